@@ -1,0 +1,179 @@
+"""CPU oracle — TEST INFRASTRUCTURE, NOT THE PRODUCT (see oracle/oracle.cpp header).
+
+ctypes marshalling around oracle/liboracle.so; every function here only converts numpy
+arrays to pointers and back.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It imports nothing from
+paper_2411_18511_b200.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 the oracle into oracle/liboracle.so (plain C++, no intrinsics)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-pthread", "-o", _LIB, _SRC])
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _L(L):
+    return (ctypes.c_int * 4)(*[int(v) for v in L])
+
+
+def _c(a):
+    a = np.ascontiguousarray(a)
+    assert a.dtype in (np.complex128, np.float64), a.dtype
+    return a
+
+
+def _vol(L):
+    return int(L[0]) * int(L[1]) * int(L[2]) * int(L[3])
+
+
+def available_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def gamma() -> np.ndarray:
+    """A2 gamma matrices, complex128 [4,4,4]."""
+    g = np.empty((4, 4, 4), dtype=np.complex128)
+    lib().orc_gamma(_p(g))
+    return g
+
+
+def dirac(L, rep, m0, U, psi, begin=0, end=None, nthreads=1, out=None):
+    """O1: D psi on lex sites [begin,end) (other sites of `out` untouched / zero)."""
+    U, psi = _c(U), _c(psi)
+    V = _vol(L)
+    end = V if end is None else end
+    if out is None:
+        out = np.zeros_like(psi)
+    lib().orc_dirac(_L(L), int(rep), ctypes.c_double(m0), _p(U), _p(psi), _p(out),
+                    ctypes.c_long(begin), ctypes.c_long(end), int(nthreads))
+    return out
+
+
+def dirac_sites(L, rep, m0, U, psi, sites):
+    U, psi = _c(U), _c(psi)
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((len(sites),) + psi.shape[1:], dtype=np.complex128)
+    lib().orc_dirac_sites(_L(L), int(rep), ctypes.c_double(m0), _p(U), _p(psi),
+                          ctypes.c_long(len(sites)), _p(sites), _p(out))
+    return out
+
+
+def hop(L, rep, out_parity, U, psi, begin=0, end=None, nthreads=1, out=None):
+    """O2: out[x] = H psi(x) on sites of parity out_parity, zero elsewhere."""
+    U, psi = _c(U), _c(psi)
+    V = _vol(L)
+    end = V if end is None else end
+    if out is None:
+        out = np.zeros_like(psi)
+    lib().orc_hop(_L(L), int(rep), int(out_parity), _p(U), _p(psi), _p(out),
+                  ctypes.c_long(begin), ctypes.c_long(end), int(nthreads))
+    return out
+
+
+def hop_sites(L, rep, U, psi, sites):
+    U, psi = _c(U), _c(psi)
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.empty((len(sites),) + psi.shape[1:], dtype=np.complex128)
+    lib().orc_hop_sites(_L(L), int(rep), _p(U), _p(psi), ctypes.c_long(len(sites)), _p(sites), _p(out))
+    return out
+
+
+def dirac_eo(L, rep, m0, U, psi, nthreads=1):
+    """O3: even-odd preconditioned operator on the even entries of psi (odd output = 0)."""
+    U, psi = _c(U), _c(psi)
+    out = np.zeros_like(psi)
+    lib().orc_dirac_eo(_L(L), int(rep), ctypes.c_double(m0), _p(U), _p(psi), _p(out), int(nthreads))
+    return out
+
+
+def represent(Ufund):
+    """O4: adjoint links [...,3,3] float64 from fundamental links [...,2,2]; also max |imag|."""
+    Ufund = _c(Ufund)
+    n = Ufund.size // 4
+    out = np.empty(Ufund.shape[:-2] + (3, 3), dtype=np.float64)
+    mi = ctypes.c_double(0.0)
+    lib().orc_represent(ctypes.c_long(n), _p(Ufund), _p(out), ctypes.byref(mi))
+    return out, mi.value
+
+
+def field_strength(L, U, mu, nu):
+    """O5: F^_mu,nu(x), complex128 [V,2,2]."""
+    U = _c(U)
+    F = np.empty((_vol(L), 2, 2), dtype=np.complex128)
+    lib().orc_field_strength(_L(L), _p(U), int(mu), int(nu), _p(F))
+    return F
+
+
+def clover_dense(L, diag, csw, U, begin=0, end=None, nthreads=1):
+    """O5/O6: dense [V,8,8] site matrices diag*1 + C(x) (rows/cols = spin*2 + colour)."""
+    U = _c(U)
+    V = _vol(L)
+    end = V if end is None else end
+    A = np.zeros((V, 8, 8), dtype=np.complex128)
+    lib().orc_clover_dense(_L(L), ctypes.c_double(diag), ctypes.c_double(csw), _p(U), _p(A),
+                           ctypes.c_long(begin), ctypes.c_long(end), int(nthreads))
+    return A
+
+
+def invert(A):
+    """Generic dense inverse of a stack of n x n complex matrices."""
+    A = _c(A)
+    n = A.shape[-1]
+    out = np.empty_like(A)
+    rc = lib().orc_invert(int(n), ctypes.c_long(A.size // (n * n)), _p(A), _p(out))
+    if rc:
+        raise ZeroDivisionError("singular matrix in oracle.invert")
+    return out
+
+
+def site_matvec(L, parity_mask, M, psi, begin=0, end=None):
+    M, psi = _c(M), _c(psi)
+    V = _vol(L)
+    end = V if end is None else end
+    out = np.zeros_like(psi)
+    lib().orc_site_matvec(_L(L), int(parity_mask), _p(M), _p(psi), _p(out), ctypes.c_long(begin), ctypes.c_long(end))
+    return out
+
+
+def dirac_clover(L, m0, U, Cdense, psi, nthreads=1):
+    """D_sw psi = D psi + C psi on all sites (Cdense built with diag = 0)."""
+    U, Cdense, psi = _c(U), _c(Cdense), _c(psi)
+    out = np.zeros_like(psi)
+    lib().orc_dirac_clover(_L(L), ctypes.c_double(m0), _p(U), _p(Cdense), _p(psi), _p(out), int(nthreads))
+    return out
+
+
+def dirac_eo_clover(L, U, A, Ainv, psi, nthreads=1):
+    """O7 on the even entries of psi (odd output = 0)."""
+    U, A, Ainv, psi = _c(U), _c(A), _c(Ainv), _c(psi)
+    out = np.zeros_like(psi)
+    lib().orc_dirac_eo_clover(_L(L), _p(U), _p(A), _p(Ainv), _p(psi), _p(out), int(nthreads))
+    return out

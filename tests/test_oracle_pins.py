@@ -1,0 +1,429 @@
+"""Pins P1-P14: what holds the CPU oracle in place.
+
+The paper (arXiv 2411.18511) prints no formula and no worked numeric example (PAPER.md:29-39,
+51-61 describe kernels only), so the oracle is pinned to what physics and mathematics fix:
+closed forms, invariants, special cases, brute force.  Everything on the right-hand side of an
+assert here is typed in this file / tests/helpers.py / tests/golden, or computed by numpy —
+never by the CUDA path.
+"""
+import numpy as np
+import pytest
+
+from paper_2411_18511_b200 import inputs
+from helpers import (PAULI, bwd, dagger, flat, fwd, gauge_transform, golden_gamma, grid, rel_l2,
+                     wilson_dirac_numpy)
+
+GAM = golden_gamma()
+G5 = np.diag([1.0, 1.0, -1.0, -1.0]).astype(np.complex128)
+
+
+def inner(a, b):
+    return np.vdot(a.ravel(), b.ravel())
+
+
+# ---------------------------------------------------------------- gamma basis (A2)
+def test_gamma_basis_is_the_golden_one(orc):
+    g = orc.gamma()
+    assert np.array_equal(g, GAM)
+    for mu in range(4):
+        assert np.array_equal(g[mu], dagger(g[mu]))
+        for nu in range(4):
+            anti = g[mu] @ g[nu] + g[nu] @ g[mu]
+            assert np.allclose(anti, 2.0 * np.eye(4) * (mu == nu), atol=0)
+    assert np.array_equal(g[0] @ g[1] @ g[2] @ g[3], G5)
+
+
+# ---------------------------------------------------------------- P1 plane wave
+@pytest.mark.parametrize("rep,N", [(0, 2), (1, 3)])
+@pytest.mark.parametrize("n", [(1, 0, 3, 2), (1, 0, 0, 0), (0, 2, 0, 0), (0, 0, 1, 0), (0, 0, 0, 3)])
+def test_P1_plane_wave(orc, rep, N, n):
+    L = (4, 6, 4, 8)
+    m0 = -0.2
+    V = inputs.volume(L)
+    x = inputs.site_coords(L)
+    p = 2.0 * np.pi * np.array(n) / np.array(L)
+    phase = np.exp(1j * (x @ p))
+    rng = np.random.default_rng(11)
+    w = rng.normal(size=(4, N)) + 1j * rng.normal(size=(4, N))
+    psi = phase[:, None, None] * w[None]
+    if rep == 0:
+        U = inputs.unit_gauge(L)
+    else:
+        U = np.tile(np.eye(3), (V, 4, 1, 1))
+    out = orc.dirac(L, rep, m0, U, psi)
+    M = (m0 + np.sum(1.0 - np.cos(p))) * np.eye(4) + 1j * sum(GAM[mu] * np.sin(p[mu]) for mu in range(4))
+    expect = phase[:, None, None] * (M @ w)[None]
+    assert rel_l2(out, expect) < 1e-14
+    # eigenvalues (basis independent): m0 + sum(1 - cos p) +- i sqrt(sum sin^2 p), each twice
+    ev = np.linalg.eigvals(M)
+    lam = m0 + np.sum(1.0 - np.cos(p))
+    s = np.sqrt(np.sum(np.sin(p) ** 2))
+    ev = ev[np.argsort(ev.imag)]
+    assert np.allclose(ev, np.array([lam - 1j * s] * 2 + [lam + 1j * s] * 2), atol=1e-14)
+
+
+# ---------------------------------------------------------------- P14 brute force / independent restatement
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 4, 4, 4), (2, 4, 6, 4)])
+def test_P14_independent_restatement_fund(orc, L):
+    U = inputs.haar_gauge(L, seed=1)
+    psi = inputs.gaussian_spinor(L, 2, seed=2)
+    out = orc.dirac(L, 0, -0.2, U, psi)
+    ref = wilson_dirac_numpy(L, U, psi, -0.2, GAM)
+    assert rel_l2(out, ref) < 1e-14
+
+
+def test_P14_independent_restatement_adj(orc):
+    L = (4, 2, 4, 6)
+    Ua, _ = orc.represent(inputs.haar_gauge(L, seed=1))
+    psi = inputs.gaussian_spinor(L, 3, seed=2)
+    out = orc.dirac(L, 1, -0.3, Ua, psi)
+    ref = wilson_dirac_numpy(L, Ua, psi, -0.3, GAM)
+    assert rel_l2(out, ref) < 1e-14
+
+
+def test_P14_dense_matrix_columns(orc):
+    """2^4: assemble D column by column from the oracle and from the numpy restatement."""
+    L = (2, 2, 2, 2)
+    V = 16
+    U = inputs.haar_gauge(L, seed=1)
+    n = V * 8
+    Do = np.empty((n, n), dtype=np.complex128)
+    Dn = np.empty((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1.0
+        e = e.reshape(V, 4, 2)
+        Do[:, k] = orc.dirac(L, 0, -0.2, U, e).ravel()
+        Dn[:, k] = wilson_dirac_numpy(L, U, e, -0.2, GAM).ravel()
+    assert np.abs(Do - Dn).max() < 1e-14
+
+
+# ---------------------------------------------------------------- P2 gamma5-hermiticity
+@pytest.mark.parametrize("rep,N", [(0, 2), (1, 3)])
+def test_P2_gamma5_hermiticity(orc, rep, N):
+    L = (4, 4, 4, 4)
+    U = inputs.haar_gauge(L, seed=1)
+    if rep == 1:
+        U, _ = orc.represent(U)
+    psi = inputs.gaussian_spinor(L, N, seed=2)
+    chi = inputs.gaussian_spinor(L, N, seed=3, field=inputs.FIELD_SPINOR2)
+    g5 = lambda v: np.einsum("st,xtc->xsc", G5, v)
+    lhs = inner(chi, orc.dirac(L, rep, -0.2, U, psi))
+    rhs = inner(g5(orc.dirac(L, rep, -0.2, U, g5(chi))), psi)
+    assert abs(lhs - rhs) / abs(lhs) < 1e-14
+
+
+def test_P2_gamma5_hermiticity_clover(orc):
+    L = (4, 4, 4, 4)
+    U = inputs.weak_gauge(L, 0.3, seed=1)
+    C = orc.clover_dense(L, 0.0, 1.2, U)
+    psi = inputs.gaussian_spinor(L, 2, seed=2)
+    chi = inputs.gaussian_spinor(L, 2, seed=3, field=inputs.FIELD_SPINOR2)
+    g5 = lambda v: np.einsum("st,xtc->xsc", G5, v)
+    lhs = inner(chi, orc.dirac_clover(L, -0.25, U, C, psi))
+    rhs = inner(g5(orc.dirac_clover(L, -0.25, U, C, g5(chi))), psi)
+    assert abs(lhs - rhs) / abs(lhs) < 1e-14
+
+
+# ---------------------------------------------------------------- P3 gauge covariance
+def test_P3_gauge_covariance_fund(orc):
+    L = (4, 6, 4, 4)
+    U = inputs.haar_gauge(L, seed=1)
+    g = inputs.haar_sites(L, seed=4)
+    psi = inputs.gaussian_spinor(L, 2, seed=2)
+    Ug = gauge_transform(U, g, L)
+    gpsi = np.einsum("xcd,xsd->xsc", g, psi)
+    lhs = orc.dirac(L, 0, -0.2, Ug, gpsi)
+    rhs = np.einsum("xcd,xsd->xsc", g, orc.dirac(L, 0, -0.2, U, psi))
+    assert rel_l2(lhs, rhs) < 1e-14
+
+
+def test_P3_gauge_covariance_adj(orc):
+    L = (4, 4, 6, 4)
+    U = inputs.haar_gauge(L, seed=1)
+    g = inputs.haar_sites(L, seed=4)
+    psi = inputs.gaussian_spinor(L, 3, seed=2)
+    Ra, _ = orc.represent(U)
+    Rg, _ = orc.represent(gauge_transform(U, g, L))
+    Rsite, _ = orc.represent(g)
+    gpsi = np.einsum("xcd,xsd->xsc", Rsite, psi)
+    lhs = orc.dirac(L, 1, -0.3, Rg, gpsi)
+    rhs = np.einsum("xcd,xsd->xsc", Rsite, orc.dirac(L, 1, -0.3, Ra, psi))
+    assert rel_l2(lhs, rhs) < 1e-14
+
+
+# ---------------------------------------------------------------- P9 EO vs full on a parity-supported vector
+@pytest.mark.parametrize("rep,N", [(0, 2), (1, 3)])
+def test_P9_hop_is_offdiagonal_part_of_D(orc, rep, N):
+    L = (4, 4, 2, 6)
+    m0 = -0.2
+    U = inputs.haar_gauge(L, seed=1)
+    if rep == 1:
+        U, _ = orc.represent(U)
+    par = inputs.site_parity(L)
+    psi = inputs.gaussian_spinor(L, N, seed=2)
+    psi_e = psi * (par == 0)[:, None, None]
+    Dpsi = orc.dirac(L, rep, m0, U, psi_e)
+    H = orc.hop(L, rep, 1, U, psi_e)
+    assert np.array_equal(H[par == 0], np.zeros_like(H[par == 0]))
+    assert rel_l2(Dpsi[par == 1], -0.5 * H[par == 1]) < 1e-15
+    assert rel_l2(Dpsi[par == 0], (4 + m0) * psi_e[par == 0]) < 1e-15
+    # hop_sites agrees with hop on a list of sites
+    sites = np.nonzero(par == 1)[0][::7]
+    assert np.array_equal(orc.hop_sites(L, rep, U, psi_e, sites), H[sites])
+    assert np.array_equal(orc.dirac_sites(L, rep, m0, U, psi_e, sites), Dpsi[sites])
+
+
+# ---------------------------------------------------------------- P4 Schur identity (no solve)
+@pytest.mark.parametrize("rep,N", [(0, 2), (1, 3)])
+def test_P4_schur_identity(orc, rep, N):
+    L = (4, 4, 4, 6)
+    m0 = -0.1
+    d = 4.0 + m0
+    U = inputs.haar_gauge(L, seed=1)
+    if rep == 1:
+        U, _ = orc.represent(U)
+    par = inputs.site_parity(L)
+    even = (par == 0)[:, None, None]
+    x = inputs.gaussian_spinor(L, N, seed=2)
+    eta = orc.dirac(L, rep, m0, U, x)
+    # D^ x_e = eta_e - D_eo D_oo^-1 eta_o,  D_eo = -1/2 H_eo, D_oo = (4+m0)
+    rhs = eta * even + 0.5 / d * orc.hop(L, rep, 0, U, eta * ~even)
+    lhs = orc.dirac_eo(L, rep, m0, U, x)
+    assert rel_l2(lhs, rhs) < 1e-14
+    # x_o = D_oo^-1 (eta_o - D_oe x_e)
+    xo = (eta * ~even + 0.5 * orc.hop(L, rep, 1, U, x * even)) / d
+    assert rel_l2(xo, x * ~even) < 1e-14
+
+
+def test_P4_schur_identity_clover(orc):
+    L = (4, 4, 4, 4)
+    m0, csw = -0.25, 1.2
+    U = inputs.weak_gauge(L, 0.3, seed=1)
+    par = inputs.site_parity(L)
+    even = (par == 0)[:, None, None]
+    C = orc.clover_dense(L, 0.0, csw, U)
+    A = orc.clover_dense(L, 4.0 + m0, csw, U)
+    assert np.abs(A - C - (4.0 + m0) * np.eye(8)).max() < 1e-15
+    Ainv = orc.invert(A)
+    x = inputs.gaussian_spinor(L, 2, seed=2)
+    eta = orc.dirac_clover(L, m0, U, C, x)
+    Ainv_eta_o = orc.site_matvec(L, 2, Ainv, eta)
+    rhs = eta * even + 0.5 * orc.hop(L, 0, 0, U, Ainv_eta_o)
+    lhs = orc.dirac_eo_clover(L, U, A, Ainv, x)
+    assert rel_l2(lhs, rhs) < 1e-14
+
+
+# ---------------------------------------------------------------- P5 Schur complement vs full solve at 4^4
+def test_P5_schur_vs_full_solve(orc):
+    L = (4, 4, 4, 4)
+    m0 = -0.2
+    d = 4.0 + m0
+    V = 256
+    n = V * 8
+    U = inputs.haar_gauge(L, seed=1)
+    par = inputs.site_parity(L)
+    even = (par == 0)[:, None, None]
+    D = np.empty((n, n), dtype=np.complex128)
+    Dhat = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1.0
+        e = e.reshape(V, 4, 2)
+        D[:, k] = orc.dirac(L, 0, m0, U, e).ravel()
+        if par[k // 8] == 0:
+            Dhat[:, k] = orc.dirac_eo(L, 0, m0, U, e).ravel()
+    eta = inputs.gaussian_spinor(L, 2, seed=2)
+    x = np.linalg.solve(D, eta.ravel()).reshape(V, 4, 2)
+    assert np.linalg.cond(D) < 10.0
+    ev = np.repeat(par == 0, 8)
+    rhs_e = (eta * even + 0.5 / d * orc.hop(L, 0, 0, U, eta * ~even)).ravel()[ev]
+    xe = np.linalg.solve(Dhat[np.ix_(ev, ev)], rhs_e)
+    assert rel_l2(xe, x.ravel()[ev]) < 1e-12
+    x_e_full = np.zeros(n, dtype=np.complex128)
+    x_e_full[ev] = xe
+    xo = (eta * ~even + 0.5 * orc.hop(L, 0, 1, U, x_e_full.reshape(V, 4, 2))) / d
+    assert rel_l2(xo.ravel()[~ev], x.ravel()[~ev]) < 1e-12
+
+
+# ---------------------------------------------------------------- P6-P8 adjoint links
+def _quaternion(U):
+    """U = a0 + i a.sigma  ->  a0 [n], a [n,3]  (A14)"""
+    a0 = U[..., 0, 0].real
+    a = np.stack([U[..., 0, 1].imag, U[..., 0, 1].real, U[..., 0, 0].imag], axis=-1)
+    return a0, a
+
+
+def test_P6_P7_P8_adjoint(orc):
+    U1 = inputs.haar_su2(500, 1, inputs.FIELD_GAUGE)
+    U2 = inputs.haar_su2(500, 7, inputs.FIELD_GAUGE)
+    R1, mi = orc.represent(U1)
+    R2, _ = orc.represent(U2)
+    assert mi < 1e-15
+    eye = np.eye(3)
+    # P6 orthogonal, det +1
+    assert np.abs(R1 @ np.swapaxes(R1, -1, -2) - eye).max() < 1e-14
+    assert np.abs(np.linalg.det(R1) - 1.0).max() < 1e-14
+    # P7 homomorphism
+    R12, _ = orc.represent(U1 @ U2)
+    assert np.abs(R12 - R1 @ R2).max() < 1e-14
+    Rd, _ = orc.represent(dagger(U1))
+    assert np.abs(Rd - np.swapaxes(R1, -1, -2)).max() < 1e-15
+    Rm, _ = orc.represent(-U1)
+    assert np.abs(Rm - R1).max() < 1e-15
+    # P8 orientation: U sigma_b U^dag = sum_a sigma_a R_ab
+    lhs = np.einsum("nij,bjk,nkl->nbil", U1, PAULI, dagger(U1))
+    rhs = np.einsum("aij,nab->nbij", PAULI, R1)
+    assert np.abs(lhs - rhs).max() < 1e-14
+    # closed form (O4): R_ab = (a0^2 - |a|^2) d_ab + 2 a_a a_b + 2 a0 eps_abc a_c
+    a0, a = _quaternion(U1)
+    eps = np.zeros((3, 3, 3))
+    eps[0, 1, 2] = eps[1, 2, 0] = eps[2, 0, 1] = 1.0
+    eps[0, 2, 1] = eps[2, 1, 0] = eps[1, 0, 2] = -1.0
+    cf = ((a0 ** 2 - (a * a).sum(-1))[:, None, None] * eye + 2.0 * a[:, :, None] * a[:, None, :]
+          + 2.0 * a0[:, None, None] * np.einsum("abc,nc->nab", eps, a))
+    assert np.abs(cf - R1).max() < 1e-14
+    # identity and a rotation about axis 3 by angle 2*theta: U = exp(i theta sigma_3)
+    Rid, _ = orc.represent(np.eye(2, dtype=np.complex128)[None])
+    assert np.array_equal(Rid[0], eye)
+    th = 0.37
+    Rz, _ = orc.represent(np.diag([np.exp(1j * th), np.exp(-1j * th)])[None])
+    c, s = np.cos(2 * th), np.sin(2 * th)
+    assert np.abs(Rz[0] - np.array([[c, s, 0], [-s, c, 0], [0, 0, 1]])).max() < 1e-15
+
+
+# ---------------------------------------------------------------- P10 clover structure
+def test_P10_clover_structure(orc):
+    L = (4, 4, 4, 4)
+    U = inputs.haar_gauge(L, seed=1)
+    g = inputs.haar_sites(L, seed=4)
+    Ug = gauge_transform(U, g, L)
+    for mu in range(4):
+        for nu in range(4):
+            if mu == nu:
+                continue
+            F = orc.field_strength(L, U, mu, nu)
+            assert np.abs(F + dagger(F)).max() < 1e-15                       # anti-hermitian
+            assert np.abs(np.trace(F, axis1=-1, axis2=-2)).max() < 1e-15       # traceless
+            assert np.abs(F + orc.field_strength(L, U, nu, mu)).max() < 1e-15  # antisymmetric in mu,nu
+            Fg = orc.field_strength(L, Ug, mu, nu)
+            assert np.abs(Fg - g @ F @ dagger(g)).max() < 1e-14                # covariant at x
+    C = orc.clover_dense(L, 0.0, 1.0, U)
+    assert np.abs(C - dagger(C)).max() < 1e-15
+    assert np.abs(np.trace(C, axis1=-1, axis2=-2)).max() < 1e-14
+    g5 = np.kron(G5, np.eye(2))
+    assert np.abs(C @ g5 - g5 @ C).max() < 1e-15
+    assert np.abs(C[:, :4, 4:]).max() < 1e-15 and np.abs(C[:, 4:, :4]).max() < 1e-15
+    # pure gauge links U_mu(x) = g(x) g(x+mu)^dag  =>  C = 0
+    Upure = gauge_transform(inputs.unit_gauge(L), g, L)
+    assert np.abs(orc.clover_dense(L, 0.0, 1.0, Upure)).max() < 1e-14
+
+
+def test_O6_block_formula(orc):
+    """A+- = (4+m0) + (csw/2)[tau1 x i(+-F01 - F23) + tau2 x i(+-F02 + F13) + tau3 x i(+-F03 - F12)]."""
+    L = (4, 4, 4, 4)
+    m0, csw = -0.25, 1.2
+    U = inputs.weak_gauge(L, 0.3, seed=1)
+    A = orc.clover_dense(L, 4.0 + m0, csw, U)
+    F = {(m, n): orc.field_strength(L, U, m, n) for m in range(4) for n in range(m + 1, 4)}
+    for sign, sl in ((+1, slice(0, 4)), (-1, slice(4, 8))):
+        blk = (4.0 + m0) * np.eye(4)[None] + 0.5 * csw * (
+            np.einsum("st,xcd->xsctd", PAULI[0], 1j * (sign * F[0, 1] - F[2, 3])).reshape(-1, 4, 4)
+            + np.einsum("st,xcd->xsctd", PAULI[1], 1j * (sign * F[0, 2] + F[1, 3])).reshape(-1, 4, 4)
+            + np.einsum("st,xcd->xsctd", PAULI[2], 1j * (sign * F[0, 3] - F[1, 2])).reshape(-1, 4, 4))
+        assert np.abs(A[:, sl, sl] - blk).max() < 1e-15
+
+
+# ---------------------------------------------------------------- P11 abelian closed form
+def test_P11_abelian_closed_form(orc):
+    L = (4, 6, 4, 4)
+    V = inputs.volume(L)
+    rng = np.random.default_rng(5)
+    phi = rng.uniform(-np.pi, np.pi, size=(V, 4))
+    U = np.zeros((V, 4, 2, 2), dtype=np.complex128)
+    U[..., 0, 0] = np.exp(1j * phi)
+    U[..., 1, 1] = np.exp(-1j * phi)
+    ph = grid(phi, L)
+    for mu in range(4):
+        for nu in range(4):
+            if mu == nu:
+                continue
+            P = ph[..., mu] + fwd(ph[..., nu], mu) - fwd(ph[..., mu], nu) - ph[..., nu]
+            S = np.sin(P) + np.sin(bwd(P, mu)) + np.sin(bwd(bwd(P, mu), nu)) + np.sin(bwd(P, nu))
+            expect = (0.25j * S)[..., None, None] * PAULI[2]
+            F = orc.field_strength(L, U, mu, nu)
+            assert np.abs(F - flat(expect, L)).max() < 1e-15
+
+
+# ---------------------------------------------------------------- P12 sign of the clover term
+def test_P12_clover_sign(orc):
+    """Tree-level improvement identity: -1/2 sum_{mu!=nu} g_mu g_nu Dl_mu Dl_nu psi ~ C psi (c_sw = 1),
+    Dl = symmetric covariant difference; residual is the O(k^2) lattice artefact."""
+    L = (12, 12, 12, 12)
+    V = inputs.volume(L)
+    k = 2.0 * np.pi / 12.0
+    x = inputs.site_coords(L).astype(np.float64)
+    rng = np.random.default_rng(3)
+    q = np.zeros((V, 4, 4))
+    for mu in range(4):
+        f = np.empty((V, 3))
+        for c in range(3):
+            n = rng.integers(0, 2, size=4)
+            f[:, c] = 0.2 * np.cos(k * (x @ n) + rng.uniform(0, 2 * np.pi))
+        r = np.sqrt((f * f).sum(-1))
+        q[:, mu, 0] = np.cos(r)
+        q[:, mu, 1:] = f * (np.sin(r) / r)[:, None]
+    U = np.empty((V, 4, 2, 2), dtype=np.complex128)
+    inputs._quaternion_to_su2(q, U)
+    w = rng.normal(size=(4, 2)) + 1j * rng.normal(size=(4, 2))
+    psi = (np.cos(k * x[:, 0] + 0.3) * np.sin(k * (x[:, 1] + x[:, 2])))[:, None, None] * w[None]
+
+    Ug = grid(U, L)
+
+    def cdiff(v, mu):
+        u = Ug[..., mu, :, :]
+        f = np.einsum("...cd,...sd->...sc", u, fwd(v, mu))
+        b = bwd(np.einsum("...dc,...sd->...sc", np.conj(u), v), mu)
+        return 0.5 * (f - b)
+
+    p = grid(psi, L)
+    lhs = np.zeros_like(p)
+    for mu in range(4):
+        for nu in range(4):
+            if mu != nu:
+                lhs += -0.5 * np.einsum("st,...tc->...sc", GAM[mu] @ GAM[nu], cdiff(cdiff(p, nu), mu))
+    lhs = flat(lhs, L)
+    C = orc.clover_dense(L, 0.0, 1.0, U)
+    Cpsi = orc.site_matvec(L, 3, C, psi)
+    nC = np.linalg.norm(Cpsi)
+    assert np.linalg.norm(lhs - Cpsi) < 0.5 * nC
+    assert np.linalg.norm(lhs + Cpsi) > 1.5 * nC
+
+
+# ---------------------------------------------------------------- P13 inverse
+def test_P13_clover_inverse(orc):
+    L = (4, 4, 4, 4)
+    U = inputs.weak_gauge(L, 0.3, seed=1)
+    A = orc.clover_dense(L, 4.0 - 0.25, 1.2, U)
+    Ainv = orc.invert(A)
+    assert np.abs(A @ Ainv - np.eye(8)).max() < 1e-14
+    assert np.abs(Ainv - np.linalg.inv(A)).max() < 1e-14
+    ev = np.linalg.eigvalsh(A[:, :4, :4])
+    # each chirality block of C is traceless (tr tau_k = 0): eigenvalues average to 4+m0 exactly;
+    # SURVEY P13 saw [2.7, 4.8] with its own random field at these parameters: same scale here
+    assert np.abs(ev.mean(axis=1) - 3.75).max() < 1e-14
+    assert ev.min() > 2.4 and ev.max() < 5.1 and (ev.max(axis=1) / ev.min(axis=1)).max() < 2.0
+    # the generic inverse on a matrix that needs pivoting
+    M = np.array([[[0, 2], [3, 1]]], dtype=np.complex128)
+    assert np.abs(orc.invert(M) - np.linalg.inv(M)).max() < 1e-15
+
+
+# ---------------------------------------------------------------- threads give the same bits
+def test_threads_bitwise_identical(orc):
+    L = (4, 4, 4, 6)
+    U = inputs.haar_gauge(L, seed=1)
+    psi = inputs.gaussian_spinor(L, 2, seed=2)
+    a = orc.dirac(L, 0, -0.2, U, psi, nthreads=1)
+    b = orc.dirac(L, 0, -0.2, U, psi, nthreads=3)
+    assert np.array_equal(a, b)
+    assert np.array_equal(orc.dirac_eo(L, 0, -0.2, U, psi, 1), orc.dirac_eo(L, 0, -0.2, U, psi, 4))
