@@ -1,0 +1,155 @@
+/* hr_dslash.h — C-ABI of the B200-native Wilson-Dirac hot path of HiRep (arXiv 2411.18511).
+ *
+ * What the paper describes (§2.1 "Wilson-Dirac Operator", §2.2 "Clover
+ * improvement") is a set of device kernels; it prints no formula.  The operator is the one written in
+ * BASELINE.json `north_star`,
+ *
+ *     D psi(x) = (4+m0) psi(x) - 1/2 sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^dag psi(x-mu) ],
+ *
+ * on a 4-D periodic lattice, gauge group SU(2), fermions in the fundamental (2 complex colours) or
+ * adjoint (3 colours, real 3x3 links) representation, with the conventions of SURVEY.md §8(c) /
+ * DESIGN.md §3 (gamma basis A2, site order A3, canonical formats A4).
+ *
+ * Conventions of every call
+ *   - extern "C", plain C types, no torch types.  `stream` is a cudaStream_t passed as void* (NULL = default).
+ *   - Unless the name ends in `_host`, every data pointer is a DEVICE pointer, 16-byte aligned.
+ *   - Return value: HR_OK, or an error code below; hr_last_error() gives the text of the last failure
+ *     of the calling thread.  Argument checks happen before anything is enqueued.
+ *   - Device calls only enqueue work on `stream`: no allocation, no host-device synchronisation.
+ *   - The caller owns every buffer, including temporaries, and sizes them with the hr_*_bytes queries.
+ *   - "canonical" = array-of-structs in lexicographic site order (x3 fastest), real type of geom->prec:
+ *         spinor        [V][4 spin][N colour][re,im]
+ *         fund gauge    [V][4 mu][2 row][2 col][re,im]
+ *         adj gauge     [V][4 mu][3 a][3 b]                       (real)
+ *         clover blocks [V][2 chirality +,-][16 reals]            (4 real diagonal entries, then the 6
+ *                        strictly-lower complex entries (1,0) (2,0) (3,0) (2,1) (3,1) (3,2) as re,im;
+ *                        block index = (spin mod 2)*2 + colour)
+ *     "device layout" = the library's parity-split, x3-row-blocked structure of arrays;
+ *     opaque to the caller except through hr_pack_* / hr_unpack_*.  A full-lattice device field is the
+ *     even half followed by the odd half, each hr_*_bytes(geom, 0) long, so `field + half` is the odd half.
+ *   - Lattice extents must be even and >= 2 (odd extents break the even-odd colouring under wrap-around).
+ */
+#ifndef HR_DSLASH_H
+#define HR_DSLASH_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { HR_OK = 0, HR_EINVAL = 1, HR_EUNSUPPORTED = 2, HR_EALIGN = 3, HR_ECUDA = 4 };
+
+enum { HR_REP_FUND = 0, HR_REP_ADJ = 1 };
+enum { HR_PREC_F64 = 0, HR_PREC_F32 = 1 };
+/* fundamental links are stored as their first row (alpha, beta): U = [[alpha, beta], [-conj(beta), conj(alpha)]]
+ * is exact for SU(2).  HR_LINKS_FULL (all four entries) is declared for the byte model only and is
+ * rejected with HR_EUNSUPPORTED by the kernels. */
+enum { HR_LINKS_FULL = 0, HR_LINKS_COMPRESSED = 1 };
+/* which hopping kernel runs: AUTO picks the x0-marching tiled kernel when the lattice allows it and is
+ * large enough to need it, else the generic one-thread-per-site kernel.  The other two values force a
+ * kernel (HR_KERNEL_TILED fails with HR_EUNSUPPORTED if the lattice does not fit its tiles). */
+enum { HR_KERNEL_AUTO = 0, HR_KERNEL_GENERIC = 1, HR_KERNEL_TILED = 2 };
+
+typedef struct hr_geom {
+    int L[4];         /* extents, L[0] = T (slowest) ... L[3] (fastest); all even, >= 2 */
+    int rep;          /* HR_REP_*: representation of the FERMION (and of the links the operators read) */
+    int prec;         /* HR_PREC_* : arithmetic and storage type of every field */
+    int link_storage; /* HR_LINKS_* (fundamental links only) */
+    int kernel;       /* HR_KERNEL_* */
+} hr_geom;
+
+/* parity arguments */
+enum { HR_EVEN = 0, HR_ODD = 1, HR_BOTH = 2 };
+
+/* ---- sizes (host-only, no CUDA call).  0 is returned for an invalid geometry. ---- */
+size_t hr_spinor_bytes(const hr_geom* g, int parity);      /* device layout; parity HR_EVEN/HR_ODD: half field, HR_BOTH: full */
+size_t hr_gauge_bytes(const hr_geom* g, int rep);           /* device layout, all 4V links of representation `rep` */
+size_t hr_clover_bytes(const hr_geom* g);                   /* device layout, one set of blocks (forward OR inverse), all V sites */
+size_t hr_canonical_spinor_bytes(const hr_geom* g);         /* canonical, V sites */
+size_t hr_canonical_gauge_bytes(const hr_geom* g, int rep); /* canonical, 4V links */
+size_t hr_canonical_clover_bytes(const hr_geom* g);         /* canonical, V sites x 2 x 16 reals */
+
+/* ---- canonical <-> device layout (both pointers on the device; pure permutations, no arithmetic) ---- */
+int hr_pack_spinor(const hr_geom* g, const void* canon, void* dev, void* stream);
+int hr_unpack_spinor(const hr_geom* g, const void* dev, void* canon, void* stream);
+int hr_pack_gauge(const hr_geom* g, int rep, const void* canon, void* dev, void* stream);
+int hr_unpack_gauge(const hr_geom* g, int rep, const void* dev, void* canon, void* stream);
+int hr_pack_clover(const hr_geom* g, const void* canon, void* dev, void* stream);
+int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* stream);
+
+/* R1 (BASELINE.json north_star "Representation kernel"; "higher representations"):
+ *   R^{ab}(x,mu) = 1/2 tr(sigma_a U_mu(x) sigma_b U_mu(x)^dag), a,b = 1..3, real 3x3, for all 4V links.
+ * u_fund: fundamental gauge field, u_adj: adjoint gauge field, both device layout, sized by
+ * hr_gauge_bytes(g, HR_REP_FUND / HR_REP_ADJ).  g->rep is ignored. */
+int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* stream);
+
+/* H3 (north_star "full form"): out = D psi on all V sites, one launch.
+ * u: gauge field in representation g->rep; psi, out: full-lattice spinors (out must not alias psi). */
+int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, void* out, void* stream);
+
+/* H1/H2/E1/E2 (north_star "even-odd preconditioned form D_ee - D_eo D_oo^-1 D_oe as used in the HMC";
+ * PAPER.md:39 "even-odd preconditioned version of the Dirac operator used mainly in the HMC").
+ *   op = HR_EO_HOP_OE : out_o = H_oe in_e   (bare hopping sum, no -1/2), in: even half field, out: odd half field
+ *   op = HR_EO_HOP_EO : out_e = H_eo in_o
+ *   op = HR_EO_DHAT   : out_e = Dhat in_e, in and out even half fields, tmp an odd half field;
+ *        without clover (clover_fwd == clover_inv == NULL):
+ *              Dhat = (4+m0) - H_eo H_oe / (4 (4+m0))
+ *        with clover (both non-NULL, built by hr_clover_build with the same m0; fundamental rep only):
+ *              Dhat = A_ee - 1/4 H_eo A_oo^-1 H_oe            (m0 is then ignored: it lives inside A)
+ *        Two dependent launches on `stream` (the paper's "impossible to parallelise" pair of halves).
+ * out must not alias in; tmp must alias neither. */
+enum { HR_EO_HOP_OE = 0, HR_EO_HOP_EO = 1, HR_EO_DHAT = 2 };
+int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const void* clover_fwd,
+                      const void* clover_inv, const void* in, void* out, void* tmp, void* stream);
+
+/* C1 ("precomputing certain fields ... recomputed whenever the gauge field is updated"):
+ * from the FUNDAMENTAL gauge field build, for every site, the two hermitian 4x4 chirality blocks of
+ *   A(x) = (4+m0) + csw (i/4) sum_{mu,nu} sigma_mu,nu F^_mu,nu(x)      (F^ from the four-leaf clover)
+ * into clover_fwd and their inverses into clover_inv (either may be NULL to skip it).  Setup step. */
+int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
+                    void* clover_inv, void* stream);
+
+/* C2/C3 ("application of another diagonal term"): out(x) = B(x) in(x) on the sites of
+ * `parity` (HR_EVEN, HR_ODD: in/out are half fields; HR_BOTH: full fields).  `blocks` is the full-lattice
+ * block field (forward blocks: C2; inverse blocks: C3 — same kernel).  Fundamental rep only. */
+int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream);
+
+/* M1 ("measured in terms of memory bandwidth"): the work model, per OUTPUT site of `op`,
+ * for the storage described by g.  bytes_compulsory: every distinct datum crosses DRAM once per kernel;
+ * bytes_requested: no reuse at all (every neighbour spinor counted), the paper-style figure. Host-only. */
+enum {
+    HR_OP_HOP = 0,        /* bare parity hop H1                     */
+    HR_OP_DIRAC = 1,      /* full D, one launch (H3), per site of V */
+    HR_OP_DHAT = 2,       /* E1, per even site                      */
+    HR_OP_CLOVER = 3,     /* C2/C3                                  */
+    HR_OP_DHAT_CLOVER = 4,/* E2, per even site                      */
+    HR_OP_REPRESENT = 5   /* R1, per site (4 links)                 */
+};
+int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, double* bytes_compulsory,
+                         double* bytes_requested);
+
+/* ---- host-buffer entry points (the end-to-end path a user without device buffers calls) ----
+ * All data pointers are HOST pointers to canonical arrays (pinned memory makes the copies asynchronous);
+ * `workspace` is a DEVICE buffer of at least hr_host_workspace_bytes(g) bytes.  The call uploads gauge
+ * and spinor, packs, applies, unpacks, downloads, and synchronises `stream` before returning.
+ *   hr_dirac_apply_host    : out[V] = D psi[V]
+ *   hr_dirac_eo_apply_host : op as in hr_dirac_eo_apply without clover; full-lattice canonical arrays, only
+ *                            the entries of the input parity are read, only those of the output parity written. */
+size_t hr_host_workspace_bytes(const hr_geom* g);
+int hr_dirac_apply_host(const hr_geom* g, double m0, const void* u_canon_host, const void* psi_canon_host,
+                        void* out_canon_host, void* workspace, void* stream);
+int hr_dirac_eo_apply_host(const hr_geom* g, int op, double m0, const void* u_canon_host,
+                           const void* in_canon_host, void* out_canon_host, void* workspace, void* stream);
+
+/* ---- diagnostics ---- */
+size_t hr_last_error(char* buf, size_t len);   /* copies the last error text (NUL-terminated); returns its length */
+/* number of kernels this library has launched since load (bench.py's gpu_launches) */
+unsigned long long hr_launch_count(void);
+/* name of the hopping kernel hr_dirac_eo_apply/hr_dirac_apply would run for g: "generic" or "tiled" */
+const char* hr_kernel_name(const hr_geom* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HR_DSLASH_H */

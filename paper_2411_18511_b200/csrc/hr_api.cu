@@ -1,0 +1,355 @@
+// hr_api.cu — the extern "C" entry points of libhr_dslash (include/hr_dslash.h): argument checks,
+// size queries, the work model M1, composition of the operators from the kernels, host-buffer path.
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "hr_hop_generic.cuh"
+
+namespace hr {
+
+// hr_fields.cu
+int permute_chunks(bool pack, const Geo& g, int NI, int NCH, int SRC, const void* src, void* dst, cudaStream_t st);
+int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st);
+int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st);
+int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
+int run_clover_build(const Geo& g, int prec, double diag, double csw, const void* ufund, void* fwd, void* inv, cudaStream_t st);
+int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
+
+static thread_local char g_err[512] = "";
+static std::atomic<unsigned long long> g_launches{0};
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+void count_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+int check_launch(const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        set_error("%s: %s", what, cudaGetErrorString(e));
+        return HR_ECUDA;
+    }
+    return HR_OK;
+}
+
+static int check_geom(const hr_geom* g) {
+    if (!geom_ok(g)) {
+        set_error("invalid hr_geom (extents must be even and >= 2, volume < 2e9, enums in range)");
+        return HR_EINVAL;
+    }
+    return HR_OK;
+}
+static int check_ptr(const void* p, const char* name) {
+    if (!p) {
+        set_error("%s is NULL", name);
+        return HR_EINVAL;
+    }
+    if (reinterpret_cast<uintptr_t>(p) & 15) {
+        set_error("%s is not 16-byte aligned", name);
+        return HR_EALIGN;
+    }
+    return HR_OK;
+}
+static int check_links(const hr_geom* g) {
+    if (g->rep == HR_REP_FUND && g->link_storage != HR_LINKS_COMPRESSED) {
+        set_error("HR_LINKS_FULL is a byte-model option only; kernels read HR_LINKS_COMPRESSED fundamental links");
+        return HR_EUNSUPPORTED;
+    }
+    return HR_OK;
+}
+static bool overlap(const void* a, size_t na, const void* b, size_t nb) {
+    const char* x = (const char*)a;
+    const char* y = (const char*)b;
+    return x < y + nb && y < x + na;
+}
+#define HR_TRY(expr)                 \
+    do {                             \
+        int rc_ = (expr);            \
+        if (rc_ != HR_OK) return rc_; \
+    } while (0)
+
+static size_t half_spinor_bytes(const hr_geom* g) {
+    const Geo geo = make_geo(g);
+    return (size_t)geo.Vh * spinor_chunks(g->rep, g->prec) * 16;
+}
+
+}  // namespace hr
+
+using namespace hr;
+
+extern "C" {
+
+size_t hr_spinor_bytes(const hr_geom* g, int parity) {
+    if (!geom_ok(g) || parity < HR_EVEN || parity > HR_BOTH) return 0;
+    return half_spinor_bytes(g) * (parity == HR_BOTH ? 2 : 1);
+}
+
+size_t hr_gauge_bytes(const hr_geom* g, int rep) {
+    if (!geom_ok(g) || (rep != HR_REP_FUND && rep != HR_REP_ADJ)) return 0;
+    const Geo geo = make_geo(g);
+    const size_t links = 8 * (size_t)geo.Vh;
+    if (rep == HR_REP_FUND) return links * link_chunks(g->prec) * 16;
+    return links * 9 * real_bytes(g->prec);
+}
+
+size_t hr_clover_bytes(const hr_geom* g) {
+    if (!geom_ok(g)) return 0;
+    const Geo geo = make_geo(g);
+    return 2 * (size_t)geo.Vh * clover_chunks(g->prec) * 16;
+}
+
+size_t hr_canonical_spinor_bytes(const hr_geom* g) {
+    if (!geom_ok(g)) return 0;
+    const Geo geo = make_geo(g);
+    return 2 * (size_t)geo.Vh * 8 * ncolour(g->rep) * real_bytes(g->prec);
+}
+
+size_t hr_canonical_gauge_bytes(const hr_geom* g, int rep) {
+    if (!geom_ok(g) || (rep != HR_REP_FUND && rep != HR_REP_ADJ)) return 0;
+    const Geo geo = make_geo(g);
+    return 8 * (size_t)geo.Vh * (rep == HR_REP_FUND ? 8 : 9) * real_bytes(g->prec);
+}
+
+size_t hr_canonical_clover_bytes(const hr_geom* g) {
+    if (!geom_ok(g)) return 0;
+    const Geo geo = make_geo(g);
+    return 2 * (size_t)geo.Vh * 32 * real_bytes(g->prec);
+}
+
+// ---------------------------------------------------------------- pack / unpack
+int hr_pack_spinor(const hr_geom* g, const void* canon, void* dev, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
+    const int nch = spinor_chunks(g->rep, g->prec);
+    return permute_chunks(true, make_geo(g), 1, nch, nch, canon, dev, (cudaStream_t)stream);
+}
+int hr_unpack_spinor(const hr_geom* g, const void* dev, void* canon, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
+    const int nch = spinor_chunks(g->rep, g->prec);
+    return permute_chunks(false, make_geo(g), 1, nch, nch, dev, canon, (cudaStream_t)stream);
+}
+int hr_pack_gauge(const hr_geom* g, int rep, const void* canon, void* dev, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
+    if (rep == HR_REP_FUND) {
+        if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+        const int lch = link_chunks(g->prec);
+        return permute_chunks(true, make_geo(g), 4, lch, 2 * lch, canon, dev, (cudaStream_t)stream);
+    }
+    if (rep == HR_REP_ADJ) return permute_adj(true, make_geo(g), g->prec, canon, dev, (cudaStream_t)stream);
+    set_error("unknown representation %d", rep);
+    return HR_EINVAL;
+}
+int hr_unpack_gauge(const hr_geom* g, int rep, const void* dev, void* canon, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
+    if (rep == HR_REP_FUND) {
+        if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+        const int lch = link_chunks(g->prec);
+        const Geo geo = make_geo(g);
+        HR_TRY(permute_chunks(false, geo, 4, lch, 2 * lch, dev, canon, (cudaStream_t)stream));
+        return rebuild_second_row(geo, g->prec, canon, (cudaStream_t)stream);
+    }
+    if (rep == HR_REP_ADJ) return permute_adj(false, make_geo(g), g->prec, dev, canon, (cudaStream_t)stream);
+    set_error("unknown representation %d", rep);
+    return HR_EINVAL;
+}
+int hr_pack_clover(const hr_geom* g, const void* canon, void* dev, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
+    const int cch = clover_chunks(g->prec);
+    return permute_chunks(true, make_geo(g), 1, cch, cch, canon, dev, (cudaStream_t)stream);
+}
+int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
+    const int cch = clover_chunks(g->prec);
+    return permute_chunks(false, make_geo(g), 1, cch, cch, dev, canon, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------- R1
+int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund")); HR_TRY(check_ptr(u_adj, "u_adj"));
+    if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+    return run_represent(make_geo(g), g->prec, u_fund, u_adj, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------- H3
+int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, void* out, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(psi, "psi")); HR_TRY(check_ptr(out, "out"));
+    const size_t full = 2 * half_spinor_bytes(g);
+    if (overlap(psi, full, out, full)) { set_error("hr_dirac_apply: out aliases psi (gather operation)"); return HR_EINVAL; }
+    HopArgs a;
+    a.gauge = u; a.in = psi; a.out = out; a.phi = psi; a.clover = nullptr;
+    a.a = 4.0 + m0; a.c = -0.5; a.parity = 0; a.both = 1;
+    return run_hop(g, a, EPI_AXPY, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------- H1 / E1 / E2
+int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const void* clover_fwd,
+                      const void* clover_inv, const void* in, void* out, void* tmp, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
+    const size_t half = half_spinor_bytes(g);
+    if (overlap(in, half, out, half)) { set_error("hr_dirac_eo_apply: out aliases in (gather operation)"); return HR_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    HopArgs a;
+    a.gauge = u; a.phi = nullptr; a.clover = nullptr; a.a = 0.0; a.c = 1.0; a.both = 0;
+    if (op == HR_EO_HOP_OE || op == HR_EO_HOP_EO) {
+        a.in = in; a.out = out; a.parity = (op == HR_EO_HOP_OE) ? HR_ODD : HR_EVEN;
+        return run_hop(g, a, EPI_NONE, st);
+    }
+    if (op != HR_EO_DHAT) { set_error("hr_dirac_eo_apply: unknown op %d", op); return HR_EINVAL; }
+    HR_TRY(check_ptr(tmp, "tmp"));
+    if (overlap(tmp, half, in, half) || overlap(tmp, half, out, half)) { set_error("hr_dirac_eo_apply: tmp aliases in or out"); return HR_EINVAL; }
+    const bool clover = clover_fwd || clover_inv;
+    if (clover) {
+        if (!clover_fwd || !clover_inv) { set_error("hr_dirac_eo_apply: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
+        HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(clover_inv, "clover_inv"));
+        if (g->rep != HR_REP_FUND) { set_error("clover operators exist for the fundamental representation only"); return HR_EUNSUPPORTED; }
+        // E2: tmp_o = A_oo^-1 H_oe in_e ;  out_e = A_ee in_e - 1/4 H_eo tmp_o
+        a.in = in; a.out = tmp; a.parity = HR_ODD; a.clover = clover_inv;
+        HR_TRY(run_hop(g, a, EPI_CLOVER_INV, st));
+        a.in = tmp; a.out = out; a.parity = HR_EVEN; a.clover = clover_fwd; a.phi = in; a.c = -0.25;
+        return run_hop(g, a, EPI_CLOVER_AXPY, st);
+    }
+    // E1: tmp_o = H_oe in_e ;  out_e = (4+m0) in_e - H_eo tmp_o / (4 (4+m0))
+    const double d = 4.0 + m0;
+    if (d == 0.0) { set_error("hr_dirac_eo_apply: 4+m0 = 0, D_oo is singular"); return HR_EINVAL; }
+    a.in = in; a.out = tmp; a.parity = HR_ODD;
+    HR_TRY(run_hop(g, a, EPI_NONE, st));
+    a.in = tmp; a.out = out; a.parity = HR_EVEN; a.phi = in; a.a = d; a.c = -1.0 / (4.0 * d);
+    return run_hop(g, a, EPI_AXPY, st);
+}
+
+// ---------------------------------------------------------------- C1 / C2 / C3
+int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
+                    void* clover_inv, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund"));
+    if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+    if (!clover_fwd && !clover_inv) { set_error("hr_clover_build: nothing to build"); return HR_EINVAL; }
+    if (clover_fwd) HR_TRY(check_ptr(clover_fwd, "clover_fwd"));
+    if (clover_inv) HR_TRY(check_ptr(clover_inv, "clover_inv"));
+    return run_clover_build(make_geo(g), g->prec, 4.0 + m0, csw, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
+}
+
+int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream) {
+    HR_TRY(check_geom(g));
+    if (g->rep != HR_REP_FUND) { set_error("clover operators exist for the fundamental representation only"); return HR_EUNSUPPORTED; }
+    if (parity < HR_EVEN || parity > HR_BOTH) { set_error("hr_clover_apply: parity %d", parity); return HR_EINVAL; }
+    HR_TRY(check_ptr(blocks, "blocks")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
+    return run_clover_apply(make_geo(g), g->prec, parity, blocks, in, out, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------- M1
+int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, double* bytes_compulsory,
+                         double* bytes_requested) {
+    HR_TRY(check_geom(g));
+    const double N = ncolour(g->rep), w = (double)real_bytes(g->prec);
+    const double nr = 8.0 * N, S = nr * w;
+    const double Gf = (g->link_storage == HR_LINKS_COMPRESSED ? 4.0 : 8.0) * w, Ga = 9.0 * w;
+    const double G = g->rep == HR_REP_FUND ? Gf : Ga;
+    const double Bk = 32.0 * w;
+    // per direction: 4N adds to project, two colour mat-vecs, 8N adds to accumulate; x8, minus the first accumulate
+    const double Fhop = g->rep == HR_REP_FUND ? 8.0 * N * (16.0 * N + 7.0) : 8.0 * N * (8.0 * N + 7.0);
+    const double Fblk = 208.0;  // two hermitian 4x4 mat-vecs
+    double f = 0, bc = 0, br = 0;
+    switch (op) {
+        case HR_OP_HOP: f = Fhop; bc = 2 * S + 8 * G; br = 9 * S + 8 * G; break;
+        case HR_OP_DIRAC: f = Fhop + 3 * nr; bc = 2 * S + 4 * G; br = 10 * S + 8 * G; break;
+        case HR_OP_DHAT: f = 2 * Fhop + 3 * nr; bc = 5 * S + 16 * G; br = 19 * S + 16 * G; break;
+        case HR_OP_CLOVER:
+            if (g->rep != HR_REP_FUND) { set_error("clover: fundamental representation only"); return HR_EUNSUPPORTED; }
+            f = Fblk; bc = 2 * S + Bk; br = bc; break;
+        case HR_OP_DHAT_CLOVER:
+            if (g->rep != HR_REP_FUND) { set_error("clover: fundamental representation only"); return HR_EUNSUPPORTED; }
+            f = 2 * Fhop + 2 * Fblk + 2 * nr; bc = 5 * S + 16 * G + 2 * Bk; br = 19 * S + 16 * G + 2 * Bk; break;
+        case HR_OP_REPRESENT: f = 4 * 30.0; bc = 4 * Gf + 4 * Ga; br = bc; break;
+        default: set_error("hr_dirac_flops_bytes: unknown op %d", op); return HR_EINVAL;
+    }
+    if (flops_per_site) *flops_per_site = f;
+    if (bytes_compulsory) *bytes_compulsory = bc;
+    if (bytes_requested) *bytes_requested = br;
+    return HR_OK;
+}
+
+// ---------------------------------------------------------------- host-buffer path
+static size_t up256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+size_t hr_host_workspace_bytes(const hr_geom* g) {
+    if (!geom_ok(g)) return 0;
+    return up256(hr_canonical_gauge_bytes(g, g->rep)) + 2 * up256(hr_canonical_spinor_bytes(g)) +
+           up256(hr_gauge_bytes(g, g->rep)) + 3 * up256(hr_spinor_bytes(g, HR_BOTH));
+}
+
+static int host_apply(const hr_geom* g, int op, double m0, const void* u_h, const void* in_h, void* out_h,
+                      void* workspace, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    if (!u_h || !in_h || !out_h) { set_error("host pointer is NULL"); return HR_EINVAL; }
+    HR_TRY(check_ptr(workspace, "workspace"));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t cg = hr_canonical_gauge_bytes(g, g->rep), cs = hr_canonical_spinor_bytes(g);
+    const size_t dg = hr_gauge_bytes(g, g->rep), ds = hr_spinor_bytes(g, HR_BOTH), half = ds / 2;
+    char* w = (char*)workspace;
+    char* c_u = w; w += up256(cg);
+    char* c_in = w; w += up256(cs);
+    char* c_out = w; w += up256(cs);
+    char* d_u = w; w += up256(dg);
+    char* d_in = w; w += up256(ds);
+    char* d_out = w; w += up256(ds);
+    char* d_tmp = w;
+#define HR_CUDA(call)                                                         \
+    do {                                                                      \
+        cudaError_t e_ = (call);                                              \
+        if (e_ != cudaSuccess) { set_error("%s: %s", #call, cudaGetErrorString(e_)); return HR_ECUDA; } \
+    } while (0)
+    HR_CUDA(cudaMemcpyAsync(c_u, u_h, cg, cudaMemcpyHostToDevice, st));
+    HR_CUDA(cudaMemcpyAsync(c_in, in_h, cs, cudaMemcpyHostToDevice, st));
+    HR_TRY(hr_pack_gauge(g, g->rep, c_u, d_u, stream));
+    HR_TRY(hr_pack_spinor(g, c_in, d_in, stream));
+    if (op < 0) {
+        HR_TRY(hr_dirac_apply(g, m0, d_u, d_in, d_out, stream));
+    } else {
+        // outputs of the untouched parity come back as zeros
+        HR_CUDA(cudaMemsetAsync(d_out, 0, ds, st));
+        const int in_par = (op == HR_EO_HOP_EO) ? HR_ODD : HR_EVEN;
+        const int out_par = (op == HR_EO_HOP_OE) ? HR_ODD : HR_EVEN;
+        HR_TRY(hr_dirac_eo_apply(g, op, m0, d_u, nullptr, nullptr, d_in + in_par * half, d_out + out_par * half, d_tmp, stream));
+    }
+    HR_TRY(hr_unpack_spinor(g, d_out, c_out, stream));
+    HR_CUDA(cudaMemcpyAsync(out_h, c_out, cs, cudaMemcpyDeviceToHost, st));
+    HR_CUDA(cudaStreamSynchronize(st));
+#undef HR_CUDA
+    return HR_OK;
+}
+
+int hr_dirac_apply_host(const hr_geom* g, double m0, const void* u_canon_host, const void* psi_canon_host,
+                        void* out_canon_host, void* workspace, void* stream) {
+    return host_apply(g, -1, m0, u_canon_host, psi_canon_host, out_canon_host, workspace, stream);
+}
+
+int hr_dirac_eo_apply_host(const hr_geom* g, int op, double m0, const void* u_canon_host,
+                           const void* in_canon_host, void* out_canon_host, void* workspace, void* stream) {
+    if (op < HR_EO_HOP_OE || op > HR_EO_DHAT) { set_error("hr_dirac_eo_apply_host: unknown op %d", op); return HR_EINVAL; }
+    return host_apply(g, op, m0, u_canon_host, in_canon_host, out_canon_host, workspace, stream);
+}
+
+// ---------------------------------------------------------------- diagnostics
+size_t hr_last_error(char* buf, size_t len) {
+    const size_t n = strlen(g_err);
+    if (buf && len) {
+        const size_t m = n < len - 1 ? n : len - 1;
+        memcpy(buf, g_err, m);
+        buf[m] = 0;
+    }
+    return n;
+}
+
+unsigned long long hr_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char* hr_kernel_name(const hr_geom* g) {
+    if (!geom_ok(g)) return "invalid";
+    return tiled_chosen(g) ? "tiled" : "generic";
+}
+
+}  // extern "C"

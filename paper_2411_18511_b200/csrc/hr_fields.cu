@@ -1,0 +1,342 @@
+// hr_fields.cu — layout permutations (pack/unpack), the representation kernel R1 and the clover
+// kernels C1/C2/C3 of libhr_dslash.
+#include "hr_common.cuh"
+
+namespace hr {
+
+// lexicographic site -> (parity, row, h)
+struct SiteRef {
+    int par, row, h;
+};
+__device__ __forceinline__ SiteRef site_of_lex(const Geo& g, int lex) {
+    const int L3 = 2 * g.L3h;
+    const int x3 = lex % L3;
+    const int row = lex / L3;
+    const int x0 = row / g.s0, rem = row - x0 * g.s0;
+    const int x1 = rem / g.s1, x2 = rem - x1 * g.s1;
+    SiteRef s;
+    s.par = (x0 + x1 + x2 + x3) & 1;
+    s.row = row;
+    s.h = x3 >> 1;
+    return s;
+}
+// coordinates (any integers, wrapped periodically) -> (parity, row, h)
+__device__ __forceinline__ SiteRef site_of_coords(const Geo& g, int x0, int x1, int x2, int x3) {
+    const int L3 = 2 * g.L3h;
+    x0 = (x0 + g.L0) % g.L0; x1 = (x1 + g.L1) % g.L1; x2 = (x2 + g.L2) % g.L2; x3 = (x3 + L3) % L3;
+    SiteRef s;
+    s.par = (x0 + x1 + x2 + x3) & 1;
+    s.row = (x0 * g.L1 + x1) * g.L2 + x2;
+    s.h = x3 >> 1;
+    return s;
+}
+
+// ------------------------------------------------------------------ pack / unpack: pure permutations
+// Generic 16-byte-chunk permutation.  Canonical: [lex][item 0..NI-1][SRC chunks]; of each item the first
+// NCH chunks are kept (NCH == SRC except for compressed links, where SRC = 2*NCH).  Device:
+//   [par][item][row][NCH][h].   Spinor and clover use NI = 1; compressed links NI = 4 (mu).
+template <bool PACK>
+__global__ void permute_chunks_kernel(Geo g, int NI, int NCH, int SRC, const uint4* __restrict__ src, uint4* __restrict__ dst) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = 2LL * g.Vh * NI * NCH;
+    if (t >= total) return;
+    const int c = (int)(t % NCH);
+    const int item = (int)((t / NCH) % NI);
+    const int lex = (int)(t / ((long long)NCH * NI));
+    const SiteRef s = site_of_lex(g, lex);
+    const size_t ic = ((size_t)lex * NI + item) * SRC + c;
+    const size_t id = (((size_t)(s.par * NI + item) * g.R + s.row) * NCH + c) * g.L3h + s.h;
+    if (PACK) dst[id] = src[ic];
+    else dst[ic] = src[id];
+}
+
+// second row of an unpacked fundamental link: (-conj(beta), conj(alpha))
+template <typename T>
+__global__ void rebuild_second_row_kernel(long long nlinks, T* canon) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nlinks) return;
+    T* u = canon + k * 8;
+    u[4] = -u[2]; u[5] = u[3];
+    u[6] = u[0]; u[7] = -u[1];
+}
+
+// adjoint links: canonical [lex][mu][9] reals <-> device [par][mu][row][9][h]
+template <typename T, bool PACK>
+__global__ void permute_adj_kernel(Geo g, const T* __restrict__ src, T* __restrict__ dst) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = 2LL * g.Vh * 36;
+    if (t >= total) return;
+    const int k = (int)(t % 9);
+    const int mu = (int)((t / 9) % 4);
+    const int lex = (int)(t / 36);
+    const SiteRef s = site_of_lex(g, lex);
+    const size_t id = (((size_t)(s.par * 4 + mu) * g.R + s.row) * 9 + k) * g.L3h + s.h;
+    if (PACK) dst[id] = src[t];
+    else dst[t] = src[id];
+}
+
+static inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+int permute_chunks(bool pack, const Geo& g, int NI, int NCH, int SRC, const void* src, void* dst, cudaStream_t st) {
+    const long long total = 2LL * g.Vh * NI * NCH;
+    if (pack)
+        permute_chunks_kernel<true><<<blocks_for(total, 256), 256, 0, st>>>(g, NI, NCH, SRC, (const uint4*)src, (uint4*)dst);
+    else
+        permute_chunks_kernel<false><<<blocks_for(total, 256), 256, 0, st>>>(g, NI, NCH, SRC, (const uint4*)src, (uint4*)dst);
+    count_launch();
+    return check_launch("permute_chunks_kernel");
+}
+
+int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st) {
+    const long long nl = 8LL * g.Vh;
+    if (prec == HR_PREC_F64) rebuild_second_row_kernel<double><<<blocks_for(nl, 256), 256, 0, st>>>(nl, (double*)canon);
+    else rebuild_second_row_kernel<float><<<blocks_for(nl, 256), 256, 0, st>>>(nl, (float*)canon);
+    count_launch();
+    return check_launch("rebuild_second_row_kernel");
+}
+
+int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st) {
+    const long long total = 2LL * g.Vh * 36;
+    const unsigned nb = blocks_for(total, 256);
+    if (prec == HR_PREC_F64) {
+        if (pack) permute_adj_kernel<double, true><<<nb, 256, 0, st>>>(g, (const double*)src, (double*)dst);
+        else permute_adj_kernel<double, false><<<nb, 256, 0, st>>>(g, (const double*)src, (double*)dst);
+    } else {
+        if (pack) permute_adj_kernel<float, true><<<nb, 256, 0, st>>>(g, (const float*)src, (float*)dst);
+        else permute_adj_kernel<float, false><<<nb, 256, 0, st>>>(g, (const float*)src, (float*)dst);
+    }
+    count_launch();
+    return check_launch("permute_adj_kernel");
+}
+
+// ------------------------------------------------------------------ R1: adjoint links from fundamental ones
+// R^{ab} = 1/2 tr(sigma_a U sigma_b U^dag)  (BASELINE.json north_star).  With U = a0 + i a.sigma
+// (alpha = a0 + i a3, beta = a2 + i a1) the trace evaluates to
+//     R_ab = (a0^2 - |a|^2) delta_ab + 2 a_a a_b + 2 a0 eps_abc a_c .
+// One thread per link; fundamental and adjoint gauge fields share the [par][mu][row][..][h] indexing.
+template <typename T>
+__global__ void represent_kernel(Geo g, const void* __restrict__ ufund, T* __restrict__ uadj) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = 8LL * g.Vh;  // 2 parities x 4 mu x Vh
+    if (t >= total) return;
+    const int h = (int)(t % g.L3h);
+    const long long pr = t / g.L3h;  // (par*4+mu)*R + row
+    cplx<T> ab[2];
+    constexpr int LCH = SiteIO<T, 2>::NCH;
+    SiteIO<T, 2>::template load<LD_STREAM>(ab, ufund, (size_t)pr * (LCH * g.L3h) + h, g.L3h);
+    const T a0 = ab[0].re, a3 = ab[0].im, a2 = ab[1].re, a1 = ab[1].im;
+    const T d = a0 * a0 - (a1 * a1 + a2 * a2 + a3 * a3);
+    T r[9];
+    r[0] = d + 2 * a1 * a1;           r[1] = 2 * (a1 * a2 + a0 * a3);   r[2] = 2 * (a1 * a3 - a0 * a2);
+    r[3] = 2 * (a2 * a1 - a0 * a3);   r[4] = d + 2 * a2 * a2;           r[5] = 2 * (a2 * a3 + a0 * a1);
+    r[6] = 2 * (a3 * a1 + a0 * a2);   r[7] = 2 * (a3 * a2 - a0 * a1);   r[8] = d + 2 * a3 * a3;
+    T* o = uadj + (size_t)pr * (9 * g.L3h) + h;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) __stcs(o + (size_t)k * g.L3h, r[k]);
+}
+
+int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st) {
+    const long long total = 8LL * g.Vh;
+    if (prec == HR_PREC_F64) represent_kernel<double><<<blocks_for(total, 256), 256, 0, st>>>(g, ufund, (double*)uadj);
+    else represent_kernel<float><<<blocks_for(total, 256), 256, 0, st>>>(g, ufund, (float*)uadj);
+    count_launch();
+    return check_launch("represent_kernel");
+}
+
+// ------------------------------------------------------------------ C1: clover blocks and their inverses
+// SU(2) matrices as quaternions q = (q0, q1, q2, q3) <-> q0 + i (q1 s1 + q2 s2 + q3 s3):
+//   product (a0,a)(b0,b) = (a0 b0 - a.b, a0 b + b0 a - a x b),  dagger = (a0, -a).
+struct Quat {
+    double q0, q1, q2, q3;
+};
+__device__ __forceinline__ Quat qmul(const Quat& a, const Quat& b) {
+    Quat c;
+    c.q0 = a.q0 * b.q0 - (a.q1 * b.q1 + a.q2 * b.q2 + a.q3 * b.q3);
+    c.q1 = a.q0 * b.q1 + b.q0 * a.q1 - (a.q2 * b.q3 - a.q3 * b.q2);
+    c.q2 = a.q0 * b.q2 + b.q0 * a.q2 - (a.q3 * b.q1 - a.q1 * b.q3);
+    c.q3 = a.q0 * b.q3 + b.q0 * a.q3 - (a.q1 * b.q2 - a.q2 * b.q1);
+    return c;
+}
+__device__ __forceinline__ Quat qdag(const Quat& a) {
+    Quat c;
+    c.q0 = a.q0; c.q1 = -a.q1; c.q2 = -a.q2; c.q3 = -a.q3;
+    return c;
+}
+template <typename T>
+__device__ __forceinline__ Quat link_quat(const void* ufund, const Geo& g, int x0, int x1, int x2, int x3, int mu) {
+    const SiteRef s = site_of_coords(g, x0, x1, x2, x3);
+    Link<T, 2> u;
+    load_link<T, LD_KEEP>(u, ufund, g, s.par, mu, s.row, s.h);
+    Quat q;
+    q.q0 = (double)u.a.re; q.q3 = (double)u.a.im; q.q2 = (double)u.b.re; q.q1 = (double)u.b.im;
+    return q;
+}
+
+// vector part of Q_mu,nu(x) = sum of the four plaquette leaves in the mu-nu plane that start and end at x,
+// all traversed in the mu -> nu sense:
+//   P1 = U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+//   P2 = U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+//   P3 = U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+//   P4 = U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+// F^_mu,nu = (Q - Q^dag)/8 = (i/4) vec(Q).sigma, so  i F^_mu,nu = -(1/4) vec(Q).sigma.
+template <typename T>
+__device__ void clover_leaves(double* v, const void* ufund, const Geo& g, const int* x, int mu, int nu) {
+    int e[4] = {0, 0, 0, 0}, f[4] = {0, 0, 0, 0};
+    e[mu] = 1;
+    f[nu] = 1;
+#define HR_U(DM, DN, DIR) link_quat<T>(ufund, g, x[0] + (DM) * e[0] + (DN) * f[0], x[1] + (DM) * e[1] + (DN) * f[1], \
+                                       x[2] + (DM) * e[2] + (DN) * f[2], x[3] + (DM) * e[3] + (DN) * f[3], DIR)
+    Quat p1 = qmul(qmul(HR_U(0, 0, mu), HR_U(1, 0, nu)), qmul(qdag(HR_U(0, 1, mu)), qdag(HR_U(0, 0, nu))));
+    Quat p2 = qmul(qmul(HR_U(0, 0, nu), qdag(HR_U(-1, 1, mu))), qmul(qdag(HR_U(-1, 0, nu)), HR_U(-1, 0, mu)));
+    Quat p3 = qmul(qmul(qdag(HR_U(-1, 0, mu)), qdag(HR_U(-1, -1, nu))), qmul(HR_U(-1, -1, mu), HR_U(0, -1, nu)));
+    Quat p4 = qmul(qmul(qdag(HR_U(0, -1, nu)), HR_U(0, -1, mu)), qmul(HR_U(1, -1, nu), qdag(HR_U(0, 0, mu))));
+#undef HR_U
+    v[0] = p1.q1 + p2.q1 + p3.q1 + p4.q1;
+    v[1] = p1.q2 + p2.q2 + p3.q2 + p4.q2;
+    v[2] = p1.q3 + p2.q3 + p3.q3 + p4.q3;
+}
+
+struct dcplx {
+    double re, im;
+};
+__device__ __forceinline__ dcplx dmul(dcplx a, dcplx b) { dcplx r; r.re = a.re * b.re - a.im * b.im; r.im = a.re * b.im + a.im * b.re; return r; }
+__device__ __forceinline__ dcplx dsub(dcplx a, dcplx b) { dcplx r; r.re = a.re - b.re; r.im = a.im - b.im; return r; }
+
+// in-place inverse of a hermitian positive-definite 4x4 (Gauss-Jordan, no pivoting: the diagonal of a
+// positive-definite matrix stays positive under elimination)
+__device__ void invert4(dcplx A[4][4]) {
+    dcplx B[4][4];
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) { B[i][j].re = (i == j) ? 1.0 : 0.0; B[i][j].im = 0.0; }
+    for (int k = 0; k < 4; ++k) {
+        const double n2 = A[k][k].re * A[k][k].re + A[k][k].im * A[k][k].im;
+        dcplx inv;
+        inv.re = A[k][k].re / n2;
+        inv.im = -A[k][k].im / n2;
+        for (int j = 0; j < 4; ++j) { A[k][j] = dmul(A[k][j], inv); B[k][j] = dmul(B[k][j], inv); }
+        for (int i = 0; i < 4; ++i) {
+            if (i == k) continue;
+            const dcplx f = A[i][k];
+            for (int j = 0; j < 4; ++j) { A[i][j] = dsub(A[i][j], dmul(f, A[k][j])); B[i][j] = dsub(B[i][j], dmul(f, B[k][j])); }
+        }
+    }
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) A[i][j] = B[i][j];
+}
+
+// hermitian 4x4 -> 16 reals (diagonal, then lower entries column-major), hermitian part taken
+template <typename T>
+__device__ void herm_to_reals(T* out, dcplx A[4][4]) {
+    for (int i = 0; i < 4; ++i) out[i] = (T)A[i][i].re;
+    int k = 4;
+    for (int j = 0; j < 4; ++j)
+        for (int i = j + 1; i < 4; ++i) {
+            out[k++] = (T)(0.5 * (A[i][j].re + A[j][i].re));
+            out[k++] = (T)(0.5 * (A[i][j].im - A[j][i].im));
+        }
+}
+
+// chirality blocks (pinned against the dense 8x8 form by tests/test_oracle_pins.py::test_O6_block_formula):
+//   A+- = (4+m0) + (csw/2) [ tau1 (x) i(+-F01 - F23) + tau2 (x) i(+-F02 + F13) + tau3 (x) i(+-F03 - F12) ],
+// tau_k on the spin index within the chirality, i F on colour; block index = spin*2 + colour.
+template <typename T>
+__global__ void clover_build_kernel(Geo g, double diag, double csw, const void* __restrict__ ufund, void* fwd, void* inv) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 2 * g.Vh) return;
+    const int par = t / g.Vh, cb = t - par * g.Vh;
+    const int row = cb / g.L3h, h = cb - row * g.L3h;
+    int x[4];
+    x[0] = row / g.s0;
+    const int rem = row - x[0] * g.s0;
+    x[1] = rem / g.s1;
+    x[2] = rem - x[1] * g.s1;
+    x[3] = 2 * h + ((x[0] + x[1] + x[2] + par) & 1);
+
+    double a01[3], a02[3], a03[3], a12[3], a13[3], a23[3];
+    clover_leaves<T>(a01, ufund, g, x, 0, 1);
+    clover_leaves<T>(a02, ufund, g, x, 0, 2);
+    clover_leaves<T>(a03, ufund, g, x, 0, 3);
+    clover_leaves<T>(a12, ufund, g, x, 1, 2);
+    clover_leaves<T>(a13, ufund, g, x, 1, 3);
+    clover_leaves<T>(a23, ufund, g, x, 2, 3);
+
+    // Pauli matrices as [k][row][col]
+    const dcplx Z = {0.0, 0.0}, P1 = {1.0, 0.0}, M1 = {-1.0, 0.0}, PI = {0.0, 1.0}, MI = {0.0, -1.0};
+    const dcplx pauli[3][2][2] = {{{Z, P1}, {P1, Z}}, {{Z, MI}, {PI, Z}}, {{P1, Z}, {Z, M1}}};
+
+    T reals_f[32], reals_i[32];
+    for (int chi = 0; chi < 2; ++chi) {
+        const double s = chi == 0 ? 1.0 : -1.0;
+        // m[k][j]: i F-combination of tau_{k+1} = sum_j m[k][j] sigma_{j+1}
+        double m[3][3];
+        for (int j = 0; j < 3; ++j) {
+            m[0][j] = -0.25 * (s * a01[j] - a23[j]);
+            m[1][j] = -0.25 * (s * a02[j] + a13[j]);
+            m[2][j] = -0.25 * (s * a03[j] - a12[j]);
+        }
+        dcplx A[4][4];
+        for (int sp = 0; sp < 2; ++sp)
+            for (int c = 0; c < 2; ++c)
+                for (int tp = 0; tp < 2; ++tp)
+                    for (int d = 0; d < 2; ++d) {
+                        dcplx acc = {(sp == tp && c == d) ? diag : 0.0, 0.0};
+                        for (int k = 0; k < 3; ++k) {
+                            dcplx X = {0.0, 0.0};
+                            for (int j = 0; j < 3; ++j) { X.re += m[k][j] * pauli[j][c][d].re; X.im += m[k][j] * pauli[j][c][d].im; }
+                            const dcplx tx = dmul(pauli[k][sp][tp], X);
+                            acc.re += 0.5 * csw * tx.re;
+                            acc.im += 0.5 * csw * tx.im;
+                        }
+                        A[sp * 2 + c][tp * 2 + d] = acc;
+                    }
+        herm_to_reals<T>(reals_f + 16 * chi, A);
+        invert4(A);
+        herm_to_reals<T>(reals_i + 16 * chi, A);
+    }
+    constexpr int CCH = 32 * sizeof(T) / 16;
+    constexpr int PER = 16 / sizeof(T);
+    typedef typename Chunk<T>::type chunk_t;
+    const size_t first = ((size_t)par * g.R + row) * (CCH * g.L3h) + h;
+    for (int c = 0; c < CCH; ++c) {
+        if (fwd) reinterpret_cast<chunk_t*>(fwd)[first + (size_t)c * g.L3h] = reals_to_chunk(reals_f + c * PER);
+        if (inv) reinterpret_cast<chunk_t*>(inv)[first + (size_t)c * g.L3h] = reals_to_chunk(reals_i + c * PER);
+    }
+}
+
+int run_clover_build(const Geo& g, int prec, double diag, double csw, const void* ufund, void* fwd, void* inv, cudaStream_t st) {
+    const unsigned nb = blocks_for(2LL * g.Vh, 128);
+    if (prec == HR_PREC_F64) clover_build_kernel<double><<<nb, 128, 0, st>>>(g, diag, csw, ufund, fwd, inv);
+    else clover_build_kernel<float><<<nb, 128, 0, st>>>(g, diag, csw, ufund, fwd, inv);
+    count_launch();
+    return check_launch("clover_build_kernel");
+}
+
+// ------------------------------------------------------------------ C2/C3: out(x) = B(x) in(x)
+template <typename T>
+__global__ void __launch_bounds__(128) clover_apply_kernel(Geo g, int parity, const void* __restrict__ blocks,
+                                                           const void* __restrict__ in, void* __restrict__ out) {
+    typedef SiteIO<T, 8> IO;
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const int p = parity == HR_BOTH ? (int)blockIdx.y : parity;
+    const size_t half_bytes = (size_t)g.Vh * IO::NCH * 16;
+    const size_t off = parity == HR_BOTH ? (size_t)p * half_bytes : 0;
+    const int row = cb / g.L3h, h = cb - row * g.L3h;
+    const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
+    T blk[32];
+    cplx<T> x[8], y[8];
+    load_clover<T>(blk, blocks, g, p, row, h);
+    IO::template load<LD_STREAM>(x, reinterpret_cast<const char*>(in) + off, first, g.L3h);
+    clover_matvec<T>(y, blk, x);
+    IO::store(reinterpret_cast<char*>(out) + off, first, g.L3h, y);
+}
+
+int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st) {
+    dim3 grid(blocks_for(g.Vh, 128), parity == HR_BOTH ? 2 : 1);
+    if (prec == HR_PREC_F64) clover_apply_kernel<double><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+    else clover_apply_kernel<float><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+    count_launch();
+    return check_launch("clover_apply_kernel");
+}
+
+}  // namespace hr

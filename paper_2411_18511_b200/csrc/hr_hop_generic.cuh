@@ -1,0 +1,138 @@
+// hr_hop_generic.cuh — the generic hopping kernel: one thread per output site, any even extents >= 2.
+// Steps H1/H2/H3 of DESIGN.md §2 (BASELINE.json north_star "Hopping kernel"; PAPER.md:31, 39
+// "inner Dirac kernel").  Used for small or oddly-shaped lattices and as the fallback of the tiled kernel.
+#pragma once
+
+#include "hr_common.cuh"
+
+namespace hr {
+
+// epilogue of a hop (H2): what is written for output site x, with h = H in(x) the bare hopping sum
+enum {
+    EPI_NONE = 0,        // out = h
+    EPI_AXPY = 1,        // out = a*phi(x) + c*h
+    EPI_CLOVER_INV = 2,  // out = B(x) h                 (B = blocks of `clover`, e.g. A_oo^-1)
+    EPI_CLOVER_AXPY = 3  // out = B(x) phi(x) + c*h      (B = A_ee)
+};
+
+struct HopArgs {
+    const void* gauge;   // gauge field in the fermion representation, device layout
+    const void* in;      // both == 0: half field of parity 1-parity; both == 1: full field
+    void* out;           // both == 0: half field of parity `parity`;  both == 1: full field
+    const void* phi;     // same shape as out (EPI_AXPY, EPI_CLOVER_AXPY)
+    const void* clover;  // full-lattice block field (EPI_CLOVER_*)
+    double a, c;
+    int parity;          // output parity when both == 0
+    int both;            // 1: gridDim.y == 2 and blockIdx.y is the output parity (full D in one launch)
+};
+
+template <typename T, int N, int EPI>
+__device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const HopArgs& a, const void* phi_half,
+                                             void* out_half, int p, int row, int h) {
+    constexpr int NC = 4 * N;
+    typedef SiteIO<T, NC> IO;
+    const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
+    if (EPI == EPI_AXPY) {
+        cplx<T> phi[NC];
+        IO::template load<LD_STREAM>(phi, phi_half, first, g.L3h);
+        const T ca = (T)a.a, cc = (T)a.c;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            acc[k].re = fma(cc, acc[k].re, ca * phi[k].re);
+            acc[k].im = fma(cc, acc[k].im, ca * phi[k].im);
+        }
+    } else if (EPI == EPI_CLOVER_INV) {
+        if (N == 2) {
+            T blk[32];
+            cplx<T> y[NC];
+            load_clover<T>(blk, a.clover, g, p, row, h);
+            clover_matvec<T>(y, blk, acc);
+#pragma unroll
+            for (int k = 0; k < NC; ++k) acc[k] = y[k];
+        }
+    } else if (EPI == EPI_CLOVER_AXPY) {
+        if (N == 2) {
+            T blk[32];
+            cplx<T> phi[NC], y[NC];
+            load_clover<T>(blk, a.clover, g, p, row, h);
+            IO::template load<LD_STREAM>(phi, phi_half, first, g.L3h);
+            clover_matvec<T>(y, blk, phi);
+            const T cc = (T)a.c;
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                acc[k].re = fma(cc, acc[k].re, y[k].re);
+                acc[k].im = fma(cc, acc[k].im, y[k].im);
+            }
+        }
+    }
+    IO::store(out_half, first, g.L3h, acc);
+}
+
+template <typename T, int N, int EPI>
+__global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
+    constexpr int NC = 4 * N;
+    typedef SiteIO<T, NC> IO;
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const int p = a.both ? (int)blockIdx.y : a.parity;
+    const size_t half_bytes = (size_t)g.Vh * IO::NCH * 16;
+    const char* in_half = reinterpret_cast<const char*>(a.in) + (a.both ? (size_t)(1 - p) * half_bytes : 0);
+    char* out_half = reinterpret_cast<char*>(a.out) + (a.both ? (size_t)p * half_bytes : 0);
+    const char* phi_half = a.phi ? reinterpret_cast<const char*>(a.phi) + (a.both ? (size_t)p * half_bytes : 0) : nullptr;
+
+    const int row = cb / g.L3h, h = cb - row * g.L3h;
+    const int x0 = row / g.s0, rem = row - x0 * g.s0;
+    const int x1 = rem / g.s1, x2 = rem - x1 * g.s1;
+    const int r = (x0 + x1 + x2 + p) & 1;  // x3 = 2h + r
+
+    // neighbour rows (periodic) and pair indices in the opposite-parity arrays
+    const int row_f0 = row + (x0 == g.L0 - 1 ? -(g.L0 - 1) * g.s0 : g.s0);
+    const int row_b0 = row + (x0 == 0 ? (g.L0 - 1) * g.s0 : -g.s0);
+    const int row_f1 = row + (x1 == g.L1 - 1 ? -(g.L1 - 1) * g.s1 : g.s1);
+    const int row_b1 = row + (x1 == 0 ? (g.L1 - 1) * g.s1 : -g.s1);
+    const int row_f2 = row + (x2 == g.L2 - 1 ? -(g.L2 - 1) : 1);
+    const int row_b2 = row + (x2 == 0 ? (g.L2 - 1) : -1);
+    const int h_f3 = r ? (h == g.L3h - 1 ? 0 : h + 1) : h;
+    const int h_b3 = r ? h : (h == 0 ? g.L3h - 1 : h - 1);
+
+    cplx<T> acc[NC];
+#pragma unroll
+    for (int k = 0; k < NC; ++k) acc[k] = mk<T>((T)0, (T)0);
+
+    const int stride = g.L3h;
+    const int rowlen = IO::NCH * g.L3h;
+#define HR_HOP_DIR(MU, ROWF, HF, ROWB, HB)                                                      \
+    {                                                                                           \
+        cplx<T> nb[NC];                                                                         \
+        Link<T, N> u;                                                                           \
+        load_link<T, LD_STREAM>(u, a.gauge, g, p, MU, row, h);                                  \
+        IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWF) * rowlen + (HF), stride);        \
+        hop_term<T, N, MU, true>(acc, nb, u);                                                   \
+        load_link<T, LD_STREAM>(u, a.gauge, g, 1 - p, MU, ROWB, HB);                            \
+        IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWB) * rowlen + (HB), stride);        \
+        hop_term<T, N, MU, false>(acc, nb, u);                                                  \
+    }
+    HR_HOP_DIR(0, row_f0, h, row_b0, h)
+    HR_HOP_DIR(1, row_f1, h, row_b1, h)
+    HR_HOP_DIR(2, row_f2, h, row_b2, h)
+    HR_HOP_DIR(3, row, h_f3, row, h_b3)
+#undef HR_HOP_DIR
+
+    hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row, h);
+}
+
+template <typename T, int N>
+inline int launch_hop_generic(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
+    dim3 block(128), grid((g.Vh + 127) / 128, a.both ? 2 : 1);
+    switch (epi) {
+        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY><<<grid, block, 0, st>>>(g, a); break;
+        default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
+    }
+    count_launch();
+    return check_launch("hop_generic_kernel");
+}
+
+}  // namespace hr

@@ -1,0 +1,219 @@
+"""Thin ctypes binding of libhr_dslash (include/hr_dslash.h): same names, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; this module converts Python objects to
+pointers and raises on a non-zero status.  PyTorch is used by callers only to allocate device memory
+and streams (`device_buffer`, `stream_ptr`).  There is no CPU fallback: if the shared library is
+missing, importing `lib()` fails loudly.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libhr_dslash.so")
+
+OK, EINVAL, EUNSUPPORTED, EALIGN, ECUDA = 0, 1, 2, 3, 4
+REP_FUND, REP_ADJ = 0, 1
+PREC_F64, PREC_F32 = 0, 1
+LINKS_FULL, LINKS_COMPRESSED = 0, 1
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
+EVEN, ODD, BOTH = 0, 1, 2
+EO_HOP_OE, EO_HOP_EO, EO_DHAT = 0, 1, 2
+OP_HOP, OP_DIRAC, OP_DHAT, OP_CLOVER, OP_DHAT_CLOVER, OP_REPRESENT = 0, 1, 2, 3, 4, 5
+
+# every symbol include/hr_dslash.h declares (tests/test_abi.py checks the header against this list)
+SYMBOLS = [
+    "hr_spinor_bytes", "hr_gauge_bytes", "hr_clover_bytes", "hr_canonical_spinor_bytes",
+    "hr_canonical_gauge_bytes", "hr_canonical_clover_bytes", "hr_pack_spinor", "hr_unpack_spinor",
+    "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
+    "hr_dirac_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_apply", "hr_dirac_flops_bytes",
+    "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
+    "hr_launch_count", "hr_kernel_name",
+]
+
+
+class hr_geom(ctypes.Structure):
+    _fields_ = [("L", ctypes.c_int * 4), ("rep", ctypes.c_int), ("prec", ctypes.c_int),
+                ("link_storage", ctypes.c_int), ("kernel", ctypes.c_int)]
+
+
+class HrError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("libhr_dslash status %d: %s" % (status, text))
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load libhr_dslash.so (built in-tree by paper_2411_18511_b200.build).  No fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("%s is missing: run `python -m paper_2411_18511_b200.build` "
+                              "(there is no CPU fallback)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        G, V, I, D, S = ctypes.POINTER(hr_geom), ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        PD = ctypes.POINTER(ctypes.c_double)
+        sig = {
+            "hr_spinor_bytes": (S, [G, I]), "hr_gauge_bytes": (S, [G, I]), "hr_clover_bytes": (S, [G]),
+            "hr_canonical_spinor_bytes": (S, [G]), "hr_canonical_gauge_bytes": (S, [G, I]),
+            "hr_canonical_clover_bytes": (S, [G]),
+            "hr_pack_spinor": (I, [G, V, V, V]), "hr_unpack_spinor": (I, [G, V, V, V]),
+            "hr_pack_gauge": (I, [G, I, V, V, V]), "hr_unpack_gauge": (I, [G, I, V, V, V]),
+            "hr_pack_clover": (I, [G, V, V, V]), "hr_unpack_clover": (I, [G, V, V, V]),
+            "hr_represent_gauge": (I, [G, V, V, V]),
+            "hr_dirac_apply": (I, [G, D, V, V, V, V]),
+            "hr_dirac_eo_apply": (I, [G, I, D, V, V, V, V, V, V, V]),
+            "hr_clover_build": (I, [G, D, D, V, V, V, V]),
+            "hr_clover_apply": (I, [G, I, V, V, V, V]),
+            "hr_dirac_flops_bytes": (I, [G, I, PD, PD, PD]),
+            "hr_host_workspace_bytes": (S, [G]),
+            "hr_dirac_apply_host": (I, [G, D, V, V, V, V, V]),
+            "hr_dirac_eo_apply_host": (I, [G, I, D, V, V, V, V, V]),
+            "hr_last_error": (S, [ctypes.c_char_p, S]),
+            "hr_launch_count": (ctypes.c_ulonglong, []),
+            "hr_kernel_name": (ctypes.c_char_p, [G]),
+        }
+        for name, (res, args) in sig.items():
+            f = getattr(L, name)
+            f.restype, f.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def geom(L, rep=REP_FUND, prec=PREC_F64, link_storage=LINKS_COMPRESSED, kernel=KERNEL_AUTO) -> hr_geom:
+    g = hr_geom()
+    for i in range(4):
+        g.L[i] = int(L[i])
+    g.rep, g.prec, g.link_storage, g.kernel = int(rep), int(prec), int(link_storage), int(kernel)
+    return g
+
+
+def _ptr(x):
+    """torch tensor / numpy array / int / None -> integer address (or None)"""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError("cannot take the address of %r" % type(x))
+
+
+def stream_ptr(stream=None):
+    """cudaStream_t of a torch.cuda.Stream (None: torch's current stream)."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def last_error() -> str:
+    buf = ctypes.create_string_buffer(512)
+    lib().hr_last_error(buf, 512)
+    return buf.value.decode()
+
+
+def _check(status):
+    if status != OK:
+        raise HrError(status, last_error())
+
+
+# ------------------------------------------------------------------ sizes
+def hr_spinor_bytes(g, parity=BOTH): return lib().hr_spinor_bytes(ctypes.byref(g), parity)
+def hr_gauge_bytes(g, rep): return lib().hr_gauge_bytes(ctypes.byref(g), rep)
+def hr_clover_bytes(g): return lib().hr_clover_bytes(ctypes.byref(g))
+def hr_canonical_spinor_bytes(g): return lib().hr_canonical_spinor_bytes(ctypes.byref(g))
+def hr_canonical_gauge_bytes(g, rep): return lib().hr_canonical_gauge_bytes(ctypes.byref(g), rep)
+def hr_canonical_clover_bytes(g): return lib().hr_canonical_clover_bytes(ctypes.byref(g))
+def hr_host_workspace_bytes(g): return lib().hr_host_workspace_bytes(ctypes.byref(g))
+
+
+# ------------------------------------------------------------------ layout
+def hr_pack_spinor(g, canon, dev, stream=0): _check(lib().hr_pack_spinor(ctypes.byref(g), _ptr(canon), _ptr(dev), stream))
+def hr_unpack_spinor(g, dev, canon, stream=0): _check(lib().hr_unpack_spinor(ctypes.byref(g), _ptr(dev), _ptr(canon), stream))
+def hr_pack_gauge(g, rep, canon, dev, stream=0): _check(lib().hr_pack_gauge(ctypes.byref(g), rep, _ptr(canon), _ptr(dev), stream))
+def hr_unpack_gauge(g, rep, dev, canon, stream=0): _check(lib().hr_unpack_gauge(ctypes.byref(g), rep, _ptr(dev), _ptr(canon), stream))
+def hr_pack_clover(g, canon, dev, stream=0): _check(lib().hr_pack_clover(ctypes.byref(g), _ptr(canon), _ptr(dev), stream))
+def hr_unpack_clover(g, dev, canon, stream=0): _check(lib().hr_unpack_clover(ctypes.byref(g), _ptr(dev), _ptr(canon), stream))
+
+
+# ------------------------------------------------------------------ operators
+def hr_represent_gauge(g, u_fund, u_adj, stream=0):
+    _check(lib().hr_represent_gauge(ctypes.byref(g), _ptr(u_fund), _ptr(u_adj), stream))
+
+
+def hr_dirac_apply(g, m0, u, psi, out, stream=0):
+    _check(lib().hr_dirac_apply(ctypes.byref(g), float(m0), _ptr(u), _ptr(psi), _ptr(out), stream))
+
+
+def hr_dirac_eo_apply(g, op, m0, u, clover_fwd, clover_inv, inp, out, tmp, stream=0):
+    _check(lib().hr_dirac_eo_apply(ctypes.byref(g), int(op), float(m0), _ptr(u), _ptr(clover_fwd), _ptr(clover_inv),
+                                   _ptr(inp), _ptr(out), _ptr(tmp), stream))
+
+
+def hr_clover_build(g, m0, csw, u_fund, clover_fwd, clover_inv, stream=0):
+    _check(lib().hr_clover_build(ctypes.byref(g), float(m0), float(csw), _ptr(u_fund), _ptr(clover_fwd), _ptr(clover_inv), stream))
+
+
+def hr_clover_apply(g, parity, blocks, inp, out, stream=0):
+    _check(lib().hr_clover_apply(ctypes.byref(g), int(parity), _ptr(blocks), _ptr(inp), _ptr(out), stream))
+
+
+def hr_dirac_flops_bytes(g, op):
+    """-> (flops per output site, compulsory bytes per site, requested bytes per site)"""
+    f, bc, br = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(lib().hr_dirac_flops_bytes(ctypes.byref(g), int(op), ctypes.byref(f), ctypes.byref(bc), ctypes.byref(br)))
+    return f.value, bc.value, br.value
+
+
+def hr_dirac_apply_host(g, m0, u_canon_host, psi_canon_host, out_canon_host, workspace, stream=0):
+    _check(lib().hr_dirac_apply_host(ctypes.byref(g), float(m0), _ptr(u_canon_host), _ptr(psi_canon_host),
+                                     _ptr(out_canon_host), _ptr(workspace), stream))
+
+
+def hr_dirac_eo_apply_host(g, op, m0, u_canon_host, in_canon_host, out_canon_host, workspace, stream=0):
+    _check(lib().hr_dirac_eo_apply_host(ctypes.byref(g), int(op), float(m0), _ptr(u_canon_host), _ptr(in_canon_host),
+                                        _ptr(out_canon_host), _ptr(workspace), stream))
+
+
+def hr_launch_count() -> int: return int(lib().hr_launch_count())
+def hr_kernel_name(g) -> str: return lib().hr_kernel_name(ctypes.byref(g)).decode()
+
+
+# ------------------------------------------------------------------ plumbing: device memory via torch
+def device_buffer(nbytes: int, device="cuda:0"):
+    """A torch uint8 buffer of nbytes on the device (256-byte aligned by the caching allocator)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("libhr_dslash needs a CUDA device; there is no CPU fallback")
+    return torch.empty(int(nbytes), dtype=torch.uint8, device=device)
+
+
+def np_real(g):
+    import numpy as np
+    return np.float64 if g.prec == PREC_F64 else np.float32
+
+
+def np_complex(g):
+    import numpy as np
+    return np.complex128 if g.prec == PREC_F64 else np.complex64
+
+
+def upload(array, device="cuda:0"):
+    """numpy array -> device uint8 buffer holding the same bytes"""
+    import numpy as np
+    import torch
+    a = np.ascontiguousarray(array)
+    return torch.from_numpy(a.view(np.uint8).reshape(-1)).to(device)
+
+
+def download(buf, dtype, shape):
+    """device uint8 buffer -> numpy array of dtype/shape"""
+    import numpy as np
+    return buf.cpu().numpy().view(dtype).reshape(shape)

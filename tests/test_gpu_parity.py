@@ -1,0 +1,410 @@
+"""GPU parity: libhr_dslash (through the C-ABI) against the CPU oracle on the same seeded inputs.
+
+BASELINE.json `north_star` bar: relative L2 error over the compared outputs <= 1e-13 (fp64), <= 1e-5 (fp32);
+for fp32 both sides see the inputs rounded to float.  The five BASELINE.json configs are
+covered at full size; edge cases (extent 2, ragged extents, both kernels) at sizes the oracle does in
+seconds.  Expected values always come from oracle/ or from identities — never from the CUDA path."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2411_18511_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {0: 1e-13, 1: 1e-5}   # hr.PREC_F64, hr.PREC_F32
+NTHREADS = max(1, len(os.sched_getaffinity(0)))
+
+
+@pytest.fixture(scope="module")
+def hr():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2411_18511_b200 import build, hr as _hr
+    build.build()
+    _hr.lib()
+    return _hr
+
+
+def lattice(hr, L, rep=0, prec=0, kernel=0):
+    from paper_2411_18511_b200.lattice import Lattice
+    return Lattice(L, rep, prec, kernel)
+
+
+def rel(a, b):
+    return float(np.linalg.norm((a.astype(np.complex128) - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+def rounded(a, prec):
+    return inputs.to_f32_rounded(a) if prec == 1 else a
+
+
+def kernels_for(hr, L, rep, prec):
+    """kernel selectors to test on this lattice: generic always, tiled where the lattice fits it"""
+    ks = [hr.KERNEL_GENERIC]
+    if hr.hr_kernel_name(hr.geom(L, rep, prec, hr.LINKS_COMPRESSED, hr.KERNEL_TILED)) == "tiled":
+        ks.append(hr.KERNEL_TILED)
+    return ks
+
+
+def dense_to_blocks(A):
+    """oracle dense [n,8,8] -> canonical blocks [n,2,16]: 4 real diagonal entries, then the strictly-lower
+    entries (1,0) (2,0) (3,0) (2,1) (3,1) (3,2) as re,im (include/hr_dslash.h)."""
+    out = np.empty((A.shape[0], 2, 16))
+    for chi in range(2):
+        B = A[:, 4 * chi:4 * chi + 4, 4 * chi:4 * chi + 4]
+        for i in range(4):
+            out[:, chi, i] = B[:, i, i].real
+        k = 4
+        for j in range(4):
+            for i in range(j + 1, 4):
+                out[:, chi, k] = B[:, i, j].real
+                out[:, chi, k + 1] = B[:, i, j].imag
+                k += 2
+    return out
+
+
+def gpu_ops(hr, lat, U_dev, psi, m0):
+    """run hop_oe, hop_eo, full D and Dhat on the GPU; return canonical arrays (untouched parity = 0)"""
+    import torch
+    psi_dev = lat.put_spinor(psi)
+    res = {}
+    out = torch.zeros_like(psi_dev)
+    lat.hop(hr.EO_HOP_OE, U_dev, lat.even(psi_dev), lat.odd(out))
+    lat.hop(hr.EO_HOP_EO, U_dev, lat.odd(psi_dev), lat.even(out))
+    res["hop"] = lat.get_spinor(out)
+    res["dirac"] = lat.get_spinor(lat.dirac(m0, U_dev, psi_dev))
+    out2 = torch.zeros_like(psi_dev)
+    lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out2))
+    res["dhat"] = lat.get_spinor(out2)
+    torch.cuda.synchronize()
+    return res
+
+
+def oracle_ops(orc, L, rep, U, psi, m0):
+    res = {}
+    h = orc.hop(L, rep, 0, U, psi, nthreads=NTHREADS)
+    res["hop"] = orc.hop(L, rep, 1, U, psi, nthreads=NTHREADS, out=h)
+    res["dirac"] = orc.dirac(L, rep, m0, U, psi, nthreads=NTHREADS)
+    res["dhat"] = orc.dirac_eo(L, rep, m0, U, psi, nthreads=NTHREADS)
+    return res
+
+
+# ------------------------------------------------------------------ layout permutations
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 4, 6, 8), (2, 2, 2, 2), (6, 4, 2, 10)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_pack_unpack_roundtrip_is_exact(hr, L, prec):
+    U = rounded(inputs.haar_gauge(L, 1), prec)
+    for rep, N in ((0, 2), (1, 3)):
+        lat = lattice(hr, L, rep, prec)
+        psi = rounded(inputs.gaussian_spinor(L, N, 2), prec)
+        assert np.array_equal(lat.get_spinor(lat.put_spinor(psi)).astype(np.complex128), psi)
+    lat = lattice(hr, L, 0, prec)
+    assert np.array_equal(lat.get_gauge_fund(lat.put_gauge_fund(U)).astype(np.complex128), U)
+    R = rounded(inputs.normals(7, 9, 0, lat.V * 36).reshape(lat.V, 4, 3, 3), prec)
+    assert np.array_equal(lat.get_gauge_adj(lat.put_gauge_adj(R)).astype(np.float64), R)
+    B = rounded(inputs.normals(8, 9, 0, lat.V * 32).reshape(lat.V, 2, 16), prec)
+    assert np.array_equal(lat.get_clover(lat.put_clover(B)).astype(np.float64), B)
+
+
+def test_device_layout_is_the_documented_one(hr):
+    """chunk c of site (row,h) of parity p sits at 16-byte index p*Vh*NCH + (row*NCH + c)*L3h + h."""
+    L = (2, 4, 6, 8)
+    lat = lattice(hr, L, 0, 0)
+    psi = inputs.gaussian_spinor(L, 2, 2)
+    raw = lat.put_spinor(psi).cpu().numpy().view(np.complex128)
+    x = inputs.site_coords(L)
+    par = x.sum(1) % 2
+    row = (x[:, 0] * L[1] + x[:, 1]) * L[2] + x[:, 2]
+    h = x[:, 3] // 2
+    L3h, Vh = L[3] // 2, lat.V // 2
+    for c in (0, 3, 7):
+        idx = par * Vh * 8 + (row * 8 + c) * L3h + h
+        assert np.array_equal(raw[idx], psi.reshape(lat.V, 8)[:, c])
+
+
+# ------------------------------------------------------------------ config 0 and the edge lattices
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (4, 4, 4, 2), (6, 2, 4, 12), (8, 4, 4, 16), (4, 8, 8, 8)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_fundamental_small_lattices(hr, orc, L, prec):
+    """configs[0] (4^4, Haar links, m0 = -0.2: full D and even-odd operator) plus degenerate and ragged extents"""
+    m0 = -0.2
+    U = rounded(inputs.haar_gauge(L, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 2, 2), prec)
+    want = oracle_ops(orc, L, 0, U, psi, m0)
+    for kernel in kernels_for(hr, L, 0, prec):
+        lat = lattice(hr, L, 0, prec, kernel)
+        got = gpu_ops(hr, lat, lat.put_gauge_fund(U), psi, m0)
+        for k in want:
+            assert rel(got[k], want[k]) <= TOL[prec], (k, kernel)
+        odd = inputs.site_parity(L) == 1
+        assert not got["dhat"][odd].any()
+
+
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (4, 6, 4, 2)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_adjoint_small_lattices(hr, orc, L, prec):
+    m0 = -0.3
+    Uf = rounded(inputs.haar_gauge(L, 1), prec)
+    R, _ = orc.represent(Uf)
+    psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
+    lat = lattice(hr, L, 1, prec)
+    R_dev = lat.represent(lat.put_gauge_fund(Uf))
+    got_R = lat.get_gauge_adj(R_dev).astype(np.float64)
+    assert np.abs(got_R - R).max() <= (1e-14 if prec == 0 else 1e-6)
+    # the adjoint operator is compared on the links the oracle built (rounded for fp32), packed directly
+    Rr = rounded(R, prec)
+    want = oracle_ops(orc, L, 1, Rr, psi, m0)
+    got = gpu_ops(hr, lat, lat.put_gauge_adj(Rr), psi, m0)
+    for k in want:
+        assert rel(got[k], want[k]) <= TOL[prec], k
+    if prec == 0:   # and end to end on the links the GPU built
+        got2 = gpu_ops(hr, lat, R_dev, psi, m0)
+        for k in want:
+            assert rel(got2[k], want[k]) <= TOL[prec], k
+
+
+# ------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("prec", [0, 1])
+def test_config1_16to4_dhat_100_repetitions(hr, orc, prec):
+    """configs[1]: 16^4, links exp(i 0.3 a.sigma), m0 = -0.1, Dhat on the even spinor, 100 repetitions of the
+    same application; every repetition must give the same bits."""
+    import torch
+    L, m0 = (16, 16, 16, 16), -0.1
+    U = rounded(inputs.weak_gauge(L, 0.3, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 2, 2), prec)
+    want = orc.dirac_eo(L, 0, m0, U, psi, nthreads=NTHREADS)
+    for kernel in kernels_for(hr, L, 0, prec):
+        lat = lattice(hr, L, 0, prec, kernel)
+        U_dev, psi_dev = lat.put_gauge_fund(U), lat.put_spinor(psi)
+        first = torch.zeros_like(psi_dev)
+        last = torch.zeros_like(psi_dev)
+        tmp = lat.empty_spinor(hr.ODD)
+        lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(first), tmp)
+        for _ in range(99):
+            lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(last), tmp)
+        torch.cuda.synchronize()
+        assert torch.equal(first, last)
+        assert rel(lat.get_spinor(last), want) <= TOL[prec], kernel
+
+
+# ------------------------------------------------------------------ config 2
+def test_config2_24to4_adjoint(hr, orc):
+    """configs[2]: 24^4 adjoint fp64, links built from Haar fundamental links by hr_represent_gauge, m0 = -0.3"""
+    L, m0 = (24, 24, 24, 24), -0.3
+    Uf = inputs.haar_gauge(L, 1)
+    psi = inputs.gaussian_spinor(L, 3, 2)
+    R, max_imag = orc.represent(Uf)
+    assert max_imag < 1e-15
+    lat = lattice(hr, L, 1, 0)
+    R_dev = lat.represent(lat.put_gauge_fund(Uf))
+    got_R = lat.get_gauge_adj(R_dev)
+    assert np.abs(got_R - R).max() <= 1e-14
+    # P6 on the GPU's own output: real orthogonal with det +1
+    RRt = np.einsum("xmab,xmcb->xmac", got_R, got_R)
+    assert np.abs(RRt - np.eye(3)).max() < 1e-14
+    assert np.abs(np.linalg.det(got_R) - 1.0).max() < 1e-14
+    want = oracle_ops(orc, L, 1, R, psi, m0)
+    got = gpu_ops(hr, lat, R_dev, psi, m0)
+    for k in want:
+        assert rel(got[k], want[k]) <= 1e-13, k
+
+
+# ------------------------------------------------------------------ config 3
+@pytest.fixture(scope="module")
+def big_inputs():
+    L = (48, 48, 48, 48)
+    return L, inputs.haar_gauge(L, 1), inputs.gaussian_spinor(L, 2, 2)
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+def test_config3_48to4_fundamental(hr, orc, big_inputs, prec):
+    """configs[3]: 48^4, Haar links, m0 = -0.2: bare hops, full D and Dhat against the oracle on the whole
+    field, in the launch configuration bench.py times (kernel = AUTO), plus the forced generic kernel."""
+    L, U, psi = big_inputs
+    m0 = -0.2
+    U, psi = rounded(U, prec), rounded(psi, prec)
+    want = oracle_ops(orc, L, 0, U, psi, m0)
+    kernels = [hr.KERNEL_AUTO]
+    if hr.hr_kernel_name(hr.geom(L, 0, prec)) != "generic":
+        kernels.append(hr.KERNEL_GENERIC)
+    for kernel in kernels:
+        lat = lattice(hr, L, 0, prec, kernel)
+        got = gpu_ops(hr, lat, lat.put_gauge_fund(U), psi, m0)
+        for k in want:
+            assert rel(got[k], want[k]) <= TOL[prec], (k, kernel)
+
+
+def test_config3_invariants_on_the_gpu(hr, big_inputs):
+    """P2 (gamma5-hermiticity) and P4 (Schur identity) hold at any size and need no oracle run: evaluated at 48^4
+    on GPU outputs, in fp64."""
+    import torch
+    L, U, psi = big_inputs
+    m0 = -0.2
+    lat = lattice(hr, L, 0, 0)
+    U_dev = lat.put_gauge_fund(U)
+    chi = inputs.gaussian_spinor(L, 2, 3, inputs.FIELD_SPINOR2)
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+    Dpsi = lat.get_spinor(lat.dirac(m0, U_dev, lat.put_spinor(psi)))
+    Dg5chi = lat.get_spinor(lat.dirac(m0, U_dev, lat.put_spinor(g5 * chi)))
+    lhs = np.vdot(chi.ravel(), Dpsi.ravel())
+    rhs = np.vdot((g5 * Dg5chi).ravel(), psi.ravel())
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+    # P4: eta = D x  =>  Dhat x_e = eta_e - D_eo D_oo^-1 eta_o = eta_e + H_eo eta_o / (2 (4+m0))
+    eta = Dpsi
+    eta_dev = lat.put_spinor(eta)
+    psi_dev = lat.put_spinor(psi)
+    dh = torch.zeros_like(psi_dev)
+    lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(dh))
+    hop = torch.zeros_like(psi_dev)
+    lat.hop(hr.EO_HOP_EO, U_dev, lat.odd(eta_dev), lat.even(hop))
+    even = inputs.site_parity(L) == 0
+    lhs = lat.get_spinor(dh)[even]
+    rhs = eta[even] + lat.get_spinor(hop)[even] / (2.0 * (4.0 + m0))
+    assert rel(lhs, rhs) <= 1e-13
+
+
+# ------------------------------------------------------------------ clover (config 4)
+def clover_oracle(orc, L, U, m0, csw):
+    A = orc.clover_dense(L, 4.0 + m0, csw, U, nthreads=NTHREADS)
+    return A, orc.invert(A)
+
+
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 4, 6, 8), (8, 8, 8, 8), (2, 2, 2, 2)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_clover_small_lattices(hr, orc, L, prec):
+    """C1 blocks and inverses, C2/C3 application, E2 (Dhat with clover) against the oracle's dense 8x8 route"""
+    import torch
+    m0, csw = -0.25, 1.2
+    U = rounded(inputs.weak_gauge(L, 0.3, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 2, 2), prec)
+    A, Ainv = clover_oracle(orc, L, U, m0, csw)
+    for kernel in kernels_for(hr, L, 0, prec):
+        lat = lattice(hr, L, 0, prec, kernel)
+        U_dev, psi_dev = lat.put_gauge_fund(U), lat.put_spinor(psi)
+        fwd, inv = lat.clover_build(m0, csw, U_dev)
+        tol_blk = 1e-13 if prec == 0 else 1e-6
+        bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+        assert np.linalg.norm(lat.get_clover(fwd) - bf) <= tol_blk * np.linalg.norm(bf)
+        assert np.linalg.norm(lat.get_clover(inv) - bi) <= tol_blk * np.linalg.norm(bi)
+        # C2 / C3 on both parities at once and on one parity
+        got = lat.get_spinor(lat.clover_apply(hr.BOTH, fwd, psi_dev))
+        assert rel(got, orc.site_matvec(L, 3, A, psi)) <= TOL[prec]
+        got = lat.get_spinor(lat.clover_apply(hr.BOTH, inv, psi_dev))
+        assert rel(got, orc.site_matvec(L, 3, Ainv, psi)) <= TOL[prec]
+        half = torch.zeros_like(psi_dev)
+        lat.clover_apply(hr.ODD, inv, lat.odd(psi_dev), lat.odd(half))
+        assert rel(lat.get_spinor(half), orc.site_matvec(L, 2, Ainv, psi)) <= TOL[prec]
+        # E2 with the GPU's own blocks
+        out = torch.zeros_like(psi_dev)
+        lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
+        want = orc.dirac_eo_clover(L, U, A, Ainv, psi, nthreads=NTHREADS)
+        assert rel(lat.get_spinor(out), want) <= TOL[prec], kernel
+        # ... and with the oracle's blocks packed in (a pure mat-vec + hop check)
+        if prec == 0:
+            out2 = torch.zeros_like(psi_dev)
+            lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out2), clover_fwd=lat.put_clover(bf), clover_inv=lat.put_clover(bi))
+            assert rel(lat.get_spinor(out2), want) <= TOL[prec]
+
+
+def test_config4_48to4_clover(hr, orc):
+    """configs[4]: 48^4 fp64, links exp(i 0.3 a.sigma), c_sw = 1.2, m0 = -0.25.  Blocks, C2/C3 and E2 are
+    compared with the oracle on sampled sites (the dense 8x8 oracle field would need 11 GB at this size);
+    the Schur identity with clover (P4) checks E2 on every even site."""
+    import torch
+    L, m0, csw = (48, 48, 48, 48), -0.25, 1.2
+    V = inputs.volume(L)
+    U = inputs.weak_gauge(L, 0.3, 1)
+    psi = inputs.gaussian_spinor(L, 2, 2)
+    lat = lattice(hr, L, 0, 0)
+    U_dev, psi_dev = lat.put_gauge_fund(U), lat.put_spinor(psi)
+    fwd, inv = lat.clover_build(m0, csw, U_dev)
+    got_f, got_i = lat.get_clover(fwd), lat.get_clover(inv)
+    got_Apsi = lat.get_spinor(lat.clover_apply(hr.BOTH, fwd, psi_dev))
+    got_Aipsi = lat.get_spinor(lat.clover_apply(hr.BOTH, inv, psi_dev))
+    # sampled ranges: lattice corners (wrap-around in every direction), the middle, a ragged interior stretch
+    for b, e in [(0, 96), (V - 96, V), (V // 2 - 48, V // 2 + 48), (1234567, 1234567 + 101), (47 * 48 ** 3, 47 * 48 ** 3 + 64)]:
+        A = orc.clover_dense(L, 4.0 + m0, csw, U, begin=b, end=e)[b:e]
+        Ainv = orc.invert(A)
+        bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+        assert np.linalg.norm(got_f[b:e] - bf) <= 1e-13 * np.linalg.norm(bf)
+        assert np.linalg.norm(got_i[b:e] - bi) <= 1e-13 * np.linalg.norm(bi)
+        want = np.einsum("xij,xj->xi", A, psi[b:e].reshape(-1, 8)).reshape(-1, 4, 2)
+        assert rel(got_Apsi[b:e], want) <= 1e-13
+        want = np.einsum("xij,xj->xi", Ainv, psi[b:e].reshape(-1, 8)).reshape(-1, 4, 2)
+        assert rel(got_Aipsi[b:e], want) <= 1e-13
+    # E2 on sampled even sites, step by step with oracle calls: the 8 neighbours y of x, t(y) = A(y)^-1 (H psi)(y),
+    # then one more hop at x of the field that is t on those neighbours
+    out = torch.zeros_like(psi_dev)
+    lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
+    got = lat.get_spinor(out)
+    coords = inputs.site_coords(L)
+    rng = np.random.default_rng(5)
+    cand = np.concatenate([[0, V - 2, 47 * 48 ** 3 + 47 * 48 ** 2], rng.integers(0, V, 40)])
+    sites = [int(s) for s in cand if coords[s].sum() % 2 == 0][:24]
+    scratch = np.zeros_like(psi)
+    Lv = np.array(L)
+    strides = np.array([L[1] * L[2] * L[3], L[2] * L[3], L[3], 1])
+    want, have = [], []
+    for x in sites:
+        nb = []
+        for mu in range(4):
+            for d in (+1, -1):
+                y = coords[x].copy()
+                y[mu] = (y[mu] + d) % Lv[mu]
+                nb.append(int(y @ strides))
+        nb = np.array(sorted(set(nb)), dtype=np.int64)
+        t1 = orc.hop_sites(L, 0, U, psi, nb).reshape(-1, 8)
+        for k, y in enumerate(nb):
+            Ay = orc.clover_dense(L, 4.0 + m0, csw, U, begin=y, end=y + 1)[y]
+            scratch[y] = (orc.invert(Ay[None])[0] @ t1[k]).reshape(4, 2)
+        h = orc.hop_sites(L, 0, U, scratch, np.array([x]))[0]
+        scratch[nb] = 0.0
+        Ax = orc.clover_dense(L, 4.0 + m0, csw, U, begin=x, end=x + 1)[x]
+        want.append((Ax @ psi[x].reshape(8)).reshape(4, 2) - 0.25 * h)
+        have.append(got[x])
+    assert rel(np.array(have), np.array(want)) <= 1e-13
+    # P4 with clover on all even sites: eta = D_sw x = D x + (A - (4+m0)) x;
+    #   Dhat x_e = eta_e - D_eo D_oo^-1 eta_o = eta_e + 1/2 H_eo A_oo^-1 eta_o
+    Dx = lat.get_spinor(lat.dirac(m0, U_dev, psi_dev))
+    eta = Dx + got_Apsi - (4.0 + m0) * psi
+    eta_dev = lat.put_spinor(eta)
+    t = torch.zeros_like(psi_dev)
+    lat.clover_apply(hr.ODD, inv, lat.odd(eta_dev), lat.odd(t))
+    hop = torch.zeros_like(psi_dev)
+    lat.hop(hr.EO_HOP_EO, U_dev, lat.odd(t), lat.even(hop))
+    even = inputs.site_parity(L) == 0
+    assert rel(got[even], eta[even] + 0.5 * lat.get_spinor(hop)[even]) <= 1e-13
+
+
+# ------------------------------------------------------------------ host-buffer path
+@pytest.mark.parametrize("prec", [0, 1])
+def test_host_entry_points(hr, orc, prec):
+    import torch
+    L, m0 = (4, 6, 8, 8), -0.2
+    U = rounded(inputs.haar_gauge(L, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 2, 2), prec)
+    lat = lattice(hr, L, 0, prec)
+    ws = hr.device_buffer(hr.hr_host_workspace_bytes(lat.g))
+    Uh = torch.from_numpy(U.astype(lat.cplx)).pin_memory()
+    ph = torch.from_numpy(psi.astype(lat.cplx)).pin_memory()
+    oh = torch.empty_like(ph).pin_memory()
+    hr.hr_dirac_apply_host(lat.g, m0, Uh, ph, oh, ws, hr.stream_ptr())
+    assert rel(oh.numpy(), orc.dirac(L, 0, m0, U, psi)) <= TOL[prec]
+    hr.hr_dirac_eo_apply_host(lat.g, hr.EO_DHAT, m0, Uh, ph, oh, ws, hr.stream_ptr())
+    assert rel(oh.numpy(), orc.dirac_eo(L, 0, m0, U, psi)) <= TOL[prec]
+    hr.hr_dirac_eo_apply_host(lat.g, hr.EO_HOP_OE, m0, Uh, ph, oh, ws, hr.stream_ptr())
+    assert rel(oh.numpy(), orc.hop(L, 0, 1, U, psi)) <= TOL[prec]
+
+
+def test_native_library_is_the_one_loaded(hr):
+    """the product path is the in-tree shared object, and it counts its own launches"""
+    import torch
+    n0 = hr.hr_launch_count()
+    lat = lattice(hr, (4, 4, 4, 4))
+    lat.put_spinor(inputs.gaussian_spinor((4, 4, 4, 4), 2, 2))
+    torch.cuda.synchronize()
+    assert hr.hr_launch_count() == n0 + 1
+    with open("/proc/self/maps") as f:
+        assert "paper_2411_18511_b200/libhr_dslash.so" in f.read()
