@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py — whole-hot-path benchmark of libhr_dslash on BASELINE.json configs[3]/[4] (48^4).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--L 48]
+
+One "step" = one pass of every hot-path row of DESIGN.md §2 over one 48^4 lattice of synthetic seeded
+fields (Haar links, Gaussian spinors; clover links exp(i 0.3 a.sigma)), inputs resident in HBM:
+    fp64: H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat, C2 clover, C3 clover inverse, E2 Dhat+clover, R1 represent
+    fp32: H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat
+`value` = compulsory (algorithmic) bytes of the step (hr_dirac_flops_bytes) / step time, in GB/s — the paper's
+bandwidth metric.  Prints ONE JSON line (rank 0).  See DESIGN.md §7 for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "dslash_hbm_bandwidth_48^4"
+UNIT = "GB/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--L", type=int, default=48, help="lattice extent (48 = BASELINE.json configs[3]; others for debugging)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    """roofline denominator: measured copy bandwidth of this pool's B200s (MEASURED_PEAKS.json), else the
+    profiling guide's fallback 6650 GB/s"""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons through NVML (what nvidia-smi reads) while the timed region runs"""
+
+    def __init__(self, device_index, period=0.02):
+        super().__init__(daemon=True)
+        self.period = period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self.stop_flag = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            h = None
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                if not uuid.startswith("GPU-"):
+                    uuid = "GPU-" + uuid
+                h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if hasattr(uuid, "encode") else uuid)
+            except Exception:
+                h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+            self.h = h
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self.stop_flag.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def finish(self):
+        self.stop_flag.set()
+        if self.is_alive():
+            self.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_2411_18511_b200 import build, hr, inputs
+    from paper_2411_18511_b200.dist import Ranks, whole_job_throughput
+    from paper_2411_18511_b200.lattice import Lattice
+
+    ranks = Ranks()
+    assert ranks.world == args.gpus or ranks.world == 1, "launch N ranks with torchrun for --gpus N"
+    dev_index = ranks.local_rank
+    torch.cuda.set_device(dev_index)
+    device = "cuda:%d" % dev_index
+    build.build()
+    hr.lib()
+
+    L = (args.L,) * 4
+    V = args.L ** 4
+    Vh = V // 2
+    kernel = {"auto": hr.KERNEL_AUTO, "generic": hr.KERNEL_GENERIC, "tiled": hr.KERNEL_TILED}[args.kernel]
+    m0, m0c, csw = -0.2, -0.25, 1.2
+
+    # ---- seeded synthetic inputs: configs[3] Haar links; configs[4] links exp(i 0.3 a.sigma)
+    U = inputs.haar_gauge(L, 1)
+    Uw = inputs.weak_gauge(L, 0.3, 1)
+    psi = inputs.gaussian_spinor(L, 2, 2)
+
+    S = {}
+    for prec, tag in ((hr.PREC_F64, "f64"), (hr.PREC_F32, "f32")):
+        lat = Lattice(L, hr.REP_FUND, prec, kernel, device)
+        s = {"lat": lat, "U": lat.put_gauge_fund(U), "psi": lat.put_spinor(psi), "out": lat.empty_spinor(),
+             "tmp": lat.empty_spinor(hr.ODD)}
+        S[tag] = s
+    lat64 = S["f64"]["lat"]
+    S["f64"]["Uw"] = lat64.put_gauge_fund(Uw)
+    S["f64"]["fwd"], S["f64"]["inv"] = lat64.clover_build(m0c, csw, S["f64"]["Uw"])
+    S["f64"]["Uadj"] = lat64.empty_gauge(hr.REP_ADJ)
+    torch.cuda.synchronize()
+    del U, Uw
+    st = hr.stream_ptr()
+
+    # ---- the step: (name, precision, model op, output sites, callable)
+    def mk(tag):
+        s = S[tag]
+        lat, g = s["lat"], s["lat"].g
+        ev, od = lat.even, lat.odd
+        ops = [
+            ("hop_oe_" + tag, g, hr.OP_HOP, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_OE, 0.0, s["U"], None, None, ev(s["psi"]), od(s["out"]), None, st)),
+            ("hop_eo_" + tag, g, hr.OP_HOP, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_EO, 0.0, s["U"], None, None, od(s["psi"]), ev(s["out"]), None, st)),
+            ("dirac_" + tag, g, hr.OP_DIRAC, V, lambda: hr.hr_dirac_apply(g, m0, s["U"], s["psi"], s["out"], st)),
+            ("dhat_" + tag, g, hr.OP_DHAT, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, m0, s["U"], None, None, ev(s["psi"]), ev(s["out"]), s["tmp"], st)),
+        ]
+        if tag == "f64":
+            ops += [
+                ("clover_" + tag, g, hr.OP_CLOVER, V, lambda: hr.hr_clover_apply(g, hr.BOTH, s["fwd"], s["psi"], s["out"], st)),
+                ("clover_inv_" + tag, g, hr.OP_CLOVER, V, lambda: hr.hr_clover_apply(g, hr.BOTH, s["inv"], s["psi"], s["out"], st)),
+                ("dhat_clover_" + tag, g, hr.OP_DHAT_CLOVER, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, m0c, s["Uw"], s["fwd"], s["inv"], ev(s["psi"]), ev(s["out"]), s["tmp"], st)),
+                ("represent_" + tag, g, hr.OP_REPRESENT, V, lambda: hr.hr_represent_gauge(g, s["U"], s["Uadj"], st)),
+            ]
+        return ops
+
+    ops = mk("f64") + mk("f32")
+    model = {}
+    for name, g, op, sites, _ in ops:
+        f, bc, br = hr.hr_dirac_flops_bytes(g, op)
+        model[name] = {"sites": sites, "flops": f * sites, "bytes": bc * sites, "bytes_requested": br * sites}
+    step_bytes = sum(m["bytes"] for m in model.values())
+    step_flops = sum(m["flops"] for m in model.values())
+    step_sites = sum(m["sites"] for m in model.values())
+
+    def step(events=None):
+        for i, (name, g, op, sites, fn) in enumerate(ops):
+            if events is not None:
+                events[i][0].record()
+            fn()
+            if events is not None:
+                events[i][1].record()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+
+    K = args.steps
+    per_op_events = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in ops] for _ in range(K)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(dev_index)
+    launches0 = hr.hr_launch_count()
+    ranks.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    e0.record()
+    for k in range(K):
+        step(per_op_events[k])
+    e1.record()
+    torch.cuda.synchronize()
+    ranks.barrier()
+    clocks = sampler.finish()
+    launches = hr.hr_launch_count() - launches0
+    seconds = e0.elapsed_time(e1) * 1e-3
+    value, tmax = whole_job_throughput(ranks, step_bytes * K / 1e9, seconds)
+    ms_per_step = tmax * 1e3 / K
+
+    op_report = {}
+    for i, (name, g, op, sites, _) in enumerate(ops):
+        ms = sum(per_op_events[k][i][0].elapsed_time(per_op_events[k][i][1]) for k in range(K)) / K
+        m = model[name]
+        op_report[name] = {
+            "ms": round(ms, 4), "gbs": round(m["bytes"] / ms / 1e6, 1), "gbs_requested": round(m["bytes_requested"] / ms / 1e6, 1),
+            "gflops": round(m["flops"] / ms / 1e6, 1), "gsites_per_s": round(m["sites"] / ms / 1e6, 3),
+            "kernel": hr.hr_kernel_name(g) if "clover_" not in name[:7] and "represent" not in name else "site-diagonal",
+        }
+
+    # ---- roofline of the dominant kernel: the fp64 parity hop (2 launches per step as H1, same kernel inside E1/E2)
+    peak, peak_src = peaks()
+    hop_ms = 0.5 * (op_report["hop_oe_f64"]["ms"] + op_report["hop_eo_f64"]["ms"])
+    hop_bytes = model["hop_oe_f64"]["bytes"]
+    achieved = hop_bytes / hop_ms / 1e6
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "hop_f64_traffic.json")
+    if os.path.exists(tp):
+        try:
+            with open(tp) as f:
+                traffic = json.load(f).get(hr.hr_kernel_name(S["f64"]["lat"].g))
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": "parity hop fp64 (%s)" % hr.hr_kernel_name(S["f64"]["lat"].g), "achieved": round(achieved, 1),
+                "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                "frac_of_datasheet_8000": round(achieved / 8000.0, 4), "bytes_per_launch": hop_bytes,
+                "avg_launch_ms": round(hop_ms, 4), "traffic": traffic,
+                "fp32": {"achieved": round(model["hop_oe_f32"]["bytes"] / (0.5 * (op_report["hop_oe_f32"]["ms"] + op_report["hop_eo_f32"]["ms"])) / 1e6, 1)}}
+    roofline["fp32"]["frac"] = round(roofline["fp32"]["achieved"] / peak, 4)
+
+    # ---- end to end through the host-buffer C-ABI entry points (pinned host memory, copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(args, ranks, hr, S, psi, L, m0, model)
+
+    # ---- the oracle beside it (rank 0, N = 1 only)
+    cpu = None
+    if not args.no_cpu and ranks.rank == 0 and ranks.world == 1:
+        cpu = cpu_baseline(L, m0, seconds_budget=15.0)
+
+    if ranks.rank == 0:
+        line = {
+            "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": ranks.world, "steps": K, "warmup": max(3, args.warmup),
+            "ms_per_step": round(ms_per_step, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64+f32", "data": "synthetic",
+            "config": {"workload": "configs[3]+[4]: %d^4 SU(2) fundamental, Haar links (clover: exp(i 0.3 a.sigma), csw 1.2); "
+                                   "step = hop_oe, hop_eo, D, Dhat (f64 and f32) + clover, clover_inv, Dhat_clover, represent (f64)" % args.L,
+                       "lattice": list(L), "l2_policy": "working set per op (>= 1.3 GB at 48^4) far exceeds the 126 MB L2; no flush needed",
+                       "kernel": hr.hr_kernel_name(S["f64"]["lat"].g), "link_storage": "compressed first row (32 B fp64 / 16 B fp32)",
+                       "parallelism": "replicas x%d (no data-path collective)" % ranks.world},
+            "gflops": round(step_flops * K / tmax / 1e9 * ranks.world, 1),
+            "gsites_per_s": round(step_sites * K / tmax / 1e9 * ranks.world, 3),
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu, "ops": op_report,
+        }
+        print(json.dumps(line))
+    ranks.close()
+
+
+def run_e2e(args, ranks, hr, S, psi, L, m0, model):
+    """same metric through hr_dirac_apply_host / hr_dirac_eo_apply_host: canonical fields in pinned host memory,
+    H2D + pack + operator + unpack + D2H inside the timed region, every step."""
+    import numpy as np
+    import torch
+    from paper_2411_18511_b200 import inputs
+    steps = max(1, min(args.steps, 3))
+    total_s, total_bytes, h2d, d2h = 0.0, 0.0, 0, 0
+    names = []
+    U = inputs.haar_gauge(L, 1)
+    for tag in ("f64", "f32"):
+        lat = S[tag]["lat"]
+        g = lat.g
+        ws = hr.device_buffer(hr.hr_host_workspace_bytes(g), lat.device)
+        Uh = torch.from_numpy(U.astype(lat.cplx)).pin_memory()
+        ph = torch.from_numpy(psi.astype(lat.cplx)).pin_memory()
+        oh = torch.empty_like(ph).pin_memory()
+        st = hr.stream_ptr()
+        calls = [("dirac_" + tag, lambda: hr.hr_dirac_apply_host(g, m0, Uh, ph, oh, ws, st)),
+                 ("dhat_" + tag, lambda: hr.hr_dirac_eo_apply_host(g, hr.EO_DHAT, m0, Uh, ph, oh, ws, st))]
+        for _, fn in calls:
+            fn()  # warm-up (page-locks, first-touch)
+        ranks.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            for _, fn in calls:
+                fn()  # each call synchronises its stream before returning
+        torch.cuda.synchronize()
+        total_s += time.perf_counter() - t0
+        ranks.barrier()
+        for name, _ in calls:
+            total_bytes += model[name]["bytes"]
+            names.append(name)
+        h2d += len(calls) * (Uh.numel() * Uh.element_size() + ph.numel() * ph.element_size())
+        d2h += len(calls) * (oh.numel() * oh.element_size())
+        del ws, Uh, ph, oh
+    from paper_2411_18511_b200.dist import whole_job_throughput
+    value, tmax = whole_job_throughput(ranks, total_bytes * steps / 1e9, total_s)
+    return {"value": round(value, 2), "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+            "steps": steps, "ms_per_step": round(tmax * 1e3 / steps, 2), "ops": names,
+            "note": "host canonical arrays -> H2D -> pack -> operator -> unpack -> D2H per call; bytes = same compulsory model"}
+
+
+# ------------------------------------------------------------------------------------------ oracle timing
+def oracle_sample(L, m0, nthreads, nsites):
+    """time the oracle, as it stands, on a contiguous slab of `nsites` output sites of the 48^4 full-D workload"""
+    import numpy as np
+    import oracle
+    from paper_2411_18511_b200 import inputs
+    U = inputs.haar_gauge(L, 1)
+    psi = inputs.gaussian_spinor(L, 2, 2)
+    out = np.zeros_like(psi)
+    oracle.lib()
+    V = inputs.volume(L)
+    nsites = min(nsites, V)
+    oracle.dirac(L, 0, m0, U, psi, 0, min(4096, V), nthreads, out)  # touch
+    return oracle, U, psi, out, nsites
+
+
+def cpu_baseline(L, m0, seconds_budget=15.0):
+    import oracle
+    cores = oracle.available_cores()
+    orc, U, psi, out, _ = oracle_sample(L, m0, cores, 0)
+    V = 1
+    for v in L:
+        V *= v
+    # calibrate on 1/64 of the lattice, then size the sample to the budget
+    n0 = max(4096, V // 64)
+    t = time.perf_counter()
+    orc.dirac(L, 0, m0, U, psi, 0, n0, cores, out)
+    dt = time.perf_counter() - t
+    n = int(min(V, max(n0, n0 * seconds_budget * 0.5 / max(dt, 1e-6))))
+    t = time.perf_counter()
+    orc.dirac(L, 0, m0, U, psi, 0, n, cores, out)
+    dt_all = time.perf_counter() - t
+    n1 = max(4096, n // max(1, cores))
+    t = time.perf_counter()
+    orc.dirac(L, 0, m0, U, psi, 0, n1, 1, out)
+    dt_one = time.perf_counter() - t
+    bytes_per_site = 384.0  # same compulsory model as the GPU's fused full D, fp64, compressed links
+    return {"value": round(n / dt_all * bytes_per_site / 1e9, 3), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "oracle full D (fp64) on the first %d of %d sites of the %d^4 workload, %d threads; GB/s by the GPU's byte model (384 B/site)" % (n, V, L[0], cores),
+            "msites_per_s": round(n / dt_all / 1e6, 3), "single_thread_msites_per_s": round(n1 / dt_one / 1e6, 3),
+            "label": "unoptimised CPU oracle, reported baseline, not a tuned CPU Dslash"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores; each step = full D on a bounded slab."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    L = (args.L,) * 4
+    m0 = -0.2
+    cores = oracle.available_cores()
+    V = args.L ** 4
+    orc, U, psi, out, _ = oracle_sample(L, m0, cores, 0)
+    n0 = max(4096, V // 256)
+    t = time.perf_counter()
+    orc.dirac(L, 0, m0, U, psi, 0, n0, cores, out)
+    dt = time.perf_counter() - t
+    total_steps = args.steps + max(3, args.warmup)
+    n = int(min(V, max(n0, n0 * (60.0 / total_steps) / max(dt, 1e-6))))   # whole run ~ 1 minute
+    for _ in range(max(3, args.warmup)):
+        orc.dirac(L, 0, m0, U, psi, 0, n, cores, out)
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        orc.dirac(L, 0, m0, U, psi, 0, n, cores, out)
+    dt = time.perf_counter() - t
+    value = n * args.steps / dt * 384.0 / 1e9
+    sample = "oracle full D (fp64) on the first %d of %d sites of %d^4 per step, %d threads; GB/s by the 384 B/site compulsory model" % (n, V, args.L, cores)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": round(dt * 1e3 / args.steps, 3), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[3]: %d^4 SU(2) fundamental, Haar links; oracle (CPU) full D on a slab per step" % args.L,
+                   "lattice": list(L), "parallelism": "host threads x%d" % cores},
+        "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": round(value, 3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
