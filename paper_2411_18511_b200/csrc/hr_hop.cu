@@ -1,10 +1,35 @@
 // hr_hop.cu — dispatch of the hopping kernels (H1/H2/H3).
-#include "hr_hop_generic.cuh"
+#include "hr_hop_tiled.cuh"
 
 namespace hr {
 
-bool tiled_supported(const hr_geom*) { return false; }
-bool tiled_chosen(const hr_geom* g) { return g->kernel == HR_KERNEL_TILED && tiled_supported(g); }
+// lattices below this many sites fit L2 several times over and are launch-bound: the generic kernel's
+// many small CTAs spread better there than one marching CTA per tile
+static const double TILED_AUTO_MIN_SITES = 32.0 * 32.0 * 32.0 * 32.0;
+
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+            (void)cudaGetLastError();
+            n = 148;
+        }
+    }
+    return n;
+}
+
+bool tiled_supported(const hr_geom* g) {
+    TiledPlan pl;
+    return tiled_plan(g, 0, 148, pl);
+}
+
+bool tiled_chosen(const hr_geom* g) {
+    if (g->kernel == HR_KERNEL_GENERIC || !tiled_supported(g)) return false;
+    if (g->kernel == HR_KERNEL_TILED) return true;
+    const double v = (double)g->L[0] * g->L[1] * g->L[2] * g->L[3];
+    return v >= TILED_AUTO_MIN_SITES;
+}
 
 int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
     const Geo geo = make_geo(g);
@@ -12,13 +37,23 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
         set_error("HR_KERNEL_TILED: lattice %dx%dx%dx%d does not fit the tiled kernel", g->L[0], g->L[1], g->L[2], g->L[3]);
         return HR_EUNSUPPORTED;
     }
+    if (g->rep != HR_REP_FUND && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) {
+        set_error("clover epilogues exist for the fundamental representation only");
+        return HR_EUNSUPPORTED;
+    }
+    if (tiled_chosen(g)) {
+        TiledPlan pl;
+        tiled_plan(g, a.both, sm_count(), pl);
+        if (g->rep == HR_REP_FUND) {
+            if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 2>(geo, a, epi, pl, st);
+            return launch_hop_tiled<float, 2>(geo, a, epi, pl, st);
+        }
+        if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 3>(geo, a, epi, pl, st);
+        return launch_hop_tiled<float, 3>(geo, a, epi, pl, st);
+    }
     if (g->rep == HR_REP_FUND) {
         if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 2>(geo, a, epi, st);
         return launch_hop_generic<float, 2>(geo, a, epi, st);
-    }
-    if (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY) {
-        set_error("clover epilogues exist for the fundamental representation only");
-        return HR_EUNSUPPORTED;
     }
     if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 3>(geo, a, epi, st);
     return launch_hop_generic<float, 3>(geo, a, epi, st);

@@ -1,0 +1,361 @@
+// hr_hop_tiled.cuh — the x0-marching tiled hopping kernel (steps H1/H2/H3 of DESIGN.md §2, design in §5.2).
+//
+// One CTA owns a T1 x T2 tile of x3-rows in the (x1,x2) plane and marches along x0 through a segment of
+// planes.  A producer thread moves whole x3-rows of the input half field (contiguous runs of the device
+// layout) into shared memory with 1-D bulk asynchronous copies (cp.async.bulk, completion on
+// an mbarrier): the tile rows of plane x0+1 into a 4-slot ring (each plane serves three steps: as x0+1, x0
+// and x0-1 neighbour) and the one-row halo of the centre plane in x1 and x2 into a double buffer.
+// Consumer threads (one per output site of the tile) gather the 8 neighbour spinors from shared memory;
+// links are read straight from global memory (each is used once per kernel) and re-loaded into the same
+// registers right after their use, for the next step, so a link load has a whole step to complete.
+// Bytes in flight are therefore bounded by shared memory, not by registers (the generic kernel's limit:
+// profiles/r01_generic_hop.md), and an input row crosses L2->SM (1 + 2/T1 + 2/T2) times instead of ~5.4.
+#pragma once
+
+#include <cstdlib>
+
+#include "hr_hop_generic.cuh"
+
+namespace hr {
+
+constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live + one being filled
+constexpr int TILED_MAX_THREADS = 256;  // consumer threads (<= 224) + one producer warp
+
+// ------------------------------------------------------------------ mbarrier / bulk-copy primitives (PTX)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "HR_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra HR_DONE_%=;\n"
+        "bra HR_WAIT_%=;\n"
+        "HR_DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned); completes on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+// NC complex numbers of one site from a shared-memory row image (chunk c at byte offset c*L3h*16 from `p`)
+template <typename T, int NC>
+__device__ __forceinline__ void lds_site(cplx<T>* s, const char* p, int chunk_stride_bytes);
+template <>
+__device__ __forceinline__ void lds_site<double, 8>(cplx<double>* s, const char* p, int cs) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const double2 v = *reinterpret_cast<const double2*>(p + c * cs);
+        s[c] = mk<double>(v.x, v.y);
+    }
+}
+template <>
+__device__ __forceinline__ void lds_site<double, 12>(cplx<double>* s, const char* p, int cs) {
+#pragma unroll
+    for (int c = 0; c < 12; ++c) {
+        const double2 v = *reinterpret_cast<const double2*>(p + c * cs);
+        s[c] = mk<double>(v.x, v.y);
+    }
+}
+template <>
+__device__ __forceinline__ void lds_site<float, 8>(cplx<float>* s, const char* p, int cs) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const float4 v = *reinterpret_cast<const float4*>(p + c * cs);
+        s[2 * c] = mk<float>(v.x, v.y);
+        s[2 * c + 1] = mk<float>(v.z, v.w);
+    }
+}
+template <>
+__device__ __forceinline__ void lds_site<float, 12>(cplx<float>* s, const char* p, int cs) {
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const float4 v = *reinterpret_cast<const float4*>(p + c * cs);
+        s[2 * c] = mk<float>(v.x, v.y);
+        s[2 * c + 1] = mk<float>(v.z, v.w);
+    }
+}
+
+// launch geometry chosen on the host (hr_hop.cu)
+struct TiledPlan {
+    int nt1, nt2;      // tiles along x1, x2
+    int nseg, seglen;  // x0 segments per tile and their length (nseg*seglen == L0)
+    int nconsumer;     // consumer threads (multiple of 32, >= T1*T2*L3h)
+    int rowb;          // bytes of one x3-row of the input half field
+    size_t smem;       // dynamic shared memory
+};
+
+// ------------------------------------------------------------------ the kernel
+// grid.x = (both ? 2 : 1) * nt1 * nt2 * nseg; with both == 1 the output parity is the fastest-varying part
+// of blockIdx.x, so the two CTAs that use a link (forward term of parity p, backward term of parity 1-p)
+// run next to each other and the second use hits L2.
+// Shared memory: [16 mbarriers][ring: TILED_RING planes of T1*T2 rows][halo: 2 buffers of 2*T2 + 2*T1 rows]
+//   halo buffer rows: [x1-1 line: T2 rows][x1+T1 line: T2 rows][x2-1 rows: T1][x2+T2 rows: T1]
+template <typename T, int N, int EPI, int T1, int T2>
+__global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) ? 2 : 1)
+    hop_tiled_kernel(Geo g, HopArgs a, TiledPlan pl) {
+    constexpr int NC = 4 * N;
+    typedef SiteIO<T, NC> IO;
+    constexpr int TR = T1 * T2;            // tile rows
+    constexpr int HR = 2 * T2 + 2 * T1;    // halo rows
+    extern __shared__ __align__(128) char smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
+    char* ring = smem + 128;
+    const int rowb = pl.rowb;
+    const int planeb = TR * rowb;
+    const int halob = HR * rowb;
+    char* halo = ring + TILED_RING * planeb;
+    const uint32_t bar_full = smem_u32(bars);            // [TILED_RING]
+    const uint32_t bar_empty = smem_u32(bars + 4);       // [TILED_RING]
+    const uint32_t bar_hempty = smem_u32(bars + 8);      // [2]
+
+    const int tid = threadIdx.x;
+    const int ncw = pl.nconsumer >> 5;  // consumer warps
+    if (tid == 0) {
+        for (int i = 0; i < TILED_RING; ++i) {
+            mbar_init(bar_full + 8 * i, 1);
+            mbar_init(bar_empty + 8 * i, ncw);
+        }
+        mbar_init(bar_hempty, ncw);
+        mbar_init(bar_hempty + 8, ncw);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    // ---- which work: parity, tile, x0 segment
+    int bid = blockIdx.x;
+    int p = a.parity;
+    if (a.both) { p = bid & 1; bid >>= 1; }
+    const int seg = bid / (pl.nt1 * pl.nt2);
+    const int tile = bid - seg * (pl.nt1 * pl.nt2);
+    const int t1 = tile / pl.nt2, t2 = tile - t1 * pl.nt2;
+    const int xs = seg * pl.seglen, nsteps = pl.seglen;
+    const int L0 = g.L0, L1 = g.s0 / g.s1, L2 = g.s1;
+
+    const size_t half_bytes = (size_t)g.Vh * IO::NCH * 16;
+    const char* in_half = reinterpret_cast<const char*>(a.in) + (a.both ? (size_t)(1 - p) * half_bytes : 0);
+    char* out_half = reinterpret_cast<char*>(a.out) + (a.both ? (size_t)p * half_bytes : 0);
+    const char* phi_half = a.phi ? reinterpret_cast<const char*>(a.phi) + (a.both ? (size_t)p * half_bytes : 0) : nullptr;
+
+    if (tid >= pl.nconsumer) {
+        // ================================================================ producer (one thread)
+        if (tid != pl.nconsumer) return;
+        const int x1base = t1 * T1, x2base = t2 * T2;
+        const int x1lo = (x1base - 1 + L1) % L1, x1hi = (x1base + T1) % L1;
+        const int x2lo = (x2base - 1 + L2) % L2, x2hi = (x2base + T2) % L2;
+        for (int j = 0; j < nsteps + 2; ++j) {   // iteration j: plane x0 = xs-1+j into ring slot j%4, halo of plane xs-2+j
+            const int slot = j & (TILED_RING - 1);
+            const uint32_t use = (uint32_t)(j / TILED_RING);
+            mbar_wait(bar_empty + 8 * slot, (use & 1) ^ 1);
+            const bool with_halo = (j >= 2);     // halo of centre plane j-1, used by step j-2
+            const int hb = (j - 1) & 1;
+            if (with_halo) mbar_wait(bar_hempty + 8 * hb, ((uint32_t)((j - 2) >> 1) & 1) ^ 1);
+            const uint32_t full = bar_full + 8 * slot;
+            mbar_expect_tx(full, (uint32_t)(planeb + (with_halo ? halob : 0)));
+            const int x0p = (xs - 1 + j + L0) % L0;
+            const uint32_t dst = smem_u32(ring + slot * planeb);
+#pragma unroll
+            for (int aa = 0; aa < T1; ++aa) {
+                const size_t row = ((size_t)x0p * L1 + x1base + aa) * L2 + x2base;
+                bulk_g2s(dst + aa * T2 * rowb, in_half + row * rowb, (uint32_t)(T2 * rowb), full);
+            }
+            if (with_halo) {
+                const int x0h = (xs - 2 + j + L0) % L0;
+                const uint32_t hd = smem_u32(halo + hb * halob);
+                bulk_g2s(hd, in_half + (((size_t)x0h * L1 + x1lo) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
+                bulk_g2s(hd + T2 * rowb, in_half + (((size_t)x0h * L1 + x1hi) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
+#pragma unroll
+                for (int aa = 0; aa < T1; ++aa) {
+                    const size_t rb = ((size_t)x0h * L1 + x1base + aa) * L2;
+                    bulk_g2s(hd + (2 * T2 + aa) * rowb, in_half + (rb + x2lo) * rowb, (uint32_t)rowb, full);
+                    bulk_g2s(hd + (2 * T2 + T1 + aa) * rowb, in_half + (rb + x2hi) * rowb, (uint32_t)rowb, full);
+                }
+            }
+        }
+        return;
+    }
+
+    // ================================================================ consumers: one thread per output site
+    const int L3h = g.L3h;
+    const bool active = tid < TR * L3h;
+    const int ctid = active ? tid : 0;               // idle threads shadow site 0 (no global access)
+    const int lr = ctid / L3h, h = ctid - lr * L3h;   // local row in the tile, pair index
+    const int la = lr / T2, lb = lr - la * T2;
+    const int x1 = t1 * T1 + la, x2 = t2 * T2 + lb;
+    const int cs = L3h * 16;                          // byte stride between chunks of a site in a row image
+    // shared-memory byte offsets of the neighbour rows, relative to the centre ring slot (in-tile) or the
+    // halo buffer; constant over the march
+    const bool f1_in = la + 1 < T1, b1_in = la > 0, f2_in = lb + 1 < T2, b2_in = lb > 0;
+    const int off_f1 = (f1_in ? (lr + T2) : (T2 + lb)) * rowb;
+    const int off_b1 = (b1_in ? (lr - T2) : lb) * rowb;
+    const int off_f2 = (f2_in ? (lr + 1) : (2 * T2 + T1 + la)) * rowb;
+    const int off_b2 = (b2_in ? (lr - 1) : (2 * T2 + la)) * rowb;
+    const int off_c = lr * rowb;
+    // global rows: own row at plane x0 is row0 + x0*s0; backward-link rows in x1, x2 likewise
+    const int row0 = x1 * g.s1 + x2;
+    const int rowb1_0 = ((x1 == 0 ? L1 - 1 : x1 - 1)) * g.s1 + x2;
+    const int rowb2_0 = x1 * g.s1 + (x2 == 0 ? L2 - 1 : x2 - 1);
+
+    Link<T, N> uf[4], ub[4];
+    auto load_links = [&](int x0) {
+        const int row = row0 + x0 * g.s0;
+        const int xm = (x0 == 0 ? L0 - 1 : x0 - 1);
+        const int r = (x0 + x1 + x2 + p) & 1;
+        const int hb3 = r ? h : (h == 0 ? L3h - 1 : h - 1);
+        load_link<T, LD_STREAM>(uf[0], a.gauge, g, p, 0, row, h);
+        load_link<T, LD_STREAM>(ub[0], a.gauge, g, 1 - p, 0, row0 + xm * g.s0, h);
+        load_link<T, LD_STREAM>(uf[1], a.gauge, g, p, 1, row, h);
+        load_link<T, LD_STREAM>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + x0 * g.s0, h);
+        load_link<T, LD_STREAM>(uf[2], a.gauge, g, p, 2, row, h);
+        load_link<T, LD_STREAM>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + x0 * g.s0, h);
+        load_link<T, LD_STREAM>(uf[3], a.gauge, g, p, 3, row, h);
+        load_link<T, LD_STREAM>(ub[3], a.gauge, g, 1 - p, 3, row, hb3);
+    };
+    load_links(xs);
+
+    for (int k = 0; k < nsteps; ++k) {
+        const int x0 = xs + k;
+        const int r = (x0 + x1 + x2 + p) & 1;
+        const int hf3 = r ? (h == L3h - 1 ? 0 : h + 1) : h;
+        const int hb3 = r ? h : (h == 0 ? L3h - 1 : h - 1);
+        const char* sprev = ring + (k & 3) * planeb;
+        const char* scur = ring + ((k + 1) & 3) * planeb;
+        const char* snext = ring + ((k + 2) & 3) * planeb;
+        const int hb = (k + 1) & 1;
+        const char* shalo = halo + hb * halob;
+        if (k == 0) {
+            mbar_wait(bar_full, 0);
+            mbar_wait(bar_full + 8, 0);
+        }
+        mbar_wait(bar_full + 8 * ((k + 2) & 3), ((uint32_t)(k + 2) >> 2) & 1);
+
+        // next step's plane (clamped on the last step: the reload is then harmless and unused)
+        const int xn = (k + 1 < nsteps) ? x0 + 1 : x0;
+        const int rown = row0 + xn * g.s0;
+        const int rn = (xn + x1 + x2 + p) & 1;
+        const int hb3n = rn ? h : (h == 0 ? L3h - 1 : h - 1);
+
+        cplx<T> acc[NC], nb[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc[c] = mk<T>((T)0, (T)0);
+
+        lds_site<T, NC>(nb, snext + off_c + h * 16, cs);
+        hop_term<T, N, 0, true>(acc, nb, uf[0]);
+        load_link<T, LD_STREAM>(uf[0], a.gauge, g, p, 0, rown, h);
+        lds_site<T, NC>(nb, sprev + off_c + h * 16, cs);
+        hop_term<T, N, 0, false>(acc, nb, ub[0]);
+        load_link<T, LD_STREAM>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
+
+        lds_site<T, NC>(nb, (f1_in ? scur : shalo) + off_f1 + h * 16, cs);
+        hop_term<T, N, 1, true>(acc, nb, uf[1]);
+        load_link<T, LD_STREAM>(uf[1], a.gauge, g, p, 1, rown, h);
+        lds_site<T, NC>(nb, (b1_in ? scur : shalo) + off_b1 + h * 16, cs);
+        hop_term<T, N, 1, false>(acc, nb, ub[1]);
+        load_link<T, LD_STREAM>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
+
+        lds_site<T, NC>(nb, (f2_in ? scur : shalo) + off_f2 + h * 16, cs);
+        hop_term<T, N, 2, true>(acc, nb, uf[2]);
+        load_link<T, LD_STREAM>(uf[2], a.gauge, g, p, 2, rown, h);
+        lds_site<T, NC>(nb, (b2_in ? scur : shalo) + off_b2 + h * 16, cs);
+        hop_term<T, N, 2, false>(acc, nb, ub[2]);
+        load_link<T, LD_STREAM>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
+
+        lds_site<T, NC>(nb, scur + off_c + hf3 * 16, cs);
+        hop_term<T, N, 3, true>(acc, nb, uf[3]);
+        load_link<T, LD_STREAM>(uf[3], a.gauge, g, p, 3, rown, h);
+        lds_site<T, NC>(nb, scur + off_c + hb3 * 16, cs);
+        hop_term<T, N, 3, false>(acc, nb, ub[3]);
+        load_link<T, LD_STREAM>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
+
+        // all shared-memory reads of this step are consumed: hand the oldest plane and the halo buffer back
+        __syncwarp();
+        if ((tid & 31) == 0) {
+            mbar_arrive(bar_empty + 8 * (k & 3));
+            mbar_arrive(bar_hempty + 8 * hb);
+        }
+        if (active) hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
+    }
+}
+
+// ------------------------------------------------------------------ host side
+constexpr int TILED_T1 = 2, TILED_T2 = 4;
+constexpr size_t TILED_SMEM_LIMIT = 227 * 1024;
+
+// fills pl; false if the lattice does not fit the T1 x T2 tile, the thread budget or shared memory
+inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) {
+    const Geo g = make_geo(hg);
+    const int L1 = hg->L[1], L2 = hg->L[2], L0 = hg->L[0];
+    if (L1 % TILED_T1 || L2 % TILED_T2) return false;
+    const int sites = TILED_T1 * TILED_T2 * g.L3h;
+    if (sites > TILED_MAX_THREADS - 32) return false;
+    pl.nconsumer = (sites + 31) & ~31;
+    pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
+    pl.smem = 128 + (size_t)pl.rowb * (TILED_RING * TILED_T1 * TILED_T2 + 2 * (2 * TILED_T1 + 2 * TILED_T2));
+    if (pl.smem > TILED_SMEM_LIMIT) return false;
+    pl.nt1 = L1 / TILED_T1;
+    pl.nt2 = L2 / TILED_T2;
+    // x0 segments: minimise waves x (segment length + pipeline fill) over the divisors of L0
+    const int cps = (2 * pl.smem + 2048 <= 228 * 1024) ? 2 : 1;   // CTAs resident per SM (shared-memory bound)
+    const long tiles = (long)pl.nt1 * pl.nt2 * (both ? 2 : 1);
+    const long slots = (long)(num_sms > 0 ? num_sms : 148) * cps;
+    double best = 1e300;
+    pl.nseg = 1;
+    for (int ns = 1; ns <= L0; ++ns) {
+        if (L0 % ns) continue;
+        const long waves = (tiles * ns + slots - 1) / slots;
+        const double cost = (double)waves * (L0 / ns + 3);
+        if (cost < best - 1e-9) { best = cost; pl.nseg = ns; }
+    }
+    // tuning / test knob: HR_TILED_NSEG=<divisor of L0> overrides the choice
+    if (const char* e = getenv("HR_TILED_NSEG")) {
+        const int ns = atoi(e);
+        if (ns >= 1 && ns <= L0 && L0 % ns == 0) pl.nseg = ns;
+    }
+    pl.seglen = L0 / pl.nseg;
+    return true;
+}
+
+template <typename T, int N, int EPI>
+inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
+    auto kern = hop_tiled_kernel<T, N, EPI, TILED_T1, TILED_T2>;
+    static bool configured = false;   // per instantiation
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
+        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute(hop_tiled_kernel): %s", cudaGetErrorString(e)); return HR_ECUDA; }
+        configured = true;
+    }
+    const unsigned grid = (unsigned)((a.both ? 2 : 1) * pl.nt1 * pl.nt2 * pl.nseg);
+    kern<<<grid, pl.nconsumer + 32, pl.smem, st>>>(g, a, pl);
+    count_launch();
+    return check_launch("hop_tiled_kernel");
+}
+
+template <typename T, int N>
+inline int launch_hop_tiled(const Geo& g, const HopArgs& a, int epi, const TiledPlan& pl, cudaStream_t st) {
+    switch (epi) {
+        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE>(g, a, pl, st);
+        case EPI_AXPY: return launch_hop_tiled_epi<T, N, EPI_AXPY>(g, a, pl, st);
+        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV>(g, a, pl, st);
+        case EPI_CLOVER_AXPY: return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY>(g, a, pl, st);
+        default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
+    }
+}
+
+}  // namespace hr

@@ -156,13 +156,33 @@ def test_adjoint_small_lattices(hr, orc, L, prec):
     # the adjoint operator is compared on the links the oracle built (rounded for fp32), packed directly
     Rr = rounded(R, prec)
     want = oracle_ops(orc, L, 1, Rr, psi, m0)
-    got = gpu_ops(hr, lat, lat.put_gauge_adj(Rr), psi, m0)
-    for k in want:
-        assert rel(got[k], want[k]) <= TOL[prec], k
+    for kernel in kernels_for(hr, L, 1, prec):
+        latk = lattice(hr, L, 1, prec, kernel)
+        got = gpu_ops(hr, latk, latk.put_gauge_adj(Rr), psi, m0)
+        for k in want:
+            assert rel(got[k], want[k]) <= TOL[prec], (k, kernel)
     if prec == 0:   # and end to end on the links the GPU built
         got2 = gpu_ops(hr, lat, R_dev, psi, m0)
         for k in want:
             assert rel(got2[k], want[k]) <= TOL[prec], k
+
+
+@pytest.mark.parametrize("nseg", [1, 2, 4, 8])
+@pytest.mark.parametrize("rep,N", [(0, 2), (1, 3)])
+def test_tiled_kernel_segment_lengths(hr, orc, monkeypatch, nseg, rep, N):
+    """the x0-marching kernel with segments of 8, 4, 2 and 1 planes (HR_TILED_NSEG), tiles that wrap onto
+    themselves in x1 (L1 = T1) and several tiles in x2; all four operators against the oracle"""
+    L, m0 = (8, 2, 8, 6), -0.2
+    monkeypatch.setenv("HR_TILED_NSEG", str(nseg))
+    Uf = inputs.haar_gauge(L, 1)
+    U = Uf if rep == 0 else orc.represent(Uf)[0]
+    psi = inputs.gaussian_spinor(L, N, 2)
+    want = oracle_ops(orc, L, rep, U, psi, m0)
+    lat = lattice(hr, L, rep, 0, hr.KERNEL_TILED)
+    assert hr.hr_kernel_name(lat.g) == "tiled"
+    got = gpu_ops(hr, lat, lat.put_gauge_fund(U) if rep == 0 else lat.put_gauge_adj(U), psi, m0)
+    for k in want:
+        assert rel(got[k], want[k]) <= TOL[0], (k, nseg)
 
 
 # ------------------------------------------------------------------ config 1
