@@ -89,26 +89,41 @@ template <> struct Chunk<float> { typedef float4 type; };
 
 // cache behaviour of a global access: spinors are re-read by neighbouring sites and should
 // stay in L1/L2; links, clover blocks and outputs are touched once per kernel and are streamed.
-enum { LD_KEEP = 0, LD_STREAM = 1 };
+enum { LD_KEEP = 0, LD_STREAM = 1, LD_NOALLOC = 2 };
 
 template <int POLICY> __device__ __forceinline__ double2 ldg16(const double2* p) {
     if (POLICY == LD_STREAM) return __ldcs(p);
+    if (POLICY == LD_NOALLOC) {
+        double2 v;
+        asm("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+        return v;
+    }
     return __ldg(p);
 }
 template <int POLICY> __device__ __forceinline__ float4 ldg16(const float4* p) {
     if (POLICY == LD_STREAM) return __ldcs(p);
+    if (POLICY == LD_NOALLOC) {
+        float4 v;
+        asm("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+        return v;
+    }
     return __ldg(p);
 }
 template <int POLICY> __device__ __forceinline__ double ldg_real(const double* p) {
-    if (POLICY == LD_STREAM) return __ldcs(p);
+    if (POLICY != LD_KEEP) return __ldcs(p);
     return __ldg(p);
 }
 template <int POLICY> __device__ __forceinline__ float ldg_real(const float* p) {
-    if (POLICY == LD_STREAM) return __ldcs(p);
+    if (POLICY != LD_KEEP) return __ldcs(p);
     return __ldg(p);
 }
+#ifdef HR_STORE_PLAIN
+__device__ __forceinline__ void stg16_stream(double2* p, double2 v) { *p = v; }
+__device__ __forceinline__ void stg16_stream(float4* p, float4 v) { *p = v; }
+#else
 __device__ __forceinline__ void stg16_stream(double2* p, double2 v) { __stcs(p, v); }
 __device__ __forceinline__ void stg16_stream(float4* p, float4 v) { __stcs(p, v); }
+#endif
 
 __device__ __forceinline__ void chunk_to_reals(double2 v, double* e) { e[0] = v.x; e[1] = v.y; }
 __device__ __forceinline__ void chunk_to_reals(float4 v, float* e) { e[0] = v.x; e[1] = v.y; e[2] = v.z; e[3] = v.w; }

@@ -26,7 +26,9 @@ struct HopArgs {
     int both;            // 1: gridDim.y == 2 and blockIdx.y is the output parity (full D in one launch)
 };
 
-template <typename T, int N, int EPI>
+// PHI_POLICY: LD_STREAM when phi is read by this kernel only; LD_KEEP in the full-lattice launch (H3), where
+// phi is the other parity pass's gather input
+template <typename T, int N, int EPI, int PHI_POLICY = LD_STREAM>
 __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const HopArgs& a, const void* phi_half,
                                              void* out_half, int p, int row, int h) {
     constexpr int NC = 4 * N;
@@ -34,7 +36,7 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
     const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
     if (EPI == EPI_AXPY) {
         cplx<T> phi[NC];
-        IO::template load<LD_STREAM>(phi, phi_half, first, g.L3h);
+        IO::template load<PHI_POLICY>(phi, phi_half, first, g.L3h);
         const T ca = (T)a.a, cc = (T)a.c;
 #pragma unroll
         for (int k = 0; k < NC; ++k) {

@@ -19,7 +19,37 @@
 namespace hr {
 
 constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live + one being filled
-constexpr int TILED_MAX_THREADS = 256;  // consumer threads (<= 224) + one producer warp
+#ifndef HR_T_HALO
+#define HR_T_HALO 2
+#endif
+// consumer scheduling, per precision (measured at 48^4, profiles/r01_tiled_variants.md):
+//   PIN  : __syncwarp() after each link re-load, which stops ptxas from sinking the loads to the end of the step
+//   NBDB : read the neighbour of term t+1 from shared memory before computing term t (two register images)
+#ifndef HR_T_PIN_F64
+#define HR_T_PIN_F64 0
+#endif
+#ifndef HR_T_PIN_F32
+#define HR_T_PIN_F32 1
+#endif
+#ifndef HR_T_NBDB_F64
+#define HR_T_NBDB_F64 0
+#endif
+#ifndef HR_T_NBDB_F32
+#define HR_T_NBDB_F32 1
+#endif
+constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, two being filled (the halo is 60 % of a step's bytes)
+//   LINKPOL : cache policy of the link loads (LD_STREAM = ld.global.cs, LD_KEEP = ld.global.nc)
+#ifndef HR_T_LINKPOL_F64
+#define HR_T_LINKPOL_F64 LD_KEEP
+#endif
+#ifndef HR_T_LINKPOL_F32
+#define HR_T_LINKPOL_F32 LD_STREAM
+#endif
+#ifndef HR_T_F32_WIDE
+#define HR_T_F32_WIDE 1
+#endif
+// threads per CTA the kernel is compiled for: one per site of a T1 x T2 tile of rows with L3h <= 24, + producer warp
+constexpr int tiled_max_threads(int t1, int t2) { return ((t1 * t2 * 24 + 31) / 32) * 32 + 32; }
 
 // ------------------------------------------------------------------ mbarrier / bulk-copy primitives (PTX)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -95,6 +125,7 @@ __device__ __forceinline__ void lds_site<float, 12>(cplx<float>* s, const char* 
 
 // launch geometry chosen on the host (hr_hop.cu)
 struct TiledPlan {
+    int t1, t2;        // tile shape in rows (x1, x2): selects the kernel instantiation
     int nt1, nt2;      // tiles along x1, x2
     int nseg, seglen;  // x0 segments per tile and their length (nseg*seglen == L0)
     int nconsumer;     // consumer threads (multiple of 32, >= T1*T2*L3h)
@@ -106,15 +137,19 @@ struct TiledPlan {
 // grid.x = (both ? 2 : 1) * nt1 * nt2 * nseg; with both == 1 the output parity is the fastest-varying part
 // of blockIdx.x, so the two CTAs that use a link (forward term of parity p, backward term of parity 1-p)
 // run next to each other and the second use hits L2.
-// Shared memory: [16 mbarriers][ring: TILED_RING planes of T1*T2 rows][halo: 2 buffers of 2*T2 + 2*T1 rows]
+// Shared memory: [16 mbarriers][ring: TILED_RING planes of T1*T2 rows][halo: TILED_HALO buffers of 2*T2 + 2*T1 rows]
 //   halo buffer rows: [x1-1 line: T2 rows][x1+T1 line: T2 rows][x2-1 rows: T1][x2+T2 rows: T1]
-template <typename T, int N, int EPI, int T1, int T2>
-__global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) ? 2 : 1)
+// SHARE: links and phi are also read by the CTA of the other parity (full-lattice launch): keep them in L2
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE>
+__global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g, HopArgs a, TiledPlan pl) {
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
     constexpr int TR = T1 * T2;            // tile rows
     constexpr int HR = 2 * T2 + 2 * T1;    // halo rows
+    constexpr int LP = SHARE ? LD_KEEP : (sizeof(T) == 4 ? HR_T_LINKPOL_F32 : HR_T_LINKPOL_F64);
+    constexpr bool PIN = sizeof(T) == 4 ? HR_T_PIN_F32 : HR_T_PIN_F64;
+    constexpr bool NBDB = sizeof(T) == 4 ? HR_T_NBDB_F32 : HR_T_NBDB_F64;
     extern __shared__ __align__(128) char smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
     char* ring = smem + 128;
@@ -124,7 +159,7 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
     char* halo = ring + TILED_RING * planeb;
     const uint32_t bar_full = smem_u32(bars);            // [TILED_RING]
     const uint32_t bar_empty = smem_u32(bars + 4);       // [TILED_RING]
-    const uint32_t bar_hempty = smem_u32(bars + 8);      // [2]
+    const uint32_t bar_hempty = smem_u32(bars + 8);      // [TILED_HALO]
 
     const int tid = threadIdx.x;
     const int ncw = pl.nconsumer >> 5;  // consumer warps
@@ -133,8 +168,7 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
             mbar_init(bar_full + 8 * i, 1);
             mbar_init(bar_empty + 8 * i, ncw);
         }
-        mbar_init(bar_hempty, ncw);
-        mbar_init(bar_hempty + 8, ncw);
+        for (int i = 0; i < TILED_HALO; ++i) mbar_init(bar_hempty + 8 * i, ncw);
         mbar_fence_init();
     }
     __syncthreads();
@@ -160,13 +194,14 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
         const int x1base = t1 * T1, x2base = t2 * T2;
         const int x1lo = (x1base - 1 + L1) % L1, x1hi = (x1base + T1) % L1;
         const int x2lo = (x2base - 1 + L2) % L2, x2hi = (x2base + T2) % L2;
-        for (int j = 0; j < nsteps + 2; ++j) {   // iteration j: plane x0 = xs-1+j into ring slot j%4, halo of plane xs-2+j
+        for (int j = 0; j < nsteps + 2; ++j) {   // iteration j: plane x0 = xs-1+j into ring slot j%4, with its halo if it will be a centre
             const int slot = j & (TILED_RING - 1);
             const uint32_t use = (uint32_t)(j / TILED_RING);
             mbar_wait(bar_empty + 8 * slot, (use & 1) ^ 1);
-            const bool with_halo = (j >= 2);     // halo of centre plane j-1, used by step j-2
-            const int hb = (j - 1) & 1;
-            if (with_halo) mbar_wait(bar_hempty + 8 * hb, ((uint32_t)((j - 2) >> 1) & 1) ^ 1);
+            const int hc = j - (3 - TILED_HALO);              // centre plane whose halo rides with this iteration
+            const bool with_halo = (hc >= 1 && hc <= nsteps);   // plane hc is the centre of step hc-1
+            const int hb = hc % TILED_HALO;
+            if (with_halo) mbar_wait(bar_hempty + 8 * hb, ((uint32_t)((hc - 1) / TILED_HALO) & 1) ^ 1);
             const uint32_t full = bar_full + 8 * slot;
             mbar_expect_tx(full, (uint32_t)(planeb + (with_halo ? halob : 0)));
             const int x0p = (xs - 1 + j + L0) % L0;
@@ -177,7 +212,7 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
                 bulk_g2s(dst + aa * T2 * rowb, in_half + row * rowb, (uint32_t)(T2 * rowb), full);
             }
             if (with_halo) {
-                const int x0h = (xs - 2 + j + L0) % L0;
+                const int x0h = (xs - 1 + hc + L0) % L0;
                 const uint32_t hd = smem_u32(halo + hb * halob);
                 bulk_g2s(hd, in_half + (((size_t)x0h * L1 + x1lo) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
                 bulk_g2s(hd + T2 * rowb, in_half + (((size_t)x0h * L1 + x1hi) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
@@ -214,21 +249,18 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
     const int rowb2_0 = x1 * g.s1 + (x2 == 0 ? L2 - 1 : x2 - 1);
 
     Link<T, N> uf[4], ub[4];
-    auto load_links = [&](int x0) {
-        const int row = row0 + x0 * g.s0;
-        const int xm = (x0 == 0 ? L0 - 1 : x0 - 1);
-        const int r = (x0 + x1 + x2 + p) & 1;
-        const int hb3 = r ? h : (h == 0 ? L3h - 1 : h - 1);
-        load_link<T, LD_STREAM>(uf[0], a.gauge, g, p, 0, row, h);
-        load_link<T, LD_STREAM>(ub[0], a.gauge, g, 1 - p, 0, row0 + xm * g.s0, h);
-        load_link<T, LD_STREAM>(uf[1], a.gauge, g, p, 1, row, h);
-        load_link<T, LD_STREAM>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + x0 * g.s0, h);
-        load_link<T, LD_STREAM>(uf[2], a.gauge, g, p, 2, row, h);
-        load_link<T, LD_STREAM>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + x0 * g.s0, h);
-        load_link<T, LD_STREAM>(uf[3], a.gauge, g, p, 3, row, h);
-        load_link<T, LD_STREAM>(ub[3], a.gauge, g, 1 - p, 3, row, hb3);
-    };
-    load_links(xs);
+    {   // links of the first step
+        const int row = row0 + xs * g.s0;
+        const int r = (xs + x1 + x2 + p) & 1;
+        load_link<T, LP>(uf[0], a.gauge, g, p, 0, row, h);
+        load_link<T, LP>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
+        load_link<T, LP>(uf[1], a.gauge, g, p, 1, row, h);
+        load_link<T, LP>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xs * g.s0, h);
+        load_link<T, LP>(uf[2], a.gauge, g, p, 2, row, h);
+        load_link<T, LP>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xs * g.s0, h);
+        load_link<T, LP>(uf[3], a.gauge, g, p, 3, row, h);
+        load_link<T, LP>(ub[3], a.gauge, g, 1 - p, 3, row, r ? h : (h == 0 ? L3h - 1 : h - 1));
+    }
 
     for (int k = 0; k < nsteps; ++k) {
         const int x0 = xs + k;
@@ -238,7 +270,7 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
         const char* sprev = ring + (k & 3) * planeb;
         const char* scur = ring + ((k + 1) & 3) * planeb;
         const char* snext = ring + ((k + 2) & 3) * planeb;
-        const int hb = (k + 1) & 1;
+        const int hb = (k + 1) % TILED_HALO;
         const char* shalo = halo + hb * halob;
         if (k == 0) {
             mbar_wait(bar_full, 0);
@@ -252,37 +284,62 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
         const int rn = (xn + x1 + x2 + p) & 1;
         const int hb3n = rn ? h : (h == 0 ? L3h - 1 : h - 1);
 
-        cplx<T> acc[NC], nb[NC];
+        // Eight terms.  The neighbour of term t+1 is read from shared memory before term t is computed
+        // (two register images, nbA / nbB), and each link is re-loaded for the next step right after its
+        // use; __syncwarp() keeps the compiler from sinking those loads to the end of the step (where
+        // their latency would be exposed at the top of the next one).
+        cplx<T> acc[NC], nbA[NC], nbB[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[c] = mk<T>((T)0, (T)0);
 
-        lds_site<T, NC>(nb, snext + off_c + h * 16, cs);
-        hop_term<T, N, 0, true>(acc, nb, uf[0]);
-        load_link<T, LD_STREAM>(uf[0], a.gauge, g, p, 0, rown, h);
-        lds_site<T, NC>(nb, sprev + off_c + h * 16, cs);
-        hop_term<T, N, 0, false>(acc, nb, ub[0]);
-        load_link<T, LD_STREAM>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
-
-        lds_site<T, NC>(nb, (f1_in ? scur : shalo) + off_f1 + h * 16, cs);
-        hop_term<T, N, 1, true>(acc, nb, uf[1]);
-        load_link<T, LD_STREAM>(uf[1], a.gauge, g, p, 1, rown, h);
-        lds_site<T, NC>(nb, (b1_in ? scur : shalo) + off_b1 + h * 16, cs);
-        hop_term<T, N, 1, false>(acc, nb, ub[1]);
-        load_link<T, LD_STREAM>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
-
-        lds_site<T, NC>(nb, (f2_in ? scur : shalo) + off_f2 + h * 16, cs);
-        hop_term<T, N, 2, true>(acc, nb, uf[2]);
-        load_link<T, LD_STREAM>(uf[2], a.gauge, g, p, 2, rown, h);
-        lds_site<T, NC>(nb, (b2_in ? scur : shalo) + off_b2 + h * 16, cs);
-        hop_term<T, N, 2, false>(acc, nb, ub[2]);
-        load_link<T, LD_STREAM>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
-
-        lds_site<T, NC>(nb, scur + off_c + hf3 * 16, cs);
-        hop_term<T, N, 3, true>(acc, nb, uf[3]);
-        load_link<T, LD_STREAM>(uf[3], a.gauge, g, p, 3, rown, h);
-        lds_site<T, NC>(nb, scur + off_c + hb3 * 16, cs);
-        hop_term<T, N, 3, false>(acc, nb, ub[3]);
-        load_link<T, LD_STREAM>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
+#define HR_NB_NEXT(BUF, ADDR) if (NBDB) lds_site<T, NC>(BUF, ADDR, cs)
+#define HR_NB_NOW(BUF, ADDR) if (!NBDB) lds_site<T, NC>(BUF, ADDR, cs)
+#define HR_PIN() if (PIN) __syncwarp()
+        cplx<T>* const nb0 = nbA;
+        cplx<T>* const nb1 = NBDB ? nbB : nbA;
+        const char* const a0f = snext + off_c + h * 16;
+        const char* const a0b = sprev + off_c + h * 16;
+        const char* const a1f = (f1_in ? scur : shalo) + off_f1 + h * 16;
+        const char* const a1b = (b1_in ? scur : shalo) + off_b1 + h * 16;
+        const char* const a2f = (f2_in ? scur : shalo) + off_f2 + h * 16;
+        const char* const a2b = (b2_in ? scur : shalo) + off_b2 + h * 16;
+        const char* const a3f = scur + off_c + hf3 * 16;
+        const char* const a3b = scur + off_c + hb3 * 16;
+        HR_NB_NEXT(nb0, a0f);
+        HR_NB_NEXT(nb1, a0b); HR_NB_NOW(nb0, a0f);
+        hop_term<T, N, 0, true>(acc, nb0, uf[0]);
+        load_link<T, LP>(uf[0], a.gauge, g, p, 0, rown, h);
+        HR_PIN();
+        HR_NB_NEXT(nb0, a1f); HR_NB_NOW(nb1, a0b);
+        hop_term<T, N, 0, false>(acc, nb1, ub[0]);
+        load_link<T, LP>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
+        HR_PIN();
+        HR_NB_NEXT(nb1, a1b); HR_NB_NOW(nb0, a1f);
+        hop_term<T, N, 1, true>(acc, nb0, uf[1]);
+        load_link<T, LP>(uf[1], a.gauge, g, p, 1, rown, h);
+        HR_PIN();
+        HR_NB_NEXT(nb0, a2f); HR_NB_NOW(nb1, a1b);
+        hop_term<T, N, 1, false>(acc, nb1, ub[1]);
+        load_link<T, LP>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
+        HR_PIN();
+        HR_NB_NEXT(nb1, a2b); HR_NB_NOW(nb0, a2f);
+        hop_term<T, N, 2, true>(acc, nb0, uf[2]);
+        load_link<T, LP>(uf[2], a.gauge, g, p, 2, rown, h);
+        HR_PIN();
+        HR_NB_NEXT(nb0, a3f); HR_NB_NOW(nb1, a2b);
+        hop_term<T, N, 2, false>(acc, nb1, ub[2]);
+        load_link<T, LP>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
+        HR_PIN();
+        HR_NB_NEXT(nb1, a3b); HR_NB_NOW(nb0, a3f);
+        hop_term<T, N, 3, true>(acc, nb0, uf[3]);
+        load_link<T, LP>(uf[3], a.gauge, g, p, 3, rown, h);
+        HR_PIN();
+        HR_NB_NOW(nb1, a3b);
+        hop_term<T, N, 3, false>(acc, nb1, ub[3]);
+        load_link<T, LP>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
+#undef HR_NB_NEXT
+#undef HR_NB_NOW
+#undef HR_PIN
 
         // all shared-memory reads of this step are consumed: hand the oldest plane and the halo buffer back
         __syncwarp();
@@ -290,29 +347,29 @@ __global__ void __launch_bounds__(TILED_MAX_THREADS, (sizeof(T) == 4 && N == 2) 
             mbar_arrive(bar_empty + 8 * (k & 3));
             mbar_arrive(bar_hempty + 8 * hb);
         }
-        if (active) hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
+        if (active) hop_epilogue<T, N, EPI, LP>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
     }
 }
 
 // ------------------------------------------------------------------ host side
-constexpr int TILED_T1 = 2, TILED_T2 = 4;
 constexpr size_t TILED_SMEM_LIMIT = 227 * 1024;
 
-// fills pl; false if the lattice does not fit the T1 x T2 tile, the thread budget or shared memory
-inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) {
+inline bool tiled_plan_shape(const hr_geom* hg, int both, int num_sms, int t1, int t2, TiledPlan& pl) {
     const Geo g = make_geo(hg);
     const int L1 = hg->L[1], L2 = hg->L[2], L0 = hg->L[0];
-    if (L1 % TILED_T1 || L2 % TILED_T2) return false;
-    const int sites = TILED_T1 * TILED_T2 * g.L3h;
-    if (sites > TILED_MAX_THREADS - 32) return false;
+    if (L1 % t1 || L2 % t2) return false;
+    const int sites = t1 * t2 * g.L3h;
+    if (sites > tiled_max_threads(t1, t2) - 32) return false;
+    pl.t1 = t1;
+    pl.t2 = t2;
     pl.nconsumer = (sites + 31) & ~31;
     pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
-    pl.smem = 128 + (size_t)pl.rowb * (TILED_RING * TILED_T1 * TILED_T2 + 2 * (2 * TILED_T1 + 2 * TILED_T2));
+    pl.smem = 128 + (size_t)pl.rowb * (TILED_RING * t1 * t2 + TILED_HALO * (2 * t1 + 2 * t2));
     if (pl.smem > TILED_SMEM_LIMIT) return false;
-    pl.nt1 = L1 / TILED_T1;
-    pl.nt2 = L2 / TILED_T2;
+    pl.nt1 = L1 / t1;
+    pl.nt2 = L2 / t2;
     // x0 segments: minimise waves x (segment length + pipeline fill) over the divisors of L0
-    const int cps = (2 * pl.smem + 2048 <= 228 * 1024) ? 2 : 1;   // CTAs resident per SM (shared-memory bound)
+    const int cps = (2 * pl.smem + 2048 <= 228 * 1024 && hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND) ? 2 : 1;  // CTAs per SM
     const long tiles = (long)pl.nt1 * pl.nt2 * (both ? 2 : 1);
     const long slots = (long)(num_sms > 0 ? num_sms : 148) * cps;
     double best = 1e300;
@@ -332,9 +389,18 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) 
     return true;
 }
 
-template <typename T, int N, int EPI>
-inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    auto kern = hop_tiled_kernel<T, N, EPI, TILED_T1, TILED_T2>;
+// fills pl; false if the lattice fits no instantiated tile shape.  fp32 fundamental rows are half as long,
+// so a 4 x 4 tile fits (2 row-loads per site instead of 2.5); everything else uses 2 x 4.
+inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) {
+#if HR_T_F32_WIDE
+    if (hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, num_sms, 4, 4, pl)) return true;
+#endif
+    return tiled_plan_shape(hg, both, num_sms, 2, 4, pl);
+}
+
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2>
+inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
+    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE>;
     static bool configured = false;   // per instantiation
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
@@ -347,13 +413,25 @@ inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan&
     return check_launch("hop_tiled_kernel");
 }
 
+template <typename T, int N, int EPI, bool SHARE>
+inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
+    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4>(g, a, pl, st);
+#if HR_T_F32_WIDE
+    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4>(g, a, pl, st);
+#endif
+    set_error("hop_tiled_kernel: no instantiation for a %d x %d tile", pl.t1, pl.t2);
+    return HR_EUNSUPPORTED;
+}
+
 template <typename T, int N>
 inline int launch_hop_tiled(const Geo& g, const HopArgs& a, int epi, const TiledPlan& pl, cudaStream_t st) {
     switch (epi) {
-        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE>(g, a, pl, st);
-        case EPI_AXPY: return launch_hop_tiled_epi<T, N, EPI_AXPY>(g, a, pl, st);
-        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV>(g, a, pl, st);
-        case EPI_CLOVER_AXPY: return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY>(g, a, pl, st);
+        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE, false>(g, a, pl, st);
+        case EPI_AXPY:
+            if (a.both) return launch_hop_tiled_epi<T, N, EPI_AXPY, true>(g, a, pl, st);
+            return launch_hop_tiled_epi<T, N, EPI_AXPY, false>(g, a, pl, st);
+        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV, false>(g, a, pl, st);
+        case EPI_CLOVER_AXPY: return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, false>(g, a, pl, st);
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
 }
