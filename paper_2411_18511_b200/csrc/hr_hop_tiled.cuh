@@ -347,6 +347,7 @@ __global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && 
             mbar_arrive(bar_empty + 8 * (k & 3));
             mbar_arrive(bar_hempty + 8 * hb);
         }
+        // (requesting phi before the eight terms was measured slower at 48^4: 412 -> 425 us for fp64 H3)
         if (active) hop_epilogue<T, N, EPI, LP>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
     }
 }
