@@ -45,7 +45,11 @@ enum { HR_PREC_F64 = 0, HR_PREC_F32 = 1 };
 /* fundamental links are stored as their first row (alpha, beta): U = [[alpha, beta], [-conj(beta), conj(alpha)]]
  * is exact for SU(2).  HR_LINKS_FULL (all four entries) is declared for the byte model only and is
  * rejected with HR_EUNSUPPORTED by the kernels. */
-enum { HR_LINKS_FULL = 0, HR_LINKS_COMPRESSED = 1 };
+enum { HR_LINKS_FULL = 0, HR_LINKS_COMPRESSED = 1,
+       /* adjoint fermions only: the operators are handed the FUNDAMENTAL (compressed) gauge field and rebuild the
+        * real 3x3 link R^{ab} = 1/2 tr(sigma_a U sigma_b U^dag) in registers — 32 B instead of 72 B per fp64 link,
+        * and no adjoint gauge field in memory ("higher representations") */
+       HR_LINKS_ONTHEFLY = 2 };
 /* which hopping kernel runs: AUTO picks the x0-marching tiled kernel when the lattice allows it and is
  * large enough to need it, else the generic one-thread-per-site kernel.  The other two values force a
  * kernel (HR_KERNEL_TILED fails with HR_EUNSUPPORTED if the lattice does not fit its tiles). */
@@ -55,7 +59,7 @@ typedef struct hr_geom {
     int L[4];         /* extents, L[0] = T (slowest) ... L[3] (fastest); all even, >= 2 */
     int rep;          /* HR_REP_*: representation of the FERMION (and of the links the operators read) */
     int prec;         /* HR_PREC_* : arithmetic and storage type of every field */
-    int link_storage; /* HR_LINKS_* (fundamental links only) */
+    int link_storage; /* HR_LINKS_*: FULL/COMPRESSED describe fundamental links; ONTHEFLY is for rep == HR_REP_ADJ */
     int kernel;       /* HR_KERNEL_* */
 } hr_geom;
 
@@ -85,7 +89,8 @@ int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* strea
 int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* stream);
 
 /* H3 (north_star "full form"): out = D psi on all V sites, one launch.
- * u: gauge field in representation g->rep; psi, out: full-lattice spinors (out must not alias psi). */
+ * u: gauge field in representation g->rep (the fundamental field if g->link_storage == HR_LINKS_ONTHEFLY);
+ * psi, out: full-lattice spinors (out must not alias psi). */
 int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, void* out, void* stream);
 
 /* H1/H2/E1/E2 (north_star "even-odd preconditioned form D_ee - D_eo D_oo^-1 D_oe as used in the HMC";

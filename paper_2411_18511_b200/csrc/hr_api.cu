@@ -134,7 +134,7 @@ int hr_unpack_spinor(const hr_geom* g, const void* dev, void* canon, void* strea
 int hr_pack_gauge(const hr_geom* g, int rep, const void* canon, void* dev, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
     if (rep == HR_REP_FUND) {
-        if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+        if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
         const int lch = link_chunks(g->prec);
         return permute_chunks(true, make_geo(g), 4, lch, 2 * lch, canon, dev, (cudaStream_t)stream);
     }
@@ -145,7 +145,7 @@ int hr_pack_gauge(const hr_geom* g, int rep, const void* canon, void* dev, void*
 int hr_unpack_gauge(const hr_geom* g, int rep, const void* dev, void* canon, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
     if (rep == HR_REP_FUND) {
-        if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+        if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
         const int lch = link_chunks(g->prec);
         const Geo geo = make_geo(g);
         HR_TRY(permute_chunks(false, geo, 4, lch, 2 * lch, dev, canon, (cudaStream_t)stream));
@@ -169,7 +169,7 @@ int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* strea
 // ---------------------------------------------------------------- R1
 int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund")); HR_TRY(check_ptr(u_adj, "u_adj"));
-    if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+    if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     return run_represent(make_geo(g), g->prec, u_fund, u_adj, (cudaStream_t)stream);
 }
 
@@ -226,7 +226,7 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
 int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
                     void* clover_inv, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund"));
-    if (g->link_storage != HR_LINKS_COMPRESSED) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+    if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     if (!clover_fwd && !clover_inv) { set_error("hr_clover_build: nothing to build"); return HR_EINVAL; }
     if (clover_fwd) HR_TRY(check_ptr(clover_fwd, "clover_fwd"));
     if (clover_inv) HR_TRY(check_ptr(clover_inv, "clover_inv"));
@@ -247,10 +247,11 @@ int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, doubl
     HR_TRY(check_geom(g));
     const double N = ncolour(g->rep), w = (double)real_bytes(g->prec);
     const double nr = 8.0 * N, S = nr * w;
-    const double Gf = (g->link_storage == HR_LINKS_COMPRESSED ? 4.0 : 8.0) * w, Ga = 9.0 * w;
-    const double G = g->rep == HR_REP_FUND ? Gf : Ga;
+    const double Gf = (g->link_storage != HR_LINKS_FULL ? 4.0 : 8.0) * w, Ga = 9.0 * w;
+    const double G = g->rep == HR_REP_FUND ? Gf : (g->link_storage == HR_LINKS_ONTHEFLY ? 4.0 * w : Ga);
     const double Bk = 32.0 * w;
     // per direction: 4N adds to project, two colour mat-vecs, 8N adds to accumulate; x8, minus the first accumulate
+    // (rebuilding R from the quaternion, ~30 flops per link, is not counted: the model counts the operator's flops)
     const double Fhop = g->rep == HR_REP_FUND ? 8.0 * N * (16.0 * N + 7.0) : 8.0 * N * (8.0 * N + 7.0);
     const double Fblk = 208.0;  // two hermitian 4x4 mat-vecs
     double f = 0, bc = 0, br = 0;
@@ -278,8 +279,9 @@ static size_t up256(size_t n) { return (n + 255) & ~(size_t)255; }
 
 size_t hr_host_workspace_bytes(const hr_geom* g) {
     if (!geom_ok(g)) return 0;
-    return up256(hr_canonical_gauge_bytes(g, g->rep)) + 2 * up256(hr_canonical_spinor_bytes(g)) +
-           up256(hr_gauge_bytes(g, g->rep)) + 3 * up256(hr_spinor_bytes(g, HR_BOTH));
+    const int urep = g->link_storage == HR_LINKS_ONTHEFLY ? HR_REP_FUND : g->rep;   // representation of the links handed in
+    return up256(hr_canonical_gauge_bytes(g, urep)) + 2 * up256(hr_canonical_spinor_bytes(g)) +
+           up256(hr_gauge_bytes(g, urep)) + 3 * up256(hr_spinor_bytes(g, HR_BOTH));
 }
 
 static int host_apply(const hr_geom* g, int op, double m0, const void* u_h, const void* in_h, void* out_h,
@@ -288,8 +290,9 @@ static int host_apply(const hr_geom* g, int op, double m0, const void* u_h, cons
     if (!u_h || !in_h || !out_h) { set_error("host pointer is NULL"); return HR_EINVAL; }
     HR_TRY(check_ptr(workspace, "workspace"));
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t cg = hr_canonical_gauge_bytes(g, g->rep), cs = hr_canonical_spinor_bytes(g);
-    const size_t dg = hr_gauge_bytes(g, g->rep), ds = hr_spinor_bytes(g, HR_BOTH), half = ds / 2;
+    const int urep = g->link_storage == HR_LINKS_ONTHEFLY ? HR_REP_FUND : g->rep;
+    const size_t cg = hr_canonical_gauge_bytes(g, urep), cs = hr_canonical_spinor_bytes(g);
+    const size_t dg = hr_gauge_bytes(g, urep), ds = hr_spinor_bytes(g, HR_BOTH), half = ds / 2;
     char* w = (char*)workspace;
     char* c_u = w; w += up256(cg);
     char* c_in = w; w += up256(cs);
@@ -305,7 +308,7 @@ static int host_apply(const hr_geom* g, int op, double m0, const void* u_h, cons
     } while (0)
     HR_CUDA(cudaMemcpyAsync(c_u, u_h, cg, cudaMemcpyHostToDevice, st));
     HR_CUDA(cudaMemcpyAsync(c_in, in_h, cs, cudaMemcpyHostToDevice, st));
-    HR_TRY(hr_pack_gauge(g, g->rep, c_u, d_u, stream));
+    HR_TRY(hr_pack_gauge(g, urep, c_u, d_u, stream));
     HR_TRY(hr_pack_spinor(g, c_in, d_in, stream));
     if (op < 0) {
         HR_TRY(hr_dirac_apply(g, m0, d_u, d_in, d_out, stream));

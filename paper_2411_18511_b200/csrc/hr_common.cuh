@@ -33,7 +33,8 @@ inline bool geom_ok(const hr_geom* g) {
     if (v > 2.0e9) return false;  // 32-bit site indices
     if (g->rep != HR_REP_FUND && g->rep != HR_REP_ADJ) return false;
     if (g->prec != HR_PREC_F64 && g->prec != HR_PREC_F32) return false;
-    if (g->link_storage != HR_LINKS_FULL && g->link_storage != HR_LINKS_COMPRESSED) return false;
+    if (g->link_storage != HR_LINKS_FULL && g->link_storage != HR_LINKS_COMPRESSED && g->link_storage != HR_LINKS_ONTHEFLY) return false;
+    if (g->link_storage == HR_LINKS_ONTHEFLY && g->rep != HR_REP_ADJ) return false;
     if (g->kernel < HR_KERNEL_AUTO || g->kernel > HR_KERNEL_TILED) return false;
     return true;
 }
@@ -192,6 +193,28 @@ __device__ __forceinline__ void load_link(Link<T, 3>& u, const void* gauge, cons
     const T* p = reinterpret_cast<const T*>(gauge) + ((size_t)(par * 4 + mu) * g.R + row) * (9 * g.L3h) + h;
 #pragma unroll
     for (int k = 0; k < 9; ++k) u.r[k] = ldg_real<POLICY>(p + (size_t)k * g.L3h);
+}
+
+// ONFLY: the gauge field handed to the kernel is the fundamental one; an adjoint link is rebuilt in registers,
+//   R_ab = (a0^2 - |a|^2) delta_ab + 2 a_a a_b + 2 a0 eps_abc a_c,   U = a0 + i a.sigma  (alpha = a0 + i a3, beta = a2 + i a1)
+// — the closed form of R^{ab} = 1/2 tr(sigma_a U sigma_b U^dag) also used by represent_kernel.
+template <typename T, int POLICY, bool ONFLY>
+__device__ __forceinline__ void load_link_rep(Link<T, 2>& u, const void* gauge, const Geo& g, int par, int mu, int row, int h) {
+    load_link<T, POLICY>(u, gauge, g, par, mu, row, h);
+}
+template <typename T, int POLICY, bool ONFLY>
+__device__ __forceinline__ void load_link_rep(Link<T, 3>& u, const void* gauge, const Geo& g, int par, int mu, int row, int h) {
+    if (!ONFLY) {
+        load_link<T, POLICY>(u, gauge, g, par, mu, row, h);
+        return;
+    }
+    Link<T, 2> f;
+    load_link<T, POLICY>(f, gauge, g, par, mu, row, h);
+    const T a0 = f.a.re, a3 = f.a.im, a2 = f.b.re, a1 = f.b.im;
+    const T d = a0 * a0 - (a1 * a1 + a2 * a2 + a3 * a3);
+    u.r[0] = d + 2 * a1 * a1;          u.r[1] = 2 * (a1 * a2 + a0 * a3);  u.r[2] = 2 * (a1 * a3 - a0 * a2);
+    u.r[3] = 2 * (a2 * a1 - a0 * a3);  u.r[4] = d + 2 * a2 * a2;          u.r[5] = 2 * (a2 * a3 + a0 * a1);
+    u.r[6] = 2 * (a3 * a1 + a0 * a2);  u.r[7] = 2 * (a3 * a2 - a0 * a1);  u.r[8] = d + 2 * a3 * a3;
 }
 
 // chi = U h  /  chi = U^dag h  on the colour index of one spin component

@@ -48,12 +48,20 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
             if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 2>(geo, a, epi, pl, st);
             return launch_hop_tiled<float, 2>(geo, a, epi, pl, st);
         }
+        if (g->link_storage == HR_LINKS_ONTHEFLY) {
+            if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 3, true>(geo, a, epi, pl, st);
+            return launch_hop_tiled<float, 3, true>(geo, a, epi, pl, st);
+        }
         if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 3>(geo, a, epi, pl, st);
         return launch_hop_tiled<float, 3>(geo, a, epi, pl, st);
     }
     if (g->rep == HR_REP_FUND) {
         if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 2>(geo, a, epi, st);
         return launch_hop_generic<float, 2>(geo, a, epi, st);
+    }
+    if (g->link_storage == HR_LINKS_ONTHEFLY) {
+        if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 3, true>(geo, a, epi, st);
+        return launch_hop_generic<float, 3, true>(geo, a, epi, st);
     }
     if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 3>(geo, a, epi, st);
     return launch_hop_generic<float, 3>(geo, a, epi, st);

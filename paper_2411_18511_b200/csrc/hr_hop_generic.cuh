@@ -70,7 +70,7 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
     IO::store(out_half, first, g.L3h, acc);
 }
 
-template <typename T, int N, int EPI>
+template <typename T, int N, int EPI, bool ONFLY>
 __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
@@ -107,10 +107,10 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     {                                                                                           \
         cplx<T> nb[NC];                                                                         \
         Link<T, N> u;                                                                           \
-        load_link<T, LD_STREAM>(u, a.gauge, g, p, MU, row, h);                                  \
+        load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, p, MU, row, h);                                  \
         IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWF) * rowlen + (HF), stride);        \
         hop_term<T, N, MU, true>(acc, nb, u);                                                   \
-        load_link<T, LD_STREAM>(u, a.gauge, g, 1 - p, MU, ROWB, HB);                            \
+        load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, 1 - p, MU, ROWB, HB);                            \
         IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWB) * rowlen + (HB), stride);        \
         hop_term<T, N, MU, false>(acc, nb, u);                                                  \
     }
@@ -123,14 +123,14 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row, h);
 }
 
-template <typename T, int N>
+template <typename T, int N, bool ONFLY = false>
 inline int launch_hop_generic(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
     dim3 block(128), grid((g.Vh + 127) / 128, a.both ? 2 : 1);
     switch (epi) {
-        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE, ONFLY><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY, ONFLY><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY><<<grid, block, 0, st>>>(g, a); break;
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
     count_launch();

@@ -140,7 +140,7 @@ struct TiledPlan {
 // Shared memory: [16 mbarriers][ring: TILED_RING planes of T1*T2 rows][halo: TILED_HALO buffers of 2*T2 + 2*T1 rows]
 //   halo buffer rows: [x1-1 line: T2 rows][x1+T1 line: T2 rows][x2-1 rows: T1][x2+T2 rows: T1]
 // SHARE: links and phi are also read by the CTA of the other parity (full-lattice launch): keep them in L2
-template <typename T, int N, int EPI, int T1, int T2, bool SHARE>
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY>
 __global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g, HopArgs a, TiledPlan pl) {
     constexpr int NC = 4 * N;
@@ -252,14 +252,14 @@ __global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && 
     {   // links of the first step
         const int row = row0 + xs * g.s0;
         const int r = (xs + x1 + x2 + p) & 1;
-        load_link<T, LP>(uf[0], a.gauge, g, p, 0, row, h);
-        load_link<T, LP>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
-        load_link<T, LP>(uf[1], a.gauge, g, p, 1, row, h);
-        load_link<T, LP>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xs * g.s0, h);
-        load_link<T, LP>(uf[2], a.gauge, g, p, 2, row, h);
-        load_link<T, LP>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xs * g.s0, h);
-        load_link<T, LP>(uf[3], a.gauge, g, p, 3, row, h);
-        load_link<T, LP>(ub[3], a.gauge, g, 1 - p, 3, row, r ? h : (h == 0 ? L3h - 1 : h - 1));
+        load_link_rep<T, LP, ONFLY>(uf[0], a.gauge, g, p, 0, row, h);
+        load_link_rep<T, LP, ONFLY>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
+        load_link_rep<T, LP, ONFLY>(uf[1], a.gauge, g, p, 1, row, h);
+        load_link_rep<T, LP, ONFLY>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xs * g.s0, h);
+        load_link_rep<T, LP, ONFLY>(uf[2], a.gauge, g, p, 2, row, h);
+        load_link_rep<T, LP, ONFLY>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xs * g.s0, h);
+        load_link_rep<T, LP, ONFLY>(uf[3], a.gauge, g, p, 3, row, h);
+        load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, row, r ? h : (h == 0 ? L3h - 1 : h - 1));
     }
 
     for (int k = 0; k < nsteps; ++k) {
@@ -308,35 +308,35 @@ __global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && 
         HR_NB_NEXT(nb0, a0f);
         HR_NB_NEXT(nb1, a0b); HR_NB_NOW(nb0, a0f);
         hop_term<T, N, 0, true>(acc, nb0, uf[0]);
-        load_link<T, LP>(uf[0], a.gauge, g, p, 0, rown, h);
+        load_link_rep<T, LP, ONFLY>(uf[0], a.gauge, g, p, 0, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a1f); HR_NB_NOW(nb1, a0b);
         hop_term<T, N, 0, false>(acc, nb1, ub[0]);
-        load_link<T, LP>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
+        load_link_rep<T, LP, ONFLY>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a1b); HR_NB_NOW(nb0, a1f);
         hop_term<T, N, 1, true>(acc, nb0, uf[1]);
-        load_link<T, LP>(uf[1], a.gauge, g, p, 1, rown, h);
+        load_link_rep<T, LP, ONFLY>(uf[1], a.gauge, g, p, 1, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a2f); HR_NB_NOW(nb1, a1b);
         hop_term<T, N, 1, false>(acc, nb1, ub[1]);
-        load_link<T, LP>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
+        load_link_rep<T, LP, ONFLY>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a2b); HR_NB_NOW(nb0, a2f);
         hop_term<T, N, 2, true>(acc, nb0, uf[2]);
-        load_link<T, LP>(uf[2], a.gauge, g, p, 2, rown, h);
+        load_link_rep<T, LP, ONFLY>(uf[2], a.gauge, g, p, 2, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a3f); HR_NB_NOW(nb1, a2b);
         hop_term<T, N, 2, false>(acc, nb1, ub[2]);
-        load_link<T, LP>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
+        load_link_rep<T, LP, ONFLY>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a3b); HR_NB_NOW(nb0, a3f);
         hop_term<T, N, 3, true>(acc, nb0, uf[3]);
-        load_link<T, LP>(uf[3], a.gauge, g, p, 3, rown, h);
+        load_link_rep<T, LP, ONFLY>(uf[3], a.gauge, g, p, 3, rown, h);
         HR_PIN();
         HR_NB_NOW(nb1, a3b);
         hop_term<T, N, 3, false>(acc, nb1, ub[3]);
-        load_link<T, LP>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
+        load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
 #undef HR_NB_NEXT
 #undef HR_NB_NOW
 #undef HR_PIN
@@ -399,9 +399,9 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) 
     return tiled_plan_shape(hg, both, num_sms, 2, 4, pl);
 }
 
-template <typename T, int N, int EPI, bool SHARE, int T1, int T2>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY>
 inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE>;
+    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY>;
     static bool configured = false;   // per instantiation
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
@@ -414,25 +414,25 @@ inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPla
     return check_launch("hop_tiled_kernel");
 }
 
-template <typename T, int N, int EPI, bool SHARE>
+template <typename T, int N, int EPI, bool SHARE, bool ONFLY>
 inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4>(g, a, pl, st);
+    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4, ONFLY>(g, a, pl, st);
 #if HR_T_F32_WIDE
-    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4>(g, a, pl, st);
+    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4, false>(g, a, pl, st);
 #endif
     set_error("hop_tiled_kernel: no instantiation for a %d x %d tile", pl.t1, pl.t2);
     return HR_EUNSUPPORTED;
 }
 
-template <typename T, int N>
+template <typename T, int N, bool ONFLY = false>
 inline int launch_hop_tiled(const Geo& g, const HopArgs& a, int epi, const TiledPlan& pl, cudaStream_t st) {
     switch (epi) {
-        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE, false>(g, a, pl, st);
+        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE, false, ONFLY>(g, a, pl, st);
         case EPI_AXPY:
-            if (a.both) return launch_hop_tiled_epi<T, N, EPI_AXPY, true>(g, a, pl, st);
-            return launch_hop_tiled_epi<T, N, EPI_AXPY, false>(g, a, pl, st);
-        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV, false>(g, a, pl, st);
-        case EPI_CLOVER_AXPY: return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, false>(g, a, pl, st);
+            if (a.both) return launch_hop_tiled_epi<T, N, EPI_AXPY, true, ONFLY>(g, a, pl, st);
+            return launch_hop_tiled_epi<T, N, EPI_AXPY, false, ONFLY>(g, a, pl, st);
+        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV, false, ONFLY>(g, a, pl, st);
+        case EPI_CLOVER_AXPY: return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, false, ONFLY>(g, a, pl, st);
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
 }

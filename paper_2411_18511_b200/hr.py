@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libhr_dslash.so")
 OK, EINVAL, EUNSUPPORTED, EALIGN, ECUDA = 0, 1, 2, 3, 4
 REP_FUND, REP_ADJ = 0, 1
 PREC_F64, PREC_F32 = 0, 1
-LINKS_FULL, LINKS_COMPRESSED = 0, 1
+LINKS_FULL, LINKS_COMPRESSED, LINKS_ONTHEFLY = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 EVEN, ODD, BOTH = 0, 1, 2
 EO_HOP_OE, EO_HOP_EO, EO_DHAT = 0, 1, 2

@@ -11,11 +11,12 @@ from . import hr
 
 
 class Lattice:
-    def __init__(self, L, rep=hr.REP_FUND, prec=hr.PREC_F64, kernel=hr.KERNEL_AUTO, device="cuda:0"):
+    def __init__(self, L, rep=hr.REP_FUND, prec=hr.PREC_F64, kernel=hr.KERNEL_AUTO, device="cuda:0",
+                 link_storage=hr.LINKS_COMPRESSED):
         self.L = tuple(int(v) for v in L)
         self.V = int(np.prod(self.L))
         self.N = 2 if rep == hr.REP_FUND else 3
-        self.g = hr.geom(self.L, rep, prec, hr.LINKS_COMPRESSED, kernel)
+        self.g = hr.geom(self.L, rep, prec, link_storage, kernel)
         self.device = device
         self.real = hr.np_real(self.g)
         self.cplx = hr.np_complex(self.g)

@@ -120,6 +120,10 @@ def test_work_model_matches_survey_table(L):
     assert hr.hr_dirac_flops_bytes(f32, hr.OP_HOP)[:2] == (624.0, 256.0)
     assert hr.hr_dirac_flops_bytes(f32full, hr.OP_HOP) == (624.0, 384.0, 832.0)
     assert hr.hr_dirac_flops_bytes(adj, hr.OP_HOP) == (744.0, 960.0, 2304.0)
+    adjfly = hr.geom((24,) * 4, hr.REP_ADJ, hr.PREC_F64, hr.LINKS_ONTHEFLY)
+    assert hr.hr_dirac_flops_bytes(adjfly, hr.OP_HOP) == (744.0, 640.0, 9 * 192 + 8 * 32)   # 960 -> 640
+    assert hr.hr_dirac_flops_bytes(adjfly, hr.OP_DIRAC)[:2] == (816.0, 2 * 192 + 4 * 32)
+    assert hr.hr_spinor_bytes(hr.geom((4, 4, 4, 4), hr.REP_FUND, hr.PREC_F64, hr.LINKS_ONTHEFLY)) == 0   # adjoint only
     assert hr.hr_dirac_flops_bytes(f64, hr.OP_DIRAC)[:2] == (672.0, 384.0)
     assert hr.hr_dirac_flops_bytes(f64full, hr.OP_DIRAC)[:2] == (672.0, 512.0)
     assert hr.hr_dirac_flops_bytes(adj, hr.OP_DIRAC)[:2] == (816.0, 672.0)

@@ -185,6 +185,24 @@ def test_tiled_kernel_segment_lengths(hr, orc, monkeypatch, nseg, rep, N):
         assert rel(got[k], want[k]) <= TOL[0], (k, nseg)
 
 
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (8, 2, 8, 6), (6, 2, 4, 12)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_adjoint_on_the_fly_links(hr, orc, L, prec):
+    """the adjoint operators handed the FUNDAMENTAL gauge field (HR_LINKS_ONTHEFLY) rebuild
+    R in registers; expected values = the oracle's adjoint operators on the oracle's R(U)"""
+    m0 = -0.3
+    Uf = rounded(inputs.haar_gauge(L, 1), prec)
+    R, _ = orc.represent(Uf)
+    psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
+    want = oracle_ops(orc, L, 1, R, psi, m0)
+    from paper_2411_18511_b200.lattice import Lattice
+    for kernel in kernels_for(hr, L, 1, prec):
+        lat = Lattice(L, hr.REP_ADJ, prec, kernel, link_storage=hr.LINKS_ONTHEFLY)
+        got = gpu_ops(hr, lat, lat.put_gauge_fund(Uf), psi, m0)
+        for k in want:
+            assert rel(got[k], want[k]) <= TOL[prec], (k, kernel)
+
+
 # ------------------------------------------------------------------ config 1
 @pytest.mark.parametrize("prec", [0, 1])
 def test_config1_16to4_dhat_100_repetitions(hr, orc, prec):
@@ -229,6 +247,13 @@ def test_config2_24to4_adjoint(hr, orc):
     got = gpu_ops(hr, lat, R_dev, psi, m0)
     for k in want:
         assert rel(got[k], want[k]) <= 1e-13, k
+    # the same operators with the links rebuilt on the fly from the fundamental field, both kernels
+    from paper_2411_18511_b200.lattice import Lattice
+    for kernel in kernels_for(hr, L, 1, 0):
+        fly = Lattice(L, hr.REP_ADJ, hr.PREC_F64, kernel, link_storage=hr.LINKS_ONTHEFLY)
+        got = gpu_ops(hr, fly, fly.put_gauge_fund(Uf), psi, m0)
+        for k in want:
+            assert rel(got[k], want[k]) <= 1e-13, (k, kernel, "on the fly")
 
 
 # ------------------------------------------------------------------ config 3
@@ -428,3 +453,49 @@ def test_native_library_is_the_one_loaded(hr):
     assert hr.hr_launch_count() == n0 + 1
     with open("/proc/self/maps") as f:
         assert "paper_2411_18511_b200/libhr_dslash.so" in f.read()
+
+
+# ------------------------------------------------------------------ bounds (compute-sanitizer is closed on this pool)
+@pytest.mark.parametrize("L,rep", [((8, 2, 8, 6), 0), ((8, 4, 4, 16), 0), ((6, 2, 4, 12), 1), ((2, 2, 2, 2), 0), ((2, 4, 6, 8), 1)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_operators_write_only_their_output(hr, L, rep, prec):
+    """every output / temporary buffer sits between two guard regions holding a byte pattern; after all hop
+    variants (both kernels, every epilogue) the guards are intact and bytes outside the output are unchanged"""
+    import torch
+    N = 2 if rep == 0 else 3
+    U = inputs.haar_gauge(L, 1)
+    psi = inputs.gaussian_spinor(L, N, 2)
+    G = 1 << 16
+    for kernel in kernels_for(hr, L, rep, prec):
+        lat = lattice(hr, L, rep, prec, kernel)
+        Uf = lat.put_gauge_fund(U)
+        U_dev = Uf if rep == 0 else lat.represent(Uf)
+        psi_dev = lat.put_spinor(psi)
+        half = lat.half
+        arena = torch.full((4 * G + 2 * half + half,), 0xA5, dtype=torch.uint8, device="cuda")
+        out = arena[G:G + 2 * half]
+        tmp = arena[3 * G + 2 * half:3 * G + 3 * half]
+        st = hr.stream_ptr()
+
+        def guards_ok():
+            torch.cuda.synchronize()
+            a = arena
+            return bool((a[:G] == 0xA5).all() and (a[G + 2 * half:3 * G + 2 * half] == 0xA5).all() and (a[3 * G + 3 * half:] == 0xA5).all())
+
+        hr.hr_dirac_apply(lat.g, -0.2, U_dev, psi_dev, out, st)
+        assert guards_ok(), ("dirac", kernel)
+        out.fill_(0xA5)
+        hr.hr_dirac_eo_apply(lat.g, hr.EO_HOP_OE, 0.0, U_dev, None, None, lat.even(psi_dev), out[half:], None, st)
+        assert guards_ok() and bool((out[:half] == 0xA5).all()), ("hop_oe", kernel)
+        out.fill_(0xA5)
+        hr.hr_dirac_eo_apply(lat.g, hr.EO_DHAT, -0.2, U_dev, None, None, lat.even(psi_dev), out[:half], tmp, st)
+        assert guards_ok() and bool((out[half:] == 0xA5).all()), ("dhat", kernel)
+        if rep == 0:
+            fwd, inv = lat.clover_build(-0.25, 1.2, Uf)
+            out.fill_(0xA5)
+            tmp.fill_(0xA5)
+            hr.hr_dirac_eo_apply(lat.g, hr.EO_DHAT, -0.25, U_dev, fwd, inv, lat.even(psi_dev), out[:half], tmp, st)
+            assert guards_ok() and bool((out[half:] == 0xA5).all()), ("dhat clover", kernel)
+            out.fill_(0xA5)
+            hr.hr_clover_apply(lat.g, hr.ODD, inv, lat.odd(psi_dev), out[half:], st)
+            assert guards_ok() and bool((out[:half] == 0xA5).all()), ("clover odd", kernel)
