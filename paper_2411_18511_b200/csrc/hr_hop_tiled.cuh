@@ -45,6 +45,12 @@ constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, two b
 #ifndef HR_T_LINKPOL_F32
 #define HR_T_LINKPOL_F32 LD_STREAM
 #endif
+#ifndef HR_T_PHIPOL_SHARE
+#define HR_T_PHIPOL_SHARE LD_KEEP
+#endif
+#ifndef HR_T_LINKPOL_SHARE
+#define HR_T_LINKPOL_SHARE LD_KEEP
+#endif
 #ifndef HR_T_F32_WIDE
 #define HR_T_F32_WIDE 1
 #endif
@@ -140,20 +146,24 @@ struct TiledPlan {
 // Shared memory: [16 mbarriers][ring: TILED_RING planes of T1*T2 rows][halo: TILED_HALO buffers of 2*T2 + 2*T1 rows]
 //   halo buffer rows: [x1-1 line: T2 rows][x1+T1 line: T2 rows][x2-1 rows: T1][x2+T2 rows: T1]
 // SHARE: links and phi are also read by the CTA of the other parity (full-lattice launch): keep them in L2
-template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY>
+// L3H: compile-time L3/2 (0 = read it from the geometry): the strides between the 16-byte chunks of a site are then
+// immediates in every LDS / LDG / STG (about a quarter fewer instructions per site)
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H>
 __global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
-    hop_tiled_kernel(Geo g, HopArgs a, TiledPlan pl) {
+    hop_tiled_kernel(Geo g_in, HopArgs a, TiledPlan pl) {
+    Geo g = g_in;
+    if (L3H > 0) g.L3h = L3H;
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
     constexpr int TR = T1 * T2;            // tile rows
     constexpr int HR = 2 * T2 + 2 * T1;    // halo rows
-    constexpr int LP = SHARE ? LD_KEEP : (sizeof(T) == 4 ? HR_T_LINKPOL_F32 : HR_T_LINKPOL_F64);
+    constexpr int LP = SHARE ? HR_T_LINKPOL_SHARE : (sizeof(T) == 4 ? HR_T_LINKPOL_F32 : HR_T_LINKPOL_F64);
     constexpr bool PIN = sizeof(T) == 4 ? HR_T_PIN_F32 : HR_T_PIN_F64;
     constexpr bool NBDB = sizeof(T) == 4 ? HR_T_NBDB_F32 : HR_T_NBDB_F64;
     extern __shared__ __align__(128) char smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
     char* ring = smem + 128;
-    const int rowb = pl.rowb;
+    const int rowb = L3H > 0 ? SiteIO<T, 4 * N>::NCH * L3H * 16 : pl.rowb;
     const int planeb = TR * rowb;
     const int halob = HR * rowb;
     char* halo = ring + TILED_RING * planeb;
@@ -348,7 +358,7 @@ __global__ void __launch_bounds__(tiled_max_threads(T1, T2), (sizeof(T) == 4 && 
             mbar_arrive(bar_hempty + 8 * hb);
         }
         // (requesting phi before the eight terms was measured slower at 48^4: 412 -> 425 us for fp64 H3)
-        if (active) hop_epilogue<T, N, EPI, LP>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
+        if (active) hop_epilogue<T, N, EPI, (SHARE ? HR_T_PHIPOL_SHARE : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
     }
 }
 
@@ -399,9 +409,9 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) 
     return tiled_plan_shape(hg, both, num_sms, 2, 4, pl);
 }
 
-template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY>
-inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY>;
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H>
+inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
+    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H>;
     static bool configured = false;   // per instantiation
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
@@ -412,6 +422,13 @@ inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPla
     kern<<<grid, pl.nconsumer + 32, pl.smem, st>>>(g, a, pl);
     count_launch();
     return check_launch("hop_tiled_kernel");
+}
+
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY>
+inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
+    // (measured at 48^4: fp64 hop 219.3 -> 216.1 us, H3 411 -> 408; the fp32 4x4 H3 got slower, so fp64 only)
+    if (N == 2 && sizeof(T) == 8 && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, ((N == 2 && sizeof(T) == 8) ? 24 : 0)>(g, a, pl, st);
+    return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, 0>(g, a, pl, st);
 }
 
 template <typename T, int N, int EPI, bool SHARE, bool ONFLY>
