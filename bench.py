@@ -37,6 +37,7 @@ def parse():
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-other", action="store_true", help="skip the 16^4 / 24^4 side report")
     return ap.parse_args()
 
 
@@ -249,6 +250,15 @@ def run_ours(args):
     if not args.no_e2e:
         e2e = run_e2e(args, ranks, hr, S, psi, L, m0, model)
 
+    # ---- the parity configs, timed for the record (not part of the step): configs[1] 16^4 Dhat as a CUDA graph of
+    # 100 repetitions (launch-bound: the lattice fits L2), configs[2] 24^4 adjoint with stored and on-the-fly links
+    other = None
+    if not args.no_other and ranks.rank == 0:
+        try:
+            other = other_configs(hr, inputs, Lattice)
+        except Exception as e:  # never let the side report break the bench line
+            other = {"error": repr(e)}
+
     # ---- the oracle beside it (rank 0, N = 1 only)
     cpu = None
     if not args.no_cpu and ranks.rank == 0 and ranks.world == 1:
@@ -266,10 +276,84 @@ def run_ours(args):
                        "parallelism": "replicas x%d (no data-path collective)" % ranks.world},
             "gflops": round(step_flops * K / tmax / 1e9 * ranks.world, 1),
             "gsites_per_s": round(step_sites * K / tmax / 1e9 * ranks.world, 3),
-            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu, "ops": op_report,
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu, "ops": op_report, "other_configs": other,
         }
         print(json.dumps(line))
     ranks.close()
+
+
+def other_configs(hr, inputs, Lattice):
+    """per-apply device time of BASELINE.json configs[1] (16^4 fund, Dhat, 100 repetitions replayed as one CUDA graph)
+    and configs[2] (24^4 adjoint: hop, D, Dhat; links stored as 3x3 reals and rebuilt on the fly)"""
+    import torch
+    out = {}
+    reps = 100
+
+    def timed(fn, n):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    # configs[1]
+    L = (16,) * 4
+    U = inputs.weak_gauge(L, 0.3, 1)
+    psi = inputs.gaussian_spinor(L, 2, 2)
+    for prec, tag in ((hr.PREC_F64, "f64"), (hr.PREC_F32, "f32")):
+        lat = Lattice(L, hr.REP_FUND, prec)
+        g = lat.g
+        U_dev, p_dev, o_dev, tmp = lat.put_gauge_fund(U), lat.put_spinor(psi), lat.empty_spinor(), lat.empty_spinor(hr.ODD)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            st = hr.stream_ptr(side)
+            call = lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.1, U_dev, None, None, lat.even(p_dev), lat.even(o_dev), tmp, st)
+            call()
+            side.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                stc = hr.stream_ptr(torch.cuda.current_stream())
+                for _ in range(reps):
+                    hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.1, U_dev, None, None, lat.even(p_dev), lat.even(o_dev), tmp, stc)
+        torch.cuda.current_stream().wait_stream(side)
+        ms_graph = timed(graph.replay, 5) / reps
+        st0 = hr.stream_ptr()
+        ms_plain = timed(lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.1, U_dev, None, None, lat.even(p_dev), lat.even(o_dev), tmp, st0), reps)
+        f, bc, _ = hr.hr_dirac_flops_bytes(g, hr.OP_DHAT)
+        sites = 16 ** 4 // 2
+        out["config1_16^4_dhat_" + tag] = {"us_per_apply_graph": round(ms_graph * 1e3, 2), "us_per_apply_launches": round(ms_plain * 1e3, 2),
+                                          "gsites_per_s": round(sites / ms_graph / 1e6, 3), "gflops": round(f * sites / ms_graph / 1e6, 1),
+                                          "gbs_requested_from_l2": round(bc * sites / ms_graph / 1e6, 1), "kernel": hr.hr_kernel_name(g),
+                                          "note": "fits L2 (24 MiB): HBM fraction not meaningful"}
+    # configs[2]
+    L = (24,) * 4
+    V = 24 ** 4
+    Uf = inputs.haar_gauge(L, 1)
+    psi = inputs.gaussian_spinor(L, 3, 2)
+    for storage, tag in ((hr.LINKS_COMPRESSED, "stored"), (hr.LINKS_ONTHEFLY, "onthefly")):
+        lat = Lattice(L, hr.REP_ADJ, hr.PREC_F64, hr.KERNEL_AUTO, link_storage=storage)
+        g = lat.g
+        Uf_dev = lat.put_gauge_fund(Uf)
+        U_dev = lat.represent(Uf_dev) if storage == hr.LINKS_COMPRESSED else Uf_dev
+        p_dev, o_dev, tmp = lat.put_spinor(psi), lat.empty_spinor(), lat.empty_spinor(hr.ODD)
+        st0 = hr.stream_ptr()
+        for name, op, sites, fn in (
+                ("hop", hr.OP_HOP, V // 2, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_OE, 0.0, U_dev, None, None, lat.even(p_dev), lat.odd(o_dev), None, st0)),
+                ("dirac", hr.OP_DIRAC, V, lambda: hr.hr_dirac_apply(g, -0.3, U_dev, p_dev, o_dev, st0)),
+                ("dhat", hr.OP_DHAT, V // 2, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.3, U_dev, None, None, lat.even(p_dev), lat.even(o_dev), tmp, st0))):
+            ms = timed(fn, 50)
+            f, bc, _ = hr.hr_dirac_flops_bytes(g, op)
+            out["config2_24^4_adj_%s_%s_f64" % (name, tag)] = {"us_per_apply": round(ms * 1e3, 2), "gsites_per_s": round(sites / ms / 1e6, 3),
+                                                            "gflops": round(f * sites / ms / 1e6, 1), "gbs": round(bc * sites / ms / 1e6, 1),
+                                                            "kernel": hr.hr_kernel_name(g),
+                                                            "note": "working set 0.1-0.2 GB: partly L2-resident, HBM fraction indicative only"}
+    return out
 
 
 def run_e2e(args, ranks, hr, S, psi, L, m0, model):

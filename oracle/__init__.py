@@ -177,3 +177,37 @@ def dirac_eo_clover(L, U, A, Ainv, psi, nthreads=1):
     out = np.zeros_like(psi)
     lib().orc_dirac_eo_clover(_L(L), _p(U), _p(A), _p(Ainv), _p(psi), _p(out), int(nthreads))
     return out
+
+
+# ------------------------------------------------------------------ O8: conjugate gradient on the normal equations
+def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1):
+    """O8 (the HMC inverts the even-odd operator): solve
+        Dhat^dag Dhat x = b        on the even sites,   Dhat^dag = gamma5 Dhat gamma5  (pin P2),
+    by the textbook conjugate-gradient iteration (Hestenes-Stiefel) from x = 0, in the order
+        r = b, p = r;  loop:  q = Dhat^dag Dhat p;  alpha = <r,r>/<p,q>;  x += alpha p;  r -= alpha q;
+                              stop when |r| <= tol |b|;  beta = <r,r>_new/<r,r>_old;  p = r + beta p.
+    b, x: complex [V,4,N] with zero odd entries.  Returns (x, iterations, |r|/|b|).  Plain numpy on top of
+    dirac_eo; no preconditioning, no restarts, no reordering."""
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+
+    def M(v):
+        t = dirac_eo(L, rep, m0, U, v, nthreads)
+        return g5 * dirac_eo(L, rep, m0, U, g5 * t, nthreads)
+
+    b = _c(b)
+    x = np.zeros_like(b)
+    r = b.copy()
+    p = r.copy()
+    rr = float(np.vdot(r, r).real)
+    bb = rr
+    it = 0
+    while it < max_iter and rr > tol * tol * bb:
+        q = M(p)
+        alpha = rr / float(np.vdot(p, q).real)
+        x += alpha * p
+        r -= alpha * q
+        rr_new = float(np.vdot(r, r).real)
+        p = r + (rr_new / rr) * p
+        rr = rr_new
+        it += 1
+    return x, it, float(np.sqrt(rr / bb))

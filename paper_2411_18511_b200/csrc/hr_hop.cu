@@ -27,6 +27,9 @@ bool tiled_supported(const hr_geom* g) {
 bool tiled_chosen(const hr_geom* g) {
     if (g->kernel == HR_KERNEL_GENERIC || !tiled_supported(g)) return false;
     if (g->kernel == HR_KERNEL_TILED) return true;
+    // adjoint rows are 1.5x longer: the 2x4 tile then takes > 200 KiB of shared memory, which starves the L1 the link
+    // loads go through; measured slower than the generic kernel at every size (L = 16..40), so AUTO keeps generic
+    if (g->rep == HR_REP_ADJ) return false;
     const double v = (double)g->L[0] * g->L[1] * g->L[2] * g->L[3];
     return v >= TILED_AUTO_MIN_SITES;
 }
