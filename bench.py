@@ -256,6 +256,7 @@ def run_ours(args):
     if not args.no_other and ranks.rank == 0:
         try:
             other = other_configs(hr, inputs, Lattice)
+            other.update(cg_report(hr, S, m0))
         except Exception as e:  # never let the side report break the bench line
             other = {"error": repr(e)}
 
@@ -353,6 +354,35 @@ def other_configs(hr, inputs, Lattice):
                                                             "gflops": round(f * sites / ms / 1e6, 1), "gbs": round(bc * sites / ms / 1e6, 1),
                                                             "kernel": hr.hr_kernel_name(g),
                                                             "note": "working set 0.1-0.2 GB: partly L2-resident, HBM fraction indicative only"}
+    return out
+
+
+def cg_report(hr, S, m0):
+    """hr_cg_solve on the bench lattice: 20 iterations of CG on Dhat^dag Dhat, no convergence read-back
+    in between; bytes per even site and iteration = 2 (5S + 16G) for the two Dhat + 11 S for the three vector kernels"""
+    import torch
+    out = {}
+    for tag in ("f64", "f32"):
+        s = S[tag]
+        lat, g = s["lat"], s["lat"].g
+        ws = hr.device_buffer(hr.hr_cg_workspace_bytes(g), lat.device)
+        x = lat.empty_spinor(hr.EVEN)
+        st = hr.stream_ptr()
+        hr.hr_cg_solve(g, m0, s["U"], None, None, lat.even(s["psi"]), x, ws, 1e-30, 3, 1000, st)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n = 20
+        e0.record()
+        it, rel = hr.hr_cg_solve(g, m0, s["U"], None, None, lat.even(s["psi"]), x, ws, 1e-30, n, 1000, st)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / max(it, 1)
+        _, bc, _ = hr.hr_dirac_flops_bytes(g, hr.OP_DHAT)
+        w = 8 if tag == "f64" else 4
+        bytes_site = 2 * bc + 11 * 16 * w
+        Vh = lat.V // 2
+        out["cg_48^4_" + tag] = {"ms_per_iteration": round(ms, 4), "iterations": it, "relres_after": rel,
+                                 "gbs": round(bytes_site * Vh / ms / 1e6, 1), "bytes_per_even_site_per_iteration": bytes_site}
+        del ws, x
     return out
 
 

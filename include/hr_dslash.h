@@ -134,6 +134,21 @@ enum {
 int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, double* bytes_compulsory,
                          double* bytes_requested);
 
+/* S1 ("a range of inverters", PAPER.md:39 the even-odd operator is the one
+ * "used mainly in the HMC"): conjugate gradient on the normal equations of the even-odd operator,
+ *       Dhat^dag Dhat x = b      on the even sites,      Dhat^dag = gamma5 Dhat gamma5,
+ * Dhat as in hr_dirac_eo_apply(op = HR_EO_DHAT) (with clover if both block fields are given), started from x = 0,
+ * textbook Hestenes-Stiefel recurrences in the field precision with double-precision, fixed-order reductions.
+ * Stops when |r| <= tol |b| or after max_iter iterations; the residual is read back every check_every iterations
+ * (so up to check_every - 1 extra iterations are made) — the one call of this library that synchronises `stream`.
+ *   b, x: even half fields (device); workspace: device, hr_cg_workspace_bytes(g) bytes; iters, relres: HOST
+ *   outputs (may be NULL): iterations made and the recurrence residual |r|/|b|.
+ * Returns HR_OK also when max_iter was reached without convergence (check *relres). */
+size_t hr_cg_workspace_bytes(const hr_geom* g);
+int hr_cg_solve(const hr_geom* g, double m0, const void* u, const void* clover_fwd, const void* clover_inv,
+                const void* b, void* x, void* workspace, double tol, int max_iter, int check_every,
+                int* iters, double* relres, void* stream);
+
 /* ---- host-buffer entry points (the end-to-end path a user without device buffers calls) ----
  * All data pointers are HOST pointers to canonical arrays (pinned memory makes the copies asynchronous);
  * `workspace` is a DEVICE buffer of at least hr_host_workspace_bytes(g) bytes.  The call uploads gauge

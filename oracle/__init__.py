@@ -180,19 +180,23 @@ def dirac_eo_clover(L, U, A, Ainv, psi, nthreads=1):
 
 
 # ------------------------------------------------------------------ O8: conjugate gradient on the normal equations
-def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1):
+def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1, A=None, Ainv=None):
     """O8 (the HMC inverts the even-odd operator): solve
         Dhat^dag Dhat x = b        on the even sites,   Dhat^dag = gamma5 Dhat gamma5  (pin P2),
     by the textbook conjugate-gradient iteration (Hestenes-Stiefel) from x = 0, in the order
         r = b, p = r;  loop:  q = Dhat^dag Dhat p;  alpha = <r,r>/<p,q>;  x += alpha p;  r -= alpha q;
                               stop when |r| <= tol |b|;  beta = <r,r>_new/<r,r>_old;  p = r + beta p.
     b, x: complex [V,4,N] with zero odd entries.  Returns (x, iterations, |r|/|b|).  Plain numpy on top of
-    dirac_eo; no preconditioning, no restarts, no reordering."""
+    dirac_eo (dirac_eo_clover when A, Ainv are given); no preconditioning, no restarts, no reordering."""
     g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
 
+    def Dhat(v):   # O3, or O7 when the dense clover matrices A, A^-1 are given (fundamental representation)
+        if A is None:
+            return dirac_eo(L, rep, m0, U, v, nthreads)
+        return dirac_eo_clover(L, U, A, Ainv, v, nthreads)
+
     def M(v):
-        t = dirac_eo(L, rep, m0, U, v, nthreads)
-        return g5 * dirac_eo(L, rep, m0, U, g5 * t, nthreads)
+        return g5 * Dhat(g5 * Dhat(v))
 
     b = _c(b)
     x = np.zeros_like(b)

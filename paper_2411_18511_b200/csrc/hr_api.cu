@@ -17,6 +17,11 @@ int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStr
 int run_clover_build(const Geo& g, int prec, double diag, double csw, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
 
+// hr_solver.cu
+size_t cg_workspace_bytes(const hr_geom* g);
+int run_cg(const hr_geom* g, double m0, const void* u, const void* cf, const void* ci, const void* b, void* x, void* workspace, double tol,
+           int max_iter, int check_every, int* iters_out, double* relres_out, cudaStream_t st);
+
 static thread_local char g_err[512] = "";
 static std::atomic<unsigned long long> g_launches{0};
 
@@ -239,6 +244,28 @@ int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void
     if (parity < HR_EVEN || parity > HR_BOTH) { set_error("hr_clover_apply: parity %d", parity); return HR_EINVAL; }
     HR_TRY(check_ptr(blocks, "blocks")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
     return run_clover_apply(make_geo(g), g->prec, parity, blocks, in, out, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------- S1
+size_t hr_cg_workspace_bytes(const hr_geom* g) {
+    if (!geom_ok(g)) return 0;
+    return cg_workspace_bytes(g);
+}
+
+int hr_cg_solve(const hr_geom* g, double m0, const void* u, const void* clover_fwd, const void* clover_inv,
+                const void* b, void* x, void* workspace, double tol, int max_iter, int check_every,
+                int* iters, double* relres, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(b, "b")); HR_TRY(check_ptr(x, "x")); HR_TRY(check_ptr(workspace, "workspace"));
+    if (!(tol > 0.0) || max_iter < 0 || check_every < 1) { set_error("hr_cg_solve: tol must be > 0, max_iter >= 0, check_every >= 1"); return HR_EINVAL; }
+    if ((clover_fwd == nullptr) != (clover_inv == nullptr)) { set_error("hr_cg_solve: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
+    const size_t half = half_spinor_bytes(g);
+    if (overlap(b, half, x, half)) { set_error("hr_cg_solve: x aliases b"); return HR_EINVAL; }
+    if (overlap(workspace, cg_workspace_bytes(g), x, half) || overlap(workspace, cg_workspace_bytes(g), b, half)) {
+        set_error("hr_cg_solve: workspace aliases b or x");
+        return HR_EINVAL;
+    }
+    return run_cg(g, m0, u, clover_fwd, clover_inv, b, x, workspace, tol, max_iter, check_every, iters, relres, (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------- M1

@@ -1,0 +1,243 @@
+// hr_solver.cu — conjugate gradient on the normal equations of the even-odd operator (
+// PAPER.md:13 "range of inverters", PAPER.md:39 the even-odd operator "used mainly in the HMC"):
+//     Dhat^dag Dhat x = b   on the even sites,   Dhat^dag = gamma5 Dhat gamma5.
+// The operator applications are hr_dirac_eo_apply (the hopping kernels); this file adds the linear algebra
+// between them as three fused streaming kernels and keeps every scalar on the device, so an iteration is
+// enqueued without a host round trip.  Reductions are two-stage with a fixed order (per-block partial sums in
+// double, then one block sums them): results are bitwise reproducible from run to run.
+#include "hr_common.cuh"
+
+namespace hr {
+
+constexpr int CG_BLOCK = 256;
+constexpr int CG_MAX_PARTIALS = 148 * 8;
+
+// device scalars of the iteration
+struct CgScalars {
+    double rr;      // <r,r>
+    double rr_new;
+    double pap;     // <p, Dhat^dag Dhat p> = |Dhat p|^2
+    double bb;      // <b,b>
+    double alpha, beta;
+};
+
+// sign of gamma5 = diag(1,1,-1,-1) on 16-byte chunk number `chunk` of a half field laid out [row][NCH][L3h]
+__device__ __forceinline__ double g5_sign(size_t chunk, int L3h, int NCH) {
+    const int c = (int)((chunk / (size_t)L3h) % (size_t)NCH);
+    return c < NCH / 2 ? 1.0 : -1.0;
+}
+
+template <typename T> struct RealsPerChunk { static constexpr int value = 16 / sizeof(T); };
+
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sm[CG_BLOCK / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < CG_BLOCK / 32; ++i) t += sm[i];
+    return t;   // valid in thread 0
+}
+
+// s = gamma5 t, partial[blockIdx] = sum |t|^2            (t = Dhat p;  |t|^2 = <p, Dhat^dag Dhat p>)
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_g5_norm_kernel(size_t nchunks, int L3h, int NCH, const void* __restrict__ t_, void* __restrict__ s_,
+                                                              double* __restrict__ partial) {
+    typedef typename Chunk<T>::type chunk_t;
+    constexpr int R = RealsPerChunk<T>::value;
+    const chunk_t* t = reinterpret_cast<const chunk_t*>(t_);
+    chunk_t* s = reinterpret_cast<chunk_t*>(s_);
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
+        T e[R];
+        chunk_to_reals(ldg16<LD_STREAM>(t + i), e);
+        const T sg = (T)g5_sign(i, L3h, NCH);
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            acc += (double)e[k] * (double)e[k];
+            e[k] *= sg;
+        }
+        s[i] = reals_to_chunk(e);
+    }
+    const double tot = block_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
+// which scalar a finalize step produces
+enum { CG_FIN_INIT = 0, CG_FIN_PAP = 1, CG_FIN_RR = 2 };
+
+// one block: sums the partials in index order and updates the scalars
+__global__ void __launch_bounds__(CG_BLOCK) cg_finalize_kernel(int what, int npartial, const double* __restrict__ partial, CgScalars* sc) {
+    __shared__ double sm[CG_BLOCK];
+    double v = 0.0;
+    for (int i = threadIdx.x; i < npartial; i += CG_BLOCK) v += partial[i];
+    sm[threadIdx.x] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int i = 0; i < CG_BLOCK; ++i) t += sm[i];
+        if (what == CG_FIN_INIT) {
+            sc->rr = t; sc->bb = t; sc->rr_new = t; sc->alpha = 0.0; sc->beta = 0.0; sc->pap = 0.0;
+        } else if (what == CG_FIN_PAP) {
+            sc->pap = t;
+            sc->alpha = t > 0.0 ? sc->rr / t : 0.0;
+        } else {
+            sc->rr_new = t;
+            sc->beta = sc->rr > 0.0 ? t / sc->rr : 0.0;
+            sc->rr = t;
+        }
+    }
+}
+
+// x += alpha p;  r -= alpha gamma5 w;  partial = sum |r|^2          (w = Dhat gamma5 Dhat p, so gamma5 w = Dhat^dag Dhat p)
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_update_kernel(size_t nchunks, int L3h, int NCH, const CgScalars* __restrict__ sc, const void* __restrict__ p_,
+                                                             const void* __restrict__ w_, void* __restrict__ x_, void* __restrict__ r_,
+                                                             double* __restrict__ partial) {
+    typedef typename Chunk<T>::type chunk_t;
+    constexpr int R = RealsPerChunk<T>::value;
+    const chunk_t* p = reinterpret_cast<const chunk_t*>(p_);
+    const chunk_t* w = reinterpret_cast<const chunk_t*>(w_);
+    chunk_t* x = reinterpret_cast<chunk_t*>(x_);
+    chunk_t* r = reinterpret_cast<chunk_t*>(r_);
+    const T alpha = (T)sc->alpha;
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
+        T ep[R], ew[R], ex[R], er[R];
+        chunk_to_reals(ldg16<LD_KEEP>(p + i), ep);
+        chunk_to_reals(ldg16<LD_STREAM>(w + i), ew);
+        chunk_to_reals(x[i], ex);
+        chunk_to_reals(r[i], er);
+        const T sg = (T)g5_sign(i, L3h, NCH);
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            ex[k] = fma(alpha, ep[k], ex[k]);
+            er[k] = fma(-alpha * sg, ew[k], er[k]);
+            acc += (double)er[k] * (double)er[k];
+        }
+        x[i] = reals_to_chunk(ex);
+        r[i] = reals_to_chunk(er);
+    }
+    const double tot = block_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
+// p = r + beta p
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_direction_kernel(size_t nchunks, const CgScalars* __restrict__ sc, const void* __restrict__ r_, void* __restrict__ p_) {
+    typedef typename Chunk<T>::type chunk_t;
+    constexpr int R = RealsPerChunk<T>::value;
+    const chunk_t* r = reinterpret_cast<const chunk_t*>(r_);
+    chunk_t* p = reinterpret_cast<chunk_t*>(p_);
+    const T beta = (T)sc->beta;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
+        T er[R], ep[R];
+        chunk_to_reals(r[i], er);
+        chunk_to_reals(p[i], ep);
+#pragma unroll
+        for (int k = 0; k < R; ++k) ep[k] = fma(beta, ep[k], er[k]);
+        p[i] = reals_to_chunk(ep);
+    }
+}
+
+// r = b, p = b, x = 0, partial = sum |b|^2
+template <typename T>
+__global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(size_t nchunks, const void* __restrict__ b_, void* __restrict__ x_, void* __restrict__ r_,
+                                                           void* __restrict__ p_, double* __restrict__ partial) {
+    typedef typename Chunk<T>::type chunk_t;
+    constexpr int R = RealsPerChunk<T>::value;
+    const chunk_t* b = reinterpret_cast<const chunk_t*>(b_);
+    chunk_t* x = reinterpret_cast<chunk_t*>(x_);
+    chunk_t* r = reinterpret_cast<chunk_t*>(r_);
+    chunk_t* p = reinterpret_cast<chunk_t*>(p_);
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
+        T e[R], z[R];
+        const chunk_t v = b[i];
+        chunk_to_reals(v, e);
+#pragma unroll
+        for (int k = 0; k < R; ++k) { acc += (double)e[k] * (double)e[k]; z[k] = (T)0; }
+        r[i] = v;
+        p[i] = v;
+        x[i] = reals_to_chunk(z);
+    }
+    const double tot = block_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
+// ------------------------------------------------------------------ host driver
+static size_t up256s(size_t n) { return (n + 255) & ~(size_t)255; }
+
+size_t cg_workspace_bytes(const hr_geom* g) {
+    const size_t half = hr_spinor_bytes(g, HR_EVEN);
+    return 256 + up256s(CG_MAX_PARTIALS * sizeof(double)) + 5 * up256s(half);
+}
+
+template <typename T>
+static int cg_run(const hr_geom* g, double m0, const void* u, const void* cf, const void* ci, const void* b, void* x, void* workspace,
+                  double tol, int max_iter, int check_every, int* iters_out, double* relres_out, cudaStream_t st) {
+    const Geo geo = make_geo(g);
+    const int NCH = spinor_chunks(g->rep, g->prec);
+    const size_t half = hr_spinor_bytes(g, HR_EVEN);
+    const size_t nchunks = half / 16;
+    char* w8 = (char*)workspace;
+    CgScalars* sc = (CgScalars*)w8; w8 += 256;
+    double* partial = (double*)w8; w8 += up256s(CG_MAX_PARTIALS * sizeof(double));
+    void* r = w8; w8 += up256s(half);
+    void* p = w8; w8 += up256s(half);
+    void* t = w8; w8 += up256s(half);
+    void* w = w8; w8 += up256s(half);
+    void* tmp = w8;
+    int nblk = (int)((nchunks + CG_BLOCK - 1) / CG_BLOCK);
+    if (nblk > CG_MAX_PARTIALS) nblk = CG_MAX_PARTIALS;
+    void* strm = (void*)st;
+
+    cg_init_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, b, x, r, p, partial);
+    cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_INIT, nblk, partial, sc);
+    count_launch(2);
+    int rc = check_launch("cg_init_kernel");
+    if (rc != HR_OK) return rc;
+
+    CgScalars h;
+    int it = 0;
+    double relres = 1.0;
+    bool done = false;
+    while (!done) {
+        // convergence is read back every check_every iterations (the only host round trip of the solve)
+        if (it % check_every == 0 || it >= max_iter) {
+            cudaError_t e = cudaMemcpyAsync(&h, sc, sizeof(h), cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) { set_error("hr_cg_solve: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+            relres = h.bb > 0.0 ? sqrt(h.rr / h.bb) : 0.0;
+            if (h.bb == 0.0 || h.rr <= tol * tol * h.bb || it >= max_iter) { done = true; break; }
+            if (!(h.rr == h.rr)) { set_error("hr_cg_solve: residual is NaN at iteration %d", it); return HR_ECUDA; }
+        }
+        // t = Dhat p ; s = gamma5 t (into w), |t|^2 ; t = Dhat s ; x += alpha p, r -= alpha gamma5 t ; p = r + beta p
+        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u, cf, ci, p, t, tmp, strm);
+        if (rc != HR_OK) return rc;
+        cg_g5_norm_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, t, w, partial);
+        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_PAP, nblk, partial, sc);
+        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u, cf, ci, w, t, tmp, strm);
+        if (rc != HR_OK) return rc;
+        cg_update_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, sc, p, t, x, r, partial);
+        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_RR, nblk, partial, sc);
+        cg_direction_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, sc, r, p);
+        count_launch(5);
+        rc = check_launch("cg iteration");
+        if (rc != HR_OK) return rc;
+        ++it;
+    }
+    if (iters_out) *iters_out = it;
+    if (relres_out) *relres_out = relres;
+    return HR_OK;
+}
+
+int run_cg(const hr_geom* g, double m0, const void* u, const void* cf, const void* ci, const void* b, void* x, void* workspace, double tol,
+           int max_iter, int check_every, int* iters_out, double* relres_out, cudaStream_t st) {
+    if (g->prec == HR_PREC_F64) return cg_run<double>(g, m0, u, cf, ci, b, x, workspace, tol, max_iter, check_every, iters_out, relres_out, st);
+    return cg_run<float>(g, m0, u, cf, ci, b, x, workspace, tol, max_iter, check_every, iters_out, relres_out, st);
+}
+
+}  // namespace hr

@@ -29,7 +29,7 @@ SYMBOLS = [
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
     "hr_dirac_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_apply", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
-    "hr_launch_count", "hr_kernel_name",
+    "hr_launch_count", "hr_kernel_name", "hr_cg_workspace_bytes", "hr_cg_solve",
 ]
 
 
@@ -76,6 +76,8 @@ def lib():
             "hr_last_error": (S, [ctypes.c_char_p, S]),
             "hr_launch_count": (ctypes.c_ulonglong, []),
             "hr_kernel_name": (ctypes.c_char_p, [G]),
+            "hr_cg_workspace_bytes": (S, [G]),
+            "hr_cg_solve": (I, [G, D, V, V, V, V, V, V, D, I, I, ctypes.POINTER(ctypes.c_int), PD, V]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name)
@@ -180,6 +182,17 @@ def hr_dirac_apply_host(g, m0, u_canon_host, psi_canon_host, out_canon_host, wor
 def hr_dirac_eo_apply_host(g, op, m0, u_canon_host, in_canon_host, out_canon_host, workspace, stream=0):
     _check(lib().hr_dirac_eo_apply_host(ctypes.byref(g), int(op), float(m0), _ptr(u_canon_host), _ptr(in_canon_host),
                                         _ptr(out_canon_host), _ptr(workspace), stream))
+
+
+def hr_cg_workspace_bytes(g): return lib().hr_cg_workspace_bytes(ctypes.byref(g))
+
+
+def hr_cg_solve(g, m0, u, clover_fwd, clover_inv, b, x, workspace, tol, max_iter, check_every=5, stream=0):
+    """-> (iterations, |r|/|b|)"""
+    it, rel = ctypes.c_int(), ctypes.c_double()
+    _check(lib().hr_cg_solve(ctypes.byref(g), float(m0), _ptr(u), _ptr(clover_fwd), _ptr(clover_inv), _ptr(b), _ptr(x),
+                             _ptr(workspace), float(tol), int(max_iter), int(check_every), ctypes.byref(it), ctypes.byref(rel), stream))
+    return it.value, rel.value
 
 
 def hr_launch_count() -> int: return int(lib().hr_launch_count())

@@ -122,3 +122,10 @@ class Lattice:
         out = self.empty_spinor(parity) if out is None else out
         hr.hr_clover_apply(self.g, parity, blocks, inp, out, hr.stream_ptr())
         return out
+
+    def cg(self, m0, u, b, tol, max_iter, clover_fwd=None, clover_inv=None, check_every=5):
+        """b: even half field -> (x even half field, iterations, |r|/|b|)"""
+        x = self.empty_spinor(hr.EVEN)
+        ws = hr.device_buffer(hr.hr_cg_workspace_bytes(self.g), self.device)
+        it, rel = hr.hr_cg_solve(self.g, m0, u, clover_fwd, clover_inv, b, x, ws, tol, max_iter, check_every, hr.stream_ptr())
+        return x, it, rel

@@ -102,6 +102,13 @@ def test_argument_checks_happen_before_any_cuda_call(L):
     with pytest.raises(hr.HrError) as e:
         hr.hr_clover_apply(gadj, hr.EVEN, 4096, 1 << 20, 1 << 21)
     assert e.value.status == hr.EUNSUPPORTED
+    with pytest.raises(hr.HrError) as e:   # hr_cg_solve: tol must be positive; checked before any CUDA call
+        hr.hr_cg_solve(g, 0.0, 4096, None, None, 1 << 20, 1 << 21, 1 << 24, 0.0, 10)
+    assert e.value.status == hr.EINVAL
+    with pytest.raises(hr.HrError) as e:   # x aliases b
+        hr.hr_cg_solve(g, 0.0, 4096, None, None, 1 << 20, 1 << 20, 1 << 24, 1e-8, 10)
+    assert e.value.status == hr.EINVAL
+    assert hr.hr_cg_workspace_bytes(g) >= 5 * hr.hr_spinor_bytes(g, hr.EVEN)
     gt = hr.geom((2, 2, 2, 2), kernel=hr.KERNEL_TILED)
     with pytest.raises(hr.HrError) as e:
         hr.hr_dirac_apply(gt, 0.0, 4096, 1 << 20, 1 << 21)

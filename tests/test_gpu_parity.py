@@ -499,3 +499,62 @@ def test_operators_write_only_their_output(hr, L, rep, prec):
             out.fill_(0xA5)
             hr.hr_clover_apply(lat.g, hr.ODD, inv, lat.odd(psi_dev), out[half:], st)
             assert guards_ok() and bool((out[:half] == 0xA5).all()), ("clover odd", kernel)
+
+
+# ------------------------------------------------------------------ S1: CG on Dhat^dag Dhat
+@pytest.mark.parametrize("L,rep", [((8, 4, 4, 8), 0), ((4, 4, 4, 4), 1), ((8, 2, 8, 6), 0)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_cg_solution_matches_the_oracle(hr, orc, L, rep, prec):
+    """hr_cg_solve against the oracle's textbook CG (O8) on the same system: same solution up to the stopping
+    tolerance times the conditioning, about the same iteration count, and a true residual (evaluated with the
+    ORACLE's operator on the GPU's solution) at the requested level"""
+    import torch
+    m0 = -0.2
+    N = 2 if rep == 0 else 3
+    Uf = rounded(inputs.haar_gauge(L, 1), prec)
+    U = Uf if rep == 0 else rounded(orc.represent(Uf)[0], prec)
+    b = rounded(inputs.gaussian_spinor(L, N, 2), prec)
+    even = inputs.site_parity(L) == 0
+    b[~even] = 0
+    tol = 1e-12 if prec == 0 else 2e-6
+    x_orc, it_orc, _ = orc.cg_normal(L, rep, m0, U, b, tol=tol, max_iter=1000, nthreads=NTHREADS)
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+    for kernel in kernels_for(hr, L, rep, prec):
+        lat = lattice(hr, L, rep, prec, kernel)
+        U_dev = lat.put_gauge_fund(U) if rep == 0 else lat.put_gauge_adj(U)
+        b_dev = lat.put_spinor(b)
+        x_half, it, relres = lat.cg(m0, U_dev, lat.even(b_dev), tol, 1000, check_every=3)
+        # the count may differ by the rounding of the residual norm at the threshold, plus the check interval
+        assert relres <= tol and it_orc - 2 <= it <= it_orc + 6, (it, it_orc, relres)
+        full = torch.zeros_like(b_dev)
+        lat.even(full).copy_(x_half)
+        x = lat.get_spinor(full).astype(np.complex128)
+        assert not x[~even].any()
+        assert rel(x, x_orc) <= (1e-9 if prec == 0 else 2e-3), kernel
+        t = orc.dirac_eo(L, rep, m0, U, x, nthreads=NTHREADS)
+        r = b - g5 * orc.dirac_eo(L, rep, m0, U, g5 * t, nthreads=NTHREADS)
+        assert np.linalg.norm(r) <= (10 * tol if prec == 0 else 2e-5) * np.linalg.norm(b)
+
+
+def test_cg_with_clover_and_repeatability(hr, orc):
+    """the clover-improved system (E2 inside the solver) against the oracle, and two solves give the same bits"""
+    import torch
+    L, m0, csw = (4, 4, 4, 8), -0.25, 1.2
+    U = inputs.weak_gauge(L, 0.3, 1)
+    b = inputs.gaussian_spinor(L, 2, 2)
+    even = inputs.site_parity(L) == 0
+    b[~even] = 0
+    A, Ainv = clover_oracle(orc, L, U, m0, csw)
+    x_orc, it_orc, _ = orc.cg_normal(L, 0, m0, U, b, tol=1e-12, max_iter=500, nthreads=NTHREADS, A=A, Ainv=Ainv)
+    lat = lattice(hr, L, 0, 0)
+    U_dev, b_dev = lat.put_gauge_fund(U), lat.put_spinor(b)
+    fwd, inv = lat.clover_build(m0, csw, U_dev)
+    sols = []
+    for _ in range(2):
+        x_half, it, relres = lat.cg(m0, U_dev, lat.even(b_dev), 1e-12, 500, clover_fwd=fwd, clover_inv=inv, check_every=1)
+        assert abs(it - it_orc) <= 2 and relres <= 1e-12, (it, it_orc)
+        sols.append(x_half.clone())
+    assert torch.equal(sols[0], sols[1])
+    full = torch.zeros_like(b_dev)
+    lat.even(full).copy_(sols[0])
+    assert rel(lat.get_spinor(full), x_orc) <= 1e-9
