@@ -215,3 +215,21 @@ def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1, A=None, Ai
         rr = rr_new
         it += 1
     return x, it, float(np.sqrt(rr / bb))
+
+
+# ------------------------------------------------------------------ O9: exponential clover term
+def clover_exp_dense(L, diag, csw, U, nthreads=1):
+    """O9 ("exponential of the clover term ... the diagonal part of the Dirac operator and its inverse
+    take the same time to execute", ref [6] at PAPER.md:123; reading B4 of DESIGN.md §3): the site-diagonal term of
+    the exponential clover improvement,
+        A_exp(x) = diag * exp( C(x) / diag ),     A_exp(x)^-1 = exp( -C(x) / diag ) / diag,     diag = 4 + m0,
+    with C(x) = csw (i/4) sum_{mu,nu} sigma_mu,nu F^_mu,nu(x) the clover term of O5 (the regular term is diag + C,
+    the first two orders of this exponential).  The exponential of the hermitian 8x8 matrix C/diag is taken from
+    its eigendecomposition, exp(H) = V diag(e^lambda) V^dag.  Returns (A_exp, A_exp^-1), dense [V,8,8]."""
+    A = clover_dense(L, diag, csw, U, nthreads=nthreads)
+    C = A - diag * np.eye(8)[None]
+    lam, V = np.linalg.eigh(C / diag)
+    Vh = np.conj(np.swapaxes(V, -1, -2))
+    fwd = diag * (V * np.exp(lam)[:, None, :]) @ Vh
+    inv = (V * np.exp(-lam)[:, None, :]) @ Vh / diag
+    return fwd, inv

@@ -458,3 +458,37 @@ def test_P15_cg_against_dense_solve(orc):
     g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
     lhs = (g5 * orc.dirac_eo(L, 0, m0, U, g5 * v))[even].ravel()
     assert np.linalg.norm(lhs - Dh.conj().T @ v[even].ravel()) <= 1e-13 * np.linalg.norm(lhs)
+
+
+def test_P16_exponential_clover(orc):
+    """O9: A_exp = d exp(C/d).  Pins: the same matrix from scipy's Pade expm (another route); det A_exp = d^8 exactly
+    because tr C = 0; A_exp A_exp^-1 = 1; hermitian, commuting with gamma5; A_exp - (d + C) = C^2/(2d) + O(C^3)
+    (the regular clover term is its first two orders): the difference scales as csw^2 and matches C^2/(2d) to
+    the next order; csw = 0 gives d * 1."""
+    from scipy.linalg import expm
+    L, m0 = (4, 4, 2, 2), -0.25
+    d = 4.0 + m0
+    U = inputs.weak_gauge(L, 0.3, 1)
+    V = inputs.volume(L)
+    eye = np.eye(8)[None]
+    fwd, inv = orc.clover_exp_dense(L, d, 1.2, U)
+    C = orc.clover_dense(L, d, 1.2, U) - d * eye
+    for x in (0, 7, V - 1):
+        assert np.abs(fwd[x] - d * expm(C[x] / d)).max() <= 1e-13
+        assert np.abs(inv[x] - expm(-C[x] / d) / d).max() <= 1e-14
+    assert np.abs(np.linalg.det(fwd) - d ** 8).max() <= 1e-9 * d ** 8
+    assert np.abs(fwd @ inv - eye).max() <= 1e-14
+    assert np.abs(fwd - np.conj(np.swapaxes(fwd, -1, -2))).max() <= 1e-14
+    g5 = np.diag([1, 1, 1, 1, -1, -1, -1, -1]).astype(complex)
+    assert np.abs(g5 @ fwd - fwd @ g5).max() <= 1e-14
+    # series: A_exp - (d + C) - C^2/(2d) = O(C^3/d^2)
+    rem2 = fwd - (d * eye + C)
+    rem3 = rem2 - C @ C / (2 * d)
+    nC = np.abs(C).max()
+    assert np.abs(rem2).max() <= 2.0 * nC ** 2 / d and np.abs(rem3).max() <= 2.0 * nC ** 3 / d ** 2
+    fwd_half, _ = orc.clover_exp_dense(L, d, 0.6, U)
+    rem2_half = fwd_half - (d * eye + 0.5 * C)
+    ratio = np.abs(rem2).max() / np.abs(rem2_half).max()
+    assert 3.5 < ratio < 4.7          # quadratic in csw
+    f0, i0 = orc.clover_exp_dense(L, d, 0.0, U)
+    assert np.abs(f0 - d * eye).max() <= 1e-14 and np.abs(i0 - eye / d).max() <= 1e-15
