@@ -115,6 +115,15 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
 int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
                     void* clover_inv, void* stream);
 
+/* C1x ("exponential of the clover term"; ref [6] at PAPER.md:123): the same
+ * block fields for the EXPONENTIAL clover improvement,
+ *   A_exp(x) = (4+m0) exp( C(x) / (4+m0) ),   A_exp(x)^-1 = exp( -C(x) / (4+m0) ) / (4+m0),
+ * C(x) = csw (i/4) sum_{mu,nu} sigma_mu,nu F^_mu,nu(x) as above (the regular term (4+m0) + C is its first two
+ * orders).  hr_clover_apply and hr_dirac_eo_apply take these blocks unchanged; forward and inverse blocks cost the
+ * same to apply, as the paper notes.  Setup step; arithmetic in double for either field precision. */
+int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
+                        void* clover_inv, void* stream);
+
 /* C2/C3 ("application of another diagonal term"): out(x) = B(x) in(x) on the sites of
  * `parity` (HR_EVEN, HR_ODD: in/out are half fields; HR_BOTH: full fields).  `blocks` is the full-lattice
  * block field (forward blocks: C2; inverse blocks: C3 — same kernel).  Fundamental rep only. */

@@ -14,7 +14,7 @@ int permute_chunks(bool pack, const Geo& g, int NI, int NCH, int SRC, const void
 int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st);
 int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st);
 int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
-int run_clover_build(const Geo& g, int prec, double diag, double csw, const void* ufund, void* fwd, void* inv, cudaStream_t st);
+int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
 
 // hr_solver.cu
@@ -228,14 +228,24 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
 }
 
 // ---------------------------------------------------------------- C1 / C2 / C3
-int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
-                    void* clover_inv, void* stream) {
+static int clover_build_any(const hr_geom* g, double m0, double csw, int expo, const void* u_fund, void* clover_fwd, void* clover_inv, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund"));
     if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     if (!clover_fwd && !clover_inv) { set_error("hr_clover_build: nothing to build"); return HR_EINVAL; }
+    if (4.0 + m0 == 0.0) { set_error("hr_clover_build: 4+m0 = 0"); return HR_EINVAL; }
     if (clover_fwd) HR_TRY(check_ptr(clover_fwd, "clover_fwd"));
     if (clover_inv) HR_TRY(check_ptr(clover_inv, "clover_inv"));
-    return run_clover_build(make_geo(g), g->prec, 4.0 + m0, csw, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
+    return run_clover_build(make_geo(g), g->prec, 4.0 + m0, csw, expo, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
+}
+
+int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
+                    void* clover_inv, void* stream) {
+    return clover_build_any(g, m0, csw, 0, u_fund, clover_fwd, clover_inv, stream);
+}
+
+int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
+                        void* clover_inv, void* stream) {
+    return clover_build_any(g, m0, csw, 1, u_fund, clover_fwd, clover_inv, stream);
 }
 
 int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream) {

@@ -224,6 +224,49 @@ __device__ void invert4(dcplx A[4][4]) {
         for (int j = 0; j < 4; ++j) A[i][j] = B[i][j];
 }
 
+__device__ __forceinline__ dcplx dadd(dcplx a, dcplx b) { dcplx r; r.re = a.re + b.re; r.im = a.im + b.im; return r; }
+__device__ void matmul4(dcplx C[4][4], const dcplx A[4][4], const dcplx B[4][4]) {
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) {
+            dcplx a = {0.0, 0.0};
+            for (int k = 0; k < 4; ++k) a = dadd(a, dmul(A[i][k], B[k][j]));
+            C[i][j] = a;
+        }
+}
+// E = exp(X) for a 4x4 complex matrix: scaling and squaring with an order-16 Taylor polynomial
+// (|X / 2^s|_inf <= 1/2, truncation < 0.5^17 / 17! ~ 2e-20).  Setup-time code: clarity over speed.
+__device__ void expm4(dcplx E[4][4], const dcplx X[4][4]) {
+    double nrm = 0.0;
+    for (int i = 0; i < 4; ++i) {
+        double r = 0.0;
+        for (int j = 0; j < 4; ++j) r += fabs(X[i][j].re) + fabs(X[i][j].im);
+        nrm = fmax(nrm, r);
+    }
+    int s = 0;
+    double scale = 1.0;
+    while (nrm * scale > 0.5 && s < 60) { scale *= 0.5; ++s; }
+    dcplx Y[4][4], P[4][4], Tm[4][4];
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j) {
+            Y[i][j].re = X[i][j].re * scale; Y[i][j].im = X[i][j].im * scale;
+            P[i][j] = Y[i][j];                                   // current term Y^k / k!
+            E[i][j].re = (i == j ? 1.0 : 0.0) + Y[i][j].re; E[i][j].im = Y[i][j].im;
+        }
+    for (int k = 2; k <= 16; ++k) {
+        matmul4(Tm, P, Y);
+        for (int i = 0; i < 4; ++i)
+            for (int j = 0; j < 4; ++j) {
+                P[i][j].re = Tm[i][j].re / k; P[i][j].im = Tm[i][j].im / k;
+                E[i][j] = dadd(E[i][j], P[i][j]);
+            }
+    }
+    for (int q = 0; q < s; ++q) {
+        matmul4(Tm, E, E);
+        for (int i = 0; i < 4; ++i)
+            for (int j = 0; j < 4; ++j) E[i][j] = Tm[i][j];
+    }
+}
+
 // hermitian 4x4 -> 16 reals (diagonal, then lower entries column-major), hermitian part taken
 template <typename T>
 __device__ void herm_to_reals(T* out, dcplx A[4][4]) {
@@ -240,7 +283,7 @@ __device__ void herm_to_reals(T* out, dcplx A[4][4]) {
 //   A+- = (4+m0) + (csw/2) [ tau1 (x) i(+-F01 - F23) + tau2 (x) i(+-F02 + F13) + tau3 (x) i(+-F03 - F12) ],
 // tau_k on the spin index within the chirality, i F on colour; block index = spin*2 + colour.
 template <typename T>
-__global__ void clover_build_kernel(Geo g, double diag, double csw, const void* __restrict__ ufund, void* fwd, void* inv) {
+__global__ void clover_build_kernel(Geo g, double diag, double csw, int expo, const void* __restrict__ ufund, void* fwd, void* inv) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= 2 * g.Vh) return;
     const int par = t / g.Vh, cb = t - par * g.Vh;
@@ -289,9 +332,27 @@ __global__ void clover_build_kernel(Geo g, double diag, double csw, const void* 
                         }
                         A[sp * 2 + c][tp * 2 + d] = acc;
                     }
-        herm_to_reals<T>(reals_f + 16 * chi, A);
-        invert4(A);
-        herm_to_reals<T>(reals_i + 16 * chi, A);
+        if (expo) {
+            // exponential clover (ref [6]): A_exp = diag exp(C/diag), A_exp^-1 = exp(-C/diag)/diag, C = A - diag
+            dcplx X[4][4], E[4][4];
+            for (int i = 0; i < 4; ++i)
+                for (int j = 0; j < 4; ++j) {
+                    X[i][j].re = (A[i][j].re - (i == j ? diag : 0.0)) / diag;
+                    X[i][j].im = A[i][j].im / diag;
+                }
+            expm4(E, X);
+            for (int i = 0; i < 4; ++i)
+                for (int j = 0; j < 4; ++j) { A[i][j].re = diag * E[i][j].re; A[i][j].im = diag * E[i][j].im; X[i][j].re = -X[i][j].re; X[i][j].im = -X[i][j].im; }
+            herm_to_reals<T>(reals_f + 16 * chi, A);
+            expm4(E, X);
+            for (int i = 0; i < 4; ++i)
+                for (int j = 0; j < 4; ++j) { A[i][j].re = E[i][j].re / diag; A[i][j].im = E[i][j].im / diag; }
+            herm_to_reals<T>(reals_i + 16 * chi, A);
+        } else {
+            herm_to_reals<T>(reals_f + 16 * chi, A);
+            invert4(A);
+            herm_to_reals<T>(reals_i + 16 * chi, A);
+        }
     }
     constexpr int CCH = 32 * sizeof(T) / 16;
     constexpr int PER = 16 / sizeof(T);
@@ -303,10 +364,10 @@ __global__ void clover_build_kernel(Geo g, double diag, double csw, const void* 
     }
 }
 
-int run_clover_build(const Geo& g, int prec, double diag, double csw, const void* ufund, void* fwd, void* inv, cudaStream_t st) {
+int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st) {
     const unsigned nb = blocks_for(2LL * g.Vh, 128);
-    if (prec == HR_PREC_F64) clover_build_kernel<double><<<nb, 128, 0, st>>>(g, diag, csw, ufund, fwd, inv);
-    else clover_build_kernel<float><<<nb, 128, 0, st>>>(g, diag, csw, ufund, fwd, inv);
+    if (prec == HR_PREC_F64) clover_build_kernel<double><<<nb, 128, 0, st>>>(g, diag, csw, expo, ufund, fwd, inv);
+    else clover_build_kernel<float><<<nb, 128, 0, st>>>(g, diag, csw, expo, ufund, fwd, inv);
     count_launch();
     return check_launch("clover_build_kernel");
 }

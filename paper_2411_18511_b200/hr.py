@@ -27,7 +27,7 @@ SYMBOLS = [
     "hr_spinor_bytes", "hr_gauge_bytes", "hr_clover_bytes", "hr_canonical_spinor_bytes",
     "hr_canonical_gauge_bytes", "hr_canonical_clover_bytes", "hr_pack_spinor", "hr_unpack_spinor",
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
-    "hr_dirac_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_apply", "hr_dirac_flops_bytes",
+    "hr_dirac_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_cg_workspace_bytes", "hr_cg_solve",
 ]
@@ -68,6 +68,7 @@ def lib():
             "hr_dirac_apply": (I, [G, D, V, V, V, V]),
             "hr_dirac_eo_apply": (I, [G, I, D, V, V, V, V, V, V, V]),
             "hr_clover_build": (I, [G, D, D, V, V, V, V]),
+            "hr_clover_build_exp": (I, [G, D, D, V, V, V, V]),
             "hr_clover_apply": (I, [G, I, V, V, V, V]),
             "hr_dirac_flops_bytes": (I, [G, I, PD, PD, PD]),
             "hr_host_workspace_bytes": (S, [G]),
@@ -161,6 +162,10 @@ def hr_dirac_eo_apply(g, op, m0, u, clover_fwd, clover_inv, inp, out, tmp, strea
 
 def hr_clover_build(g, m0, csw, u_fund, clover_fwd, clover_inv, stream=0):
     _check(lib().hr_clover_build(ctypes.byref(g), float(m0), float(csw), _ptr(u_fund), _ptr(clover_fwd), _ptr(clover_inv), stream))
+
+
+def hr_clover_build_exp(g, m0, csw, u_fund, clover_fwd, clover_inv, stream=0):
+    _check(lib().hr_clover_build_exp(ctypes.byref(g), float(m0), float(csw), _ptr(u_fund), _ptr(clover_fwd), _ptr(clover_inv), stream))
 
 
 def hr_clover_apply(g, parity, blocks, inp, out, stream=0):

@@ -113,9 +113,10 @@ class Lattice:
         hr.hr_dirac_eo_apply(self.g, hr.EO_DHAT, m0, u, clover_fwd, clover_inv, inp, out, tmp, hr.stream_ptr())
         return out
 
-    def clover_build(self, m0, csw, u_fund):
+    def clover_build(self, m0, csw, u_fund, exponential=False):
         fwd, inv = self.empty_clover(), self.empty_clover()
-        hr.hr_clover_build(self.g, m0, csw, u_fund, fwd, inv, hr.stream_ptr())
+        build = hr.hr_clover_build_exp if exponential else hr.hr_clover_build
+        build(self.g, m0, csw, u_fund, fwd, inv, hr.stream_ptr())
         return fwd, inv
 
     def clover_apply(self, parity, blocks, inp, out=None):

@@ -558,3 +558,32 @@ def test_cg_with_clover_and_repeatability(hr, orc):
     full = torch.zeros_like(b_dev)
     lat.even(full).copy_(sols[0])
     assert rel(lat.get_spinor(full), x_orc) <= 1e-9
+
+
+# ------------------------------------------------------------------ C1x: exponential clover
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 4, 6, 8), (8, 2, 8, 6)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_exponential_clover(hr, orc, L, prec):
+    """hr_clover_build_exp blocks and inverses against the oracle's O9 (eigendecomposition route), then C2/C3 and the
+    even-odd operator E2 with those blocks"""
+    import torch
+    m0, csw = -0.25, 1.2
+    U = rounded(inputs.weak_gauge(L, 0.3, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 2, 2), prec)
+    A, Ainv = orc.clover_exp_dense(L, 4.0 + m0, csw, U, nthreads=NTHREADS)
+    bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+    tol_blk = 1e-13 if prec == 0 else 1e-6
+    for kernel in kernels_for(hr, L, 0, prec):
+        lat = lattice(hr, L, 0, prec, kernel)
+        U_dev, psi_dev = lat.put_gauge_fund(U), lat.put_spinor(psi)
+        fwd, inv = lat.clover_build(m0, csw, U_dev, exponential=True)
+        assert np.linalg.norm(lat.get_clover(fwd) - bf) <= tol_blk * np.linalg.norm(bf)
+        assert np.linalg.norm(lat.get_clover(inv) - bi) <= tol_blk * np.linalg.norm(bi)
+        got = lat.get_spinor(lat.clover_apply(hr.BOTH, fwd, psi_dev))
+        assert rel(got, orc.site_matvec(L, 3, A, psi)) <= TOL[prec]
+        got = lat.get_spinor(lat.clover_apply(hr.BOTH, inv, psi_dev))
+        assert rel(got, orc.site_matvec(L, 3, Ainv, psi)) <= TOL[prec]
+        out = torch.zeros_like(psi_dev)
+        lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
+        want = orc.dirac_eo_clover(L, U, A, Ainv, psi, nthreads=NTHREADS)
+        assert rel(lat.get_spinor(out), want) <= TOL[prec], kernel
