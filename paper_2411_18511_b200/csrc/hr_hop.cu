@@ -46,7 +46,7 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
     }
     if (tiled_chosen(g)) {
         TiledPlan pl;
-        tiled_plan(g, a.both, sm_count(), pl);
+        tiled_plan(g, a.both, sm_count(), pl, a.both && epi == EPI_AXPY && a.phi == a.in);
         if (g->rep == HR_REP_FUND) {
             if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 2>(geo, a, epi, pl, st);
             return launch_hop_tiled<float, 2>(geo, a, epi, pl, st);
