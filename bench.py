@@ -383,6 +383,23 @@ def cg_report(hr, S, m0):
         out["cg_48^4_" + tag] = {"ms_per_iteration": round(ms, 4), "iterations": it, "relres_after": rel,
                                  "gbs": round(bytes_site * Vh / ms / 1e6, 1), "bytes_per_even_site_per_iteration": bytes_site}
         del ws, x
+    # time to a 1e-12 solution: plain fp64 CG against fp64 defect correction around fp32 CG (hr_cg_solve_mixed)
+    s64, s32 = S["f64"], S["f32"]
+    lat, g = s64["lat"], s64["lat"].g
+    x = lat.empty_spinor(hr.EVEN)
+    b = lat.even(s64["psi"])
+    st = hr.stream_ptr()
+    ws = hr.device_buffer(max(hr.hr_cg_workspace_bytes(g), hr.hr_cg_mixed_workspace_bytes(g)), lat.device)
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record()
+    it, rel = hr.hr_cg_solve(g, m0, s64["U"], None, None, b, x, ws, 1e-12, 2000, 5, st)
+    e1.record()
+    no, ni, relm = hr.hr_cg_solve_mixed(g, m0, s64["U"], s32["U"], b, x, ws, 1e-12, 1e-4, 30, 2000, 5, st)
+    e2.record()
+    torch.cuda.synchronize()
+    out["cg_48^4_to_1e-12"] = {"f64_ms": round(e0.elapsed_time(e1), 2), "f64_iterations": it, "f64_relres": rel,
+                               "mixed_ms": round(e1.elapsed_time(e2), 2), "mixed_outer": no, "mixed_f32_iterations": ni,
+                               "mixed_true_relres": relm}
     return out
 
 

@@ -21,6 +21,9 @@ int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, con
 size_t cg_workspace_bytes(const hr_geom* g);
 int run_cg(const hr_geom* g, double m0, const void* u, const void* cf, const void* ci, const void* b, void* x, void* workspace, double tol,
            int max_iter, int check_every, int* iters_out, double* relres_out, cudaStream_t st);
+size_t cg_mixed_workspace_bytes(const hr_geom* g);
+int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, const void* b, void* x, void* workspace, double tol, double inner_tol,
+                 int max_outer, int max_inner, int check_every, int* outer_out, int* inner_out, double* relres_out, cudaStream_t st);
 
 static thread_local char g_err[512] = "";
 static std::atomic<unsigned long long> g_launches{0};
@@ -276,6 +279,31 @@ int hr_cg_solve(const hr_geom* g, double m0, const void* u, const void* clover_f
         return HR_EINVAL;
     }
     return run_cg(g, m0, u, clover_fwd, clover_inv, b, x, workspace, tol, max_iter, check_every, iters, relres, (cudaStream_t)stream);
+}
+
+size_t hr_cg_mixed_workspace_bytes(const hr_geom* g) {
+    if (!geom_ok(g) || g->prec != HR_PREC_F64) return 0;
+    return cg_mixed_workspace_bytes(g);
+}
+
+int hr_cg_solve_mixed(const hr_geom* g, double m0, const void* u_f64, const void* u_f32, const void* b, void* x, void* workspace,
+                      double tol, double inner_tol, int max_outer, int max_inner, int check_every,
+                      int* outer_iters, int* inner_iters, double* relres, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    if (g->prec != HR_PREC_F64) { set_error("hr_cg_solve_mixed: the geometry describes the fp64 fields (prec must be HR_PREC_F64)"); return HR_EINVAL; }
+    HR_TRY(check_ptr(u_f64, "u_f64")); HR_TRY(check_ptr(u_f32, "u_f32")); HR_TRY(check_ptr(b, "b")); HR_TRY(check_ptr(x, "x"));
+    HR_TRY(check_ptr(workspace, "workspace"));
+    if (!(tol > 0.0) || !(inner_tol > 0.0) || inner_tol >= 1.0 || max_outer < 0 || max_inner < 1 || check_every < 1) {
+        set_error("hr_cg_solve_mixed: need tol > 0, 0 < inner_tol < 1, max_outer >= 0, max_inner >= 1, check_every >= 1");
+        return HR_EINVAL;
+    }
+    const size_t half = half_spinor_bytes(g);
+    if (overlap(b, half, x, half) || overlap(workspace, cg_mixed_workspace_bytes(g), x, half) || overlap(workspace, cg_mixed_workspace_bytes(g), b, half)) {
+        set_error("hr_cg_solve_mixed: b, x and workspace must not overlap");
+        return HR_EINVAL;
+    }
+    return run_cg_mixed(g, m0, u_f64, u_f32, b, x, workspace, tol, inner_tol, max_outer, max_inner, check_every, outer_iters, inner_iters, relres,
+                        (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------- M1

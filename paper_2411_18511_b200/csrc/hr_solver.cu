@@ -240,4 +240,130 @@ int run_cg(const hr_geom* g, double m0, const void* u, const void* cf, const voi
     return cg_run<float>(g, m0, u, cf, ci, b, x, workspace, tol, max_iter, check_every, iters_out, relres_out, st);
 }
 
+// ------------------------------------------------------------------ mixed precision: fp64 defect correction around fp32 CG
+// (SURVEY.md §8(f) item 2 "mixed fp32/fp64 defect correction").  Outer loop in double:
+//     r = b - Dhat^dag Dhat x  (true residual, fp64 operator);  stop when |r| <= tol |b|;
+//     solve Dhat^dag Dhat e = r in fp32 to the relative accuracy inner_tol (cg_run<float>);  x += e.
+// The fp32 fields use their own device layout (two complex per 16-byte chunk), so r and e are converted site by site.
+
+// one thread per fp32 chunk: complex numbers 2c, 2c+1 of site (row, h):  f64 chunks (row*NC + 2c [+1])*L3h + h
+__global__ void __launch_bounds__(CG_BLOCK) cg_to_f32_kernel(size_t nchunks32, int L3h, int NCH32, const double2* __restrict__ src, float4* __restrict__ dst) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks32; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t h = i % L3h, rc = i / L3h;          // rc = row*NCH32 + c
+        const size_t row = rc / NCH32, c = rc % NCH32;
+        const size_t j = (row * (2 * NCH32) + 2 * c) * L3h + h;
+        const double2 a = src[j], b = src[j + L3h];
+        dst[i] = make_float4((float)a.x, (float)a.y, (float)b.x, (float)b.y);
+    }
+}
+// x += e (e in fp32 layout)
+__global__ void __launch_bounds__(CG_BLOCK) cg_add_f32_kernel(size_t nchunks32, int L3h, int NCH32, const float4* __restrict__ e, double2* __restrict__ x) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks32; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t h = i % L3h, rc = i / L3h;
+        const size_t row = rc / NCH32, c = rc % NCH32;
+        const size_t j = (row * (2 * NCH32) + 2 * c) * L3h + h;
+        const float4 v = e[i];
+        double2 a = x[j], b = x[j + L3h];
+        a.x += (double)v.x; a.y += (double)v.y; b.x += (double)v.z; b.y += (double)v.w;
+        x[j] = a;
+        x[j + L3h] = b;
+    }
+}
+// r = b - gamma5 w, partial = sum |r|^2      (w = Dhat gamma5 Dhat x)
+__global__ void __launch_bounds__(CG_BLOCK) cg_residual_kernel(size_t nchunks, int L3h, int NCH, const double2* __restrict__ b, const double2* __restrict__ w,
+                                                               double2* __restrict__ r, double* __restrict__ partial) {
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
+        const double sg = g5_sign(i, L3h, NCH);
+        const double2 bv = b[i], wv = w[i];
+        double2 rv;
+        rv.x = bv.x - sg * wv.x;
+        rv.y = bv.y - sg * wv.y;
+        acc += rv.x * rv.x + rv.y * rv.y;
+        r[i] = rv;
+    }
+    const double tot = block_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(CG_BLOCK) cg_zero_kernel(size_t nchunks, double2* __restrict__ x) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) x[i] = make_double2(0.0, 0.0);
+}
+
+static hr_geom as_f32(const hr_geom* g) {
+    hr_geom g32 = *g;
+    g32.prec = HR_PREC_F32;
+    return g32;
+}
+
+size_t cg_mixed_workspace_bytes(const hr_geom* g) {
+    const hr_geom g32 = as_f32(g);
+    const size_t half64 = hr_spinor_bytes(g, HR_EVEN), half32 = hr_spinor_bytes(&g32, HR_EVEN);
+    return 256 + up256s(CG_MAX_PARTIALS * sizeof(double)) + 4 * up256s(half64) + 2 * up256s(half32) + up256s(cg_workspace_bytes(&g32));
+}
+
+int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, const void* b, void* x, void* workspace, double tol, double inner_tol,
+                 int max_outer, int max_inner, int check_every, int* outer_out, int* inner_out, double* relres_out, cudaStream_t st) {
+    const hr_geom g32 = as_f32(g);
+    const Geo geo = make_geo(g);
+    const int NCH = spinor_chunks(g->rep, g->prec), NCH32 = spinor_chunks(g->rep, HR_PREC_F32);
+    const size_t half64 = hr_spinor_bytes(g, HR_EVEN), half32 = hr_spinor_bytes(&g32, HR_EVEN);
+    const size_t nchunks = half64 / 16, nchunks32 = half32 / 16;
+    char* w8 = (char*)workspace;
+    CgScalars* sc = (CgScalars*)w8; w8 += 256;
+    double* partial = (double*)w8; w8 += up256s(CG_MAX_PARTIALS * sizeof(double));
+    void* r = w8; w8 += up256s(half64);
+    void* t = w8; w8 += up256s(half64);
+    void* w = w8; w8 += up256s(half64);
+    void* tmp = w8; w8 += up256s(half64);
+    void* r32 = w8; w8 += up256s(half32);
+    void* e32 = w8; w8 += up256s(half32);
+    void* ws32 = w8;
+    int nblk = (int)((nchunks + CG_BLOCK - 1) / CG_BLOCK);
+    if (nblk > CG_MAX_PARTIALS) nblk = CG_MAX_PARTIALS;
+    int nblk32 = (int)((nchunks32 + CG_BLOCK - 1) / CG_BLOCK);
+    if (nblk32 > CG_MAX_PARTIALS) nblk32 = CG_MAX_PARTIALS;
+    void* strm = (void*)st;
+
+    cg_zero_kernel<<<nblk, CG_BLOCK, 0, st>>>(nchunks, (double2*)x);
+    count_launch();
+    double bb = -1.0, relres = 1.0;
+    int outer = 0, inner_total = 0;
+    for (;;) {
+        // r = b - Dhat^dag Dhat x in double (for x = 0 this is r = b, computed the same way for simplicity)
+        int rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, nullptr, nullptr, x, t, tmp, strm);
+        if (rc != HR_OK) return rc;
+        cg_g5_norm_kernel<double><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, t, w, partial);
+        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, nullptr, nullptr, w, t, tmp, strm);
+        if (rc != HR_OK) return rc;
+        cg_residual_kernel<<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, (const double2*)b, (const double2*)t, (double2*)r, partial);
+        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_INIT, nblk, partial, sc);
+        count_launch(3);
+        CgScalars h;
+        cudaError_t e = cudaMemcpyAsync(&h, sc, sizeof(h), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { set_error("hr_cg_solve_mixed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+        if (bb < 0.0) bb = h.rr;                         // first pass: x = 0, so |r|^2 = |b|^2
+        relres = bb > 0.0 ? sqrt(h.rr / bb) : 0.0;
+        if (!(h.rr == h.rr)) { set_error("hr_cg_solve_mixed: residual is NaN after %d outer iterations", outer); return HR_ECUDA; }
+        if (bb == 0.0 || relres <= tol || outer >= max_outer) break;
+        // inner solve in fp32: Dhat^dag Dhat e = r
+        cg_to_f32_kernel<<<nblk32, CG_BLOCK, 0, st>>>(nchunks32, geo.L3h, NCH32, (const double2*)r, (float4*)r32);
+        count_launch();
+        int it = 0;
+        double rel32 = 0.0;
+        rc = run_cg(&g32, m0, u32, nullptr, nullptr, r32, e32, ws32, inner_tol, max_inner, check_every, &it, &rel32, st);
+        if (rc != HR_OK) return rc;
+        inner_total += it;
+        cg_add_f32_kernel<<<nblk32, CG_BLOCK, 0, st>>>(nchunks32, geo.L3h, NCH32, (const float4*)e32, (double2*)x);
+        count_launch();
+        rc = check_launch("cg mixed outer iteration");
+        if (rc != HR_OK) return rc;
+        ++outer;
+    }
+    if (outer_out) *outer_out = outer;
+    if (inner_out) *inner_out = inner_total;
+    if (relres_out) *relres_out = relres;
+    return HR_OK;
+}
+
 }  // namespace hr

@@ -109,6 +109,14 @@ def test_argument_checks_happen_before_any_cuda_call(L):
         hr.hr_cg_solve(g, 0.0, 4096, None, None, 1 << 20, 1 << 20, 1 << 24, 1e-8, 10)
     assert e.value.status == hr.EINVAL
     assert hr.hr_cg_workspace_bytes(g) >= 5 * hr.hr_spinor_bytes(g, hr.EVEN)
+    with pytest.raises(hr.HrError) as e:   # hr_cg_solve_mixed: the geometry must describe the fp64 fields
+        hr.hr_cg_solve_mixed(hr.geom((4, 4, 4, 4), prec=hr.PREC_F32), 0.0, 4096, 8192, 1 << 20, 1 << 21, 1 << 24, 1e-10)
+    assert e.value.status == hr.EINVAL
+    with pytest.raises(hr.HrError) as e:   # inner_tol must be below 1
+        hr.hr_cg_solve_mixed(g, 0.0, 4096, 8192, 1 << 20, 1 << 21, 1 << 24, 1e-10, inner_tol=1.5)
+    assert e.value.status == hr.EINVAL
+    assert hr.hr_cg_mixed_workspace_bytes(g) > hr.hr_cg_workspace_bytes(hr.geom((4, 4, 4, 4), prec=hr.PREC_F32))
+    assert hr.hr_cg_mixed_workspace_bytes(hr.geom((4, 4, 4, 4), prec=hr.PREC_F32)) == 0
     gt = hr.geom((2, 2, 2, 2), kernel=hr.KERNEL_TILED)
     with pytest.raises(hr.HrError) as e:
         hr.hr_dirac_apply(gt, 0.0, 4096, 1 << 20, 1 << 21)

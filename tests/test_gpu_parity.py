@@ -587,3 +587,37 @@ def test_exponential_clover(hr, orc, L, prec):
         lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
         want = orc.dirac_eo_clover(L, U, A, Ainv, psi, nthreads=NTHREADS)
         assert rel(lat.get_spinor(out), want) <= TOL[prec], kernel
+
+
+@pytest.mark.parametrize("L,rep", [((8, 4, 4, 8), 0), ((4, 4, 4, 4), 1), ((8, 2, 8, 6), 0)])
+def test_mixed_precision_cg(hr, orc, L, rep):
+    """hr_cg_solve_mixed (fp64 defect correction around fp32 CG) reaches the oracle's fp64 solution: same x, a true
+    residual (evaluated with the ORACLE's operator) at the requested 1e-12, in a handful of corrections"""
+    import torch
+    m0, tol = -0.2, 1e-12
+    N = 2 if rep == 0 else 3
+    Uf = inputs.haar_gauge(L, 1)
+    U = Uf if rep == 0 else orc.represent(Uf)[0]
+    b = inputs.gaussian_spinor(L, N, 2)
+    even = inputs.site_parity(L) == 0
+    b[~even] = 0
+    x_orc, it_orc, _ = orc.cg_normal(L, rep, m0, U, b, tol=tol, max_iter=1000, nthreads=NTHREADS)
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+    for kernel in kernels_for(hr, L, rep, 0):
+        l64, l32 = lattice(hr, L, rep, 0, kernel), lattice(hr, L, rep, 1, kernel)
+        put = (lambda lat: lat.put_gauge_fund(U)) if rep == 0 else (lambda lat: lat.put_gauge_adj(U))
+        U64, U32 = put(l64), put(l32)
+        b_dev = l64.put_spinor(b)
+        x_half = l64.empty_spinor(hr.EVEN)
+        ws = hr.device_buffer(hr.hr_cg_mixed_workspace_bytes(l64.g))
+        outer, inner, relres = hr.hr_cg_solve_mixed(l64.g, m0, U64, U32, l64.even(b_dev), x_half, ws, tol, 1e-4, 20, 1000, 5, hr.stream_ptr())
+        assert relres <= tol and 2 <= outer <= 6, (outer, inner, relres)
+        assert inner <= 3 * it_orc + 30, (inner, it_orc)
+        full = torch.zeros_like(b_dev)
+        l64.even(full).copy_(x_half)
+        x = l64.get_spinor(full)
+        assert not x[~even].any()
+        assert rel(x, x_orc) <= 1e-9, kernel
+        t = orc.dirac_eo(L, rep, m0, U, x, nthreads=NTHREADS)
+        r = b - g5 * orc.dirac_eo(L, rep, m0, U, g5 * t, nthreads=NTHREADS)
+        assert np.linalg.norm(r) <= 10 * tol * np.linalg.norm(b)
