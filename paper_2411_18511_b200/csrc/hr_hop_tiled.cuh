@@ -61,6 +61,9 @@ constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, two b
 #ifndef HR_T_NBDB_FULL
 #define HR_T_NBDB_FULL 0
 #endif
+#ifndef HR_T_L3H_F32_FULL
+#define HR_T_L3H_F32_FULL 0
+#endif
 #ifndef HR_T_F32_WIDE
 #define HR_T_F32_WIDE 1
 #endif
@@ -485,7 +488,8 @@ inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan&
 template <typename T, int N, int EPI, int MODE, int T1, int T2, bool ONFLY>
 inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
     // (measured at 48^4: fp64 hop 219.3 -> 216.1 us, H3 411 -> 408; the fp32 4x4 H3 got slower, so fp64 only)
-    if (N == 2 && sizeof(T) == 8 && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, MODE, T1, T2, ONFLY, ((N == 2 && sizeof(T) == 8) ? 24 : 0)>(g, a, pl, st);
+    constexpr bool SPECIALISE = N == 2 && (sizeof(T) == 8 || (MODE == 2 && HR_T_L3H_F32_FULL));
+    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, MODE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0)>(g, a, pl, st);
     return launch_hop_tiled_l3h<T, N, EPI, MODE, T1, T2, ONFLY, 0>(g, a, pl, st);
 }
 
