@@ -244,6 +244,23 @@ def run_ours(args):
                 "avg_launch_ms": round(hop_ms, 4), "traffic": traffic,
                 "fp32": {"achieved": round(model["hop_oe_f32"]["bytes"] / (0.5 * (op_report["hop_oe_f32"]["ms"] + op_report["hop_eo_f32"]["ms"])) / 1e6, 1)}}
     roofline["fp32"]["frac"] = round(roofline["fp32"]["achieved"] / peak, 4)
+    # the same kernel timed as 30 back-to-back launches between ONE pair of events (no per-launch event gaps): context for
+    # `achieved`, which is measured inside the step with an event pair around every launch
+    b2b = {}
+    for tag in ("f64", "f32"):
+        fn = [o for o in ops if o[0] == "hop_oe_" + tag][0][4]
+        for _ in range(3):
+            fn()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for _ in range(30):
+            fn()
+        t1.record()
+        torch.cuda.synchronize()
+        ms = t0.elapsed_time(t1) / 30
+        b2b[tag] = {"avg_launch_ms": round(ms, 4), "achieved": round(model["hop_oe_" + tag]["bytes"] / ms / 1e6, 1),
+                    "frac": round(model["hop_oe_" + tag]["bytes"] / ms / 1e6 / peak, 4)}
+    roofline["back_to_back_30_launches"] = b2b
 
     # ---- end to end through the host-buffer C-ABI entry points (pinned host memory, copies inside the timed region)
     e2e = None
