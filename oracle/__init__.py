@@ -218,7 +218,7 @@ def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1, A=None, Ai
 
 
 # ------------------------------------------------------------------ O9: exponential clover term
-def clover_exp_dense(L, diag, csw, U, nthreads=1):
+def clover_exp_dense(L, diag, csw, U, nthreads=1, begin=0, end=None):
     """O9 ("exponential of the clover term ... the diagonal part of the Dirac operator and its inverse
     take the same time to execute", ref [6] at PAPER.md:123; reading B4 of DESIGN.md §3): the site-diagonal term of
     the exponential clover improvement,
@@ -226,7 +226,9 @@ def clover_exp_dense(L, diag, csw, U, nthreads=1):
     with C(x) = csw (i/4) sum_{mu,nu} sigma_mu,nu F^_mu,nu(x) the clover term of O5 (the regular term is diag + C,
     the first two orders of this exponential).  The exponential of the hermitian 8x8 matrix C/diag is taken from
     its eigendecomposition, exp(H) = V diag(e^lambda) V^dag.  Returns (A_exp, A_exp^-1), dense [V,8,8]."""
-    A = clover_dense(L, diag, csw, U, nthreads=nthreads)
+    # (begin, end: restrict to the lex sites [begin, end); the returned arrays then hold only those sites)
+    end = _vol(L) if end is None else end
+    A = clover_dense(L, diag, csw, U, begin, end, nthreads)[begin:end]
     C = A - diag * np.eye(8)[None]
     lam, V = np.linalg.eigh(C / diag)
     Vh = np.conj(np.swapaxes(V, -1, -2))

@@ -621,3 +621,46 @@ def test_mixed_precision_cg(hr, orc, L, rep):
         t = orc.dirac_eo(L, rep, m0, U, x, nthreads=NTHREADS)
         r = b - g5 * orc.dirac_eo(L, rep, m0, U, g5 * t, nthreads=NTHREADS)
         assert np.linalg.norm(r) <= 10 * tol * np.linalg.norm(b)
+
+
+# ------------------------------------------------------------------ the widened rows at the bench size
+def test_48to4_cg_and_exponential_clover(hr, orc, big_inputs):
+    """at 48^4, in the launch configuration bench.py times: (i) hr_cg_solve and hr_cg_solve_mixed reach a TRUE residual
+    (evaluated with the oracle's Dhat on the GPU's solution) at the requested level; (ii) hr_clover_build_exp
+    blocks against the oracle's O9 on a slab of sites"""
+    import torch
+    L, U, psi = big_inputs
+    m0 = -0.2
+    even = inputs.site_parity(L) == 0
+    b = psi.copy()
+    b[~even] = 0
+    l64, l32 = lattice(hr, L, 0, 0), lattice(hr, L, 0, 1)
+    U64, U32 = l64.put_gauge_fund(U), l32.put_gauge_fund(U)
+    b_dev = l64.put_spinor(b)
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+
+    def true_relres(x_half):
+        full = torch.zeros_like(b_dev)
+        l64.even(full).copy_(x_half)
+        x = l64.get_spinor(full)
+        t = orc.dirac_eo(L, 0, m0, U, x, nthreads=NTHREADS)
+        r = b - g5 * orc.dirac_eo(L, 0, m0, U, g5 * t, nthreads=NTHREADS)
+        return float(np.linalg.norm(r) / np.linalg.norm(b))
+
+    x_half, it, relres = l64.cg(m0, U64, l64.even(b_dev), 1e-10, 500)
+    assert relres <= 1e-10 and 10 < it < 200
+    assert true_relres(x_half) <= 2e-10
+    xm = l64.empty_spinor(hr.EVEN)
+    ws = hr.device_buffer(hr.hr_cg_mixed_workspace_bytes(l64.g))
+    outer, inner, rel_m = hr.hr_cg_solve_mixed(l64.g, m0, U64, U32, l64.even(b_dev), xm, ws, 1e-12, 1e-4, 20, 500, 5, hr.stream_ptr())
+    assert rel_m <= 1e-12 and outer <= 6
+    assert true_relres(xm) <= 1e-11
+    # (ii) exponential clover blocks on the first 2 x 48^3 sites
+    m0c, csw = -0.25, 1.2
+    Uw = inputs.weak_gauge(L, 0.3, 1)
+    fwd, inv = l64.clover_build(m0c, csw, l64.put_gauge_fund(Uw), exponential=True)
+    n = 2 * 48 ** 3
+    A, Ainv = orc.clover_exp_dense(L, 4.0 + m0c, csw, Uw, nthreads=NTHREADS, begin=0, end=n)
+    bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+    assert np.linalg.norm(l64.get_clover(fwd)[:n] - bf) <= 1e-13 * np.linalg.norm(bf)
+    assert np.linalg.norm(l64.get_clover(inv)[:n] - bi) <= 1e-13 * np.linalg.norm(bi)
