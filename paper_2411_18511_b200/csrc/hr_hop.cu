@@ -7,16 +7,19 @@ namespace hr {
 // many small CTAs spread better there than one marching CTA per tile
 static const double TILED_AUTO_MIN_SITES = 32.0 * 32.0 * 32.0 * 32.0;
 
-static int sm_count() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+static int sm_count() {   // of the calling thread's current device (cached per device)
+    static int cache[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return 148; }
+    if (cache[dev] == 0) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
             (void)cudaGetLastError();
             n = 148;
         }
+        cache[dev] = n;
     }
-    return n;
+    return cache[dev];
 }
 
 bool tiled_supported(const hr_geom* g) {

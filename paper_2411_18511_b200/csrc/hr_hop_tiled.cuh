@@ -473,11 +473,15 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl, 
 template <typename T, int N, int EPI, int MODE, int T1, int T2, bool ONFLY, int L3H>
 inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
     auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, MODE, ONFLY, L3H>;
-    static bool configured = false;   // per instantiation
-    if (!configured) {
+    // the opt-in to > 48 KiB of dynamic shared memory is a per-device attribute of the function: once per
+    // instantiation and device (a benign race: two threads may both set it)
+    static bool configured[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
+    if (!configured[dev]) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
         if (e != cudaSuccess) { set_error("cudaFuncSetAttribute(hop_tiled_kernel): %s", cudaGetErrorString(e)); return HR_ECUDA; }
-        configured = true;
+        configured[dev] = true;
     }
     const unsigned grid = (unsigned)(((a.both && MODE != 2) ? 2 : 1) * pl.nt1 * pl.nt2 * pl.nseg);
     kern<<<grid, pl.nconsumer + 32, pl.smem, st>>>(g, a, pl);
