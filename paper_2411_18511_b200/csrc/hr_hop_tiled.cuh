@@ -67,8 +67,12 @@ constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, two b
 #ifndef HR_T_F32_WIDE
 #define HR_T_F32_WIDE 1
 #endif
-// threads per CTA the kernel is compiled for: one per site of a T1 x T2 tile of rows with L3h <= 24, + producer warp
-constexpr int tiled_max_threads(int t1, int t2) { return ((t1 * t2 * 24 + 31) / 32) * 32 + 32; }
+// consumer threads per output parity the kernel is compiled for (one per site of a T1 x T2 tile of rows): 192 for the
+// small tiles (2 x 4 rows of L3h <= 24 sites, 2 x 2 rows of L3h <= 48), 384 for 4 x 4 rows; MODE 2 (both parities per
+// CTA, twice the threads) keeps to T1*T2*24 so that its register budget stays at 255
+constexpr int tiled_max_consumers(int t1, int t2, int mode) {
+    return mode == 2 ? ((t1 * t2 * 24 + 31) / 32) * 32 : (t1 * t2 <= 8 ? 192 : 384);
+}
 
 // ------------------------------------------------------------------ mbarrier / bulk-copy primitives (PTX)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -169,7 +173,7 @@ struct TiledPlan {
 // L3H: compile-time L3/2 (0 = read it from the geometry): the strides between the 16-byte chunks of a site are then
 // immediates in every LDS / LDG / STG (about a quarter fewer instructions per site)
 template <typename T, int N, int EPI, int T1, int T2, int MODE, bool ONFLY, int L3H>
-__global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * (tiled_max_threads(T1, T2) - 32) + 32, (MODE != 2 && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
+__global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, T2, MODE) + 32, (MODE != 2 && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g_in, HopArgs a, TiledPlan pl) {
     Geo g = g_in;
     if (L3H > 0) g.L3h = L3H;
@@ -420,7 +424,7 @@ inline bool tiled_plan_shape(const hr_geom* hg, int both, int mode, int num_sms,
     const int L1 = hg->L[1], L2 = hg->L[2], L0 = hg->L[0];
     if (L1 % t1 || L2 % t2) return false;
     const int sites = t1 * t2 * g.L3h;
-    if (sites > tiled_max_threads(t1, t2) - 32) return false;
+    if (sites > tiled_max_consumers(t1, t2, mode)) return false;
     const int npar = mode == 2 ? 2 : 1;
     pl.t1 = t1;
     pl.t2 = t2;
@@ -467,7 +471,9 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl, 
 #if HR_T_F32_WIDE
     if (hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, mode, num_sms, 4, 4, pl)) return true;
 #endif
-    return tiled_plan_shape(hg, both, mode, num_sms, 2, 4, pl);
+    if (tiled_plan_shape(hg, both, mode, num_sms, 2, 4, pl)) return true;
+    // longer rows (24 < L3/2 <= 48) or L2 not a multiple of 4: 2 x 2 rows, fundamental representation only
+    return hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, mode, num_sms, 2, 2, pl);
 }
 
 template <typename T, int N, int EPI, int MODE, int T1, int T2, bool ONFLY, int L3H>
@@ -500,6 +506,7 @@ inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPla
 template <typename T, int N, int EPI, int MODE, bool ONFLY>
 inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
     if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, MODE, 2, 4, ONFLY>(g, a, pl, st);
+    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, MODE, 2, 2, false>(g, a, pl, st);
 #if HR_T_F32_WIDE
     if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, MODE, 4, 4, false>(g, a, pl, st);
 #endif

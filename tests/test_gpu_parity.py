@@ -125,7 +125,7 @@ def test_device_layout_is_the_documented_one(hr):
 
 
 # ------------------------------------------------------------------ config 0 and the edge lattices
-@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (4, 4, 4, 2), (6, 2, 4, 12), (8, 4, 4, 16), (4, 8, 8, 8)])
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (4, 4, 4, 2), (6, 2, 4, 12), (8, 4, 4, 16), (4, 8, 8, 8), (4, 2, 4, 52), (2, 2, 2, 96)])
 @pytest.mark.parametrize("prec", [0, 1])
 def test_fundamental_small_lattices(hr, orc, L, prec):
     """configs[0] (4^4, Haar links, m0 = -0.2: full D and even-odd operator) plus degenerate and ragged extents"""
