@@ -93,6 +93,12 @@ int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* 
  * psi, out: full-lattice spinors (out must not alias psi). */
 int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, void* out, void* stream);
 
+/* H3c (north_star "optional clover-improved form"; "Clover improvement ... requires the application of
+ * another diagonal term"): the clover-improved operator on all V sites in one launch,
+ *     out = D_sw psi = A psi - 1/2 H psi,      A(x) = (4+m0) + C(x)  the forward blocks of hr_clover_build[_exp]
+ * (m0 lives inside the blocks).  Fundamental representation only; out must not alias psi. */
+int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fwd, const void* psi, void* out, void* stream);
+
 /* H1/H2/E1/E2 (north_star "even-odd preconditioned form D_ee - D_eo D_oo^-1 D_oe as used in the HMC";
  * PAPER.md:39 "even-odd preconditioned version of the Dirac operator used mainly in the HMC").
  *   op = HR_EO_HOP_OE : out_o = H_oe in_e   (bare hopping sum, no -1/2), in: even half field, out: odd half field

@@ -193,6 +193,18 @@ int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, 
     return run_hop(g, a, EPI_AXPY, (cudaStream_t)stream);
 }
 
+int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fwd, const void* psi, void* out, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    if (g->rep != HR_REP_FUND) { set_error("clover operators exist for the fundamental representation only"); return HR_EUNSUPPORTED; }
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(psi, "psi")); HR_TRY(check_ptr(out, "out"));
+    const size_t full = 2 * half_spinor_bytes(g);
+    if (overlap(psi, full, out, full)) { set_error("hr_dirac_clover_apply: out aliases psi (gather operation)"); return HR_EINVAL; }
+    HopArgs a;
+    a.gauge = u; a.in = psi; a.out = out; a.phi = psi; a.clover = clover_fwd;
+    a.a = 1.0; a.c = -0.5; a.parity = 0; a.both = 1;
+    return run_hop(g, a, EPI_CLOVER_AXPY, (cudaStream_t)stream);
+}
+
 // ---------------------------------------------------------------- H1 / E1 / E2
 int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const void* clover_fwd,
                       const void* clover_inv, const void* in, void* out, void* tmp, void* stream) {

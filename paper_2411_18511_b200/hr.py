@@ -27,7 +27,7 @@ SYMBOLS = [
     "hr_spinor_bytes", "hr_gauge_bytes", "hr_clover_bytes", "hr_canonical_spinor_bytes",
     "hr_canonical_gauge_bytes", "hr_canonical_clover_bytes", "hr_pack_spinor", "hr_unpack_spinor",
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
-    "hr_dirac_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_dirac_flops_bytes",
+    "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_cg_workspace_bytes", "hr_cg_solve",
     "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed",
@@ -67,6 +67,7 @@ def lib():
             "hr_pack_clover": (I, [G, V, V, V]), "hr_unpack_clover": (I, [G, V, V, V]),
             "hr_represent_gauge": (I, [G, V, V, V]),
             "hr_dirac_apply": (I, [G, D, V, V, V, V]),
+            "hr_dirac_clover_apply": (I, [G, V, V, V, V, V]),
             "hr_dirac_eo_apply": (I, [G, I, D, V, V, V, V, V, V, V]),
             "hr_clover_build": (I, [G, D, D, V, V, V, V]),
             "hr_clover_build_exp": (I, [G, D, D, V, V, V, V]),
@@ -156,6 +157,10 @@ def hr_represent_gauge(g, u_fund, u_adj, stream=0):
 
 def hr_dirac_apply(g, m0, u, psi, out, stream=0):
     _check(lib().hr_dirac_apply(ctypes.byref(g), float(m0), _ptr(u), _ptr(psi), _ptr(out), stream))
+
+
+def hr_dirac_clover_apply(g, u, clover_fwd, psi, out, stream=0):
+    _check(lib().hr_dirac_clover_apply(ctypes.byref(g), _ptr(u), _ptr(clover_fwd), _ptr(psi), _ptr(out), stream))
 
 
 def hr_dirac_eo_apply(g, op, m0, u, clover_fwd, clover_inv, inp, out, tmp, stream=0):

@@ -101,6 +101,11 @@ class Lattice:
         hr.hr_dirac_apply(self.g, m0, u, psi, out, hr.stream_ptr())
         return out
 
+    def dirac_clover(self, u, clover_fwd, psi, out=None):
+        out = self.empty_spinor() if out is None else out
+        hr.hr_dirac_clover_apply(self.g, u, clover_fwd, psi, out, hr.stream_ptr())
+        return out
+
     def hop(self, op, u, inp, out=None):
         """op EO_HOP_OE: inp even half -> odd half;  EO_HOP_EO: odd half -> even half"""
         out = self.empty_spinor(hr.EVEN) if out is None else out

@@ -117,9 +117,9 @@ def test_argument_checks_happen_before_any_cuda_call(L):
     assert e.value.status == hr.EINVAL
     assert hr.hr_cg_mixed_workspace_bytes(g) > hr.hr_cg_workspace_bytes(hr.geom((4, 4, 4, 4), prec=hr.PREC_F32))
     assert hr.hr_cg_mixed_workspace_bytes(hr.geom((4, 4, 4, 4), prec=hr.PREC_F32)) == 0
-    gt = hr.geom((2, 2, 2, 2), kernel=hr.KERNEL_TILED)
+    gt = hr.geom((4, 4, 4, 200), kernel=hr.KERNEL_TILED)   # rows of 100 sites per parity: no tile shape fits
     with pytest.raises(hr.HrError) as e:
-        hr.hr_dirac_apply(gt, 0.0, 4096, 1 << 20, 1 << 21)
+        hr.hr_dirac_apply(gt, 0.0, 4096, 1 << 30, 1 << 31)
     assert e.value.status == hr.EUNSUPPORTED
 
 

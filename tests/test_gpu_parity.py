@@ -341,6 +341,11 @@ def test_clover_small_lattices(hr, orc, L, prec):
         half = torch.zeros_like(psi_dev)
         lat.clover_apply(hr.ODD, inv, lat.odd(psi_dev), lat.odd(half))
         assert rel(lat.get_spinor(half), orc.site_matvec(L, 2, Ainv, psi)) <= TOL[prec]
+        # H3c: the clover-improved operator on all sites, D_sw psi = A psi - H psi / 2 (oracle: O1 + O5)
+        dsw = lat.empty_spinor()
+        hr.hr_dirac_clover_apply(lat.g, U_dev, fwd, psi_dev, dsw, hr.stream_ptr())
+        C = A - (4.0 + m0) * np.eye(8)[None]
+        assert rel(lat.get_spinor(dsw), orc.dirac_clover(L, m0, U, C, psi, nthreads=NTHREADS)) <= TOL[prec], kernel
         # E2 with the GPU's own blocks
         out = torch.zeros_like(psi_dev)
         lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
