@@ -400,6 +400,22 @@ def cg_report(hr, S, m0):
         out["cg_48^4_" + tag] = {"ms_per_iteration": round(ms, 4), "iterations": it, "relres_after": rel,
                                  "gbs": round(bytes_site * Vh / ms / 1e6, 1), "bytes_per_even_site_per_iteration": bytes_site}
         del ws, x
+    # H3c: the clover-improved full operator in one launch (not part of the step), fp64; bytes = H3 + clover blocks
+    s64 = S["f64"]
+    lat, g = s64["lat"], s64["lat"].g
+    st = hr.stream_ptr()
+    fn = lambda: hr.hr_dirac_clover_apply(g, s64["Uw"], s64["fwd"], s64["psi"], s64["out"], st)
+    for _ in range(3):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(20):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 20
+    _, bc, _ = hr.hr_dirac_flops_bytes(g, hr.OP_DIRAC)
+    out["dirac_clover_48^4_f64"] = {"ms": round(ms, 4), "gbs": round((bc + 256.0) * lat.V / ms / 1e6, 1), "bytes_per_site": bc + 256.0}
     # time to a 1e-12 solution: plain fp64 CG against fp64 defect correction around fp32 CG (hr_cg_solve_mixed)
     s64, s32 = S["f64"], S["f32"]
     lat, g = s64["lat"], s64["lat"].g

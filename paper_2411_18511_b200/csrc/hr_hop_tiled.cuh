@@ -528,7 +528,9 @@ inline int launch_hop_tiled(const Geo& g, const HopArgs& a, int epi, const Tiled
             if (a.both) return launch_hop_tiled_epi<T, N, EPI_AXPY, 1, ONFLY>(g, a, pl, st);
             return launch_hop_tiled_epi<T, N, EPI_AXPY, 0, ONFLY>(g, a, pl, st);
         case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV, 0, ONFLY>(g, a, pl, st);
-        case EPI_CLOVER_AXPY: return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, 0, ONFLY>(g, a, pl, st);
+        case EPI_CLOVER_AXPY:
+            if (a.both) return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, 1, ONFLY>(g, a, pl, st);   // H3c: links re-read by the other parity's CTA
+            return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, 0, ONFLY>(g, a, pl, st);
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
 }
