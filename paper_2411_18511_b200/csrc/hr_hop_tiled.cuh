@@ -19,6 +19,8 @@
 namespace hr {
 
 constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live + one being filled
+// Tuning switches (HR_T_*): the defaults are the measured choices of profiles/r01_tiled_variants.md; a build with
+// other values is made with HR_NVCC_DEFS="-DHR_T_...=v" python -m paper_2411_18511_b200.build --force.
 #ifndef HR_T_HALO
 #define HR_T_HALO 2
 #endif
@@ -37,7 +39,7 @@ constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live 
 #ifndef HR_T_NBDB_F32
 #define HR_T_NBDB_F32 1
 #endif
-constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, two being filled (the halo is 60 % of a step's bytes)
+constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, one being filled (a third one costs the L1 the link loads need)
 //   LINKPOL : cache policy of the link loads (LD_STREAM = ld.global.cs, LD_KEEP = ld.global.nc)
 #ifndef HR_T_LINKPOL_F64
 #define HR_T_LINKPOL_F64 LD_KEEP
