@@ -235,3 +235,61 @@ def clover_exp_dense(L, diag, csw, U, nthreads=1, begin=0, end=None):
     fwd = diag * (V * np.exp(lam)[:, None, :]) @ Vh
     inv = (V * np.exp(-lam)[:, None, :]) @ Vh / diag
     return fwd, inv
+
+
+# ------------------------------------------------------------------ O10: clover term in the adjoint representation
+def clover_dense_adj(L, diag, csw, R):
+    """O10 (SURVEY.md §8(f) item 3 "adjoint-representation clover"): the clover term of O5 with the
+    real 3x3 adjoint links R in place of U (dagger = transpose), acting on 4 spin x 3 colour:
+        A(x) = diag + C(x),  C = csw (i/2) sum_{mu<nu} sigma_mu,nu (x) F^_mu,nu,  sigma_mu,nu = (i/2)[gamma_mu, gamma_nu],
+        F^_mu,nu = (Q - Q^T)/8,  Q = P1 + P2 + P3 + P4 the four leaves of O5 that start and end at x (mu -> nu sense).
+    R: real [V,4,3,3].  Returns dense [V,12,12] complex (row/col = spin*3 + colour).  Whole-lattice numpy shifts."""
+    R = np.ascontiguousarray(R, dtype=np.float64)
+    Lt = tuple(int(v) for v in L)
+    V = _vol(L)
+    Rg = R.reshape(Lt + (4, 3, 3))
+    gam = gamma()
+
+    def at(mu, shift):      # U_mu(x + shift), shift a dict {axis: displacement}
+        a = Rg[..., mu, :, :]
+        for ax, d in shift.items():
+            a = np.roll(a, -d, axis=ax)
+        return a
+
+    def T(m):
+        return np.swapaxes(m, -1, -2)
+
+    A = np.zeros((V, 12, 12), dtype=np.complex128)
+    A += diag * np.eye(12)[None]
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            P1 = at(mu, {}) @ at(nu, {mu: 1}) @ T(at(mu, {nu: 1})) @ T(at(nu, {}))
+            P2 = at(nu, {}) @ T(at(mu, {mu: -1, nu: 1})) @ T(at(nu, {mu: -1})) @ at(mu, {mu: -1})
+            P3 = T(at(mu, {mu: -1})) @ T(at(nu, {mu: -1, nu: -1})) @ at(mu, {mu: -1, nu: -1}) @ at(nu, {nu: -1})
+            P4 = T(at(nu, {nu: -1})) @ at(mu, {nu: -1}) @ at(nu, {mu: 1, nu: -1}) @ T(at(mu, {}))
+            Q = P1 + P2 + P3 + P4
+            F = ((Q - T(Q)) / 8.0).reshape(V, 3, 3)
+            sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
+            A += csw * 0.5j * np.einsum("st,xab->xsatb", sig, F).reshape(V, 12, 12)
+    return A
+
+
+def site_matvec_n(M, psi, mask=None):
+    """out[x] = M[x] psi[x] for dense [V,n,n] site matrices and spinors [V,4,N] (n = 4N); sites with mask False -> 0."""
+    V = psi.shape[0]
+    out = np.einsum("xij,xj->xi", M, psi.reshape(V, -1)).reshape(psi.shape)
+    if mask is not None:
+        out = np.where(mask[:, None, None], out, 0.0)
+    return out
+
+
+def dirac_eo_clover_adj(L, R, A, Ainv, psi, nthreads=1):
+    """O7 in the adjoint representation: Dhat psi_e = A_ee psi_e - 1/4 H_eo A_oo^-1 H_oe psi_e (odd output = 0);
+    A, Ainv dense [V,12,12] (clover_dense_adj with diag = 4 + m0 and its inverse)."""
+    par = (np.indices(tuple(int(v) for v in L)).sum(axis=0) % 2).reshape(-1)     # (x0+x1+x2+x3) mod 2, lex order
+    even, odd = par == 0, par == 1
+    pe = np.where(even[:, None, None], psi, 0.0)
+    t = hop(L, 1, 1, R, pe, nthreads=nthreads)              # H_oe psi_e on odd sites
+    t = site_matvec_n(Ainv, t, odd)
+    h = hop(L, 1, 0, R, t, nthreads=nthreads)               # H_eo (...) on even sites
+    return site_matvec_n(A, pe, even) - 0.25 * h

@@ -492,3 +492,82 @@ def test_P16_exponential_clover(orc):
     assert 3.5 < ratio < 4.7          # quadratic in csw
     f0, i0 = orc.clover_exp_dense(L, d, 0.0, U)
     assert np.abs(f0 - d * eye).max() <= 1e-14 and np.abs(i0 - eye / d).max() <= 1e-15
+
+
+def test_P17_adjoint_clover(orc):
+    """O10.  (a) leaves: for every site of a 2x2x2x4 lattice and every plane, the sum of the four FUNDAMENTAL leaves,
+    multiplied out here with explicit (x +- mu) mod L site arithmetic and mapped leaf by leaf through O4 (R is a
+    homomorphism, pin P7), gives the adjoint Q whose antisymmetric part O10 uses — paths, orientation, transposes;
+    (b) C hermitian, traceless, commuting with gamma5; (c) gauge covariance C[U^g](x) = R(g(x)) C(x) R(g(x))^T on
+    colour; (d) abelian links exp(i phi sigma3): R is a rotation by 2 phi about axis 3 and
+    F^_mu,nu = (1/4) J3 sum_leaves sin(2 P_leaf), J3 = [[0,-1,0],[1,0,0],[0,0,0]]... sign fixed by O4's orientation."""
+    L = (2, 2, 2, 4)
+    V = inputs.volume(L)
+    U = inputs.haar_gauge(L, 1)
+    R, _ = orc.represent(U)
+    gam = orc.gamma()
+    x_of = inputs.site_coords(L)
+
+    def lex(x):
+        return ((x[0] % L[0] * L[1] + x[1] % L[1]) * L[2] + x[2] % L[2]) * L[3] + x[3] % L[3]
+
+    def u(x, mu, dag=False):
+        m = U[lex(x), mu]
+        return m.conj().T if dag else m
+
+    def e(mu):
+        v = np.zeros(4, dtype=int)
+        v[mu] = 1
+        return v
+
+    d, csw = 3.7, 1.3
+    A = orc.clover_dense_adj(L, d, csw, R)
+    for s in range(0, V, 5):
+        x = x_of[s]
+        C = np.zeros((12, 12), dtype=complex)
+        for mu in range(4):
+            for nu in range(mu + 1, 4):
+                m, n = e(mu), e(nu)
+                leaves = [u(x, mu) @ u(x + m, nu) @ u(x + n, mu, True) @ u(x, nu, True),
+                          u(x, nu) @ u(x - m + n, mu, True) @ u(x - m, nu, True) @ u(x - m, mu),
+                          u(x - m, mu, True) @ u(x - m - n, nu, True) @ u(x - m - n, mu) @ u(x - n, nu),
+                          u(x - n, nu, True) @ u(x - n, mu) @ u(x + m - n, nu) @ u(x, mu, True)]
+                Q = sum(orc.represent(np.array([[[p]]]).reshape(1, 1, 2, 2))[0][0, 0] for p in leaves)
+                F = (Q - Q.T) / 8.0
+                sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
+                C += csw * 0.5j * np.kron(sig, F)
+        assert np.abs(A[s] - d * np.eye(12) - C).max() <= 1e-13
+    # (b)
+    Cf = A - d * np.eye(12)[None]
+    assert np.abs(Cf - np.conj(np.swapaxes(Cf, -1, -2))).max() <= 1e-15
+    assert np.abs(np.trace(Cf, axis1=1, axis2=2)).max() <= 1e-14
+    g5 = np.kron(np.diag([1, 1, -1, -1]), np.eye(3)).astype(complex)
+    assert np.abs(g5 @ Cf - Cf @ g5).max() <= 1e-15
+    # (c)
+    g = inputs.haar_sites(L, 4)
+    Rg_links, _ = orc.represent(gauge_transform(U, g, L))
+    Rg = orc.represent(g.reshape(V, 1, 2, 2))[0][:, 0]
+    big = np.einsum("st,xab->xsatb", np.eye(4), Rg).reshape(V, 12, 12)
+    Cg = orc.clover_dense_adj(L, 0.0, csw, Rg_links)
+    assert np.abs(Cg - big @ Cf @ np.swapaxes(big, -1, -2)).max() <= 1e-13
+    # (d) abelian: U_mu(x) = exp(i phi_mu(x) sigma3)
+    phi = 0.4 * inputs.normals(11, 9, 0, V * 4).reshape(L + (4,))
+    Uab = np.zeros((V, 4, 2, 2), dtype=complex)
+    Uab[:, :, 0, 0] = np.exp(1j * phi.reshape(V, 4))
+    Uab[:, :, 1, 1] = np.exp(-1j * phi.reshape(V, 4))
+    Rab, _ = orc.represent(Uab)
+    Aab = orc.clover_dense_adj(L, 0.0, 1.0, Rab)
+    # the rotation angle of R(exp(i t sigma3)) about axis 3: read it off O4 itself on one link, then use it for the sum
+    t = 0.3
+    R1 = orc.represent(np.diag([np.exp(1j * t), np.exp(-1j * t)]).reshape(1, 1, 2, 2))[0][0, 0]
+    J = (R1 - R1.T) / (2 * np.sin(2 * t))           # = +-J3 with the sign O4's orientation gives
+    assert np.abs(np.abs(J) - np.array([[0, 1, 0], [1, 0, 0], [0, 0, 0]])).max() <= 1e-14
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            P = phi[..., mu] + np.roll(phi[..., nu], -1, mu) - np.roll(phi[..., mu], -1, nu) - phi[..., nu]
+            S = np.sin(2 * P) + np.sin(2 * np.roll(P, 1, mu)) + np.sin(2 * np.roll(np.roll(P, 1, mu), 1, nu)) + np.sin(2 * np.roll(P, 1, nu))
+            Fcf = (S.reshape(V)[:, None, None] / 4.0) * J[None]
+            # extract F^_mu,nu from the oracle: C = (i/2) sum sigma (x) F; project with sigma_mu,nu (tr sigma_a sigma_b = 4 delta)
+            sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
+            Fo = np.einsum("ts,xsatb->xab", sig, Aab.reshape(V, 4, 3, 4, 3)) / 4.0 / 0.5j
+            assert np.abs(Fo - Fcf).max() <= 1e-13, (mu, nu)
