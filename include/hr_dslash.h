@@ -21,9 +21,10 @@
  *         spinor        [V][4 spin][N colour][re,im]
  *         fund gauge    [V][4 mu][2 row][2 col][re,im]
  *         adj gauge     [V][4 mu][3 a][3 b]                       (real)
- *         clover blocks [V][2 chirality +,-][16 reals]            (4 real diagonal entries, then the 6
- *                        strictly-lower complex entries (1,0) (2,0) (3,0) (2,1) (3,1) (3,2) as re,im;
- *                        block index = (spin mod 2)*2 + colour)
+ *         clover blocks [V][2 chirality +,-][(2N)^2 reals]        one hermitian 2N x 2N block per chirality, N = 2 / 3
+ *                        colours: 2N real diagonal entries, then the strictly-lower complex entries column by
+ *                        column ((1,0) (2,0) .. (2N-1,0) (2,1) ..) as re,im — 16 reals (fundamental), 36 (adjoint);
+ *                        block index = (spin mod 2)*N + colour
  *     "device layout" = the library's parity-split, x3-row-blocked structure of arrays;
  *     opaque to the caller except through hr_pack_* / hr_unpack_*.  A full-lattice device field is the
  *     even half followed by the odd half, each hr_*_bytes(geom, 0) long, so `field + half` is the odd half.
@@ -96,7 +97,7 @@ int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, 
 /* H3c (north_star "optional clover-improved form"; "Clover improvement ... requires the application of
  * another diagonal term"): the clover-improved operator on all V sites in one launch,
  *     out = D_sw psi = A psi - 1/2 H psi,      A(x) = (4+m0) + C(x)  the forward blocks of hr_clover_build[_exp]
- * (m0 lives inside the blocks).  Fundamental representation only; out must not alias psi. */
+ * (m0 lives inside the blocks).  Both representations; out must not alias psi. */
 int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fwd, const void* psi, void* out, void* stream);
 
 /* H1/H2/E1/E2 (north_star "even-odd preconditioned form D_ee - D_eo D_oo^-1 D_oe as used in the HMC";
@@ -106,7 +107,7 @@ int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fw
  *   op = HR_EO_DHAT   : out_e = Dhat in_e, in and out even half fields, tmp an odd half field;
  *        without clover (clover_fwd == clover_inv == NULL):
  *              Dhat = (4+m0) - H_eo H_oe / (4 (4+m0))
- *        with clover (both non-NULL, built by hr_clover_build with the same m0; fundamental rep only):
+ *        with clover (both non-NULL, built by hr_clover_build[_exp] with the same m0, for g->rep):
  *              Dhat = A_ee - 1/4 H_eo A_oo^-1 H_oe            (m0 is then ignored: it lives inside A)
  *        Two dependent launches on `stream` (the paper's "impossible to parallelise" pair of halves).
  * out must not alias in; tmp must alias neither. */
@@ -115,7 +116,8 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
                       const void* clover_inv, const void* in, void* out, void* tmp, void* stream);
 
 /* C1 ("precomputing certain fields ... recomputed whenever the gauge field is updated"):
- * from the FUNDAMENTAL gauge field build, for every site, the two hermitian 4x4 chirality blocks of
+ * from the FUNDAMENTAL gauge field build, for every site, the two hermitian chirality blocks (4x4 for fundamental
+ * fermions, 6x6 for adjoint ones: g->rep, the leaves mapped to the adjoint representation) of
  *   A(x) = (4+m0) + csw (i/4) sum_{mu,nu} sigma_mu,nu F^_mu,nu(x)      (F^ from the four-leaf clover)
  * into clover_fwd and their inverses into clover_inv (either may be NULL to skip it).  Setup step. */
 int hr_clover_build(const hr_geom* g, double m0, double csw, const void* u_fund, void* clover_fwd,
@@ -132,7 +134,7 @@ int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_f
 
 /* C2/C3 ("application of another diagonal term"): out(x) = B(x) in(x) on the sites of
  * `parity` (HR_EVEN, HR_ODD: in/out are half fields; HR_BOTH: full fields).  `blocks` is the full-lattice
- * block field (forward blocks: C2; inverse blocks: C3 — same kernel).  Fundamental rep only. */
+ * block field (forward blocks: C2; inverse blocks: C3 — same kernel).  Both representations. */
 int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream);
 
 /* M1 ("measured in terms of memory bandwidth"): the work model, per OUTPUT site of `op`,

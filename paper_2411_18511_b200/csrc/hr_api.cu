@@ -15,7 +15,8 @@ int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st);
 int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st);
 int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
-int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
+int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
+int run_clover_apply(const Geo& g, int rep, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
 
 // hr_solver.cu
 size_t cg_workspace_bytes(const hr_geom* g);
@@ -107,7 +108,7 @@ size_t hr_gauge_bytes(const hr_geom* g, int rep) {
 size_t hr_clover_bytes(const hr_geom* g) {
     if (!geom_ok(g)) return 0;
     const Geo geo = make_geo(g);
-    return 2 * (size_t)geo.Vh * clover_chunks(g->prec) * 16;
+    return 2 * (size_t)geo.Vh * clover_chunks(g->prec, g->rep) * 16;
 }
 
 size_t hr_canonical_spinor_bytes(const hr_geom* g) {
@@ -125,7 +126,8 @@ size_t hr_canonical_gauge_bytes(const hr_geom* g, int rep) {
 size_t hr_canonical_clover_bytes(const hr_geom* g) {
     if (!geom_ok(g)) return 0;
     const Geo geo = make_geo(g);
-    return 2 * (size_t)geo.Vh * 32 * real_bytes(g->prec);
+    const size_t d = 2 * (size_t)ncolour(g->rep);
+    return 2 * (size_t)geo.Vh * 2 * d * d * real_bytes(g->prec);
 }
 
 // ---------------------------------------------------------------- pack / unpack
@@ -165,12 +167,12 @@ int hr_unpack_gauge(const hr_geom* g, int rep, const void* dev, void* canon, voi
 }
 int hr_pack_clover(const hr_geom* g, const void* canon, void* dev, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
-    const int cch = clover_chunks(g->prec);
+    const int cch = clover_chunks(g->prec, g->rep);
     return permute_chunks(true, make_geo(g), 1, cch, cch, canon, dev, (cudaStream_t)stream);
 }
 int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_ptr(canon, "canon")); HR_TRY(check_ptr(dev, "dev"));
-    const int cch = clover_chunks(g->prec);
+    const int cch = clover_chunks(g->prec, g->rep);
     return permute_chunks(false, make_geo(g), 1, cch, cch, dev, canon, (cudaStream_t)stream);
 }
 
@@ -195,7 +197,6 @@ int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, 
 
 int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fwd, const void* psi, void* out, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_links(g));
-    if (g->rep != HR_REP_FUND) { set_error("clover operators exist for the fundamental representation only"); return HR_EUNSUPPORTED; }
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(psi, "psi")); HR_TRY(check_ptr(out, "out"));
     const size_t full = 2 * half_spinor_bytes(g);
     if (overlap(psi, full, out, full)) { set_error("hr_dirac_clover_apply: out aliases psi (gather operation)"); return HR_EINVAL; }
@@ -226,8 +227,7 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
     if (clover) {
         if (!clover_fwd || !clover_inv) { set_error("hr_dirac_eo_apply: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
         HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(clover_inv, "clover_inv"));
-        if (g->rep != HR_REP_FUND) { set_error("clover operators exist for the fundamental representation only"); return HR_EUNSUPPORTED; }
-        // E2: tmp_o = A_oo^-1 H_oe in_e ;  out_e = A_ee in_e - 1/4 H_eo tmp_o
+            // E2: tmp_o = A_oo^-1 H_oe in_e ;  out_e = A_ee in_e - 1/4 H_eo tmp_o
         a.in = in; a.out = tmp; a.parity = HR_ODD; a.clover = clover_inv;
         HR_TRY(run_hop(g, a, EPI_CLOVER_INV, st));
         a.in = tmp; a.out = out; a.parity = HR_EVEN; a.clover = clover_fwd; a.phi = in; a.c = -0.25;
@@ -250,6 +250,7 @@ static int clover_build_any(const hr_geom* g, double m0, double csw, int expo, c
     if (4.0 + m0 == 0.0) { set_error("hr_clover_build: 4+m0 = 0"); return HR_EINVAL; }
     if (clover_fwd) HR_TRY(check_ptr(clover_fwd, "clover_fwd"));
     if (clover_inv) HR_TRY(check_ptr(clover_inv, "clover_inv"));
+    if (g->rep == HR_REP_ADJ) return run_clover_build_adj(make_geo(g), g->prec, 4.0 + m0, csw, expo, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
     return run_clover_build(make_geo(g), g->prec, 4.0 + m0, csw, expo, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
 }
 
@@ -265,10 +266,9 @@ int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_f
 
 int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream) {
     HR_TRY(check_geom(g));
-    if (g->rep != HR_REP_FUND) { set_error("clover operators exist for the fundamental representation only"); return HR_EUNSUPPORTED; }
     if (parity < HR_EVEN || parity > HR_BOTH) { set_error("hr_clover_apply: parity %d", parity); return HR_EINVAL; }
     HR_TRY(check_ptr(blocks, "blocks")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
-    return run_clover_apply(make_geo(g), g->prec, parity, blocks, in, out, (cudaStream_t)stream);
+    return run_clover_apply(make_geo(g), g->rep, g->prec, parity, blocks, in, out, (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------- S1
@@ -326,21 +326,19 @@ int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, doubl
     const double nr = 8.0 * N, S = nr * w;
     const double Gf = (g->link_storage != HR_LINKS_FULL ? 4.0 : 8.0) * w, Ga = 9.0 * w;
     const double G = g->rep == HR_REP_FUND ? Gf : (g->link_storage == HR_LINKS_ONTHEFLY ? 4.0 * w : Ga);
-    const double Bk = 32.0 * w;
+    const double Bk = 2.0 * (2 * N) * (2 * N) * w;            // two hermitian 2N x 2N blocks per site
     // per direction: 4N adds to project, two colour mat-vecs, 8N adds to accumulate; x8, minus the first accumulate
     // (rebuilding R from the quaternion, ~30 flops per link, is not counted: the model counts the operator's flops)
     const double Fhop = g->rep == HR_REP_FUND ? 8.0 * N * (16.0 * N + 7.0) : 8.0 * N * (8.0 * N + 7.0);
-    const double Fblk = 208.0;  // two hermitian 4x4 mat-vecs
+    const double Fblk = 2.0 * (2.0 * (2 * N) + 8.0 * (2 * N) * (2 * N - 1));   // two hermitian 2N x 2N mat-vecs: 208 (fund), 504 (adj)
     double f = 0, bc = 0, br = 0;
     switch (op) {
         case HR_OP_HOP: f = Fhop; bc = 2 * S + 8 * G; br = 9 * S + 8 * G; break;
         case HR_OP_DIRAC: f = Fhop + 3 * nr; bc = 2 * S + 4 * G; br = 10 * S + 8 * G; break;
         case HR_OP_DHAT: f = 2 * Fhop + 3 * nr; bc = 5 * S + 16 * G; br = 19 * S + 16 * G; break;
         case HR_OP_CLOVER:
-            if (g->rep != HR_REP_FUND) { set_error("clover: fundamental representation only"); return HR_EUNSUPPORTED; }
             f = Fblk; bc = 2 * S + Bk; br = bc; break;
         case HR_OP_DHAT_CLOVER:
-            if (g->rep != HR_REP_FUND) { set_error("clover: fundamental representation only"); return HR_EUNSUPPORTED; }
             f = 2 * Fhop + 2 * Fblk + 2 * nr; bc = 5 * S + 16 * G + 2 * Bk; br = 19 * S + 16 * G + 2 * Bk; break;
         case HR_OP_REPRESENT: f = 4 * 30.0; bc = 4 * Gf + 4 * Ga; br = bc; break;
         default: set_error("hr_dirac_flops_bytes: unknown op %d", op); return HR_EINVAL;

@@ -54,7 +54,7 @@ inline int ncolour(int rep) { return rep == HR_REP_FUND ? 2 : 3; }
 // 16-byte chunks per spinor / compressed fundamental link / clover site (two blocks)
 inline int spinor_chunks(int rep, int prec) { return 8 * ncolour(rep) * (int)real_bytes(prec) / 16; }
 inline int link_chunks(int prec) { return 4 * (int)real_bytes(prec) / 16; }
-inline int clover_chunks(int prec) { return 32 * (int)real_bytes(prec) / 16; }
+inline int clover_chunks(int prec, int rep = HR_REP_FUND) { const int d = 2 * ncolour(rep); return 2 * d * d * (int)real_bytes(prec) / 16; }
 
 // ------------------------------------------------------------------ complex numbers in registers
 template <typename T>
@@ -318,10 +318,30 @@ __device__ __forceinline__ void herm4_matvec(cplx<T>* y, const T* blk, const cpl
     y[3] = blk[3] * x[3]; cmad(y[3], l30, x[0]); cmad(y[3], l31, x[1]); cmad(y[3], l32, x[2]);
 }
 
-// the 32 reals (two blocks) of one site from the clover field [par][row][chunk][h]
-template <typename T>
+// hermitian D x D block times D-vector, D = 2N (2 spins of one chirality x N colours): blk = D real diagonal entries, then the
+// strictly-lower entries column by column ((1,0) (2,0) .. (D-1,0) (2,1) ..) as re,im — D*D reals.  Generic form of herm4_matvec.
+template <typename T, int D>
+__device__ __forceinline__ void herm_matvec(cplx<T>* y, const T* blk, const cplx<T>* x) {
+#pragma unroll
+    for (int i = 0; i < D; ++i) y[i] = blk[i] * x[i];
+#pragma unroll
+    for (int j = 0; j < D; ++j)
+#pragma unroll
+        for (int i = j + 1; i < D; ++i) {
+            const int k = D + 2 * (j * (2 * D - j - 1) / 2 + (i - j - 1));
+            const cplx<T> l = mk<T>(blk[k], blk[k + 1]);
+            cmad(y[i], l, x[j]);     // row i, column j: L_ij x_j
+            cmadc(y[j], l, x[i]);    // row j, column i: conj(L_ij) x_i
+        }
+}
+
+// reals of the two blocks of one site: 2 (2N)^2
+template <int N> struct CloverSize { static constexpr int reals = 2 * (2 * N) * (2 * N); };
+
+// the block reals of one site from the clover field [par][row][chunk][h]
+template <typename T, int N = 2>
 __device__ __forceinline__ void load_clover(T* blk, const void* field, const Geo& g, int par, int row, int h) {
-    constexpr int CCH = 32 * sizeof(T) / 16;
+    constexpr int CCH = CloverSize<N>::reals * sizeof(T) / 16;
     typedef typename Chunk<T>::type chunk_t;
     const chunk_t* p = reinterpret_cast<const chunk_t*>(field) + ((size_t)par * g.R + row) * (CCH * g.L3h) + h;
 #pragma unroll
@@ -330,11 +350,16 @@ __device__ __forceinline__ void load_clover(T* blk, const void* field, const Geo
     }
 }
 
-// y = B x for a fundamental spinor (8 complex): block 0 on components 0..3, block 1 on 4..7
-template <typename T>
+// y = B x for a spinor of 4N complex numbers: block 0 on components 0..2N-1 (chirality +), block 1 on the rest
+template <typename T, int N = 2>
 __device__ __forceinline__ void clover_matvec(cplx<T>* y, const T* blk, const cplx<T>* x) {
-    herm4_matvec(y, blk, x);
-    herm4_matvec(y + 4, blk + 16, x + 4);
+    if (N == 2) {
+        herm4_matvec(y, blk, x);
+        herm4_matvec(y + 4, blk + 16, x + 4);
+    } else {
+        herm_matvec<T, 2 * N>(y, blk, x);
+        herm_matvec<T, 2 * N>(y + 2 * N, blk + 4 * N * N, x + 2 * N);
+    }
 }
 
 // ------------------------------------------------------------------ host-side bookkeeping (hr_api.cu)

@@ -180,7 +180,7 @@ __device__ __forceinline__ Quat link_quat(const void* ufund, const Geo& g, int x
 //   P4 = U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
 // F^_mu,nu = (Q - Q^dag)/8 = (i/4) vec(Q).sigma, so  i F^_mu,nu = -(1/4) vec(Q).sigma.
 template <typename T>
-__device__ void clover_leaves(double* v, const void* ufund, const Geo& g, const int* x, int mu, int nu) {
+__device__ void clover_leaves(double* v, const void* ufund, const Geo& g, const int* x, int mu, int nu, double* w = nullptr) {
     int e[4] = {0, 0, 0, 0}, f[4] = {0, 0, 0, 0};
     e[mu] = 1;
     f[nu] = 1;
@@ -194,6 +194,11 @@ __device__ void clover_leaves(double* v, const void* ufund, const Geo& g, const 
     v[0] = p1.q1 + p2.q1 + p3.q1 + p4.q1;
     v[1] = p1.q2 + p2.q2 + p3.q2 + p4.q2;
     v[2] = p1.q3 + p2.q3 + p3.q3 + p4.q3;
+    if (w) {   // adjoint representation: R(P) - R(P)^T = 4 q0 eps_abc q_c per leaf, so F^adj_ab = (1/2) eps_abc w_c
+        w[0] = p1.q0 * p1.q1 + p2.q0 * p2.q1 + p3.q0 * p3.q1 + p4.q0 * p4.q1;
+        w[1] = p1.q0 * p1.q2 + p2.q0 * p2.q2 + p3.q0 * p3.q2 + p4.q0 * p4.q2;
+        w[2] = p1.q0 * p1.q3 + p2.q0 * p2.q3 + p3.q0 * p3.q3 + p4.q0 * p4.q3;
+    }
 }
 
 struct dcplx {
@@ -364,6 +369,176 @@ __global__ void clover_build_kernel(Geo g, double diag, double csw, int expo, co
     }
 }
 
+// ---- the same for D x D matrices (D = 6: adjoint blocks), generic loops
+template <int D>
+__device__ void matmul_d(dcplx (*C)[D], const dcplx (*A)[D], const dcplx (*B)[D]) {
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) {
+            dcplx a = {0.0, 0.0};
+            for (int k = 0; k < D; ++k) a = dadd(a, dmul(A[i][k], B[k][j]));
+            C[i][j] = a;
+        }
+}
+template <int D>
+__device__ void invert_d(dcplx (*A)[D]) {   // hermitian positive definite: Gauss-Jordan without pivoting
+    dcplx B[D][D];
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) { B[i][j].re = (i == j) ? 1.0 : 0.0; B[i][j].im = 0.0; }
+    for (int k = 0; k < D; ++k) {
+        const double n2 = A[k][k].re * A[k][k].re + A[k][k].im * A[k][k].im;
+        dcplx inv;
+        inv.re = A[k][k].re / n2;
+        inv.im = -A[k][k].im / n2;
+        for (int j = 0; j < D; ++j) { A[k][j] = dmul(A[k][j], inv); B[k][j] = dmul(B[k][j], inv); }
+        for (int i = 0; i < D; ++i) {
+            if (i == k) continue;
+            const dcplx f = A[i][k];
+            for (int j = 0; j < D; ++j) { A[i][j] = dsub(A[i][j], dmul(f, A[k][j])); B[i][j] = dsub(B[i][j], dmul(f, B[k][j])); }
+        }
+    }
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) A[i][j] = B[i][j];
+}
+template <int D>
+__device__ void expm_d(dcplx (*E)[D], const dcplx (*X)[D]) {   // scaling and squaring, order-16 Taylor (as expm4)
+    double nrm = 0.0;
+    for (int i = 0; i < D; ++i) {
+        double r = 0.0;
+        for (int j = 0; j < D; ++j) r += fabs(X[i][j].re) + fabs(X[i][j].im);
+        nrm = fmax(nrm, r);
+    }
+    int s = 0;
+    double scale = 1.0;
+    while (nrm * scale > 0.5 && s < 60) { scale *= 0.5; ++s; }
+    dcplx Y[D][D], P[D][D], Tm[D][D];
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) {
+            Y[i][j].re = X[i][j].re * scale; Y[i][j].im = X[i][j].im * scale;
+            P[i][j] = Y[i][j];
+            E[i][j].re = (i == j ? 1.0 : 0.0) + Y[i][j].re; E[i][j].im = Y[i][j].im;
+        }
+    for (int k = 2; k <= 16; ++k) {
+        matmul_d<D>(Tm, P, Y);
+        for (int i = 0; i < D; ++i)
+            for (int j = 0; j < D; ++j) {
+                P[i][j].re = Tm[i][j].re / k; P[i][j].im = Tm[i][j].im / k;
+                E[i][j] = dadd(E[i][j], P[i][j]);
+            }
+    }
+    for (int q = 0; q < s; ++q) {
+        matmul_d<D>(Tm, E, E);
+        for (int i = 0; i < D; ++i)
+            for (int j = 0; j < D; ++j) E[i][j] = Tm[i][j];
+    }
+}
+template <typename T, int D>
+__device__ void herm_to_reals_d(T* out, dcplx (*A)[D]) {
+    for (int i = 0; i < D; ++i) out[i] = (T)A[i][i].re;
+    int k = D;
+    for (int j = 0; j < D; ++j)
+        for (int i = j + 1; i < D; ++i) {
+            out[k++] = (T)(0.5 * (A[i][j].re + A[j][i].re));
+            out[k++] = (T)(0.5 * (A[i][j].im - A[j][i].im));
+        }
+}
+
+// C1 in the adjoint representation (oracle O10): 6 x 6 chirality blocks on (2 spin x 3 colour),
+//   A+- = (4+m0) + (csw/2) [ tau1 (x) i(+-F01 - F23) + tau2 (x) i(+-F02 + F13) + tau3 (x) i(+-F03 - F12) ],
+// with F^_mu,nu the real antisymmetric 3x3 matrix (Q - Q^T)/8 of the adjoint leaves.  The leaves are multiplied out
+// in the fundamental representation (quaternions) and mapped leaf by leaf: R(P) - R(P)^T = 4 q0 eps_abc q_c.
+// the two 6x6 blocks (72 reals) and their inverses from the six leaf vectors w[plane][c] (planes 01 02 03 12 13 23); all
+// in double, one shared non-inlined routine for both field precisions
+__device__ __noinline__ void clover_adj_blocks(double diag, double csw, int expo, const double (*w)[3], double* reals_f, double* reals_i) {
+    const dcplx Z = {0.0, 0.0}, P1 = {1.0, 0.0}, M1 = {-1.0, 0.0}, PI = {0.0, 1.0}, MI = {0.0, -1.0};
+    const dcplx pauli[3][2][2] = {{{Z, P1}, {P1, Z}}, {{Z, MI}, {PI, Z}}, {{P1, Z}, {Z, M1}}};
+    const double eps[3][3][3] = {{{0, 0, 0}, {0, 0, 1}, {0, -1, 0}}, {{0, 0, -1}, {0, 0, 0}, {1, 0, 0}}, {{0, 1, 0}, {-1, 0, 0}, {0, 0, 0}}};
+    const double *w01 = w[0], *w02 = w[1], *w03 = w[2], *w12 = w[3], *w13 = w[4], *w23 = w[5];
+    for (int chi = 0; chi < 2; ++chi) {
+        const double s = chi == 0 ? 1.0 : -1.0;
+        double gk[3][3];   // gk[k][e]: F-combination of tau_{k+1} is the antisymmetric matrix eps_cde gk[k][e]
+        for (int e = 0; e < 3; ++e) {
+            gk[0][e] = 0.5 * (s * w01[e] - w23[e]);
+            gk[1][e] = 0.5 * (s * w02[e] + w13[e]);
+            gk[2][e] = 0.5 * (s * w03[e] - w12[e]);
+        }
+        dcplx A[6][6];
+        for (int sp = 0; sp < 2; ++sp)
+            for (int c = 0; c < 3; ++c)
+                for (int tp = 0; tp < 2; ++tp)
+                    for (int d = 0; d < 3; ++d) {
+                        dcplx acc = {(sp == tp && c == d) ? diag : 0.0, 0.0};
+                        for (int k = 0; k < 3; ++k) {
+                            double G = 0.0;
+                            for (int e = 0; e < 3; ++e) G += eps[c][d][e] * gk[k][e];
+                            const dcplx iG = {0.0, G};
+                            const dcplx tx = dmul(pauli[k][sp][tp], iG);
+                            acc.re += 0.5 * csw * tx.re;
+                            acc.im += 0.5 * csw * tx.im;
+                        }
+                        A[sp * 3 + c][tp * 3 + d] = acc;
+                    }
+        if (expo) {
+            dcplx X[6][6], E[6][6];
+            for (int i = 0; i < 6; ++i)
+                for (int j = 0; j < 6; ++j) { X[i][j].re = (A[i][j].re - (i == j ? diag : 0.0)) / diag; X[i][j].im = A[i][j].im / diag; }
+            expm_d<6>(E, X);
+            for (int i = 0; i < 6; ++i)
+                for (int j = 0; j < 6; ++j) { A[i][j].re = diag * E[i][j].re; A[i][j].im = diag * E[i][j].im; X[i][j].re = -X[i][j].re; X[i][j].im = -X[i][j].im; }
+            herm_to_reals_d<double, 6>(reals_f + 36 * chi, A);
+            expm_d<6>(E, X);
+            for (int i = 0; i < 6; ++i)
+                for (int j = 0; j < 6; ++j) { A[i][j].re = E[i][j].re / diag; A[i][j].im = E[i][j].im / diag; }
+            herm_to_reals_d<double, 6>(reals_i + 36 * chi, A);
+        } else {
+            herm_to_reals_d<double, 6>(reals_f + 36 * chi, A);
+            invert_d<6>(A);
+            herm_to_reals_d<double, 6>(reals_i + 36 * chi, A);
+        }
+    }
+}
+
+template <typename T>
+__global__ void clover_build_adj_kernel(Geo g, double diag, double csw, int expo, const void* __restrict__ ufund, void* fwd, void* inv) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 2 * g.Vh) return;
+    const int par = t / g.Vh, cb = t - par * g.Vh;
+    const int row = cb / g.L3h, h = cb - row * g.L3h;
+    int x[4];
+    x[0] = row / g.s0;
+    const int rem = row - x[0] * g.s0;
+    x[1] = rem / g.s1;
+    x[2] = rem - x[1] * g.s1;
+    x[3] = 2 * h + ((x[0] + x[1] + x[2] + par) & 1);
+    double v[3], w[6][3];
+    clover_leaves<T>(v, ufund, g, x, 0, 1, w[0]);
+    clover_leaves<T>(v, ufund, g, x, 0, 2, w[1]);
+    clover_leaves<T>(v, ufund, g, x, 0, 3, w[2]);
+    clover_leaves<T>(v, ufund, g, x, 1, 2, w[3]);
+    clover_leaves<T>(v, ufund, g, x, 1, 3, w[4]);
+    clover_leaves<T>(v, ufund, g, x, 2, 3, w[5]);
+    constexpr int NR = 72;
+    double rf[NR], ri[NR];
+    clover_adj_blocks(diag, csw, expo, w, rf, ri);
+    constexpr int CCH = NR * sizeof(T) / 16;
+    constexpr int PER = 16 / sizeof(T);
+    typedef typename Chunk<T>::type chunk_t;
+    const size_t first = ((size_t)par * g.R + row) * (CCH * g.L3h) + h;
+    for (int c = 0; c < CCH; ++c) {
+        T ef[PER], ei[PER];
+        for (int k = 0; k < PER; ++k) { ef[k] = (T)rf[c * PER + k]; ei[k] = (T)ri[c * PER + k]; }
+        if (fwd) reinterpret_cast<chunk_t*>(fwd)[first + (size_t)c * g.L3h] = reals_to_chunk(ef);
+        if (inv) reinterpret_cast<chunk_t*>(inv)[first + (size_t)c * g.L3h] = reals_to_chunk(ei);
+    }
+}
+
+int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st) {
+    const unsigned nb = blocks_for(2LL * g.Vh, 64);
+    if (prec == HR_PREC_F64) clover_build_adj_kernel<double><<<nb, 64, 0, st>>>(g, diag, csw, expo, ufund, fwd, inv);
+    else clover_build_adj_kernel<float><<<nb, 64, 0, st>>>(g, diag, csw, expo, ufund, fwd, inv);
+    count_launch();
+    return check_launch("clover_build_adj_kernel");
+}
+
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st) {
     const unsigned nb = blocks_for(2LL * g.Vh, 128);
     if (prec == HR_PREC_F64) clover_build_kernel<double><<<nb, 128, 0, st>>>(g, diag, csw, expo, ufund, fwd, inv);
@@ -373,10 +548,11 @@ int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, 
 }
 
 // ------------------------------------------------------------------ C2/C3: out(x) = B(x) in(x)
-template <typename T>
+template <typename T, int N>
 __global__ void __launch_bounds__(128) clover_apply_kernel(Geo g, int parity, const void* __restrict__ blocks,
                                                            const void* __restrict__ in, void* __restrict__ out) {
-    typedef SiteIO<T, 8> IO;
+    constexpr int NC = 4 * N;
+    typedef SiteIO<T, NC> IO;
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
     const int p = parity == HR_BOTH ? (int)blockIdx.y : parity;
@@ -384,18 +560,23 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(Geo g, int parity, co
     const size_t off = parity == HR_BOTH ? (size_t)p * half_bytes : 0;
     const int row = cb / g.L3h, h = cb - row * g.L3h;
     const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
-    T blk[32];
-    cplx<T> x[8], y[8];
-    load_clover<T>(blk, blocks, g, p, row, h);
+    T blk[CloverSize<N>::reals];
+    cplx<T> x[NC], y[NC];
+    load_clover<T, N>(blk, blocks, g, p, row, h);
     IO::template load<LD_STREAM>(x, reinterpret_cast<const char*>(in) + off, first, g.L3h);
-    clover_matvec<T>(y, blk, x);
+    clover_matvec<T, N>(y, blk, x);
     IO::store(reinterpret_cast<char*>(out) + off, first, g.L3h, y);
 }
 
-int run_clover_apply(const Geo& g, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st) {
+int run_clover_apply(const Geo& g, int rep, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st) {
     dim3 grid(blocks_for(g.Vh, 128), parity == HR_BOTH ? 2 : 1);
-    if (prec == HR_PREC_F64) clover_apply_kernel<double><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
-    else clover_apply_kernel<float><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+    if (rep == HR_REP_FUND) {
+        if (prec == HR_PREC_F64) clover_apply_kernel<double, 2><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+        else clover_apply_kernel<float, 2><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+    } else {
+        if (prec == HR_PREC_F64) clover_apply_kernel<double, 3><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+        else clover_apply_kernel<float, 3><<<grid, 128, 0, st>>>(g, parity, blocks, in, out);
+    }
     count_launch();
     return check_launch("clover_apply_kernel");
 }

@@ -43,10 +43,6 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
         set_error("HR_KERNEL_TILED: lattice %dx%dx%dx%d does not fit the tiled kernel", g->L[0], g->L[1], g->L[2], g->L[3]);
         return HR_EUNSUPPORTED;
     }
-    if (g->rep != HR_REP_FUND && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) {
-        set_error("clover epilogues exist for the fundamental representation only");
-        return HR_EUNSUPPORTED;
-    }
     if (tiled_chosen(g)) {
         TiledPlan pl;
         tiled_plan(g, a.both, sm_count(), pl, a.both && epi == EPI_AXPY && a.phi == a.in);

@@ -44,27 +44,23 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
             acc[k].im = fma(cc, acc[k].im, ca * phi[k].im);
         }
     } else if (EPI == EPI_CLOVER_INV) {
-        if (N == 2) {
-            T blk[32];
-            cplx<T> y[NC];
-            load_clover<T>(blk, a.clover, g, p, row, h);
-            clover_matvec<T>(y, blk, acc);
+        T blk[CloverSize<N>::reals];
+        cplx<T> y[NC];
+        load_clover<T, N>(blk, a.clover, g, p, row, h);
+        clover_matvec<T, N>(y, blk, acc);
 #pragma unroll
-            for (int k = 0; k < NC; ++k) acc[k] = y[k];
-        }
+        for (int k = 0; k < NC; ++k) acc[k] = y[k];
     } else if (EPI == EPI_CLOVER_AXPY) {
-        if (N == 2) {
-            T blk[32];
-            cplx<T> phi[NC], y[NC];
-            load_clover<T>(blk, a.clover, g, p, row, h);
-            IO::template load<LD_STREAM>(phi, phi_half, first, g.L3h);
-            clover_matvec<T>(y, blk, phi);
-            const T cc = (T)a.c;
+        T blk[CloverSize<N>::reals];
+        cplx<T> phi[NC], y[NC];
+        load_clover<T, N>(blk, a.clover, g, p, row, h);
+        IO::template load<PHI_POLICY>(phi, phi_half, first, g.L3h);
+        clover_matvec<T, N>(y, blk, phi);
+        const T cc = (T)a.c;
 #pragma unroll
-            for (int k = 0; k < NC; ++k) {
-                acc[k].re = fma(cc, acc[k].re, y[k].re);
-                acc[k].im = fma(cc, acc[k].im, y[k].im);
-            }
+        for (int k = 0; k < NC; ++k) {
+            acc[k].re = fma(cc, acc[k].re, y[k].re);
+            acc[k].im = fma(cc, acc[k].im, y[k].im);
         }
     }
     IO::store(out_half, first, g.L3h, acc);

@@ -78,8 +78,8 @@ class Lattice:
         return hr.download(canon, self.real, (self.V, 4, 3, 3))
 
     def put_clover(self, blocks):
-        """real [V,2,16] -> packed block field"""
-        assert blocks.shape == (self.V, 2, 16), blocks.shape
+        """real [V,2,(2N)^2] -> packed block field (16 reals per block for the fundamental, 36 for the adjoint rep)"""
+        assert blocks.shape == (self.V, 2, 4 * self.N * self.N), blocks.shape
         canon = hr.upload(blocks.astype(self.real))
         dev = self.empty_clover()
         hr.hr_pack_clover(self.g, canon, dev, hr.stream_ptr())
@@ -88,7 +88,7 @@ class Lattice:
     def get_clover(self, dev):
         canon = hr.device_buffer(hr.hr_canonical_clover_bytes(self.g), self.device)
         hr.hr_unpack_clover(self.g, dev, canon, hr.stream_ptr())
-        return hr.download(canon, self.real, (self.V, 2, 16))
+        return hr.download(canon, self.real, (self.V, 2, 4 * self.N * self.N))
 
     # ---- operators (direct C-ABI calls on torch's current stream)
     def represent(self, u_fund):

@@ -99,9 +99,10 @@ def test_argument_checks_happen_before_any_cuda_call(L):
         hr.hr_dirac_apply(gfull, 0.0, 4096, 1 << 20, 1 << 21)
     assert e.value.status == hr.EUNSUPPORTED
     gadj = hr.geom((4, 4, 4, 4), rep=hr.REP_ADJ)
-    with pytest.raises(hr.HrError) as e:
-        hr.hr_clover_apply(gadj, hr.EVEN, 4096, 1 << 20, 1 << 21)
-    assert e.value.status == hr.EUNSUPPORTED
+    with pytest.raises(hr.HrError) as e:   # adjoint clover exists (6x6 blocks); a bad parity is still caught first
+        hr.hr_clover_apply(gadj, 7, 4096, 1 << 20, 1 << 21)
+    assert e.value.status == hr.EINVAL
+    assert hr.hr_clover_bytes(gadj) == 256 * 72 * 8 and hr.hr_canonical_clover_bytes(gadj) == 256 * 72 * 8
     with pytest.raises(hr.HrError) as e:   # hr_cg_solve: tol must be positive; checked before any CUDA call
         hr.hr_cg_solve(g, 0.0, 4096, None, None, 1 << 20, 1 << 21, 1 << 24, 0.0, 10)
     assert e.value.status == hr.EINVAL
@@ -151,8 +152,9 @@ def test_work_model_matches_survey_table(L):
     assert hr.hr_dirac_flops_bytes(f64full, hr.OP_DHAT_CLOVER)[:2] == (1696.0, 2176.0)
     assert hr.hr_dirac_flops_bytes(f64, hr.OP_REPRESENT)[1] == 416.0
     assert hr.hr_dirac_flops_bytes(f64full, hr.OP_REPRESENT)[1] == 544.0
-    with pytest.raises(hr.HrError):
-        hr.hr_dirac_flops_bytes(adj, hr.OP_CLOVER)
+    # adjoint clover: two hermitian 6x6 blocks per site = 72 reals; mat-vecs 2 (12 + 8*6*5) = 504 flops
+    assert hr.hr_dirac_flops_bytes(adj, hr.OP_CLOVER) == (504.0, 2 * 192 + 576.0, 2 * 192 + 576.0)
+    assert hr.hr_dirac_flops_bytes(adj, hr.OP_DHAT_CLOVER)[:2] == (2 * 744 + 2 * 504 + 2 * 24.0, 5 * 192 + 16 * 72 + 2 * 576.0)
 
 
 def test_kernel_name_and_launch_counter(L):

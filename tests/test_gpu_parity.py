@@ -51,14 +51,15 @@ def kernels_for(hr, L, rep, prec):
 def dense_to_blocks(A):
     """oracle dense [n,8,8] -> canonical blocks [n,2,16]: 4 real diagonal entries, then the strictly-lower
     entries (1,0) (2,0) (3,0) (2,1) (3,1) (3,2) as re,im (include/hr_dslash.h)."""
-    out = np.empty((A.shape[0], 2, 16))
+    D = A.shape[-1] // 2          # 4 (fundamental) or 6 (adjoint): block = one chirality, index (spin mod 2)*N + colour
+    out = np.empty((A.shape[0], 2, D * D))
     for chi in range(2):
-        B = A[:, 4 * chi:4 * chi + 4, 4 * chi:4 * chi + 4]
-        for i in range(4):
+        B = A[:, D * chi:D * chi + D, D * chi:D * chi + D]
+        for i in range(D):
             out[:, chi, i] = B[:, i, i].real
-        k = 4
-        for j in range(4):
-            for i in range(j + 1, 4):
+        k = D
+        for j in range(D):
+            for i in range(j + 1, D):
                 out[:, chi, k] = B[:, i, j].real
                 out[:, chi, k + 1] = B[:, i, j].imag
                 k += 2
@@ -669,3 +670,50 @@ def test_48to4_cg_and_exponential_clover(hr, orc, big_inputs):
     bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
     assert np.linalg.norm(l64.get_clover(fwd)[:n] - bf) <= 1e-13 * np.linalg.norm(bf)
     assert np.linalg.norm(l64.get_clover(inv)[:n] - bi) <= 1e-13 * np.linalg.norm(bi)
+
+
+# ------------------------------------------------------------------ clover in the adjoint representation
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 4, 6, 8), (2, 2, 2, 2), (8, 2, 8, 6)])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("exponential", [False, True])
+def test_adjoint_clover(hr, orc, L, prec, exponential):
+    """6x6 blocks and inverses (regular and exponential) against the oracle's O10, C2/C3 on them, the even-odd
+    operator with clover (E2) and the full clover-improved operator in the adjoint representation; stored links and
+    links rebuilt on the fly"""
+    import torch
+    m0, csw = -0.25, 1.2
+    d = 4.0 + m0
+    Uf = rounded(inputs.weak_gauge(L, 0.3, 1), prec)
+    R, _ = orc.represent(Uf)
+    psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
+    A = orc.clover_dense_adj(L, d, csw, R)
+    if exponential:
+        lam, Vv = np.linalg.eigh((A - d * np.eye(12)[None]) / d)      # A_exp = d exp(C/d), as O9
+        Vh = np.conj(np.swapaxes(Vv, -1, -2))
+        A, Ainv = d * (Vv * np.exp(lam)[:, None, :]) @ Vh, (Vv * np.exp(-lam)[:, None, :]) @ Vh / d
+    else:
+        Ainv = np.linalg.inv(A)
+    bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+    tol_blk = 1e-13 if prec == 0 else 1e-6
+    want_dhat = orc.dirac_eo_clover_adj(L, R, A, Ainv, psi, nthreads=NTHREADS)
+    H = orc.hop(L, 1, 0, R, psi, nthreads=NTHREADS)
+    H = orc.hop(L, 1, 1, R, psi, nthreads=NTHREADS, out=H)
+    want_dsw = orc.site_matvec_n(A, psi) - 0.5 * H
+    from paper_2411_18511_b200.lattice import Lattice
+    for storage in (hr.LINKS_COMPRESSED, hr.LINKS_ONTHEFLY):
+        for kernel in kernels_for(hr, L, 1, prec):
+            lat = Lattice(L, hr.REP_ADJ, prec, kernel, link_storage=storage)
+            Uf_dev, psi_dev = lat.put_gauge_fund(Uf), lat.put_spinor(psi)
+            U_dev = Uf_dev if storage == hr.LINKS_ONTHEFLY else lat.put_gauge_adj(rounded(R, prec))
+            fwd, inv = lat.clover_build(m0, csw, Uf_dev, exponential=exponential)
+            assert np.linalg.norm(lat.get_clover(fwd) - bf) <= tol_blk * np.linalg.norm(bf)
+            assert np.linalg.norm(lat.get_clover(inv) - bi) <= tol_blk * np.linalg.norm(bi)
+            got = lat.get_spinor(lat.clover_apply(hr.BOTH, fwd, psi_dev))
+            assert rel(got, orc.site_matvec_n(A, psi)) <= TOL[prec]
+            half = torch.zeros_like(psi_dev)
+            lat.clover_apply(hr.ODD, inv, lat.odd(psi_dev), lat.odd(half))
+            assert rel(lat.get_spinor(half), orc.site_matvec_n(Ainv, psi, inputs.site_parity(L) == 1)) <= TOL[prec]
+            out = torch.zeros_like(psi_dev)
+            lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
+            assert rel(lat.get_spinor(out), want_dhat) <= TOL[prec], (storage, kernel)
+            assert rel(lat.get_spinor(lat.dirac_clover(U_dev, fwd, psi_dev)), want_dsw) <= TOL[prec], (storage, kernel)
