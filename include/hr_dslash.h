@@ -73,7 +73,7 @@ size_t hr_gauge_bytes(const hr_geom* g, int rep);           /* device layout, al
 size_t hr_clover_bytes(const hr_geom* g);                   /* device layout, one set of blocks (forward OR inverse), all V sites */
 size_t hr_canonical_spinor_bytes(const hr_geom* g);         /* canonical, V sites */
 size_t hr_canonical_gauge_bytes(const hr_geom* g, int rep); /* canonical, 4V links */
-size_t hr_canonical_clover_bytes(const hr_geom* g);         /* canonical, V sites x 2 x 16 reals */
+size_t hr_canonical_clover_bytes(const hr_geom* g);         /* canonical, V sites x 2 x (2N)^2 reals (N of g->rep) */
 
 /* ---- canonical <-> device layout (both pointers on the device; pure permutations, no arithmetic) ---- */
 int hr_pack_spinor(const hr_geom* g, const void* canon, void* dev, void* stream);
