@@ -170,7 +170,7 @@ int hr_cg_solve(const hr_geom* g, double m0, const void* u, const void* clover_f
  * accuracy with the iterations done in single precision.  Outer loop (fp64): r = b - Dhat^dag Dhat x evaluated with
  * the fp64 operator; stop when |r| <= tol |b| (this is the TRUE residual) or after max_outer corrections; otherwise
  * solve Dhat^dag Dhat e = r with hr_cg_solve's iteration on the fp32 fields to the relative accuracy inner_tol
- * (at most max_inner iterations), x += e.  No clover.  g describes the fp64 fields (prec = HR_PREC_F64);
+ * (at most max_inner iterations), x += e.  g describes the fp64 fields (prec = HR_PREC_F64);
  * u_f64 / u_f32: the SAME gauge field packed in both precisions; b, x: fp64 even half fields;
  * workspace: hr_cg_mixed_workspace_bytes(g).  HOST outputs (may be NULL): corrections made, total fp32 iterations,
  * final true |r|/|b|.  Synchronises `stream` once per outer iteration (and as hr_cg_solve inside). */
@@ -178,6 +178,12 @@ size_t hr_cg_mixed_workspace_bytes(const hr_geom* g);
 int hr_cg_solve_mixed(const hr_geom* g, double m0, const void* u_f64, const void* u_f32, const void* b, void* x,
                       void* workspace, double tol, double inner_tol, int max_outer, int max_inner, int check_every,
                       int* outer_iters, int* inner_iters, double* relres, void* stream);
+/* the same with the clover-improved operator: the block fields of hr_clover_build[_exp] in both precisions */
+int hr_cg_solve_mixed_clover(const hr_geom* g, double m0, const void* u_f64, const void* u_f32,
+                             const void* clover_fwd_f64, const void* clover_inv_f64, const void* clover_fwd_f32,
+                             const void* clover_inv_f32, const void* b, void* x, void* workspace, double tol,
+                             double inner_tol, int max_outer, int max_inner, int check_every, int* outer_iters,
+                             int* inner_iters, double* relres, void* stream);
 
 /* ---- host-buffer entry points (the end-to-end path a user without device buffers calls) ----
  * All data pointers are HOST pointers to canonical arrays (pinned memory makes the copies asynchronous);

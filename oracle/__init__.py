@@ -180,7 +180,7 @@ def dirac_eo_clover(L, U, A, Ainv, psi, nthreads=1):
 
 
 # ------------------------------------------------------------------ O8: conjugate gradient on the normal equations
-def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1, A=None, Ainv=None):
+def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1, A=None, Ainv=None, dhat=None):
     """O8 (the HMC inverts the even-odd operator): solve
         Dhat^dag Dhat x = b        on the even sites,   Dhat^dag = gamma5 Dhat gamma5  (pin P2),
     by the textbook conjugate-gradient iteration (Hestenes-Stiefel) from x = 0, in the order
@@ -190,7 +190,9 @@ def cg_normal(L, rep, m0, U, b, tol=1e-12, max_iter=2000, nthreads=1, A=None, Ai
     dirac_eo (dirac_eo_clover when A, Ainv are given); no preconditioning, no restarts, no reordering."""
     g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
 
-    def Dhat(v):   # O3, or O7 when the dense clover matrices A, A^-1 are given (fundamental representation)
+    def Dhat(v):   # O3, or O7 when the dense clover matrices A, A^-1 are given (fundamental representation),
+        if dhat is not None:   # or any even-odd operator handed in (e.g. dirac_eo_clover_adj)
+            return dhat(v)
         if A is None:
             return dirac_eo(L, rep, m0, U, v, nthreads)
         return dirac_eo_clover(L, U, A, Ainv, v, nthreads)

@@ -23,7 +23,8 @@ size_t cg_workspace_bytes(const hr_geom* g);
 int run_cg(const hr_geom* g, double m0, const void* u, const void* cf, const void* ci, const void* b, void* x, void* workspace, double tol,
            int max_iter, int check_every, int* iters_out, double* relres_out, cudaStream_t st);
 size_t cg_mixed_workspace_bytes(const hr_geom* g);
-int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, const void* b, void* x, void* workspace, double tol, double inner_tol,
+int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, const void* cf64, const void* ci64, const void* cf32, const void* ci32,
+                 const void* b, void* x, void* workspace, double tol, double inner_tol,
                  int max_outer, int max_inner, int check_every, int* outer_out, int* inner_out, double* relres_out, cudaStream_t st);
 
 static thread_local char g_err[512] = "";
@@ -298,13 +299,16 @@ size_t hr_cg_mixed_workspace_bytes(const hr_geom* g) {
     return cg_mixed_workspace_bytes(g);
 }
 
-int hr_cg_solve_mixed(const hr_geom* g, double m0, const void* u_f64, const void* u_f32, const void* b, void* x, void* workspace,
-                      double tol, double inner_tol, int max_outer, int max_inner, int check_every,
-                      int* outer_iters, int* inner_iters, double* relres, void* stream) {
+static int cg_mixed_any(const hr_geom* g, double m0, const void* u_f64, const void* u_f32, const void* cf64, const void* ci64,
+                        const void* cf32, const void* ci32, const void* b, void* x, void* workspace,
+                        double tol, double inner_tol, int max_outer, int max_inner, int check_every,
+                        int* outer_iters, int* inner_iters, double* relres, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_links(g));
     if (g->prec != HR_PREC_F64) { set_error("hr_cg_solve_mixed: the geometry describes the fp64 fields (prec must be HR_PREC_F64)"); return HR_EINVAL; }
     HR_TRY(check_ptr(u_f64, "u_f64")); HR_TRY(check_ptr(u_f32, "u_f32")); HR_TRY(check_ptr(b, "b")); HR_TRY(check_ptr(x, "x"));
     HR_TRY(check_ptr(workspace, "workspace"));
+    const int nclover = (cf64 != nullptr) + (ci64 != nullptr) + (cf32 != nullptr) + (ci32 != nullptr);
+    if (nclover != 0 && nclover != 4) { set_error("hr_cg_solve_mixed_clover: the four clover block fields must all be given"); return HR_EINVAL; }
     if (!(tol > 0.0) || !(inner_tol > 0.0) || inner_tol >= 1.0 || max_outer < 0 || max_inner < 1 || check_every < 1) {
         set_error("hr_cg_solve_mixed: need tol > 0, 0 < inner_tol < 1, max_outer >= 0, max_inner >= 1, check_every >= 1");
         return HR_EINVAL;
@@ -314,8 +318,23 @@ int hr_cg_solve_mixed(const hr_geom* g, double m0, const void* u_f64, const void
         set_error("hr_cg_solve_mixed: b, x and workspace must not overlap");
         return HR_EINVAL;
     }
-    return run_cg_mixed(g, m0, u_f64, u_f32, b, x, workspace, tol, inner_tol, max_outer, max_inner, check_every, outer_iters, inner_iters, relres,
-                        (cudaStream_t)stream);
+    return run_cg_mixed(g, m0, u_f64, u_f32, cf64, ci64, cf32, ci32, b, x, workspace, tol, inner_tol, max_outer, max_inner, check_every,
+                        outer_iters, inner_iters, relres, (cudaStream_t)stream);
+}
+
+int hr_cg_solve_mixed(const hr_geom* g, double m0, const void* u_f64, const void* u_f32, const void* b, void* x, void* workspace,
+                      double tol, double inner_tol, int max_outer, int max_inner, int check_every,
+                      int* outer_iters, int* inner_iters, double* relres, void* stream) {
+    return cg_mixed_any(g, m0, u_f64, u_f32, nullptr, nullptr, nullptr, nullptr, b, x, workspace, tol, inner_tol, max_outer, max_inner,
+                        check_every, outer_iters, inner_iters, relres, stream);
+}
+
+int hr_cg_solve_mixed_clover(const hr_geom* g, double m0, const void* u_f64, const void* u_f32,
+                             const void* clover_fwd_f64, const void* clover_inv_f64, const void* clover_fwd_f32, const void* clover_inv_f32,
+                             const void* b, void* x, void* workspace, double tol, double inner_tol, int max_outer, int max_inner,
+                             int check_every, int* outer_iters, int* inner_iters, double* relres, void* stream) {
+    return cg_mixed_any(g, m0, u_f64, u_f32, clover_fwd_f64, clover_inv_f64, clover_fwd_f32, clover_inv_f32, b, x, workspace, tol, inner_tol,
+                        max_outer, max_inner, check_every, outer_iters, inner_iters, relres, stream);
 }
 
 // ---------------------------------------------------------------- M1

@@ -301,7 +301,8 @@ size_t cg_mixed_workspace_bytes(const hr_geom* g) {
     return 256 + up256s(CG_MAX_PARTIALS * sizeof(double)) + 4 * up256s(half64) + 2 * up256s(half32) + up256s(cg_workspace_bytes(&g32));
 }
 
-int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, const void* b, void* x, void* workspace, double tol, double inner_tol,
+int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, const void* cf64, const void* ci64, const void* cf32, const void* ci32,
+                 const void* b, void* x, void* workspace, double tol, double inner_tol,
                  int max_outer, int max_inner, int check_every, int* outer_out, int* inner_out, double* relres_out, cudaStream_t st) {
     const hr_geom g32 = as_f32(g);
     const Geo geo = make_geo(g);
@@ -330,10 +331,10 @@ int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, 
     int outer = 0, inner_total = 0;
     for (;;) {
         // r = b - Dhat^dag Dhat x in double (for x = 0 this is r = b, computed the same way for simplicity)
-        int rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, nullptr, nullptr, x, t, tmp, strm);
+        int rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, cf64, ci64, x, t, tmp, strm);
         if (rc != HR_OK) return rc;
         cg_g5_norm_kernel<double><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, t, w, partial);
-        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, nullptr, nullptr, w, t, tmp, strm);
+        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, cf64, ci64, w, t, tmp, strm);
         if (rc != HR_OK) return rc;
         cg_residual_kernel<<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, (const double2*)b, (const double2*)t, (double2*)r, partial);
         cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_INIT, nblk, partial, sc);
@@ -351,7 +352,7 @@ int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, 
         count_launch();
         int it = 0;
         double rel32 = 0.0;
-        rc = run_cg(&g32, m0, u32, nullptr, nullptr, r32, e32, ws32, inner_tol, max_inner, check_every, &it, &rel32, st);
+        rc = run_cg(&g32, m0, u32, cf32, ci32, r32, e32, ws32, inner_tol, max_inner, check_every, &it, &rel32, st);
         if (rc != HR_OK) return rc;
         inner_total += it;
         cg_add_f32_kernel<<<nblk32, CG_BLOCK, 0, st>>>(nchunks32, geo.L3h, NCH32, (const float4*)e32, (double2*)x);

@@ -30,7 +30,7 @@ SYMBOLS = [
     "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_cg_workspace_bytes", "hr_cg_solve",
-    "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed",
+    "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed", "hr_cg_solve_mixed_clover",
 ]
 
 
@@ -82,6 +82,7 @@ def lib():
             "hr_cg_workspace_bytes": (S, [G]),
             "hr_cg_mixed_workspace_bytes": (S, [G]),
             "hr_cg_solve_mixed": (I, [G, D, V, V, V, V, V, D, D, I, I, I, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), PD, V]),
+            "hr_cg_solve_mixed_clover": (I, [G, D, V, V, V, V, V, V, V, V, V, D, D, I, I, I, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), PD, V]),
             "hr_cg_solve": (I, [G, D, V, V, V, V, V, V, D, I, I, ctypes.POINTER(ctypes.c_int), PD, V]),
         }
         for name, (res, args) in sig.items():
@@ -217,6 +218,16 @@ def hr_cg_solve_mixed(g, m0, u_f64, u_f32, b, x, workspace, tol, inner_tol=1e-3,
     _check(lib().hr_cg_solve_mixed(ctypes.byref(g), float(m0), _ptr(u_f64), _ptr(u_f32), _ptr(b), _ptr(x), _ptr(workspace), float(tol),
                                    float(inner_tol), int(max_outer), int(max_inner), int(check_every), ctypes.byref(no), ctypes.byref(ni),
                                    ctypes.byref(rel), stream))
+    return no.value, ni.value, rel.value
+
+
+def hr_cg_solve_mixed_clover(g, m0, u_f64, u_f32, cf64, ci64, cf32, ci32, b, x, workspace, tol, inner_tol=1e-3, max_outer=30,
+                             max_inner=1000, check_every=5, stream=0):
+    """-> (outer corrections, total fp32 iterations, true |r|/|b|)"""
+    no, ni, rel = ctypes.c_int(), ctypes.c_int(), ctypes.c_double()
+    _check(lib().hr_cg_solve_mixed_clover(ctypes.byref(g), float(m0), _ptr(u_f64), _ptr(u_f32), _ptr(cf64), _ptr(ci64), _ptr(cf32), _ptr(ci32),
+                                          _ptr(b), _ptr(x), _ptr(workspace), float(tol), float(inner_tol), int(max_outer), int(max_inner),
+                                          int(check_every), ctypes.byref(no), ctypes.byref(ni), ctypes.byref(rel), stream))
     return no.value, ni.value, rel.value
 
 

@@ -717,3 +717,48 @@ def test_adjoint_clover(hr, orc, L, prec, exponential):
             lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
             assert rel(lat.get_spinor(out), want_dhat) <= TOL[prec], (storage, kernel)
             assert rel(lat.get_spinor(lat.dirac_clover(U_dev, fwd, psi_dev)), want_dsw) <= TOL[prec], (storage, kernel)
+
+
+@pytest.mark.parametrize("rep", [0, 1])
+def test_cg_with_clover_all_variants(hr, orc, rep):
+    """hr_cg_solve and hr_cg_solve_mixed_clover on the clover-improved even-odd system, fundamental and adjoint,
+    against the oracle's CG (O8) on the oracle's operators (O7 / its adjoint form)"""
+    import torch
+    L, m0, csw, tol = (4, 4, 4, 8), -0.25, 1.2, 1e-12
+    d = 4.0 + m0
+    N = 2 if rep == 0 else 3
+    Uf = inputs.weak_gauge(L, 0.3, 1)
+    b = inputs.gaussian_spinor(L, N, 2)
+    even = inputs.site_parity(L) == 0
+    b[~even] = 0
+    if rep == 0:
+        U = Uf
+        A, Ainv = clover_oracle(orc, L, Uf, m0, csw)
+        dhat = lambda v: orc.dirac_eo_clover(L, Uf, A, Ainv, v, nthreads=NTHREADS)
+    else:
+        U = orc.represent(Uf)[0]
+        A = orc.clover_dense_adj(L, d, csw, U)
+        Ainv = np.linalg.inv(A)
+        dhat = lambda v: orc.dirac_eo_clover_adj(L, U, A, Ainv, v, nthreads=NTHREADS)
+    x_orc, it_orc, _ = orc.cg_normal(L, rep, m0, U, b, tol=tol, max_iter=1000, dhat=dhat)
+    l64, l32 = lattice(hr, L, rep, 0), lattice(hr, L, rep, 1)
+    put = (lambda lat: lat.put_gauge_fund(U)) if rep == 0 else (lambda lat: lat.put_gauge_adj(U))
+    U64, U32 = put(l64), put(l32)
+    f64, i64 = l64.clover_build(m0, csw, l64.put_gauge_fund(Uf))
+    f32, i32 = l32.clover_build(m0, csw, l32.put_gauge_fund(Uf))
+    b_dev = l64.put_spinor(b)
+
+    def solution(x_half):
+        full = torch.zeros_like(b_dev)
+        l64.even(full).copy_(x_half)
+        return l64.get_spinor(full)
+
+    x_half, it, relres = l64.cg(m0, U64, l64.even(b_dev), tol, 1000, clover_fwd=f64, clover_inv=i64, check_every=1)
+    assert relres <= tol and abs(it - it_orc) <= 2
+    assert rel(solution(x_half), x_orc) <= 1e-9
+    xm = l64.empty_spinor(hr.EVEN)
+    ws = hr.device_buffer(hr.hr_cg_mixed_workspace_bytes(l64.g))
+    outer, inner, rel_m = hr.hr_cg_solve_mixed_clover(l64.g, m0, U64, U32, f64, i64, f32, i32, l64.even(b_dev), xm, ws, tol, 1e-4, 20, 1000, 5,
+                                                      hr.stream_ptr())
+    assert rel_m <= tol and 2 <= outer <= 6
+    assert rel(solution(xm), x_orc) <= 1e-9
