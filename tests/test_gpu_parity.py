@@ -762,3 +762,29 @@ def test_cg_with_clover_all_variants(hr, orc, rep):
                                                       hr.stream_ptr())
     assert rel_m <= tol and 2 <= outer <= 6
     assert rel(solution(xm), x_orc) <= 1e-9
+
+
+def test_tiled_kernel_soak_is_bitwise_repeatable(hr):
+    """2 x 2000 launches of the tiled kernels (full D with both parities per CTA, and Dhat) on a small lattice: every
+    output equals the first one bit for bit — a rare producer/consumer ordering slip in the mbarrier pipeline would show
+    up here as a changed word (or a hang, caught by the test timeout)"""
+    import torch
+    for L, rep, prec in (((8, 2, 8, 6), 0, 0), ((8, 4, 4, 16), 1, 0), ((4, 2, 4, 52), 0, 1)):
+        g = hr.geom(L, rep, prec, hr.LINKS_COMPRESSED, hr.KERNEL_TILED)
+        assert hr.hr_kernel_name(g) == "tiled"
+        U = torch.randn(hr.hr_gauge_bytes(g, rep) // 4, device="cuda").view(torch.uint8)
+        psi = torch.randn(hr.hr_spinor_bytes(g, hr.BOTH) // 4, device="cuda").view(torch.uint8)
+        out = torch.zeros_like(psi)
+        half = psi.numel() // 2
+        tmp = torch.empty(half, device="cuda", dtype=torch.uint8)
+        st = hr.stream_ptr()
+        ref = None
+        for i in range(2000):
+            hr.hr_dirac_apply(g, -0.2, U, psi, out, st)
+            hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.2, U, None, None, psi[:half], out[:half], tmp, st)
+            if i % 250 == 0:
+                if ref is None:
+                    ref = out.clone()
+                else:
+                    assert torch.equal(ref, out), (L, rep, prec, i)
+        torch.cuda.synchronize()
