@@ -232,11 +232,15 @@ def clover_exp_dense(L, diag, csw, U, nthreads=1, begin=0, end=None):
     end = _vol(L) if end is None else end
     A = clover_dense(L, diag, csw, U, begin, end, nthreads)[begin:end]
     C = A - diag * np.eye(8)[None]
+    return _exp_hermitian_pair(C, diag)
+
+
+def _exp_hermitian_pair(C, diag):
+    """(diag exp(C/diag), exp(-C/diag)/diag) for a stack of hermitian matrices C, from the eigendecomposition
+    exp(H) = V diag(e^lambda) V^dag."""
     lam, V = np.linalg.eigh(C / diag)
     Vh = np.conj(np.swapaxes(V, -1, -2))
-    fwd = diag * (V * np.exp(lam)[:, None, :]) @ Vh
-    inv = (V * np.exp(-lam)[:, None, :]) @ Vh / diag
-    return fwd, inv
+    return diag * (V * np.exp(lam)[:, None, :]) @ Vh, (V * np.exp(-lam)[:, None, :]) @ Vh / diag
 
 
 # ------------------------------------------------------------------ O10: clover term in the adjoint representation
@@ -274,6 +278,16 @@ def clover_dense_adj(L, diag, csw, R):
             sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
             A += csw * 0.5j * np.einsum("st,xab->xsatb", sig, F).reshape(V, 12, 12)
     return A
+
+
+def clover_exp_dense_adj(L, diag, csw, R):
+    """O11 (PAPER.md:59-61 exponential clover, PAPER.md:21, 53 higher representations; readings B4 + B5 of DESIGN.md
+    §3): the exponential site-diagonal term in the adjoint representation,
+        A_exp(x) = diag * exp( C(x) / diag ),     A_exp(x)^-1 = exp( -C(x) / diag ) / diag,
+    with C(x) = clover_dense_adj(L, 0, csw, R) the 12x12 hermitian clover term of O10; the exponential is taken from
+    the eigendecomposition as in O9.  Returns (A_exp, A_exp^-1), dense [V,12,12].  Pinned by P19."""
+    C = clover_dense_adj(L, 0.0, csw, R)
+    return _exp_hermitian_pair(C, diag)
 
 
 def site_matvec_n(M, psi, mask=None):

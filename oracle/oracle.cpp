@@ -12,7 +12,8 @@
 // Style: canonical array-of-structs data (A3/A4), dense 4x4 gamma matrices applied as
 // matrices (no half-spinor trick), std::complex<double>, explicit (x +- 1) mod L
 // neighbours, no blocking, no fusion, no reordering.  Pinned by tests/test_oracle_pins.py
-// (P1-P14).  Parity unpinned: nothing.
+// (P1-P14, P20 for this file; P15-P19 for the numpy routines O8-O11 of oracle/__init__.py).
+// Parity unpinned: nothing.
 //
 // Canonical layouts (A3/A4), V = L0 L1 L2 L3, lex(x) = ((x0 L1 + x1) L2 + x2) L3 + x3:
 //   spinor      [lex][spin 0..3][colour 0..N-1][re,im]

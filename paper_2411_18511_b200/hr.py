@@ -236,12 +236,18 @@ def hr_kernel_name(g) -> str: return lib().hr_kernel_name(ctypes.byref(g)).decod
 
 
 # ------------------------------------------------------------------ plumbing: device memory via torch
-def device_buffer(nbytes: int, device="cuda:0"):
-    """A torch uint8 buffer of nbytes on the device (256-byte aligned by the caching allocator)."""
+def current_device() -> str:
+    """the calling thread's current CUDA device as a torch device string (one process per GPU sets it once)"""
     import torch
     if not torch.cuda.is_available():
         raise RuntimeError("libhr_dslash needs a CUDA device; there is no CPU fallback")
-    return torch.empty(int(nbytes), dtype=torch.uint8, device=device)
+    return "cuda:%d" % torch.cuda.current_device()
+
+
+def device_buffer(nbytes: int, device=None):
+    """A torch uint8 buffer of nbytes on `device` (default: the current device; 256-byte aligned by the caching allocator)."""
+    import torch
+    return torch.empty(int(nbytes), dtype=torch.uint8, device=current_device() if device is None else device)
 
 
 def np_real(g):
@@ -254,12 +260,12 @@ def np_complex(g):
     return np.complex128 if g.prec == PREC_F64 else np.complex64
 
 
-def upload(array, device="cuda:0"):
-    """numpy array -> device uint8 buffer holding the same bytes"""
+def upload(array, device=None):
+    """numpy array -> uint8 buffer on `device` (default: the current device) holding the same bytes"""
     import numpy as np
     import torch
     a = np.ascontiguousarray(array)
-    return torch.from_numpy(a.view(np.uint8).reshape(-1)).to(device)
+    return torch.from_numpy(a.view(np.uint8).reshape(-1)).to(current_device() if device is None else device)
 
 
 def download(buf, dtype, shape):

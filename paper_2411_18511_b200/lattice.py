@@ -11,13 +11,13 @@ from . import hr
 
 
 class Lattice:
-    def __init__(self, L, rep=hr.REP_FUND, prec=hr.PREC_F64, kernel=hr.KERNEL_AUTO, device="cuda:0",
+    def __init__(self, L, rep=hr.REP_FUND, prec=hr.PREC_F64, kernel=hr.KERNEL_AUTO, device=None,
                  link_storage=hr.LINKS_COMPRESSED):
         self.L = tuple(int(v) for v in L)
         self.V = int(np.prod(self.L))
         self.N = 2 if rep == hr.REP_FUND else 3
         self.g = hr.geom(self.L, rep, prec, link_storage, kernel)
-        self.device = device
+        self.device = hr.current_device() if device is None else device     # every buffer of this object lives here
         self.real = hr.np_real(self.g)
         self.cplx = hr.np_complex(self.g)
         self.half = hr.hr_spinor_bytes(self.g, hr.EVEN)
@@ -42,7 +42,7 @@ class Lattice:
     def put_spinor(self, psi):
         """complex [V,4,N] -> packed full-lattice device field"""
         assert psi.shape == (self.V, 4, self.N), psi.shape
-        canon = hr.upload(psi.astype(self.cplx))
+        canon = hr.upload(psi.astype(self.cplx), self.device)
         dev = self.empty_spinor()
         hr.hr_pack_spinor(self.g, canon, dev, hr.stream_ptr())
         return dev
@@ -55,7 +55,7 @@ class Lattice:
     def put_gauge_fund(self, U):
         """complex [V,4,2,2] -> packed (compressed) fundamental gauge field"""
         assert U.shape == (self.V, 4, 2, 2), U.shape
-        canon = hr.upload(U.astype(self.cplx))
+        canon = hr.upload(U.astype(self.cplx), self.device)
         dev = self.empty_gauge(hr.REP_FUND)
         hr.hr_pack_gauge(self.g, hr.REP_FUND, canon, dev, hr.stream_ptr())
         return dev
@@ -67,7 +67,7 @@ class Lattice:
 
     def put_gauge_adj(self, R):
         assert R.shape == (self.V, 4, 3, 3), R.shape
-        canon = hr.upload(R.astype(self.real))
+        canon = hr.upload(R.astype(self.real), self.device)
         dev = self.empty_gauge(hr.REP_ADJ)
         hr.hr_pack_gauge(self.g, hr.REP_ADJ, canon, dev, hr.stream_ptr())
         return dev
@@ -80,7 +80,7 @@ class Lattice:
     def put_clover(self, blocks):
         """real [V,2,(2N)^2] -> packed block field (16 reals per block for the fundamental, 36 for the adjoint rep)"""
         assert blocks.shape == (self.V, 2, 4 * self.N * self.N), blocks.shape
-        canon = hr.upload(blocks.astype(self.real))
+        canon = hr.upload(blocks.astype(self.real), self.device)
         dev = self.empty_clover()
         hr.hr_pack_clover(self.g, canon, dev, hr.stream_ptr())
         return dev

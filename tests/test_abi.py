@@ -168,3 +168,23 @@ def test_missing_library_fails_loudly(monkeypatch):
     monkeypatch.setattr(hr, "LIB_PATH", "/nonexistent/libhr_dslash.so")
     with pytest.raises(ImportError):
         hr.lib()
+
+
+def test_lattice_stages_on_its_own_device(monkeypatch):
+    """every buffer a Lattice makes (canonical staging included) is requested on the Lattice's device, not on cuda:0:
+    under `bench.py --gpus N` rank k packs on cuda:k and must not read a cuda:0 pointer (no GPU needed: the
+    allocation and pack calls are recorded, not executed)"""
+    import numpy as np
+    from paper_2411_18511_b200 import hr as _hr, lattice
+    seen = []
+    monkeypatch.setattr(_hr, "upload", lambda a, device=None: seen.append(("upload", device)) or "canon")
+    monkeypatch.setattr(_hr, "device_buffer", lambda n, device=None: seen.append(("buffer", device)) or "dev")
+    monkeypatch.setattr(_hr, "stream_ptr", lambda stream=None: 0)
+    for name in ("hr_pack_spinor", "hr_pack_gauge", "hr_pack_clover"):
+        monkeypatch.setattr(_hr, name, lambda *a, **k: None)
+    lat = lattice.Lattice((4, 4, 4, 4), _hr.REP_ADJ, _hr.PREC_F64, device="cuda:3")
+    lat.put_spinor(np.zeros((256, 4, 3), dtype=np.complex128))
+    lat.put_gauge_fund(np.zeros((256, 4, 2, 2), dtype=np.complex128))
+    lat.put_gauge_adj(np.zeros((256, 4, 3, 3)))
+    lat.put_clover(np.zeros((256, 2, 36)))
+    assert len(seen) == 8 and all(dev == "cuda:3" for _, dev in seen), seen

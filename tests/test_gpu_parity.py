@@ -36,6 +36,17 @@ def rel(a, b):
     return float(np.linalg.norm((a.astype(np.complex128) - b).ravel()) / np.linalg.norm(b.ravel()))
 
 
+def site_err(a, b):
+    """largest per-site error relative to the r.m.s. site norm of the expected field: the whole-field norm of rel()
+    averages a defect confined to a few sites away (0.02 at one of 5.3 M sites is 1e-5 of the field norm); this
+    companion does not.  Arrays are [sites, spin, colour]."""
+    d = np.linalg.norm((a.astype(np.complex128) - b).reshape(b.shape[0], -1), axis=1)
+    return float(d.max() / (np.linalg.norm(b.ravel()) / np.sqrt(b.shape[0])))
+
+
+SITE_TOL = {0: 2e-13, 1: 2e-5}   # per-site companion of TOL (a single site may sit a few sigma above the r.m.s. error)
+
+
 def rounded(a, prec):
     return inputs.to_f32_rounded(a) if prec == 1 else a
 
@@ -248,6 +259,7 @@ def test_config2_24to4_adjoint(hr, orc):
     got = gpu_ops(hr, lat, R_dev, psi, m0)
     for k in want:
         assert rel(got[k], want[k]) <= 1e-13, k
+        assert site_err(got[k], want[k]) <= SITE_TOL[0], k
     # the same operators with the links rebuilt on the fly from the fundamental field, both kernels
     from paper_2411_18511_b200.lattice import Lattice
     for kernel in kernels_for(hr, L, 1, 0):
@@ -280,6 +292,7 @@ def test_config3_48to4_fundamental(hr, orc, big_inputs, prec):
         got = gpu_ops(hr, lat, lat.put_gauge_fund(U), psi, m0)
         for k in want:
             assert rel(got[k], want[k]) <= TOL[prec], (k, kernel)
+            assert site_err(got[k], want[k]) <= SITE_TOL[prec], (k, kernel)
 
 
 def test_config3_invariants_on_the_gpu(hr, big_inputs):
@@ -686,12 +699,10 @@ def test_adjoint_clover(hr, orc, L, prec, exponential):
     Uf = rounded(inputs.weak_gauge(L, 0.3, 1), prec)
     R, _ = orc.represent(Uf)
     psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
-    A = orc.clover_dense_adj(L, d, csw, R)
     if exponential:
-        lam, Vv = np.linalg.eigh((A - d * np.eye(12)[None]) / d)      # A_exp = d exp(C/d), as O9
-        Vh = np.conj(np.swapaxes(Vv, -1, -2))
-        A, Ainv = d * (Vv * np.exp(lam)[:, None, :]) @ Vh, (Vv * np.exp(-lam)[:, None, :]) @ Vh / d
+        A, Ainv = orc.clover_exp_dense_adj(L, d, csw, R)      # O11, pinned by P19
     else:
+        A = orc.clover_dense_adj(L, d, csw, R)
         Ainv = np.linalg.inv(A)
     bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
     tol_blk = 1e-13 if prec == 0 else 1e-6

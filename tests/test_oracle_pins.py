@@ -1,4 +1,4 @@
-"""Pins P1-P14: what holds the CPU oracle in place.
+"""Pins P1-P20 (P15-P20 for the oracle pieces of the §8(f) rows): what holds the CPU oracle in place.
 
 The paper (arXiv 2411.18511) prints no formula and no worked numeric example (PAPER.md:29-39,
 51-61 describe kernels only), so the oracle is pinned to what physics and mathematics fix:
@@ -571,3 +571,126 @@ def test_P17_adjoint_clover(orc):
             sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
             Fo = np.einsum("ts,xsatb->xab", sig, Aab.reshape(V, 4, 3, 4, 3)) / 4.0 / 0.5j
             assert np.abs(Fo - Fcf).max() <= 1e-13, (mu, nu)
+
+
+def _site_loop_matvec(M, psi):
+    """out[x] = M[x] psi[x], one site at a time with the @ operator (row index of M first) — the plain definition the
+    two oracle mat-vec routines are pinned to"""
+    out = np.empty_like(psi)
+    for x in range(psi.shape[0]):
+        out[x] = (M[x] @ psi[x].reshape(-1)).reshape(psi.shape[1:])
+    return out
+
+
+def test_P20_site_matvec_orientation(orc):
+    """orc_site_matvec (C++) and site_matvec_n (numpy): out[x]_i = sum_j M[x]_ij psi[x]_j with NON-hermitian random
+    site matrices (a transposed mat-vec passes every identity that only uses hermitian matrices consistently; it
+    fails here), the parity bit mask of orc_site_matvec (bit 0 even sites, bit 1 odd sites) and the mask of
+    site_matvec_n"""
+    L = (2, 4, 2, 4)
+    V = inputs.volume(L)
+    par = inputs.site_parity(L)
+    for N, n in ((2, 8), (3, 12)):
+        M = (inputs.normals(21, 5, 0, V * n * n) + 1j * inputs.normals(22, 5, 0, V * n * n)).reshape(V, n, n)
+        psi = inputs.gaussian_spinor(L, N, 2)
+        want = _site_loop_matvec(M, psi)
+        got_n = orc.site_matvec_n(M, psi)
+        assert np.abs(got_n - want).max() <= 1e-13
+        assert np.abs(got_n - _site_loop_matvec(np.swapaxes(M, -1, -2), psi)).max() > 1.0     # the transpose is far away
+        odd = par == 1
+        got_odd = orc.site_matvec_n(M, psi, odd)
+        assert np.abs(got_odd[odd] - want[odd]).max() <= 1e-13 and not got_odd[~odd].any()
+        if N == 2:
+            both = orc.site_matvec(L, 3, M, psi)
+            assert np.abs(both - want).max() <= 1e-13
+            for mask, sel in ((1, par == 0), (2, par == 1)):
+                got = orc.site_matvec(L, mask, M, psi)
+                assert np.abs(got[sel] - want[sel]).max() <= 1e-13 and not got[~sel].any()
+
+
+def test_P18_adjoint_clover_schur_identity(orc):
+    """O7 in the adjoint representation (oracle.dirac_eo_clover_adj), pinned by the Schur identity P4: with
+    eta = D_sw x on all sites (D_sw = D[R] + C, the full operator O1 in the adjoint representation plus the O10
+    clover term applied site by site here),
+        Dhat x_e = eta_e - D_eo A_oo^-1 eta_o = eta_e + 1/2 H_eo A_oo^-1 eta_o        (D_eo = -1/2 H_eo).
+    A wrong constant (-1/2 for -1/4), a swapped parity mask or A for A^-1 fails this; gamma5-hermiticity of Dhat
+    (P2) and the equivalent full solve on a 2^4 lattice (P5) ride along."""
+    L = (2, 4, 2, 4)
+    m0, csw = -0.25, 1.2
+    d = 4.0 + m0
+    Uf = inputs.weak_gauge(L, 0.3, seed=1)
+    R, _ = orc.represent(Uf)
+    par = inputs.site_parity(L)
+    even, odd = par == 0, par == 1
+    A = orc.clover_dense_adj(L, d, csw, R)
+    C = A - d * np.eye(12)[None]
+    Ainv = np.linalg.inv(A)
+    x = inputs.gaussian_spinor(L, 3, seed=2)
+    eta = orc.dirac(L, 1, m0, R, x) + _site_loop_matvec(C, x)
+    t = np.where(odd[:, None, None], _site_loop_matvec(Ainv, eta), 0.0)
+    rhs = np.where(even[:, None, None], eta, 0.0) + 0.5 * orc.hop(L, 1, 0, R, t)
+    lhs = orc.dirac_eo_clover_adj(L, R, A, Ainv, x)
+    assert rel_l2(lhs, rhs) < 1e-14
+    assert not lhs[odd].any()
+    # the other half of the identity: x_o = A_oo^-1 (eta_o + 1/2 H_oe x_e)
+    xe = np.where(even[:, None, None], x, 0.0)
+    xo = _site_loop_matvec(Ainv, np.where(odd[:, None, None], eta + 0.5 * orc.hop(L, 1, 1, R, xe), 0.0))
+    assert rel_l2(xo[odd], x[odd]) < 1e-14
+    # P2: <chi, Dhat psi> = <gamma5 Dhat gamma5 chi, psi> on even-supported vectors
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+    chi = np.where(even[:, None, None], inputs.gaussian_spinor(L, 3, 3, inputs.FIELD_SPINOR2), 0.0)
+    a = inner(chi, orc.dirac_eo_clover_adj(L, R, A, Ainv, xe))
+    b = inner(g5 * orc.dirac_eo_clover_adj(L, R, A, Ainv, g5 * chi), xe)
+    assert abs(a - b) <= 1e-13 * abs(a)
+    # P5 on 2^4: dense D_sw (192 unknowns) solved by LAPACK; its even part solves the Schur system
+    L2 = (2, 2, 2, 2)
+    V2 = 16
+    U2 = inputs.weak_gauge(L2, 0.3, seed=1)
+    R2, _ = orc.represent(U2)
+    A2 = orc.clover_dense_adj(L2, d, csw, R2)
+    A2inv = np.linalg.inv(A2)
+    C2 = A2 - d * np.eye(12)[None]
+    n = V2 * 12
+    Dsw = np.empty((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1.0
+        e = e.reshape(V2, 4, 3)
+        Dsw[:, k] = (orc.dirac(L2, 1, m0, R2, e) + _site_loop_matvec(C2, e)).ravel()
+    eta2 = inputs.gaussian_spinor(L2, 3, seed=2)
+    x2 = np.linalg.solve(Dsw, eta2.ravel()).reshape(V2, 4, 3)
+    ev2 = (inputs.site_parity(L2) == 0)[:, None, None]
+    t2 = np.where(~ev2, _site_loop_matvec(A2inv, eta2), 0.0)
+    rhs2 = np.where(ev2, eta2, 0.0) + 0.5 * orc.hop(L2, 1, 0, R2, t2)
+    assert rel_l2(orc.dirac_eo_clover_adj(L2, R2, A2, A2inv, x2), rhs2) < 1e-13
+
+
+def test_P19_adjoint_exponential_clover(orc):
+    """O11 (oracle.clover_exp_dense_adj): A_exp = d exp(C/d) on the 12x12 adjoint clover term.  Pins as P16: scipy's
+    Pade expm on three sites (another route), det A_exp = d^12 exactly (tr C = 0), A_exp A_exp^-1 = 1, hermitian,
+    commuting with gamma5, A_exp - (d + C) = C^2/(2d) + O(C^3) scaling as csw^2, and csw = 0 gives d * 1."""
+    from scipy.linalg import expm
+    L, m0 = (4, 2, 2, 2), -0.25
+    d = 4.0 + m0
+    R, _ = orc.represent(inputs.weak_gauge(L, 0.3, 1))
+    V = inputs.volume(L)
+    eye = np.eye(12)[None]
+    fwd, inv = orc.clover_exp_dense_adj(L, d, 1.2, R)
+    C = orc.clover_dense_adj(L, 0.0, 1.2, R)
+    for x in (0, 5, V - 1):
+        assert np.abs(fwd[x] - d * expm(C[x] / d)).max() <= 1e-13
+        assert np.abs(inv[x] - expm(-C[x] / d) / d).max() <= 1e-14
+    assert np.abs(np.linalg.det(fwd) - d ** 12).max() <= 1e-9 * d ** 12
+    assert np.abs(fwd @ inv - eye).max() <= 1e-14
+    assert np.abs(fwd - np.conj(np.swapaxes(fwd, -1, -2))).max() <= 1e-14
+    g5 = np.kron(np.diag([1, 1, -1, -1]), np.eye(3)).astype(complex)
+    assert np.abs(g5 @ fwd - fwd @ g5).max() <= 1e-14
+    rem2 = fwd - (d * eye + C)
+    rem3 = rem2 - C @ C / (2 * d)
+    nC = np.abs(C).max()
+    assert np.abs(rem2).max() <= 3.0 * nC ** 2 / d and np.abs(rem3).max() <= 4.0 * nC ** 3 / d ** 2
+    fwd_half, _ = orc.clover_exp_dense_adj(L, d, 0.6, R)
+    ratio = np.abs(rem2).max() / np.abs(fwd_half - (d * eye + 0.5 * C)).max()
+    assert 3.5 < ratio < 4.7          # quadratic in csw
+    f0, i0 = orc.clover_exp_dense_adj(L, d, 0.0, R)
+    assert np.abs(f0 - d * eye).max() <= 1e-14 and np.abs(i0 - eye / d).max() <= 1e-15
