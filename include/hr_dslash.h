@@ -190,8 +190,9 @@ int hr_cg_solve_mixed_clover(const hr_geom* g, double m0, const void* u_f64, con
  * `workspace` is a DEVICE buffer of at least hr_host_workspace_bytes(g) bytes.  The call uploads gauge
  * and spinor, packs, applies, unpacks, downloads, and synchronises `stream` before returning.
  *   hr_dirac_apply_host    : out[V] = D psi[V]
- *   hr_dirac_eo_apply_host : op as in hr_dirac_eo_apply without clover; full-lattice canonical arrays, only
- *                            the entries of the input parity are read, only those of the output parity written. */
+ *   hr_dirac_eo_apply_host : op as in hr_dirac_eo_apply without clover; full-lattice canonical arrays: only the
+ *                            entries of the input parity are read; ALL of out is written — the entries of the
+ *                            output parity with the result, those of the other parity with zeros. */
 size_t hr_host_workspace_bytes(const hr_geom* g);
 int hr_dirac_apply_host(const hr_geom* g, double m0, const void* u_canon_host, const void* psi_canon_host,
                         void* out_canon_host, void* workspace, void* stream);
@@ -204,6 +205,13 @@ size_t hr_last_error(char* buf, size_t len);   /* copies the last error text (NU
 unsigned long long hr_launch_count(void);
 /* name of the hopping kernel hr_dirac_eo_apply/hr_dirac_apply would run for g: "generic" or "tiled" */
 const char* hr_kernel_name(const hr_geom* g);
+/* The launch plan of the kernel behind op = HR_OP_HOP (a parity hop, also each hop of HR_OP_DHAT) or HR_OP_DIRAC
+ * (hr_dirac_apply) on the calling thread's current device; host only, nothing is launched.  info[8] receives
+ *   [0] kernel: 0 generic (the rest is then 0), 1 hop_tiled_kernel, 2 dirac_tiled_kernel
+ *   [1],[2] tile shape T1 x T2 in x3-rows   [3] x0 segments per tile   [4] planes per segment (L0 / segments)
+ *   [5] threads per CTA   [6] dynamic shared memory in bytes   [7] CTAs in the grid.
+ * For tests (which segment lengths a lattice exercises) and for the profile notes; other ops return HR_EINVAL. */
+int hr_kernel_plan(const hr_geom* g, int op, int* info);
 
 #ifdef __cplusplus
 }

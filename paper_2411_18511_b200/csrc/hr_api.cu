@@ -444,6 +444,13 @@ size_t hr_last_error(char* buf, size_t len) {
 
 unsigned long long hr_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
+int hr_kernel_plan(const hr_geom* g, int op, int* info) {
+    HR_TRY(check_geom(g));
+    if (!info) { set_error("hr_kernel_plan: info is NULL"); return HR_EINVAL; }
+    if (op != HR_OP_HOP && op != HR_OP_DIRAC) { set_error("hr_kernel_plan: op must be HR_OP_HOP or HR_OP_DIRAC"); return HR_EINVAL; }
+    return kernel_plan(g, op == HR_OP_DIRAC ? 2 : 0, info);
+}
+
 const char* hr_kernel_name(const hr_geom* g) {
     if (!geom_ok(g)) return "invalid";
     return tiled_chosen(g) ? "tiled" : "generic";

@@ -264,9 +264,10 @@ __device__ __forceinline__ void mul_link_dag(cplx<T>* chi, const Link<T, 3>& u, 
 //   mu=2: h0 = p0 - S p3,   h1 = p1 + S p2;    r2 = S h1,    r3 = -S h0
 //   mu=3: h0 = p0 - S i p2, h1 = p1 + S i p3;  r2 = S i h0,  r3 = -S i h1
 // psi and acc are [spin][colour] flattened: component spin*N + colour.
+// The two halves of a term: hop_project forms the half spinor (h0, h1) = upper two spin components of
+// (1 + S gamma_MU) psi; hop_apply multiplies it by the link and adds the rebuilt four components to acc.
 template <typename T, int N, int MU, bool FWD>
-__device__ __forceinline__ void hop_term(cplx<T>* acc, const cplx<T>* p, const Link<T, N>& u) {
-    cplx<T> h0[N], h1[N], c0[N], c1[N];
+__device__ __forceinline__ void hop_project(cplx<T>* h0, cplx<T>* h1, const cplx<T>* p) {
 #pragma unroll
     for (int c = 0; c < N; ++c) {
         const cplx<T> p0 = p[c], p1 = p[N + c], p2 = p[2 * N + c], p3 = p[3 * N + c];
@@ -284,6 +285,10 @@ __device__ __forceinline__ void hop_term(cplx<T>* acc, const cplx<T>* p, const L
             h1[c] = FWD ? p1 - timesI(p3) : p1 + timesI(p3);
         }
     }
+}
+template <typename T, int N, int MU, bool FWD>
+__device__ __forceinline__ void hop_apply(cplx<T>* acc, const cplx<T>* h0, const cplx<T>* h1, const Link<T, N>& u) {
+    cplx<T> c0[N], c1[N];
     if (FWD) { mul_link(c0, u, h0); mul_link(c1, u, h1); }
     else     { mul_link_dag(c0, u, h0); mul_link_dag(c1, u, h1); }
 #pragma unroll
@@ -304,6 +309,12 @@ __device__ __forceinline__ void hop_term(cplx<T>* acc, const cplx<T>* p, const L
             acc[3 * N + c] = FWD ? acc[3 * N + c] + timesI(c1[c]) : acc[3 * N + c] - timesI(c1[c]);
         }
     }
+}
+template <typename T, int N, int MU, bool FWD>
+__device__ __forceinline__ void hop_term(cplx<T>* acc, const cplx<T>* p, const Link<T, N>& u) {
+    cplx<T> h0[N], h1[N];
+    hop_project<T, N, MU, FWD>(h0, h1, p);
+    hop_apply<T, N, MU, FWD>(acc, h0, h1, u);
 }
 
 // ------------------------------------------------------------------ hermitian 4x4 block times 4-vector
@@ -372,5 +383,6 @@ struct HopArgs;
 int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st);
 bool tiled_supported(const hr_geom* g);
 bool tiled_chosen(const hr_geom* g);
+int kernel_plan(const hr_geom* g, int both, int* info);   // both: 0 parity hop, 1 paired-parity launch, 2 full D with phi == in
 
 }  // namespace hr

@@ -1,5 +1,5 @@
 // hr_hop.cu — dispatch of the hopping kernels (H1/H2/H3).
-#include "hr_hop_tiled.cuh"
+#include "hr_dirac_tiled.cuh"
 
 namespace hr {
 
@@ -8,23 +8,23 @@ namespace hr {
 static const double TILED_AUTO_MIN_SITES = 32.0 * 32.0 * 32.0 * 32.0;
 
 static int sm_count() {   // of the calling thread's current device (cached per device)
-    static int cache[64] = {};
+    static std::atomic<int> cache[64];
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return 148; }
-    if (cache[dev] == 0) {
-        int n = 0;
+    int n = cache[dev].load(std::memory_order_relaxed);
+    if (n == 0) {
         if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
             (void)cudaGetLastError();
             n = 148;
         }
-        cache[dev] = n;
+        cache[dev].store(n, std::memory_order_relaxed);
     }
-    return cache[dev];
+    return n;
 }
 
 bool tiled_supported(const hr_geom* g) {
     TiledPlan pl;
-    return tiled_plan(g, 0, 148, pl);
+    return tiled_plan(g, 0, 148, pl);     // (whether a tile shape fits does not depend on the SM count)
 }
 
 bool tiled_chosen(const hr_geom* g) {
@@ -37,15 +37,37 @@ bool tiled_chosen(const hr_geom* g) {
     return v >= TILED_AUTO_MIN_SITES;
 }
 
+// the launch plan of an operator on this geometry, for tests and diagnostics (hr_kernel_plan)
+int kernel_plan(const hr_geom* g, int both, int* info) {
+    for (int i = 0; i < 8; ++i) info[i] = 0;
+    if (!tiled_chosen(g)) return HR_OK;            // generic kernel: info[0] = 0
+    DiracPlan dp;
+    if (both == 2 && dirac_plan(g, sm_count(), dp)) {
+        const int v[8] = {2, dp.t1, dp.t2, dp.nseg, dp.seglen, dp.nconsumer + 32, (int)dp.smem, dp.nt1 * dp.nt2 * dp.nseg};
+        for (int i = 0; i < 8; ++i) info[i] = v[i];
+        return HR_OK;
+    }
+    TiledPlan pl;
+    if (!tiled_plan(g, both ? 1 : 0, sm_count(), pl)) return HR_OK;
+    const int v[8] = {1, pl.t1, pl.t2, pl.nseg, pl.seglen, pl.nconsumer + 32, (int)pl.smem, (both ? 2 : 1) * pl.nt1 * pl.nt2 * pl.nseg};
+    for (int i = 0; i < 8; ++i) info[i] = v[i];
+    return HR_OK;
+}
+
 int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
     const Geo geo = make_geo(g);
-    if (g->kernel == HR_KERNEL_TILED && !tiled_supported(g)) {
+    TiledPlan pl;
+    const bool fits = g->kernel != HR_KERNEL_GENERIC && tiled_plan(g, a.both, sm_count(), pl);
+    if (g->kernel == HR_KERNEL_TILED && !fits) {
         set_error("HR_KERNEL_TILED: lattice %dx%dx%dx%d does not fit the tiled kernel", g->L[0], g->L[1], g->L[2], g->L[3]);
         return HR_EUNSUPPORTED;
     }
-    if (tiled_chosen(g)) {
-        TiledPlan pl;
-        tiled_plan(g, a.both, sm_count(), pl, a.both && epi == EPI_AXPY && a.phi == a.in);
+    if (fits && tiled_chosen(g)) {
+        DiracPlan dp;
+        if (a.both && epi == EPI_AXPY && a.phi == a.in && dirac_plan(g, sm_count(), dp)) {   // H3: hr_dirac_tiled.cuh
+            if (g->prec == HR_PREC_F64) return launch_dirac_tiled<double>(geo, a, dp, st);
+            return launch_dirac_tiled<float>(geo, a, dp, st);
+        }
         if (g->rep == HR_REP_FUND) {
             if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 2>(geo, a, epi, pl, st);
             return launch_hop_tiled<float, 2>(geo, a, epi, pl, st);

@@ -12,69 +12,25 @@
 // profiles/r01_generic_hop.md), and an input row crosses L2->SM (1 + 2/T1 + 2/T2) times instead of ~5.4.
 #pragma once
 
-#include <cstdlib>
+#include <atomic>
 
 #include "hr_hop_generic.cuh"
 
 namespace hr {
 
 constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live + one being filled
-// Tuning switches (HR_T_*): the defaults are the measured choices of profiles/r01_tiled_variants.md; a build with
-// other values is made with HR_NVCC_DEFS="-DHR_T_...=v" python -m paper_2411_18511_b200.build --force.
-#ifndef HR_T_HALO
-#define HR_T_HALO 2
-#endif
-// consumer scheduling, per precision (measured at 48^4, profiles/r01_tiled_variants.md):
-//   PIN  : __syncwarp() after each link re-load, which stops ptxas from sinking the loads to the end of the step
-//   NBDB : read the neighbour of term t+1 from shared memory before computing term t (two register images)
-#ifndef HR_T_PIN_F64
-#define HR_T_PIN_F64 0
-#endif
-#ifndef HR_T_PIN_F32
-#define HR_T_PIN_F32 1
-#endif
-#ifndef HR_T_NBDB_F64
-#define HR_T_NBDB_F64 0
-#endif
-#ifndef HR_T_NBDB_F32
-#define HR_T_NBDB_F32 1
-#endif
-constexpr int TILED_HALO = HR_T_HALO;         // halo buffers: one in use, one being filled (a third one costs the L1 the link loads need)
+constexpr int TILED_HALO = 2;         // halo buffers: one in use, one being filled (a third one costs the L1 the link loads need)
+
+// Per-precision choices, each made by measurement at 48^4 (profiles/r01_tiled_variants.md):
+//   PIN     : __syncwarp() after each link re-load, which stops ptxas from sinking the loads to the end of the step
+//   NBDB    : read the neighbour of term t+1 from shared memory before computing term t (two register images)
 //   LINKPOL : cache policy of the link loads (LD_STREAM = ld.global.cs, LD_KEEP = ld.global.nc)
-#ifndef HR_T_LINKPOL_F64
-#define HR_T_LINKPOL_F64 LD_KEEP
-#endif
-#ifndef HR_T_LINKPOL_F32
-#define HR_T_LINKPOL_F32 LD_STREAM
-#endif
-#ifndef HR_T_PHIPOL_SHARE
-#define HR_T_PHIPOL_SHARE LD_KEEP
-#endif
-#ifndef HR_T_LINKPOL_SHARE
-#define HR_T_LINKPOL_SHARE LD_KEEP
-#endif
-//   FULL : H3 with both parities per CTA (kernel MODE 2) when the launch allows it
-#ifndef HR_T_FULL
-#define HR_T_FULL 1
-#endif
-#ifndef HR_T_PIN_FULL
-#define HR_T_PIN_FULL 1
-#endif
-#ifndef HR_T_NBDB_FULL
-#define HR_T_NBDB_FULL 0
-#endif
-#ifndef HR_T_L3H_F32_FULL
-#define HR_T_L3H_F32_FULL 0
-#endif
-#ifndef HR_T_F32_WIDE
-#define HR_T_F32_WIDE 1
-#endif
-// consumer threads per output parity the kernel is compiled for (one per site of a T1 x T2 tile of rows): 192 for the
-// small tiles (2 x 4 rows of L3h <= 24 sites, 2 x 2 rows of L3h <= 48), 384 for 4 x 4 rows; MODE 2 (both parities per
-// CTA, twice the threads) keeps to T1*T2*24 so that its register budget stays at 255
-constexpr int tiled_max_consumers(int t1, int t2, int mode) {
-    return mode == 2 ? ((t1 * t2 * 24 + 31) / 32) * 32 : (t1 * t2 <= 8 ? 192 : 384);
-}
+template <typename T> struct TiledTuning;
+template <> struct TiledTuning<double> { static constexpr bool PIN = false, NBDB = false; static constexpr int LINKPOL = LD_KEEP; };
+template <> struct TiledTuning<float> { static constexpr bool PIN = true, NBDB = true; static constexpr int LINKPOL = LD_STREAM; };
+// consumer threads the kernel is compiled for (one per output site of a T1 x T2 tile of rows): 192 for the small tiles
+// (2 x 4 rows of L3h <= 24 sites, 2 x 2 rows of L3h <= 48), 384 for 4 x 4 rows
+constexpr int tiled_max_consumers(int t1, int t2) { return t1 * t2 <= 8 ? 192 : 384; }
 
 // ------------------------------------------------------------------ mbarrier / bulk-copy primitives (PTX)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -151,7 +107,6 @@ __device__ __forceinline__ void lds_site<float, 12>(cplx<float>* s, const char* 
 // launch geometry chosen on the host (hr_hop.cu)
 struct TiledPlan {
     int t1, t2;        // tile shape in rows (x1, x2): selects the kernel instantiation
-    int mode;          // kernel MODE (0 one parity, 1 paired CTAs, 2 both parities per CTA)
     int nt1, nt2;      // tiles along x1, x2
     int nseg, seglen;  // x0 segments per tile and their length (nseg*seglen == L0)
     int nconsumer;     // consumer threads (multiple of 32, >= T1*T2*L3h)
@@ -165,17 +120,14 @@ struct TiledPlan {
 // run next to each other and the second use hits L2.
 // Shared memory: [16 mbarriers][ring: TILED_RING planes of T1*T2 rows][halo: TILED_HALO buffers of 2*T2 + 2*T1 rows]
 //   halo buffer rows: [x1-1 line: T2 rows][x1+T1 line: T2 rows][x2-1 rows: T1][x2+T2 rows: T1]
-// MODE 0: one output parity per launch.
-// MODE 1 (full-lattice launch, fallback): the two parities as neighbouring CTAs; links and phi are also read by the
-//         CTA of the other parity, so they are loaded with normal L2 priority.
-// MODE 2 (full-lattice launch, H3): ONE CTA computes both parities of its tile.  Every plane and halo buffer holds
-//         the even and the odd half-rows ([parity][row]); consumer thread (parity p, site) gathers from the 1-p
-//         images and takes the axpy operand phi(x) = psi(x) from the p image of the centre plane — no global load,
-//         no latency — and both uses of a link happen in the same CTA in the same step (second one hits L1/L2).
+// SHARE = false: one output parity per launch.
+// SHARE = true : full-lattice launch, the two parities as neighbouring CTAs; links and phi are also read by the CTA of
+//         the other parity, so they are loaded with normal L2 priority.  (The plain full operator D with phi == in has
+//         its own kernel, hr_dirac_tiled.cuh; this path serves the clover-improved one and the adjoint representation.)
 // L3H: compile-time L3/2 (0 = read it from the geometry): the strides between the 16-byte chunks of a site are then
 // immediates in every LDS / LDG / STG (about a quarter fewer instructions per site)
-template <typename T, int N, int EPI, int T1, int T2, int MODE, bool ONFLY, int L3H>
-__global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, T2, MODE) + 32, (MODE != 2 && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H>
+__global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g_in, HopArgs a, TiledPlan pl) {
     Geo g = g_in;
     if (L3H > 0) g.L3h = L3H;
@@ -183,18 +135,14 @@ __global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, 
     typedef SiteIO<T, NC> IO;
     constexpr int TR = T1 * T2;            // tile rows
     constexpr int HR = 2 * T2 + 2 * T1;    // halo rows
-    constexpr bool SHARE = MODE == 1;
-    constexpr bool FULL = MODE == 2;
-    constexpr int NPAR = FULL ? 2 : 1;      // parity images per plane / halo buffer
-    constexpr int LP = FULL ? LD_KEEP : SHARE ? HR_T_LINKPOL_SHARE : (sizeof(T) == 4 ? HR_T_LINKPOL_F32 : HR_T_LINKPOL_F64);
-    constexpr bool PIN = FULL ? HR_T_PIN_FULL : sizeof(T) == 4 ? HR_T_PIN_F32 : HR_T_PIN_F64;
-    constexpr bool NBDB = FULL ? HR_T_NBDB_FULL : sizeof(T) == 4 ? HR_T_NBDB_F32 : HR_T_NBDB_F64;
+    constexpr int LP = SHARE ? LD_KEEP : TiledTuning<T>::LINKPOL;
+    constexpr bool PIN = TiledTuning<T>::PIN, NBDB = TiledTuning<T>::NBDB;
     extern __shared__ __align__(128) char smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
     char* ring = smem + 128;
     const int rowb = L3H > 0 ? SiteIO<T, 4 * N>::NCH * L3H * 16 : pl.rowb;
-    const int planeb = NPAR * TR * rowb;
-    const int halob = NPAR * HR * rowb;
+    const int planeb = TR * rowb;
+    const int halob = HR * rowb;
     char* halo = ring + TILED_RING * planeb;
     const uint32_t bar_full = smem_u32(bars);            // [TILED_RING]
     const uint32_t bar_empty = smem_u32(bars + 4);       // [TILED_RING]
@@ -215,7 +163,7 @@ __global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, 
     // ---- which work: parity, tile, x0 segment
     int bid = blockIdx.x;
     int p = a.parity;
-    if (a.both && !FULL) { p = bid & 1; bid >>= 1; }
+    if (a.both) { p = bid & 1; bid >>= 1; }
     const int seg = bid / (pl.nt1 * pl.nt2);
     const int tile = bid - seg * (pl.nt1 * pl.nt2);
     const int t1 = tile / pl.nt2, t2 = tile - t1 * pl.nt2;
@@ -244,26 +192,22 @@ __global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, 
             const uint32_t full = bar_full + 8 * slot;
             mbar_expect_tx(full, (uint32_t)(planeb + (with_halo ? halob : 0)));
             const int x0p = (xs - 1 + j + L0) % L0;
+            const uint32_t dst = smem_u32(ring + slot * planeb);
 #pragma unroll
-            for (int pp = 0; pp < NPAR; ++pp) {
-                const char* src = FULL ? reinterpret_cast<const char*>(a.in) + (size_t)pp * half_bytes : in_half;
-                const uint32_t dst = smem_u32(ring + slot * planeb + pp * TR * rowb);
+            for (int aa = 0; aa < T1; ++aa) {
+                const size_t row = ((size_t)x0p * L1 + x1base + aa) * L2 + x2base;
+                bulk_g2s(dst + aa * T2 * rowb, in_half + row * rowb, (uint32_t)(T2 * rowb), full);
+            }
+            if (with_halo) {
+                const int x0h = (xs - 1 + hc + L0) % L0;
+                const uint32_t hd = smem_u32(halo + hb * halob);
+                bulk_g2s(hd, in_half + (((size_t)x0h * L1 + x1lo) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
+                bulk_g2s(hd + T2 * rowb, in_half + (((size_t)x0h * L1 + x1hi) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
 #pragma unroll
                 for (int aa = 0; aa < T1; ++aa) {
-                    const size_t row = ((size_t)x0p * L1 + x1base + aa) * L2 + x2base;
-                    bulk_g2s(dst + aa * T2 * rowb, src + row * rowb, (uint32_t)(T2 * rowb), full);
-                }
-                if (with_halo) {
-                    const int x0h = (xs - 1 + hc + L0) % L0;
-                    const uint32_t hd = smem_u32(halo + hb * halob + pp * HR * rowb);
-                    bulk_g2s(hd, src + (((size_t)x0h * L1 + x1lo) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
-                    bulk_g2s(hd + T2 * rowb, src + (((size_t)x0h * L1 + x1hi) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
-#pragma unroll
-                    for (int aa = 0; aa < T1; ++aa) {
-                        const size_t rb = ((size_t)x0h * L1 + x1base + aa) * L2;
-                        bulk_g2s(hd + (2 * T2 + aa) * rowb, src + (rb + x2lo) * rowb, (uint32_t)rowb, full);
-                        bulk_g2s(hd + (2 * T2 + T1 + aa) * rowb, src + (rb + x2hi) * rowb, (uint32_t)rowb, full);
-                    }
+                    const size_t rb = ((size_t)x0h * L1 + x1base + aa) * L2;
+                    bulk_g2s(hd + (2 * T2 + aa) * rowb, in_half + (rb + x2lo) * rowb, (uint32_t)rowb, full);
+                    bulk_g2s(hd + (2 * T2 + T1 + aa) * rowb, in_half + (rb + x2hi) * rowb, (uint32_t)rowb, full);
                 }
             }
         }
@@ -272,17 +216,8 @@ __global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, 
 
     // ================================================================ consumers: one thread per output site
     const int L3h = g.L3h;
-    const int nsp = pl.nconsumer / NPAR;              // consumer threads per output parity
-    if (FULL) {
-        p = tid >= nsp ? 1 : 0;
-        out_half = reinterpret_cast<char*>(a.out) + (size_t)p * half_bytes;
-    }
-    const int stid = FULL ? tid - p * nsp : tid;
-    const bool active = stid < TR * L3h;
-    const int ctid = active ? stid : 0;              // idle threads shadow site 0 (no global access)
-    const int qoff_plane = FULL ? (1 - p) * TR * rowb : 0;   // the gather reads the 1-p images
-    const int qoff_halo = FULL ? (1 - p) * HR * rowb : 0;
-    const int poff_plane = FULL ? p * TR * rowb : 0;
+    const bool active = tid < TR * L3h;
+    const int ctid = active ? tid : 0;               // idle threads shadow site 0 (no global access)
     const int lr = ctid / L3h, h = ctid - lr * L3h;   // local row in the tile, pair index
     const int la = lr / T2, lb = lr - la * T2;
     const int x1 = t1 * T1 + la, x2 = t2 * T2 + lb;
@@ -319,11 +254,11 @@ __global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, 
         const int r = (x0 + x1 + x2 + p) & 1;
         const int hf3 = r ? (h == L3h - 1 ? 0 : h + 1) : h;
         const int hb3 = r ? h : (h == 0 ? L3h - 1 : h - 1);
-        const char* sprev = ring + (k & 3) * planeb + qoff_plane;
-        const char* scur = ring + ((k + 1) & 3) * planeb + qoff_plane;
-        const char* snext = ring + ((k + 2) & 3) * planeb + qoff_plane;
+        const char* sprev = ring + (k & 3) * planeb;
+        const char* scur = ring + ((k + 1) & 3) * planeb;
+        const char* snext = ring + ((k + 2) & 3) * planeb;
         const int hb = (k + 1) % TILED_HALO;
-        const char* shalo = halo + hb * halob + qoff_halo;
+        const char* shalo = halo + hb * halob;
         if (k == 0) {
             mbar_wait(bar_full, 0);
             mbar_wait(bar_full + 8, 0);
@@ -399,119 +334,96 @@ __global__ void __launch_bounds__((MODE == 2 ? 2 : 1) * tiled_max_consumers(T1, 
             mbar_arrive(bar_empty + 8 * (k & 3));
             mbar_arrive(bar_hempty + 8 * hb);
         }
-        // (requesting phi before the eight terms was measured slower at 48^4: 412 -> 425 us for fp64 H3)
-        if (FULL && EPI == EPI_AXPY) {
-            // phi(x) = psi(x): the own-parity image of the centre plane (not recycled before the end of step k+1)
-            cplx<T> phi[NC];
-            lds_site<T, NC>(phi, ring + ((k + 1) & 3) * planeb + poff_plane + off_c + h * 16, cs);
-            const T ca = (T)a.a, cc = (T)a.c;
-#pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                acc[c].re = fma(cc, acc[c].re, ca * phi[c].re);
-                acc[c].im = fma(cc, acc[c].im, ca * phi[c].im);
-            }
-            if (active) IO::store(out_half, (size_t)(row0 + x0 * g.s0) * (IO::NCH * L3h) + h, L3h, acc);
-        } else if (active) {
-            hop_epilogue<T, N, EPI, (SHARE ? HR_T_PHIPOL_SHARE : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
-        }
+        // (requesting phi before the eight terms was measured slower at 48^4)
+        if (active) hop_epilogue<T, N, EPI, (SHARE ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
     }
 }
 
 // ------------------------------------------------------------------ host side
 constexpr size_t TILED_SMEM_LIMIT = 227 * 1024;
 
-// mode: 0/1 as the kernel's MODE 0/1; 2 = both parities per CTA (H3 with phi == in)
-inline bool tiled_plan_shape(const hr_geom* hg, int both, int mode, int num_sms, int t1, int t2, TiledPlan& pl) {
-    const Geo g = make_geo(hg);
-    const int L1 = hg->L[1], L2 = hg->L[2], L0 = hg->L[0];
-    if (L1 % t1 || L2 % t2) return false;
-    const int sites = t1 * t2 * g.L3h;
-    if (sites > tiled_max_consumers(t1, t2, mode)) return false;
-    const int npar = mode == 2 ? 2 : 1;
-    pl.t1 = t1;
-    pl.t2 = t2;
-    pl.mode = mode;
-    pl.nconsumer = npar * ((sites + 31) & ~31);
-    pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
-    pl.smem = 128 + (size_t)pl.rowb * npar * (TILED_RING * t1 * t2 + TILED_HALO * (2 * t1 + 2 * t2));
-    if (pl.smem > TILED_SMEM_LIMIT) return false;
-    pl.nt1 = L1 / t1;
-    pl.nt2 = L2 / t2;
-    // x0 segments: minimise waves x (segment length + pipeline fill) over the divisors of L0
-    const int cps = (mode != 2 && 2 * pl.smem + 2048 <= 228 * 1024 && hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND) ? 2 : 1;  // CTAs per SM
-    const long tiles = (long)pl.nt1 * pl.nt2 * ((both && mode != 2) ? 2 : 1);
-    const long slots = (long)(num_sms > 0 ? num_sms : 148) * cps;
+// the opt-in to > 48 KiB of dynamic shared memory is a per-device attribute of the kernel function: set once per
+// instantiation and device (`flags`: 64 zero-initialised entries owned by the launch function of that instantiation;
+// two host threads may both set the attribute, which is idempotent)
+inline int opt_in_shared_memory(const void* kern, std::atomic<unsigned char>* flags, const char* name) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); dev = 0; }
+    if (!flags[dev].load(std::memory_order_acquire)) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
+        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute(%s): %s", name, cudaGetErrorString(e)); return HR_ECUDA; }
+        flags[dev].store(1, std::memory_order_release);
+    }
+    return HR_OK;
+}
+
+// x0 segments per tile: minimise waves x (segment length + pipeline fill) over the divisors of L0
+inline int tiled_segments(int L0, long tiles, long slots) {
     double best = 1e300;
-    pl.nseg = 1;
+    int nseg = 1;
     for (int ns = 1; ns <= L0; ++ns) {
         if (L0 % ns) continue;
         const long waves = (tiles * ns + slots - 1) / slots;
         const double cost = (double)waves * (L0 / ns + 3);
-        if (cost < best - 1e-9) { best = cost; pl.nseg = ns; }
+        if (cost < best - 1e-9) { best = cost; nseg = ns; }
     }
-    // tuning / test knob: HR_TILED_NSEG=<divisor of L0> overrides the choice
-    if (const char* e = getenv("HR_TILED_NSEG")) {
-        const int ns = atoi(e);
-        if (ns >= 1 && ns <= L0 && L0 % ns == 0) pl.nseg = ns;
-    }
+    return nseg;
+}
+
+inline bool tiled_plan_shape(const hr_geom* hg, int both, int num_sms, int t1, int t2, TiledPlan& pl) {
+    const Geo g = make_geo(hg);
+    const int L1 = hg->L[1], L2 = hg->L[2], L0 = hg->L[0];
+    if (L1 % t1 || L2 % t2) return false;
+    const int sites = t1 * t2 * g.L3h;
+    if (sites > tiled_max_consumers(t1, t2)) return false;
+    pl.t1 = t1;
+    pl.t2 = t2;
+    pl.nconsumer = (sites + 31) & ~31;
+    pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
+    pl.smem = 128 + (size_t)pl.rowb * (TILED_RING * t1 * t2 + TILED_HALO * (2 * t1 + 2 * t2));
+    if (pl.smem > TILED_SMEM_LIMIT) return false;
+    pl.nt1 = L1 / t1;
+    pl.nt2 = L2 / t2;
+    const int cps = (!both && 2 * pl.smem + 2048 <= 228 * 1024 && hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND && t1 * t2 <= 8) ? 2 : 1;  // CTAs per SM
+    pl.nseg = tiled_segments(L0, (long)pl.nt1 * pl.nt2 * (both ? 2 : 1), (long)(num_sms > 0 ? num_sms : 148) * cps);
     pl.seglen = L0 / pl.nseg;
     return true;
 }
 
 // fills pl; false if the lattice fits no instantiated tile shape.  fp32 fundamental rows are half as long,
-// so a 4 x 4 tile fits (2 row-loads per site instead of 2.5); everything else uses 2 x 4.  want_full: the
-// caller is the full-lattice launch with phi == in (H3): both parities per CTA on a 2 x 2 (fp64) / 2 x 4 (fp32)
-// tile if that fits, else the paired-CTA fallback (mode 1).
-inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl, bool want_full = false) {
-#if HR_T_FULL
-    if (want_full && both && hg->rep == HR_REP_FUND) {
-        if (hg->prec == HR_PREC_F64 && tiled_plan_shape(hg, both, 2, num_sms, 2, 2, pl)) return true;
-        if (hg->prec == HR_PREC_F32 && tiled_plan_shape(hg, both, 2, num_sms, 2, 4, pl)) return true;
-    }
-#endif
-    const int mode = both ? 1 : 0;
-#if HR_T_F32_WIDE
-    if (hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, mode, num_sms, 4, 4, pl)) return true;
-#endif
-    if (tiled_plan_shape(hg, both, mode, num_sms, 2, 4, pl)) return true;
-    // longer rows (24 < L3/2 <= 48) or L2 not a multiple of 4: 2 x 2 rows, fundamental representation only
-    return hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, mode, num_sms, 2, 2, pl);
+// so a 4 x 4 tile fits (2 row-loads per site instead of 2.5); everything else uses 2 x 4, or 2 x 2 for longer rows
+// (24 < L3/2 <= 48) or L2 not a multiple of 4 (fundamental representation only).
+inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) {
+    if (hg->prec == HR_PREC_F32 && hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, num_sms, 4, 4, pl)) return true;
+    if (tiled_plan_shape(hg, both, num_sms, 2, 4, pl)) return true;
+    return hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, num_sms, 2, 2, pl);
 }
 
-template <typename T, int N, int EPI, int MODE, int T1, int T2, bool ONFLY, int L3H>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H>
 inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, MODE, ONFLY, L3H>;
-    // the opt-in to > 48 KiB of dynamic shared memory is a per-device attribute of the function: once per
-    // instantiation and device (a benign race: two threads may both set it)
-    static bool configured[64] = {};
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
-    if (!configured[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TILED_SMEM_LIMIT);
-        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute(hop_tiled_kernel): %s", cudaGetErrorString(e)); return HR_ECUDA; }
-        configured[dev] = true;
-    }
-    const unsigned grid = (unsigned)(((a.both && MODE != 2) ? 2 : 1) * pl.nt1 * pl.nt2 * pl.nseg);
+    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H>;
+    static std::atomic<unsigned char> configured[64];
+    const int rc = opt_in_shared_memory(reinterpret_cast<const void*>(kern), configured, "hop_tiled_kernel");
+    if (rc != HR_OK) return rc;
+    const unsigned grid = (unsigned)((a.both ? 2 : 1) * pl.nt1 * pl.nt2 * pl.nseg);
     kern<<<grid, pl.nconsumer + 32, pl.smem, st>>>(g, a, pl);
     count_launch();
     return check_launch("hop_tiled_kernel");
 }
 
-template <typename T, int N, int EPI, int MODE, int T1, int T2, bool ONFLY>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY>
 inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    // (measured at 48^4: fp64 hop 219.3 -> 216.1 us, H3 411 -> 408; the fp32 4x4 H3 got slower, so fp64 only)
-    constexpr bool SPECIALISE = N == 2 && (sizeof(T) == 8 || (MODE == 2 && HR_T_L3H_F32_FULL));
-    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, MODE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0)>(g, a, pl, st);
-    return launch_hop_tiled_l3h<T, N, EPI, MODE, T1, T2, ONFLY, 0>(g, a, pl, st);
+    // compile-time L3/2 = 24 for the fp64 fundamental kernels (measured at 48^4: hop 219.3 -> 216.1 us; the fp32 4 x 4
+    // kernel got slower with it)
+    constexpr bool SPECIALISE = N == 2 && sizeof(T) == 8;
+    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0)>(g, a, pl, st);
+    return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, 0>(g, a, pl, st);
 }
 
-template <typename T, int N, int EPI, int MODE, bool ONFLY>
+template <typename T, int N, int EPI, bool SHARE, bool ONFLY>
 inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, MODE, 2, 4, ONFLY>(g, a, pl, st);
-    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, MODE, 2, 2, false>(g, a, pl, st);
-#if HR_T_F32_WIDE
-    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, MODE, 4, 4, false>(g, a, pl, st);
-#endif
+    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4, ONFLY>(g, a, pl, st);
+    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, SHARE, 2, 2, false>(g, a, pl, st);
+    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4, false>(g, a, pl, st);
     set_error("hop_tiled_kernel: no instantiation for a %d x %d tile", pl.t1, pl.t2);
     return HR_EUNSUPPORTED;
 }
@@ -519,20 +431,14 @@ inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan&
 template <typename T, int N, bool ONFLY = false>
 inline int launch_hop_tiled(const Geo& g, const HopArgs& a, int epi, const TiledPlan& pl, cudaStream_t st) {
     switch (epi) {
-        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE, 0, ONFLY>(g, a, pl, st);
+        case EPI_NONE: return launch_hop_tiled_epi<T, N, EPI_NONE, false, ONFLY>(g, a, pl, st);
         case EPI_AXPY:
-#if HR_T_FULL
-            if (pl.mode == 2 && N == 2) {   // H3: both parities per CTA (plan made with want_full)
-                if (sizeof(T) == 8) return launch_hop_tiled_shape<double, 2, EPI_AXPY, 2, 2, 2, false>(g, a, pl, st);
-                return launch_hop_tiled_shape<float, 2, EPI_AXPY, 2, 2, 4, false>(g, a, pl, st);
-            }
-#endif
-            if (a.both) return launch_hop_tiled_epi<T, N, EPI_AXPY, 1, ONFLY>(g, a, pl, st);
-            return launch_hop_tiled_epi<T, N, EPI_AXPY, 0, ONFLY>(g, a, pl, st);
-        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV, 0, ONFLY>(g, a, pl, st);
+            if (a.both) return launch_hop_tiled_epi<T, N, EPI_AXPY, true, ONFLY>(g, a, pl, st);
+            return launch_hop_tiled_epi<T, N, EPI_AXPY, false, ONFLY>(g, a, pl, st);
+        case EPI_CLOVER_INV: return launch_hop_tiled_epi<T, N, EPI_CLOVER_INV, false, ONFLY>(g, a, pl, st);
         case EPI_CLOVER_AXPY:
-            if (a.both) return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, 1, ONFLY>(g, a, pl, st);   // H3c: links re-read by the other parity's CTA
-            return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, 0, ONFLY>(g, a, pl, st);
+            if (a.both) return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, true, ONFLY>(g, a, pl, st);   // H3c: links re-read by the other parity's CTA
+            return launch_hop_tiled_epi<T, N, EPI_CLOVER_AXPY, false, ONFLY>(g, a, pl, st);
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
 }

@@ -29,7 +29,7 @@ SYMBOLS = [
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
     "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
-    "hr_launch_count", "hr_kernel_name", "hr_cg_workspace_bytes", "hr_cg_solve",
+    "hr_launch_count", "hr_kernel_name", "hr_kernel_plan", "hr_cg_workspace_bytes", "hr_cg_solve",
     "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed", "hr_cg_solve_mixed_clover",
 ]
 
@@ -79,6 +79,7 @@ def lib():
             "hr_last_error": (S, [ctypes.c_char_p, S]),
             "hr_launch_count": (ctypes.c_ulonglong, []),
             "hr_kernel_name": (ctypes.c_char_p, [G]),
+            "hr_kernel_plan": (I, [G, I, ctypes.POINTER(ctypes.c_int)]),
             "hr_cg_workspace_bytes": (S, [G]),
             "hr_cg_mixed_workspace_bytes": (S, [G]),
             "hr_cg_solve_mixed": (I, [G, D, V, V, V, V, V, D, D, I, I, I, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), PD, V]),
@@ -233,6 +234,14 @@ def hr_cg_solve_mixed_clover(g, m0, u_f64, u_f32, cf64, ci64, cf32, ci32, b, x, 
 
 def hr_launch_count() -> int: return int(lib().hr_launch_count())
 def hr_kernel_name(g) -> str: return lib().hr_kernel_name(ctypes.byref(g)).decode()
+
+
+def hr_kernel_plan(g, op=OP_HOP) -> dict:
+    """launch plan of the kernel behind a parity hop (OP_HOP) or the full operator (OP_DIRAC); needs a CUDA device"""
+    info = (ctypes.c_int * 8)()
+    _check(lib().hr_kernel_plan(ctypes.byref(g), int(op), info))
+    keys = ("kernel", "t1", "t2", "nseg", "seglen", "threads", "smem", "grid")
+    return dict(zip(keys, (int(v) for v in info)))
 
 
 # ------------------------------------------------------------------ plumbing: device memory via torch

@@ -179,22 +179,30 @@ def test_adjoint_small_lattices(hr, orc, L, prec):
             assert rel(got2[k], want[k]) <= TOL[prec], k
 
 
-@pytest.mark.parametrize("nseg", [1, 2, 4, 8])
+@pytest.mark.parametrize("L,seglen", [((8, 2, 8, 6), 1), ((8, 8, 32, 6), 2), ((8, 8, 40, 6), 4), ((8, 8, 80, 6), 8)])
 @pytest.mark.parametrize("rep,N", [(0, 2), (1, 3)])
-def test_tiled_kernel_segment_lengths(hr, orc, monkeypatch, nseg, rep, N):
-    """the x0-marching kernel with segments of 8, 4, 2 and 1 planes (HR_TILED_NSEG), tiles that wrap onto
-    themselves in x1 (L1 = T1) and several tiles in x2; all four operators against the oracle"""
-    L, m0 = (8, 2, 8, 6), -0.2
-    monkeypatch.setenv("HR_TILED_NSEG", str(nseg))
+def test_tiled_kernel_segment_lengths(hr, orc, L, seglen, rep, N):
+    """the x0-marching kernels with segments of 1, 2, 4 and 8 planes: the planner minimises waves x (L0/segments + 3),
+    so the segment length follows from the number of tiles (2, 32, 40, 80 tiles of 2 x 4 rows on 148 SMs; the plan is
+    read back through hr_kernel_plan and asserted); tiles that wrap onto themselves in x1 (L1 = T1) and many tiles in
+    x2; all four operators against the oracle"""
+    m0 = -0.2
     Uf = inputs.haar_gauge(L, 1)
     U = Uf if rep == 0 else orc.represent(Uf)[0]
     psi = inputs.gaussian_spinor(L, N, 2)
     want = oracle_ops(orc, L, rep, U, psi, m0)
     lat = lattice(hr, L, rep, 0, hr.KERNEL_TILED)
     assert hr.hr_kernel_name(lat.g) == "tiled"
+    plan = hr.hr_kernel_plan(lat.g, hr.OP_HOP)
+    assert plan["kernel"] == 1 and plan["nseg"] * plan["seglen"] == L[0]
+    import torch
+    if torch.cuda.get_device_properties(0).multi_processor_count == 148:
+        assert plan["seglen"] == seglen, plan
+    full = hr.hr_kernel_plan(lat.g, hr.OP_DIRAC)
+    assert full["kernel"] == (2 if rep == 0 else 1), full
     got = gpu_ops(hr, lat, lat.put_gauge_fund(U) if rep == 0 else lat.put_gauge_adj(U), psi, m0)
     for k in want:
-        assert rel(got[k], want[k]) <= TOL[0], (k, nseg)
+        assert rel(got[k], want[k]) <= TOL[0], (k, plan, full)
 
 
 @pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (8, 2, 8, 6), (6, 2, 4, 12)])
