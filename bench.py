@@ -3,12 +3,14 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--L 48]
 
-One "step" = one pass of every hot-path row of DESIGN.md §2 over one 48^4 lattice of synthetic seeded
-fields (Haar links, Gaussian spinors; clover links exp(i 0.3 a.sigma)), inputs resident in HBM:
-    fp64: H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat, C2 clover, C3 clover inverse, E2 Dhat+clover, R1 represent
-    fp32: H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat
+One "step" = the fp64 Dslash group of BASELINE.json configs[3] over one 48^4 lattice of synthetic seeded fields (Haar
+links, Gaussian spinors), inputs resident in HBM:  H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat  (6 kernel launches).
 `value` = compulsory (algorithmic) bytes of the step (hr_dirac_flops_bytes) / step time, in GB/s — the paper's
-bandwidth metric.  Prints ONE JSON line (rank 0).  See DESIGN.md §7 for every field.
+bandwidth metric; `dtype` = "f64".  The same four operators in fp32 and the clover / represent rows
+(configs[4]: C2, C3, E2, H3c, R1) are timed right after, K steps each, and reported under `roofline.fp32_step`,
+`roofline.clover_step` and per operator under `roofline.per_op` (fraction of the measured copy bandwidth and of the
+8 TB/s datasheet figure, DRAM traffic from the ncu captures in profiles/kernel_traffic.json).
+Prints ONE JSON line (rank 0).  See DESIGN.md §7 for every field.
 """
 from __future__ import annotations
 
@@ -113,6 +115,18 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
 
 
+def workload_config(L):
+    """the `config` object, identical in both arms (the driver compares them)"""
+    return {"workload": "BASELINE.json configs[3]: %d^4 periodic lattice, SU(2) fundamental, fp64, Haar-random links (seed 1), Gaussian spinor "
+                        "(seed 2), m0 = -0.2; one step = hop o<-e, hop e<-o, full D, even-odd Dhat; GB/s by the compulsory byte model of "
+                        "hr_dirac_flops_bytes (512 / 512 / 384 / 1152 B per output site, compressed links)" % L[0],
+            "lattice": list(L), "ops": ["hop_oe", "hop_eo", "dirac", "dhat"], "precision": "fp64",
+            "l2_policy": "working set per op (>= 1.3 GB at 48^4) far exceeds the 126 MB L2; no flush needed"}
+
+
+GROUP_BYTES = {"hop_oe": 512.0, "hop_eo": 512.0, "dirac": 384.0, "dhat": 1152.0}   # fp64, per output site (DESIGN.md §5)
+
+
 # ------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import numpy as np
@@ -151,104 +165,128 @@ def run_ours(args):
     S["f64"]["fwd"], S["f64"]["inv"] = lat64.clover_build(m0c, csw, S["f64"]["Uw"])
     S["f64"]["Uadj"] = lat64.empty_gauge(hr.REP_ADJ)
     torch.cuda.synchronize()
-    del U, Uw
+    del Uw
     st = hr.stream_ptr()
 
-    # ---- the step: (name, precision, model op, output sites, callable)
-    def mk(tag):
+    # ---- operator groups: (name, geometry, model op, output sites, extra bytes per site, callable)
+    def dslash_group(tag):
         s = S[tag]
         lat, g = s["lat"], s["lat"].g
         ev, od = lat.even, lat.odd
-        ops = [
-            ("hop_oe_" + tag, g, hr.OP_HOP, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_OE, 0.0, s["U"], None, None, ev(s["psi"]), od(s["out"]), None, st)),
-            ("hop_eo_" + tag, g, hr.OP_HOP, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_EO, 0.0, s["U"], None, None, od(s["psi"]), ev(s["out"]), None, st)),
-            ("dirac_" + tag, g, hr.OP_DIRAC, V, lambda: hr.hr_dirac_apply(g, m0, s["U"], s["psi"], s["out"], st)),
-            ("dhat_" + tag, g, hr.OP_DHAT, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, m0, s["U"], None, None, ev(s["psi"]), ev(s["out"]), s["tmp"], st)),
+        return [
+            ("hop_oe_" + tag, g, hr.OP_HOP, Vh, 0.0, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_OE, 0.0, s["U"], None, None, ev(s["psi"]), od(s["out"]), None, st)),
+            ("hop_eo_" + tag, g, hr.OP_HOP, Vh, 0.0, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_EO, 0.0, s["U"], None, None, od(s["psi"]), ev(s["out"]), None, st)),
+            ("dirac_" + tag, g, hr.OP_DIRAC, V, 0.0, lambda: hr.hr_dirac_apply(g, m0, s["U"], s["psi"], s["out"], st)),
+            ("dhat_" + tag, g, hr.OP_DHAT, Vh, 0.0, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, m0, s["U"], None, None, ev(s["psi"]), ev(s["out"]), s["tmp"], st)),
         ]
-        if tag == "f64":
-            ops += [
-                ("clover_" + tag, g, hr.OP_CLOVER, V, lambda: hr.hr_clover_apply(g, hr.BOTH, s["fwd"], s["psi"], s["out"], st)),
-                ("clover_inv_" + tag, g, hr.OP_CLOVER, V, lambda: hr.hr_clover_apply(g, hr.BOTH, s["inv"], s["psi"], s["out"], st)),
-                ("dhat_clover_" + tag, g, hr.OP_DHAT_CLOVER, Vh, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, m0c, s["Uw"], s["fwd"], s["inv"], ev(s["psi"]), ev(s["out"]), s["tmp"], st)),
-                ("represent_" + tag, g, hr.OP_REPRESENT, V, lambda: hr.hr_represent_gauge(g, s["U"], s["Uadj"], st)),
-            ]
-        return ops
 
-    ops = mk("f64") + mk("f32")
+    def clover_group():
+        s = S["f64"]
+        lat, g = s["lat"], s["lat"].g
+        ev = lat.even
+        blk = hr.hr_dirac_flops_bytes(g, hr.OP_CLOVER)[1] - 2 * 128.0        # block bytes per site
+        return [
+            ("clover_f64", g, hr.OP_CLOVER, V, 0.0, lambda: hr.hr_clover_apply(g, hr.BOTH, s["fwd"], s["psi"], s["out"], st)),
+            ("clover_inv_f64", g, hr.OP_CLOVER, V, 0.0, lambda: hr.hr_clover_apply(g, hr.BOTH, s["inv"], s["psi"], s["out"], st)),
+            ("dhat_clover_f64", g, hr.OP_DHAT_CLOVER, Vh, 0.0, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, m0c, s["Uw"], s["fwd"], s["inv"], ev(s["psi"]), ev(s["out"]), s["tmp"], st)),
+            ("dirac_clover_f64", g, hr.OP_DIRAC, V, blk, lambda: hr.hr_dirac_clover_apply(g, s["Uw"], s["fwd"], s["psi"], s["out"], st)),
+            ("represent_f64", g, hr.OP_REPRESENT, V, 0.0, lambda: hr.hr_represent_gauge(g, s["U"], s["Uadj"], st)),
+        ]
+
+    groups = {"f64": dslash_group("f64"), "f32": dslash_group("f32"), "clover": clover_group()}
     model = {}
-    for name, g, op, sites, _ in ops:
-        f, bc, br = hr.hr_dirac_flops_bytes(g, op)
-        model[name] = {"sites": sites, "flops": f * sites, "bytes": bc * sites, "bytes_requested": br * sites}
-    step_bytes = sum(m["bytes"] for m in model.values())
-    step_flops = sum(m["flops"] for m in model.values())
-    step_sites = sum(m["sites"] for m in model.values())
+    for ops in groups.values():
+        for name, g, op, sites, extra, _ in ops:
+            f, bc, br = hr.hr_dirac_flops_bytes(g, op)
+            if name == "dirac_clover_f64":
+                f += hr.hr_dirac_flops_bytes(g, hr.OP_CLOVER)[0] - 3 * 16.0      # A psi replaces the (4+m0) psi axpy
+            model[name] = {"sites": sites, "flops": f * sites, "bytes": (bc + extra) * sites, "bytes_requested": (br + extra) * sites}
 
-    def step(events=None):
-        for i, (name, g, op, sites, fn) in enumerate(ops):
+    def totals(ops):
+        return tuple(sum(model[o[0]][k] for o in ops) for k in ("bytes", "flops", "sites"))
+
+    def step(ops, events=None):
+        for i, o in enumerate(ops):
             if events is not None:
                 events[i][0].record()
-            fn()
+            o[5]()
             if events is not None:
                 events[i][1].record()
 
-    for _ in range(max(3, args.warmup)):
-        step()
+    def timed_group(ops, K, count_launches=False):
+        """K steps of one group between a barrier + synchronize on both sides; per-launch event pairs inside"""
+        evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in ops] for _ in range(K)]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(dev_index) if count_launches else None
+        n0 = hr.hr_launch_count()
+        ranks.barrier()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.start()
+        e0.record()
+        for k in range(K):
+            step(ops, evs[k])
+        e1.record()
+        torch.cuda.synchronize()
+        ranks.barrier()
+        clocks = sampler.finish() if sampler else None
+        launches = hr.hr_launch_count() - n0
+        per_op = [sum(evs[k][i][0].elapsed_time(evs[k][i][1]) for k in range(K)) / K for i in range(len(ops))]
+        return e0.elapsed_time(e1) * 1e-3, per_op, launches, clocks
+
+    W, K = max(3, args.warmup), args.steps
+    for _ in range(W):
+        for ops in groups.values():
+            step(ops)
+    for _ in range(W):       # the headline group is warmed up last, so the timed region starts from its own steady state
+        step(groups["f64"])
     torch.cuda.synchronize()
 
-    K = args.steps
-    per_op_events = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in ops] for _ in range(K)]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(dev_index)
-    launches0 = hr.hr_launch_count()
-    ranks.barrier()
-    torch.cuda.synchronize()
-    sampler.start()
-    e0.record()
-    for k in range(K):
-        step(per_op_events[k])
-    e1.record()
-    torch.cuda.synchronize()
-    ranks.barrier()
-    clocks = sampler.finish()
-    launches = hr.hr_launch_count() - launches0
-    seconds = e0.elapsed_time(e1) * 1e-3
+    seconds, ms64, launches, clocks = timed_group(groups["f64"], K, count_launches=True)
+    step_bytes, step_flops, step_sites = totals(groups["f64"])
     value, tmax = whole_job_throughput(ranks, step_bytes * K / 1e9, seconds)
     ms_per_step = tmax * 1e3 / K
+    side = {}
+    op_ms = dict(zip([o[0] for o in groups["f64"]], ms64))
+    for key in ("f32", "clover"):
+        sec, ms, _, _ = timed_group(groups[key], K)
+        by, fl, si = totals(groups[key])
+        side[key] = {"value": round(by * K / sec / 1e9, 1), "unit": UNIT, "ms_per_step": round(sec * 1e3 / K, 4),
+                     "gflops": round(fl * K / sec / 1e9, 1), "gsites_per_s": round(si * K / sec / 1e9, 3), "ops": [o[0] for o in groups[key]]}
+        op_ms.update(zip([o[0] for o in groups[key]], ms))
 
-    op_report = {}
-    for i, (name, g, op, sites, _) in enumerate(ops):
-        ms = sum(per_op_events[k][i][0].elapsed_time(per_op_events[k][i][1]) for k in range(K)) / K
-        m = model[name]
-        op_report[name] = {
-            "ms": round(ms, 4), "gbs": round(m["bytes"] / ms / 1e6, 1), "gbs_requested": round(m["bytes_requested"] / ms / 1e6, 1),
-            "gflops": round(m["flops"] / ms / 1e6, 1), "gsites_per_s": round(m["sites"] / ms / 1e6, 3),
-            "kernel": hr.hr_kernel_name(g) if "clover_" not in name[:7] and "represent" not in name else "site-diagonal",
-        }
-
-    # ---- roofline of the dominant kernel: the fp64 parity hop (2 launches per step as H1, same kernel inside E1/E2)
+    # ---- per-operator report and roofline (HBM-bound: DESIGN.md §5); DRAM traffic per launch from the committed ncu captures
     peak, peak_src = peaks()
-    hop_ms = 0.5 * (op_report["hop_oe_f64"]["ms"] + op_report["hop_eo_f64"]["ms"])
-    hop_bytes = model["hop_oe_f64"]["bytes"]
-    achieved = hop_bytes / hop_ms / 1e6
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "hop_f64_traffic.json")
+    traffic_db = {}
+    tp = os.path.join(ROOT, "profiles", "kernel_traffic.json")
     if os.path.exists(tp):
         try:
             with open(tp) as f:
-                traffic = json.load(f).get(hr.hr_kernel_name(S["f64"]["lat"].g))
+                traffic_db = json.load(f)
         except Exception:
-            traffic = None
-    roofline = {"bound": "hbm", "kernel": "parity hop fp64 (%s)" % hr.hr_kernel_name(S["f64"]["lat"].g), "achieved": round(achieved, 1),
-                "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
-                "frac_of_datasheet_8000": round(achieved / 8000.0, 4), "bytes_per_launch": hop_bytes,
-                "avg_launch_ms": round(hop_ms, 4), "traffic": traffic,
-                "fp32": {"achieved": round(model["hop_oe_f32"]["bytes"] / (0.5 * (op_report["hop_oe_f32"]["ms"] + op_report["hop_eo_f32"]["ms"])) / 1e6, 1)}}
-    roofline["fp32"]["frac"] = round(roofline["fp32"]["achieved"] / peak, 4)
-    # the same kernel timed as 30 back-to-back launches between ONE pair of events (no per-launch event gaps): context for
-    # `achieved`, which is measured inside the step with an event pair around every launch
+            traffic_db = {}
+    kname = hr.hr_kernel_name(S["f64"]["lat"].g)
+    per_op = {}
+    for name, ms in op_ms.items():
+        m = model[name]
+        gbs = m["bytes"] / ms / 1e6
+        tr = traffic_db.get(kname, {}).get(name) if args.L == 48 else None
+        per_op[name] = {"ms": round(ms, 4), "gbs": round(gbs, 1), "frac": round(gbs / peak, 4), "frac_of_8000": round(gbs / 8000.0, 4),
+                        "gflops": round(m["flops"] / ms / 1e6, 1), "gsites_per_s": round(m["sites"] / ms / 1e6, 3),
+                        "bytes_per_launch_set": m["bytes"], "traffic": tr, "traffic_ratio": round(tr / m["bytes"], 4) if tr else None}
+    hop_ms = 0.5 * (op_ms["hop_oe_f64"] + op_ms["hop_eo_f64"])
+    hop_bytes = model["hop_oe_f64"]["bytes"]
+    achieved = hop_bytes / hop_ms / 1e6
+    roofline = {"bound": "hbm", "kernel": "parity hop fp64 (%s): 4 of the 6 launches of the step and %d%% of its time" % (
+                    kname, round(100 * (op_ms["hop_oe_f64"] + op_ms["hop_eo_f64"] + op_ms["dhat_f64"]) / sum(ms64))),
+                "achieved": round(achieved, 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                "frac_of_datasheet_8000": round(achieved / 8000.0, 4), "bytes_per_launch": hop_bytes, "avg_launch_ms": round(hop_ms, 4),
+                "traffic": per_op["hop_oe_f64"]["traffic"], "per_op": per_op, "fp32_step": side["f32"], "clover_step": side["clover"]}
+    # the hop kernels timed as 30 back-to-back launches between ONE pair of events (no per-launch event gaps), each parity on
+    # its own: context for `achieved`, and the check that o<-e and e<-o cost the same when neither follows another operator
     b2b = {}
-    for tag in ("f64", "f32"):
-        fn = [o for o in ops if o[0] == "hop_oe_" + tag][0][4]
+    for name in ("hop_oe_f64", "hop_eo_f64", "dirac_f64", "hop_oe_f32", "hop_eo_f32", "dirac_f32"):
+        fn = [o for ops in groups.values() for o in ops if o[0] == name][0][5]
         for _ in range(3):
             fn()
         t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -258,14 +296,14 @@ def run_ours(args):
         t1.record()
         torch.cuda.synchronize()
         ms = t0.elapsed_time(t1) / 30
-        b2b[tag] = {"avg_launch_ms": round(ms, 4), "achieved": round(model["hop_oe_" + tag]["bytes"] / ms / 1e6, 1),
-                    "frac": round(model["hop_oe_" + tag]["bytes"] / ms / 1e6 / peak, 4)}
+        b2b[name] = {"avg_launch_ms": round(ms, 4), "gbs": round(model[name]["bytes"] / ms / 1e6, 1), "frac": round(model[name]["bytes"] / ms / 1e6 / peak, 4)}
     roofline["back_to_back_30_launches"] = b2b
 
     # ---- end to end through the host-buffer C-ABI entry points (pinned host memory, copies inside the timed region)
     e2e = None
     if not args.no_e2e:
-        e2e = run_e2e(args, ranks, hr, S, psi, L, m0, model)
+        e2e = run_e2e(args, ranks, hr, S, U, psi, L, m0, model)
+    del U
 
     # ---- the parity configs, timed for the record (not part of the step): configs[1] 16^4 Dhat as a CUDA graph of
     # 100 repetitions (launch-bound: the lattice fits L2), configs[2] 24^4 adjoint with stored and on-the-fly links
@@ -283,18 +321,18 @@ def run_ours(args):
         cpu = cpu_baseline(L, m0, seconds_budget=15.0)
 
     if ranks.rank == 0:
+        cfg = workload_config(L)
         line = {
-            "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": ranks.world, "steps": K, "warmup": max(3, args.warmup),
+            "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": ranks.world, "steps": K, "warmup": W,
             "ms_per_step": round(ms_per_step, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64+f32", "data": "synthetic",
-            "config": {"workload": "configs[3]+[4]: %d^4 SU(2) fundamental, Haar links (clover: exp(i 0.3 a.sigma), csw 1.2); "
-                                   "step = hop_oe, hop_eo, D, Dhat (f64 and f32) + clover, clover_inv, Dhat_clover, represent (f64)" % args.L,
-                       "lattice": list(L), "l2_policy": "working set per op (>= 1.3 GB at 48^4) far exceeds the 126 MB L2; no flush needed",
-                       "kernel": hr.hr_kernel_name(S["f64"]["lat"].g), "link_storage": "compressed first row (32 B fp64 / 16 B fp32)",
-                       "parallelism": "replicas x%d (no data-path collective)" % ranks.world},
+            "dtype": "f64", "data": "synthetic", "config": cfg,
+            "impl_detail": {"kernel": kname, "link_storage": "compressed first row (32 B fp64 / 16 B fp32)",
+                            "parallelism": "replicas x%d (no data-path collective)" % ranks.world,
+                            "plan_hop": hr.hr_kernel_plan(S["f64"]["lat"].g, hr.OP_HOP), "plan_dirac": hr.hr_kernel_plan(S["f64"]["lat"].g, hr.OP_DIRAC)},
             "gflops": round(step_flops * K / tmax / 1e9 * ranks.world, 1),
             "gsites_per_s": round(step_sites * K / tmax / 1e9 * ranks.world, 3),
-            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu, "ops": op_report, "other_configs": other,
+            "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+            "fp32": side["f32"], "clover": side["clover"], "other_configs": other,
         }
         print(json.dumps(line))
     ranks.close()
@@ -400,22 +438,6 @@ def cg_report(hr, S, m0):
         out["cg_48^4_" + tag] = {"ms_per_iteration": round(ms, 4), "iterations": it, "relres_after": rel,
                                  "gbs": round(bytes_site * Vh / ms / 1e6, 1), "bytes_per_even_site_per_iteration": bytes_site}
         del ws, x
-    # H3c: the clover-improved full operator in one launch (not part of the step), fp64; bytes = H3 + clover blocks
-    s64 = S["f64"]
-    lat, g = s64["lat"], s64["lat"].g
-    st = hr.stream_ptr()
-    fn = lambda: hr.hr_dirac_clover_apply(g, s64["Uw"], s64["fwd"], s64["psi"], s64["out"], st)
-    for _ in range(3):
-        fn()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(20):
-        fn()
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 20
-    _, bc, _ = hr.hr_dirac_flops_bytes(g, hr.OP_DIRAC)
-    out["dirac_clover_48^4_f64"] = {"ms": round(ms, 4), "gbs": round((bc + 256.0) * lat.V / ms / 1e6, 1), "bytes_per_site": bc + 256.0}
     # time to a 1e-12 solution: plain fp64 CG against fp64 defect correction around fp32 CG (hr_cg_solve_mixed)
     s64, s32 = S["f64"], S["f32"]
     lat, g = s64["lat"], s64["lat"].g
@@ -436,128 +458,168 @@ def cg_report(hr, S, m0):
     return out
 
 
-def run_e2e(args, ranks, hr, S, psi, L, m0, model):
-    """same metric through hr_dirac_apply_host / hr_dirac_eo_apply_host: canonical fields in pinned host memory,
-    H2D + pack + operator + unpack + D2H inside the timed region, every step."""
-    import numpy as np
+def run_e2e(args, ranks, hr, S, U, psi, L, m0, model):
+    """the headline metric end to end through the host-buffer C-ABI: canonical fp64 fields in pinned host memory; every
+    step uploads its inputs and downloads its results inside the timed region.  Two readings:
+      gauge resident (the headline e2e value): hr_gauge_upload_host once (untimed: the gauge field changes once per
+        molecular-dynamics step), then per step hr_apply_host_batch of NRHS right-hand sides for each of the
+        step's operators (hop o<-e, hop e<-o, D, Dhat) — H2D, pack, operator, unpack, D2H pipelined over three streams;
+      gauge included: hr_dirac_apply_host + hr_dirac_eo_apply_host, which also upload the links on every call."""
     import torch
-    from paper_2411_18511_b200 import inputs
-    steps = max(1, min(args.steps, 3))
-    total_s, total_bytes, h2d, d2h = 0.0, 0.0, 0, 0
-    names = []
-    U = inputs.haar_gauge(L, 1)
-    for tag in ("f64", "f32"):
-        lat = S[tag]["lat"]
-        g = lat.g
-        ws = hr.device_buffer(hr.hr_host_workspace_bytes(g), lat.device)
-        Uh = torch.from_numpy(U.astype(lat.cplx)).pin_memory()
-        ph = torch.from_numpy(psi.astype(lat.cplx)).pin_memory()
-        oh = torch.empty_like(ph).pin_memory()
-        st = hr.stream_ptr()
-        calls = [("dirac_" + tag, lambda: hr.hr_dirac_apply_host(g, m0, Uh, ph, oh, ws, st)),
-                 ("dhat_" + tag, lambda: hr.hr_dirac_eo_apply_host(g, hr.EO_DHAT, m0, Uh, ph, oh, ws, st))]
-        for _, fn in calls:
-            fn()  # warm-up (page-locks, first-touch)
-        ranks.barrier()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(steps):
-            for _, fn in calls:
-                fn()  # each call synchronises its stream before returning
-        torch.cuda.synchronize()
-        total_s += time.perf_counter() - t0
-        ranks.barrier()
-        for name, _ in calls:
-            total_bytes += model[name]["bytes"]
-            names.append(name)
-        h2d += len(calls) * (Uh.numel() * Uh.element_size() + ph.numel() * ph.element_size())
-        d2h += len(calls) * (oh.numel() * oh.element_size())
-        del ws, Uh, ph, oh
     from paper_2411_18511_b200.dist import whole_job_throughput
-    value, tmax = whole_job_throughput(ranks, total_bytes * steps / 1e9, total_s)
+    steps = max(1, min(args.steps, 3))
+    nrhs = 4
+    lat = S["f64"]["lat"]
+    g, st = lat.g, hr.stream_ptr()
+    Uh = torch.from_numpy(U.astype(lat.cplx)).pin_memory()
+    ins = [torch.from_numpy(psi.astype(lat.cplx)).pin_memory()]
+    for i in range(1, nrhs):
+        ins.append(torch.roll(ins[0], i, 0).contiguous().pin_memory())
+    outs = [torch.empty_like(a).pin_memory() for a in ins]
+    nbytes = ins[0].numel() * ins[0].element_size()
+    # ---- gauge resident
+    u_dev = lat.empty_gauge(hr.REP_FUND)
+    ws = hr.device_buffer(max(hr.hr_host_batch_workspace_bytes(g), hr.hr_canonical_gauge_bytes(g, hr.REP_FUND)), lat.device)
+    hr.hr_gauge_upload_host(g, hr.REP_FUND, Uh, u_dev, ws, st)
+    calls = [("hop_oe_f64", hr.EO_HOP_OE), ("hop_eo_f64", hr.EO_HOP_EO), ("dirac_f64", hr.HOST_DIRAC), ("dhat_f64", hr.EO_DHAT)]
+
+    def resident_step():
+        for _, op in calls:
+            hr.hr_apply_host_batch(g, op, m0, u_dev, None, None, ins, outs, ws, st)
+
+    resident_step()   # warm-up (page-locks, first-touch, stream creation)
+    ranks.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        resident_step()
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    ranks.barrier()
+    by = sum(model[name]["bytes"] for name, _ in calls) * nrhs
+    value, tmax = whole_job_throughput(ranks, by * steps / 1e9, sec)
+    h2d = d2h = len(calls) * nrhs * nbytes
+    del u_dev, ws
+    # ---- gauge included (the round-1 path), one right-hand side per call
+    ws = hr.device_buffer(hr.hr_host_workspace_bytes(g), lat.device)
+    old = [("dirac_f64", lambda: hr.hr_dirac_apply_host(g, m0, Uh, ins[0], outs[0], ws, st)),
+           ("dhat_f64", lambda: hr.hr_dirac_eo_apply_host(g, hr.EO_DHAT, m0, Uh, ins[0], outs[0], ws, st))]
+    for _, fn in old:
+        fn()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _, fn in old:
+        fn()
+    torch.cuda.synchronize()
+    sec_old = time.perf_counter() - t0
+    by_old = sum(model[name]["bytes"] for name, _ in old)
+    gauge_bytes = Uh.numel() * Uh.element_size()
+    del ws
     return {"value": round(value, 2), "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-            "steps": steps, "ms_per_step": round(tmax * 1e3 / steps, 2), "ops": names,
-            "note": "host canonical arrays -> H2D -> pack -> operator -> unpack -> D2H per call; bytes = same compulsory model"}
+            "steps": steps, "ms_per_step": round(tmax * 1e3 / steps, 2), "ops": [n for n, _ in calls], "nrhs_per_op": nrhs,
+            "pcie_gbs_each_direction": round(h2d * steps / tmax / 1e9, 1),
+            "gauge_included": {"value": round(by_old / sec_old / 1e9, 2), "unit": UNIT, "ops": [n for n, _ in old],
+                               "h2d_bytes": int(len(old) * (gauge_bytes + nbytes)), "d2h_bytes": int(len(old) * nbytes), "ms": round(sec_old * 1e3, 2)},
+            "note": "gauge resident on the device (uploaded once per gauge update), 4 right-hand sides per operator pipelined "
+                    "H2D | pack+operator+unpack | D2H; GB/s by the same compulsory byte model as `value`; PCIe-bound by construction"}
 
 
 # ------------------------------------------------------------------------------------------ oracle timing
-def oracle_sample(L, m0, nthreads, nsites):
-    """time the oracle, as it stands, on a contiguous slab of `nsites` output sites of the 48^4 full-D workload"""
-    import numpy as np
-    import oracle
-    from paper_2411_18511_b200 import inputs
-    U = inputs.haar_gauge(L, 1)
-    psi = inputs.gaussian_spinor(L, 2, 2)
-    out = np.zeros_like(psi)
-    oracle.lib()
-    V = inputs.volume(L)
-    nsites = min(nsites, V)
-    oracle.dirac(L, 0, m0, U, psi, 0, min(4096, V), nthreads, out)  # touch
-    return oracle, U, psi, out, nsites
+class OracleStep:
+    """the headline step (hop o<-e, hop e<-o, full D, Dhat; fp64) on the oracle as it stands, on the first `nplanes` x0-planes
+    of the lattice (all of it when nplanes == L0).  On a slab, Dhat is composed from the oracle's own hop: H_oe on the slab and
+    its two neighbour planes, H_eo on the slab, then (4+m0) psi_e - H_eo H_oe psi_e / (4 (4+m0))."""
+
+    def __init__(self, L, m0):
+        import numpy as np
+        import oracle
+        from paper_2411_18511_b200 import inputs
+        self.np, self.orc, self.L, self.m0 = np, oracle, L, m0
+        self.V = inputs.volume(L)
+        self.s0 = self.V // L[0]
+        self.U = inputs.haar_gauge(L, 1)
+        self.psi = inputs.gaussian_spinor(L, 2, 2)
+        self.even = (inputs.site_parity(L) == 0)[:, None, None]
+        self.psi_e = np.where(self.even, self.psi, 0.0)
+        self.out = np.zeros_like(self.psi)
+        self.t = np.zeros_like(self.psi)
+        oracle.lib()
+        self.cores = oracle.available_cores()
+        oracle.dirac(L, 0, m0, self.U, self.psi, 0, min(4096, self.V), self.cores, self.out)  # touch
+
+    def bytes(self, nplanes):
+        n = nplanes * self.s0
+        return n / 2 * (GROUP_BYTES["hop_oe"] + GROUP_BYTES["hop_eo"] + GROUP_BYTES["dhat"]) + n * GROUP_BYTES["dirac"]
+
+    def run(self, nplanes, threads):
+        o, L, m0, d = self.orc, self.L, self.m0, 4.0 + self.m0
+        n = nplanes * self.s0
+        o.hop(L, 0, 1, self.U, self.psi, 0, n, threads, self.out)
+        o.hop(L, 0, 0, self.U, self.psi, 0, n, threads, self.out)
+        o.dirac(L, 0, m0, self.U, self.psi, 0, n, threads, self.out)
+        if nplanes == L[0]:
+            o.dirac_eo(L, 0, m0, self.U, self.psi, threads)
+        else:
+            o.hop(L, 0, 1, self.U, self.psi_e, 0, min(self.V, n + self.s0), threads, self.t)
+            o.hop(L, 0, 1, self.U, self.psi_e, self.V - self.s0, self.V, threads, self.t)
+            o.hop(L, 0, 0, self.U, self.t, 0, n, threads, self.out)
+            self.out[:n] = self.np.where(self.even[:n], d * self.psi_e[:n] - self.out[:n] / (4.0 * d), 0.0)
+
+    def planes_for(self, seconds, threads):
+        """how many x0-planes one step may cover to take about `seconds` (calibrated on one plane)"""
+        t = time.perf_counter()
+        self.run(1, threads)
+        dt = max(time.perf_counter() - t, 1e-6)
+        return int(max(1, min(self.L[0], seconds / dt)))
 
 
 def cpu_baseline(L, m0, seconds_budget=15.0):
-    import oracle
-    cores = oracle.available_cores()
-    orc, U, psi, out, _ = oracle_sample(L, m0, cores, 0)
-    V = 1
-    for v in L:
-        V *= v
-    # calibrate on 1/64 of the lattice, then size the sample to the budget
-    n0 = max(4096, V // 64)
-    t = time.perf_counter()
-    orc.dirac(L, 0, m0, U, psi, 0, n0, cores, out)
-    dt = time.perf_counter() - t
-    n = int(min(V, max(n0, n0 * seconds_budget * 0.5 / max(dt, 1e-6))))
-    # about two thirds of the budget on all cores (repeated passes over the slab if one pass is short), the rest on one thread
-    passes = max(1, int(seconds_budget * 0.66 / max(dt * n / n0, 1e-6)))
+    w = OracleStep(L, m0)
+    cores = w.cores
+    npl = w.planes_for(seconds_budget * 0.6 / 2, cores)        # two passes on all cores
+    passes = 2
     t = time.perf_counter()
     for _ in range(passes):
-        orc.dirac(L, 0, m0, U, psi, 0, n, cores, out)
+        w.run(npl, cores)
     dt_all = (time.perf_counter() - t) / passes
-    n1 = int(min(V, max(4096, n0 * seconds_budget * 0.33 / max(dt * cores, 1e-6))))
+    npl1 = w.planes_for(seconds_budget * 0.3, 1)
     t = time.perf_counter()
-    orc.dirac(L, 0, m0, U, psi, 0, n1, 1, out)
+    w.run(npl1, 1)
     dt_one = time.perf_counter() - t
-    bytes_per_site = 384.0  # same compulsory model as the GPU's fused full D, fp64, compressed links
-    return {"value": round(n / dt_all * bytes_per_site / 1e9, 3), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "oracle full D (fp64) on the first %d of %d sites of the %d^4 workload, %d passes on %d threads (%.1f s) and %d sites on 1 thread (%.1f s); GB/s by the GPU's byte model (384 B/site)" % (n, V, L[0], passes, cores, dt_all * passes, n1, dt_one),
-            "msites_per_s": round(n / dt_all / 1e6, 3), "single_thread_msites_per_s": round(n1 / dt_one / 1e6, 3),
+    return {"value": round(w.bytes(npl) / dt_all / 1e9, 3), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "the step's four operators (hop o<-e, hop e<-o, D, Dhat; fp64) by the oracle on the first %d of %d x0-planes of the %d^4 "
+                      "workload, %d passes on %d threads (%.1f s per pass), and on %d plane(s) on 1 thread (%.1f s); GB/s by the same byte "
+                      "model as `value`" % (npl, L[0], L[0], passes, cores, dt_all, npl1, dt_one),
+            "single_thread_value": round(w.bytes(npl1) / dt_one / 1e9, 3),
             "label": "unoptimised CPU oracle, reported baseline, not a tuned CPU Dslash"}
 
 
 def run_reference(args):
-    """--impl reference: the oracle as it stands on the host cores; each step = full D on a bounded slab."""
+    """--impl reference: the oracle as it stands on the host cores, same step (hop o<-e, hop e<-o, D, Dhat; fp64), same config,
+    metric and unit as our arm; each step covers a bounded number of x0-planes so that the run ends within a few minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import oracle
     L = (args.L,) * 4
     m0 = -0.2
-    cores = oracle.available_cores()
-    V = args.L ** 4
-    orc, U, psi, out, _ = oracle_sample(L, m0, cores, 0)
-    n0 = max(4096, V // 256)
-    t = time.perf_counter()
-    orc.dirac(L, 0, m0, U, psi, 0, n0, cores, out)
-    dt = time.perf_counter() - t
-    total_steps = args.steps + max(3, args.warmup)
-    n = int(min(V, max(n0, n0 * (60.0 / total_steps) / max(dt, 1e-6))))   # whole run ~ 1 minute
-    for _ in range(max(3, args.warmup)):
-        orc.dirac(L, 0, m0, U, psi, 0, n, cores, out)
+    w = OracleStep(L, m0)
+    W = max(3, args.warmup)
+    npl = w.planes_for(90.0 / (args.steps + W), w.cores)     # whole run ~ 1.5 minutes at most
+    for _ in range(W):
+        w.run(npl, w.cores)
     t = time.perf_counter()
     for _ in range(args.steps):
-        orc.dirac(L, 0, m0, U, psi, 0, n, cores, out)
+        w.run(npl, w.cores)
     dt = time.perf_counter() - t
-    value = n * args.steps / dt * 384.0 / 1e9
-    sample = "oracle full D (fp64) on the first %d of %d sites of %d^4 per step, %d threads; GB/s by the 384 B/site compulsory model" % (n, V, args.L, cores)
+    value = w.bytes(npl) * args.steps / dt / 1e9
+    sample = "the step's four operators by the oracle on the first %d of %d x0-planes of %d^4 per step, %d threads; GB/s by the same byte model" % (
+        npl, L[0], args.L, w.cores)
     line = {
         "impl": "reference", "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": max(3, args.warmup), "ms_per_step": round(dt * 1e3 / args.steps, 3), "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "configs[3]: %d^4 SU(2) fundamental, Haar links; oracle (CPU) full D on a slab per step" % args.L,
-                   "lattice": list(L), "parallelism": "host threads x%d" % cores},
-        "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "warmup": W, "ms_per_step": round(dt * 1e3 / args.steps, 3), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(L),
+        "impl_detail": {"parallelism": "host threads x%d" % w.cores, "planes_per_step": npl},
+        "cpu_baseline": {"value": round(value, 3), "unit": UNIT, "cores": w.cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": round(value, 3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }

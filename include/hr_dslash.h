@@ -136,6 +136,12 @@ int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_f
  * `parity` (HR_EVEN, HR_ODD: in/out are half fields; HR_BOTH: full fields).  `blocks` is the full-lattice
  * block field (forward blocks: C2; inverse blocks: C3 — same kernel).  Both representations. */
 int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream);
+/* Number of non-finite reals in a block field (forward or inverse), written as one unsigned 64-bit integer to
+ * count_dev (device memory, 8-byte aligned, caller-owned; read it after synchronising the stream).  The inverse blocks
+ * are made by Gauss-Jordan elimination with partial pivoting in double precision: accurate whenever A(x) is
+ * invertible (it is positive definite for |csw F| < 4+m0, the regime of BASELINE.json configs[4]); an exactly
+ * singular A(x) gives inf / nan entries, which this call counts — 0 means every block is usable. */
+int hr_clover_count_nonfinite(const hr_geom* g, const void* blocks, void* count_dev, void* stream);
 
 /* M1 ("measured in terms of memory bandwidth"): the work model, per OUTPUT site of `op`,
  * for the storage described by g.  bytes_compulsory: every distinct datum crosses DRAM once per kernel;
@@ -198,6 +204,28 @@ int hr_dirac_apply_host(const hr_geom* g, double m0, const void* u_canon_host, c
                         void* out_canon_host, void* workspace, void* stream);
 int hr_dirac_eo_apply_host(const hr_geom* g, int op, double m0, const void* u_canon_host,
                            const void* in_canon_host, void* out_canon_host, void* workspace, void* stream);
+
+/* ---- host path with the gauge field resident on the device ----
+ * The gauge field changes once per molecular-dynamics step and the operator is applied many times in between
+ * (PAPER.md:53-59): upload the links once, then stream right-hand sides through.
+ *   hr_gauge_upload_host : canonical host links (rep = HR_REP_FUND: [lex][mu][2][2][re,im]; HR_REP_ADJ: [lex][mu][3][3])
+ *                          -> device layout in u_dev (hr_gauge_bytes(g, rep)); workspace = hr_canonical_gauge_bytes(g, rep)
+ *                          device bytes.  Synchronises `stream` before returning.
+ *   hr_apply_host_batch  : out_i = Op in_i for i = 0 .. nrhs-1, canonical full-lattice arrays in host memory (pinned
+ *                          memory for full PCIe speed; the two pointer arrays live in host memory).  op = HR_EO_HOP_OE,
+ *                          HR_EO_HOP_EO, HR_EO_DHAT (as hr_dirac_eo_apply_host: entries of the other parity are not
+ *                          read and come back as zeros; with clover_fwd and clover_inv the clover-improved operator E2)
+ *                          or HR_HOST_DIRAC (full D; with clover_fwd the clover-improved D_sw; clover_inv must be NULL).
+ *                          Three-stage pipeline over two library-owned copy streams (created per device on first use
+ *                          and kept for the life of the process — the one place this library allocates anything) and
+ *                          the caller's stream: upload of spinor i+1, pack + operator + unpack of spinor i and download
+ *                          of result i-1 overlap, so both PCIe directions are busy.  workspace =
+ *                          hr_host_batch_workspace_bytes(g) device bytes.  Returns after the last result has arrived. */
+enum { HR_HOST_DIRAC = 3 };
+int hr_gauge_upload_host(const hr_geom* g, int rep, const void* u_canon_host, void* u_dev, void* workspace, void* stream);
+size_t hr_host_batch_workspace_bytes(const hr_geom* g);
+int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
+                        int nrhs, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream);
 
 /* ---- diagnostics ---- */
 size_t hr_last_error(char* buf, size_t len);   /* copies the last error text (NUL-terminated); returns its length */

@@ -17,6 +17,7 @@ int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStr
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_apply(const Geo& g, int rep, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
+int run_count_nonfinite(int prec, const void* x, size_t bytes, unsigned long long* count_dev, cudaStream_t st);
 
 // hr_solver.cu
 size_t cg_workspace_bytes(const hr_geom* g);
@@ -270,6 +271,12 @@ int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void
     if (parity < HR_EVEN || parity > HR_BOTH) { set_error("hr_clover_apply: parity %d", parity); return HR_EINVAL; }
     HR_TRY(check_ptr(blocks, "blocks")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
     return run_clover_apply(make_geo(g), g->rep, g->prec, parity, blocks, in, out, (cudaStream_t)stream);
+}
+
+int hr_clover_count_nonfinite(const hr_geom* g, const void* blocks, void* count_dev, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(blocks, "blocks"));
+    if (!count_dev || (reinterpret_cast<uintptr_t>(count_dev) & 7)) { set_error("hr_clover_count_nonfinite: count_dev must be an 8-byte aligned device pointer"); return HR_EINVAL; }
+    return run_count_nonfinite(g->prec, blocks, hr_clover_bytes(g), reinterpret_cast<unsigned long long*>(count_dev), (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------- S1

@@ -207,78 +207,94 @@ struct dcplx {
 __device__ __forceinline__ dcplx dmul(dcplx a, dcplx b) { dcplx r; r.re = a.re * b.re - a.im * b.im; r.im = a.re * b.im + a.im * b.re; return r; }
 __device__ __forceinline__ dcplx dsub(dcplx a, dcplx b) { dcplx r; r.re = a.re - b.re; r.im = a.im - b.im; return r; }
 
-// in-place inverse of a hermitian positive-definite 4x4 (Gauss-Jordan, no pivoting: the diagonal of a
-// positive-definite matrix stays positive under elimination)
-__device__ void invert4(dcplx A[4][4]) {
-    dcplx B[4][4];
-    for (int i = 0; i < 4; ++i)
-        for (int j = 0; j < 4; ++j) { B[i][j].re = (i == j) ? 1.0 : 0.0; B[i][j].im = 0.0; }
-    for (int k = 0; k < 4; ++k) {
-        const double n2 = A[k][k].re * A[k][k].re + A[k][k].im * A[k][k].im;
-        dcplx inv;
-        inv.re = A[k][k].re / n2;
-        inv.im = -A[k][k].im / n2;
-        for (int j = 0; j < 4; ++j) { A[k][j] = dmul(A[k][j], inv); B[k][j] = dmul(B[k][j], inv); }
-        for (int i = 0; i < 4; ++i) {
-            if (i == k) continue;
-            const dcplx f = A[i][k];
-            for (int j = 0; j < 4; ++j) { A[i][j] = dsub(A[i][j], dmul(f, A[k][j])); B[i][j] = dsub(B[i][j], dmul(f, B[k][j])); }
-        }
-    }
-    for (int i = 0; i < 4; ++i)
-        for (int j = 0; j < 4; ++j) A[i][j] = B[i][j];
-}
-
 __device__ __forceinline__ dcplx dadd(dcplx a, dcplx b) { dcplx r; r.re = a.re + b.re; r.im = a.im + b.im; return r; }
-__device__ void matmul4(dcplx C[4][4], const dcplx A[4][4], const dcplx B[4][4]) {
-    for (int i = 0; i < 4; ++i)
-        for (int j = 0; j < 4; ++j) {
+
+// ---- small dense helpers for D x D complex matrices (D = 4: fundamental chirality blocks, D = 6: adjoint ones).
+// Setup-time code (once per gauge update): clarity over speed, double precision throughout.
+template <int D>
+__device__ void matmul_d(dcplx (*C)[D], const dcplx (*A)[D], const dcplx (*B)[D]) {
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) {
             dcplx a = {0.0, 0.0};
-            for (int k = 0; k < 4; ++k) a = dadd(a, dmul(A[i][k], B[k][j]));
+            for (int k = 0; k < D; ++k) a = dadd(a, dmul(A[i][k], B[k][j]));
             C[i][j] = a;
         }
 }
-// E = exp(X) for a 4x4 complex matrix: scaling and squaring with an order-16 Taylor polynomial
-// (|X / 2^s|_inf <= 1/2, truncation < 0.5^17 / 17! ~ 2e-20).  Setup-time code: clarity over speed.
-__device__ void expm4(dcplx E[4][4], const dcplx X[4][4]) {
+// in-place inverse by Gauss-Jordan elimination with partial pivoting (row exchanges on [A | 1]).  The clover blocks
+// are positive definite for the parameters of interest (eigenvalues (4+m0) +- O(csw |F|)), where no exchange happens;
+// pivoting keeps the result finite and accurate for indefinite blocks too (small 4+m0, large csw, rough links).  An
+// exactly singular block yields non-finite entries, which hr_clover_count_nonfinite reports.
+template <int D>
+__device__ void invert_d(dcplx (*A)[D]) {
+    dcplx B[D][D];
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) { B[i][j].re = (i == j) ? 1.0 : 0.0; B[i][j].im = 0.0; }
+    for (int k = 0; k < D; ++k) {
+        int r = k;
+        double best = A[k][k].re * A[k][k].re + A[k][k].im * A[k][k].im;
+        for (int i = k + 1; i < D; ++i) {
+            const double n2 = A[i][k].re * A[i][k].re + A[i][k].im * A[i][k].im;
+            if (n2 > best) { best = n2; r = i; }
+        }
+        if (r != k)
+            for (int j = 0; j < D; ++j) {
+                const dcplx ta = A[k][j]; A[k][j] = A[r][j]; A[r][j] = ta;
+                const dcplx tb = B[k][j]; B[k][j] = B[r][j]; B[r][j] = tb;
+            }
+        dcplx inv;
+        inv.re = A[k][k].re / best;
+        inv.im = -A[k][k].im / best;
+        for (int j = 0; j < D; ++j) { A[k][j] = dmul(A[k][j], inv); B[k][j] = dmul(B[k][j], inv); }
+        for (int i = 0; i < D; ++i) {
+            if (i == k) continue;
+            const dcplx f = A[i][k];
+            for (int j = 0; j < D; ++j) { A[i][j] = dsub(A[i][j], dmul(f, A[k][j])); B[i][j] = dsub(B[i][j], dmul(f, B[k][j])); }
+        }
+    }
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) A[i][j] = B[i][j];
+}
+// E = exp(X): scaling and squaring with an order-16 Taylor polynomial (|X / 2^s|_inf <= 1/2, truncation
+// < 0.5^17 / 17! ~ 2e-20)
+template <int D>
+__device__ void expm_d(dcplx (*E)[D], const dcplx (*X)[D]) {
     double nrm = 0.0;
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < D; ++i) {
         double r = 0.0;
-        for (int j = 0; j < 4; ++j) r += fabs(X[i][j].re) + fabs(X[i][j].im);
+        for (int j = 0; j < D; ++j) r += fabs(X[i][j].re) + fabs(X[i][j].im);
         nrm = fmax(nrm, r);
     }
     int s = 0;
     double scale = 1.0;
     while (nrm * scale > 0.5 && s < 60) { scale *= 0.5; ++s; }
-    dcplx Y[4][4], P[4][4], Tm[4][4];
-    for (int i = 0; i < 4; ++i)
-        for (int j = 0; j < 4; ++j) {
+    dcplx Y[D][D], P[D][D], Tm[D][D];
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) {
             Y[i][j].re = X[i][j].re * scale; Y[i][j].im = X[i][j].im * scale;
             P[i][j] = Y[i][j];                                   // current term Y^k / k!
             E[i][j].re = (i == j ? 1.0 : 0.0) + Y[i][j].re; E[i][j].im = Y[i][j].im;
         }
     for (int k = 2; k <= 16; ++k) {
-        matmul4(Tm, P, Y);
-        for (int i = 0; i < 4; ++i)
-            for (int j = 0; j < 4; ++j) {
+        matmul_d<D>(Tm, P, Y);
+        for (int i = 0; i < D; ++i)
+            for (int j = 0; j < D; ++j) {
                 P[i][j].re = Tm[i][j].re / k; P[i][j].im = Tm[i][j].im / k;
                 E[i][j] = dadd(E[i][j], P[i][j]);
             }
     }
     for (int q = 0; q < s; ++q) {
-        matmul4(Tm, E, E);
-        for (int i = 0; i < 4; ++i)
-            for (int j = 0; j < 4; ++j) E[i][j] = Tm[i][j];
+        matmul_d<D>(Tm, E, E);
+        for (int i = 0; i < D; ++i)
+            for (int j = 0; j < D; ++j) E[i][j] = Tm[i][j];
     }
 }
-
-// hermitian 4x4 -> 16 reals (diagonal, then lower entries column-major), hermitian part taken
-template <typename T>
-__device__ void herm_to_reals(T* out, dcplx A[4][4]) {
-    for (int i = 0; i < 4; ++i) out[i] = (T)A[i][i].re;
-    int k = 4;
-    for (int j = 0; j < 4; ++j)
-        for (int i = j + 1; i < 4; ++i) {
+// hermitian D x D -> D*D reals (diagonal, then the strictly-lower entries column by column), hermitian part taken
+template <typename T, int D>
+__device__ void herm_to_reals_d(T* out, dcplx (*A)[D]) {
+    for (int i = 0; i < D; ++i) out[i] = (T)A[i][i].re;
+    int k = D;
+    for (int j = 0; j < D; ++j)
+        for (int i = j + 1; i < D; ++i) {
             out[k++] = (T)(0.5 * (A[i][j].re + A[j][i].re));
             out[k++] = (T)(0.5 * (A[i][j].im - A[j][i].im));
         }
@@ -345,18 +361,18 @@ __global__ void clover_build_kernel(Geo g, double diag, double csw, int expo, co
                     X[i][j].re = (A[i][j].re - (i == j ? diag : 0.0)) / diag;
                     X[i][j].im = A[i][j].im / diag;
                 }
-            expm4(E, X);
+            expm_d<4>(E, X);
             for (int i = 0; i < 4; ++i)
                 for (int j = 0; j < 4; ++j) { A[i][j].re = diag * E[i][j].re; A[i][j].im = diag * E[i][j].im; X[i][j].re = -X[i][j].re; X[i][j].im = -X[i][j].im; }
-            herm_to_reals<T>(reals_f + 16 * chi, A);
-            expm4(E, X);
+            herm_to_reals_d<T, 4>(reals_f + 16 * chi, A);
+            expm_d<4>(E, X);
             for (int i = 0; i < 4; ++i)
                 for (int j = 0; j < 4; ++j) { A[i][j].re = E[i][j].re / diag; A[i][j].im = E[i][j].im / diag; }
-            herm_to_reals<T>(reals_i + 16 * chi, A);
+            herm_to_reals_d<T, 4>(reals_i + 16 * chi, A);
         } else {
-            herm_to_reals<T>(reals_f + 16 * chi, A);
-            invert4(A);
-            herm_to_reals<T>(reals_i + 16 * chi, A);
+            herm_to_reals_d<T, 4>(reals_f + 16 * chi, A);
+            invert_d<4>(A);
+            herm_to_reals_d<T, 4>(reals_i + 16 * chi, A);
         }
     }
     constexpr int CCH = 32 * sizeof(T) / 16;
@@ -369,78 +385,6 @@ __global__ void clover_build_kernel(Geo g, double diag, double csw, int expo, co
     }
 }
 
-// ---- the same for D x D matrices (D = 6: adjoint blocks), generic loops
-template <int D>
-__device__ void matmul_d(dcplx (*C)[D], const dcplx (*A)[D], const dcplx (*B)[D]) {
-    for (int i = 0; i < D; ++i)
-        for (int j = 0; j < D; ++j) {
-            dcplx a = {0.0, 0.0};
-            for (int k = 0; k < D; ++k) a = dadd(a, dmul(A[i][k], B[k][j]));
-            C[i][j] = a;
-        }
-}
-template <int D>
-__device__ void invert_d(dcplx (*A)[D]) {   // hermitian positive definite: Gauss-Jordan without pivoting
-    dcplx B[D][D];
-    for (int i = 0; i < D; ++i)
-        for (int j = 0; j < D; ++j) { B[i][j].re = (i == j) ? 1.0 : 0.0; B[i][j].im = 0.0; }
-    for (int k = 0; k < D; ++k) {
-        const double n2 = A[k][k].re * A[k][k].re + A[k][k].im * A[k][k].im;
-        dcplx inv;
-        inv.re = A[k][k].re / n2;
-        inv.im = -A[k][k].im / n2;
-        for (int j = 0; j < D; ++j) { A[k][j] = dmul(A[k][j], inv); B[k][j] = dmul(B[k][j], inv); }
-        for (int i = 0; i < D; ++i) {
-            if (i == k) continue;
-            const dcplx f = A[i][k];
-            for (int j = 0; j < D; ++j) { A[i][j] = dsub(A[i][j], dmul(f, A[k][j])); B[i][j] = dsub(B[i][j], dmul(f, B[k][j])); }
-        }
-    }
-    for (int i = 0; i < D; ++i)
-        for (int j = 0; j < D; ++j) A[i][j] = B[i][j];
-}
-template <int D>
-__device__ void expm_d(dcplx (*E)[D], const dcplx (*X)[D]) {   // scaling and squaring, order-16 Taylor (as expm4)
-    double nrm = 0.0;
-    for (int i = 0; i < D; ++i) {
-        double r = 0.0;
-        for (int j = 0; j < D; ++j) r += fabs(X[i][j].re) + fabs(X[i][j].im);
-        nrm = fmax(nrm, r);
-    }
-    int s = 0;
-    double scale = 1.0;
-    while (nrm * scale > 0.5 && s < 60) { scale *= 0.5; ++s; }
-    dcplx Y[D][D], P[D][D], Tm[D][D];
-    for (int i = 0; i < D; ++i)
-        for (int j = 0; j < D; ++j) {
-            Y[i][j].re = X[i][j].re * scale; Y[i][j].im = X[i][j].im * scale;
-            P[i][j] = Y[i][j];
-            E[i][j].re = (i == j ? 1.0 : 0.0) + Y[i][j].re; E[i][j].im = Y[i][j].im;
-        }
-    for (int k = 2; k <= 16; ++k) {
-        matmul_d<D>(Tm, P, Y);
-        for (int i = 0; i < D; ++i)
-            for (int j = 0; j < D; ++j) {
-                P[i][j].re = Tm[i][j].re / k; P[i][j].im = Tm[i][j].im / k;
-                E[i][j] = dadd(E[i][j], P[i][j]);
-            }
-    }
-    for (int q = 0; q < s; ++q) {
-        matmul_d<D>(Tm, E, E);
-        for (int i = 0; i < D; ++i)
-            for (int j = 0; j < D; ++j) E[i][j] = Tm[i][j];
-    }
-}
-template <typename T, int D>
-__device__ void herm_to_reals_d(T* out, dcplx (*A)[D]) {
-    for (int i = 0; i < D; ++i) out[i] = (T)A[i][i].re;
-    int k = D;
-    for (int j = 0; j < D; ++j)
-        for (int i = j + 1; i < D; ++i) {
-            out[k++] = (T)(0.5 * (A[i][j].re + A[j][i].re));
-            out[k++] = (T)(0.5 * (A[i][j].im - A[j][i].im));
-        }
-}
 
 // C1 in the adjoint representation (oracle O10): 6 x 6 chirality blocks on (2 spin x 3 colour),
 //   A+- = (4+m0) + (csw/2) [ tau1 (x) i(+-F01 - F23) + tau2 (x) i(+-F02 + F13) + tau3 (x) i(+-F03 - F12) ],
@@ -579,6 +523,26 @@ int run_clover_apply(const Geo& g, int rep, int prec, int parity, const void* bl
     }
     count_launch();
     return check_launch("clover_apply_kernel");
+}
+
+// ---- number of non-finite reals in a block field (a singular block inverts to inf / nan)
+template <typename T>
+__global__ void count_nonfinite_kernel(const T* __restrict__ x, size_t n, unsigned long long* count) {
+    unsigned long long bad = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        if (!isfinite(x[i])) ++bad;
+    if (bad) atomicAdd(count, bad);
+}
+
+int run_count_nonfinite(int prec, const void* x, size_t bytes, unsigned long long* count_dev, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(count_dev, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) { set_error("cudaMemsetAsync: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+    const size_t n = bytes / real_bytes(prec);
+    const int grid = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+    if (prec == HR_PREC_F64) count_nonfinite_kernel<double><<<grid, 256, 0, st>>>(reinterpret_cast<const double*>(x), n, count_dev);
+    else count_nonfinite_kernel<float><<<grid, 256, 0, st>>>(reinterpret_cast<const float*>(x), n, count_dev);
+    count_launch();
+    return check_launch("count_nonfinite_kernel");
 }
 
 }  // namespace hr

@@ -210,9 +210,9 @@ static int cg_run(const hr_geom* g, double m0, const void* u, const void* cf, co
             cudaError_t e = cudaMemcpyAsync(&h, sc, sizeof(h), cudaMemcpyDeviceToHost, st);
             if (e == cudaSuccess) e = cudaStreamSynchronize(st);
             if (e != cudaSuccess) { set_error("hr_cg_solve: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+            if (!(h.rr == h.rr) || !(h.bb == h.bb)) { set_error("hr_cg_solve: residual is NaN at iteration %d", it); return HR_ECUDA; }
             relres = h.bb > 0.0 ? sqrt(h.rr / h.bb) : 0.0;
             if (h.bb == 0.0 || h.rr <= tol * tol * h.bb || it >= max_iter) { done = true; break; }
-            if (!(h.rr == h.rr)) { set_error("hr_cg_solve: residual is NaN at iteration %d", it); return HR_ECUDA; }
         }
         // t = Dhat p ; s = gamma5 t (into w), |t|^2 ; t = Dhat s ; x += alpha p, r -= alpha gamma5 t ; p = r + beta p
         rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u, cf, ci, p, t, tmp, strm);
@@ -330,22 +330,30 @@ int run_cg_mixed(const hr_geom* g, double m0, const void* u64, const void* u32, 
     double bb = -1.0, relres = 1.0;
     int outer = 0, inner_total = 0;
     for (;;) {
-        // r = b - Dhat^dag Dhat x in double (for x = 0 this is r = b, computed the same way for simplicity)
-        int rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, cf64, ci64, x, t, tmp, strm);
-        if (rc != HR_OK) return rc;
-        cg_g5_norm_kernel<double><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, t, w, partial);
-        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, cf64, ci64, w, t, tmp, strm);
-        if (rc != HR_OK) return rc;
-        cg_residual_kernel<<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, (const double2*)b, (const double2*)t, (double2*)r, partial);
+        // r = b - Dhat^dag Dhat x in double; on the first pass x = 0, so r = b and |b|^2 come from the residual kernel
+        // alone (with w = x = 0) and the two fp64 operator applications are skipped
+        int rc = HR_OK;
+        if (bb < 0.0) {
+            cg_residual_kernel<<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, (const double2*)b, (const double2*)x, (double2*)r, partial);
+            count_launch();
+        } else {
+            rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, cf64, ci64, x, t, tmp, strm);
+            if (rc != HR_OK) return rc;
+            cg_g5_norm_kernel<double><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, t, w, partial);
+            rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u64, cf64, ci64, w, t, tmp, strm);
+            if (rc != HR_OK) return rc;
+            cg_residual_kernel<<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, (const double2*)b, (const double2*)t, (double2*)r, partial);
+            count_launch(2);
+        }
         cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_INIT, nblk, partial, sc);
-        count_launch(3);
+        count_launch();
         CgScalars h;
         cudaError_t e = cudaMemcpyAsync(&h, sc, sizeof(h), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) { set_error("hr_cg_solve_mixed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+        if (!(h.rr == h.rr)) { set_error("hr_cg_solve_mixed: residual is NaN after %d outer iterations", outer); return HR_ECUDA; }
         if (bb < 0.0) bb = h.rr;                         // first pass: x = 0, so |r|^2 = |b|^2
         relres = bb > 0.0 ? sqrt(h.rr / bb) : 0.0;
-        if (!(h.rr == h.rr)) { set_error("hr_cg_solve_mixed: residual is NaN after %d outer iterations", outer); return HR_ECUDA; }
         if (bb == 0.0 || relres <= tol || outer >= max_outer) break;
         // inner solve in fp32: Dhat^dag Dhat e = r
         cg_to_f32_kernel<<<nblk32, CG_BLOCK, 0, st>>>(nchunks32, geo.L3h, NCH32, (const double2*)r, (float4*)r32);

@@ -20,6 +20,7 @@ LINKS_FULL, LINKS_COMPRESSED, LINKS_ONTHEFLY = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 EVEN, ODD, BOTH = 0, 1, 2
 EO_HOP_OE, EO_HOP_EO, EO_DHAT = 0, 1, 2
+HOST_DIRAC = 3
 OP_HOP, OP_DIRAC, OP_DHAT, OP_CLOVER, OP_DHAT_CLOVER, OP_REPRESENT = 0, 1, 2, 3, 4, 5
 
 # every symbol include/hr_dslash.h declares (tests/test_abi.py checks the header against this list)
@@ -27,8 +28,9 @@ SYMBOLS = [
     "hr_spinor_bytes", "hr_gauge_bytes", "hr_clover_bytes", "hr_canonical_spinor_bytes",
     "hr_canonical_gauge_bytes", "hr_canonical_clover_bytes", "hr_pack_spinor", "hr_unpack_spinor",
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
-    "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_dirac_flops_bytes",
-    "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_last_error",
+    "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
+    "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_gauge_upload_host",
+    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_kernel_plan", "hr_cg_workspace_bytes", "hr_cg_solve",
     "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed", "hr_cg_solve_mixed_clover",
 ]
@@ -72,10 +74,14 @@ def lib():
             "hr_clover_build": (I, [G, D, D, V, V, V, V]),
             "hr_clover_build_exp": (I, [G, D, D, V, V, V, V]),
             "hr_clover_apply": (I, [G, I, V, V, V, V]),
+            "hr_clover_count_nonfinite": (I, [G, V, V, V]),
             "hr_dirac_flops_bytes": (I, [G, I, PD, PD, PD]),
             "hr_host_workspace_bytes": (S, [G]),
             "hr_dirac_apply_host": (I, [G, D, V, V, V, V, V]),
             "hr_dirac_eo_apply_host": (I, [G, I, D, V, V, V, V, V]),
+            "hr_gauge_upload_host": (I, [G, I, V, V, V, V]),
+            "hr_host_batch_workspace_bytes": (S, [G]),
+            "hr_apply_host_batch": (I, [G, I, D, V, V, V, I, ctypes.POINTER(V), ctypes.POINTER(V), V, V]),
             "hr_last_error": (S, [ctypes.c_char_p, S]),
             "hr_launch_count": (ctypes.c_ulonglong, []),
             "hr_kernel_name": (ctypes.c_char_p, [G]),
@@ -182,6 +188,10 @@ def hr_clover_apply(g, parity, blocks, inp, out, stream=0):
     _check(lib().hr_clover_apply(ctypes.byref(g), int(parity), _ptr(blocks), _ptr(inp), _ptr(out), stream))
 
 
+def hr_clover_count_nonfinite(g, blocks, count_dev, stream=0):
+    _check(lib().hr_clover_count_nonfinite(ctypes.byref(g), _ptr(blocks), _ptr(count_dev), stream))
+
+
 def hr_dirac_flops_bytes(g, op):
     """-> (flops per output site, compulsory bytes per site, requested bytes per site)"""
     f, bc, br = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
@@ -197,6 +207,23 @@ def hr_dirac_apply_host(g, m0, u_canon_host, psi_canon_host, out_canon_host, wor
 def hr_dirac_eo_apply_host(g, op, m0, u_canon_host, in_canon_host, out_canon_host, workspace, stream=0):
     _check(lib().hr_dirac_eo_apply_host(ctypes.byref(g), int(op), float(m0), _ptr(u_canon_host), _ptr(in_canon_host),
                                         _ptr(out_canon_host), _ptr(workspace), stream))
+
+
+def hr_gauge_upload_host(g, rep, u_canon_host, u_dev, workspace, stream=0):
+    _check(lib().hr_gauge_upload_host(ctypes.byref(g), int(rep), _ptr(u_canon_host), _ptr(u_dev), _ptr(workspace), stream))
+
+
+def hr_host_batch_workspace_bytes(g): return lib().hr_host_batch_workspace_bytes(ctypes.byref(g))
+
+
+def hr_apply_host_batch(g, op, m0, u_dev, clover_fwd, clover_inv, ins, outs, workspace, stream=0):
+    """ins / outs: sequences of canonical host arrays (torch pinned tensors or numpy arrays), one per right-hand side"""
+    n = len(ins)
+    assert len(outs) == n
+    pin = (ctypes.c_void_p * n)(*[_ptr(a) for a in ins])
+    pout = (ctypes.c_void_p * n)(*[_ptr(a) for a in outs])
+    _check(lib().hr_apply_host_batch(ctypes.byref(g), int(op), float(m0), _ptr(u_dev), _ptr(clover_fwd), _ptr(clover_inv), n, pin, pout,
+                                     _ptr(workspace), stream))
 
 
 def hr_cg_workspace_bytes(g): return lib().hr_cg_workspace_bytes(ctypes.byref(g))

@@ -470,6 +470,45 @@ def test_host_entry_points(hr, orc, prec):
     assert rel(oh.numpy(), orc.hop(L, 0, 1, U, psi)) <= TOL[prec]
 
 
+@pytest.mark.parametrize("prec", [0, 1])
+def test_host_batch_with_resident_gauge(hr, orc, prec):
+    """hr_gauge_upload_host once, then hr_apply_host_batch on 5 right-hand sides (the double-buffered pipeline wraps
+    around twice): full D, the bare hop, Dhat, and the clover-improved Dhat and D_sw, each result against the oracle"""
+    import torch
+    L, m0, csw = (4, 6, 8, 8), -0.25, 1.2
+    U = rounded(inputs.weak_gauge(L, 0.3, 1), prec)
+    lat = lattice(hr, L, 0, prec)
+    g, st = lat.g, hr.stream_ptr()
+    Uh = torch.from_numpy(U.astype(lat.cplx)).pin_memory()
+    u_dev = lat.empty_gauge(hr.REP_FUND)
+    hr.hr_gauge_upload_host(g, hr.REP_FUND, Uh, u_dev, hr.device_buffer(hr.hr_canonical_gauge_bytes(g, hr.REP_FUND)), st)
+    assert torch.equal(u_dev, lat.put_gauge_fund(U))
+    fwd, inv = lat.clover_build(m0, csw, u_dev)
+    A = orc.clover_dense(L, 4.0 + m0, csw, U)
+    Ainv = orc.invert(A)
+    C = A - (4.0 + m0) * np.eye(8)[None]
+    psis = [rounded(inputs.gaussian_spinor(L, 2, 2 + i), prec) for i in range(5)]
+    ins = [torch.from_numpy(p.astype(lat.cplx)).pin_memory() for p in psis]
+    outs = [torch.empty_like(a).pin_memory() for a in ins]
+    ws = hr.device_buffer(hr.hr_host_batch_workspace_bytes(g))
+    cases = [
+        (hr.HOST_DIRAC, None, None, lambda p: orc.dirac(L, 0, m0, U, p)),
+        (hr.EO_HOP_EO, None, None, lambda p: orc.hop(L, 0, 0, U, p)),
+        (hr.EO_DHAT, None, None, lambda p: orc.dirac_eo(L, 0, m0, U, p)),
+        (hr.EO_DHAT, fwd, inv, lambda p: orc.dirac_eo_clover(L, U, A, Ainv, p)),
+        (hr.HOST_DIRAC, fwd, None, lambda p: orc.dirac_clover(L, m0, U, C, p)),
+    ]
+    for op, cf, ci, want in cases:
+        for o in outs:
+            o.fill_(7.0)
+        hr.hr_apply_host_batch(g, op, m0, u_dev, cf, ci, ins, outs, ws, st)
+        for p, o in zip(psis, outs):
+            assert rel(o.numpy(), want(p)) <= TOL[prec], (op, cf is not None)
+    hr.hr_apply_host_batch(g, hr.HOST_DIRAC, m0, u_dev, None, None, [], [], ws, st)      # empty batch: nothing to do
+    with pytest.raises(hr.HrError):
+        hr.hr_apply_host_batch(g, hr.HOST_DIRAC, m0, u_dev, fwd, inv, ins[:1], outs[:1], ws, st)
+
+
 def test_native_library_is_the_one_loaded(hr):
     """the product path is the in-tree shared object, and it counts its own launches"""
     import torch
@@ -807,3 +846,29 @@ def test_tiled_kernel_soak_is_bitwise_repeatable(hr):
                 else:
                     assert torch.equal(ref, out), (L, rep, prec, i)
         torch.cuda.synchronize()
+
+
+def test_clover_inverse_of_indefinite_blocks(hr, orc):
+    """4 + m0 small against |csw F|: A(x) is indefinite and the unpivoted elimination would divide by tiny diagonal
+    pivots; the build's Gauss-Jordan with partial pivoting must still reproduce the oracle's dense inverse, and
+    hr_clover_count_nonfinite must report 0 non-finite entries"""
+    import torch
+    L, m0, csw = (4, 4, 4, 4), -3.95, 4.0
+    U = inputs.weak_gauge(L, 0.6, 1)
+    A = orc.clover_dense(L, 4.0 + m0, csw, U)
+    ev = np.linalg.eigvalsh(A)
+    assert ev.min() < -0.1 and ev.max() > 0.1 and np.abs(ev).min() > 1e-4     # indefinite, invertible
+    Ainv = np.linalg.inv(A)
+    lat = lattice(hr, L, 0, 0)
+    fwd, inv = lat.clover_build(m0, csw, lat.put_gauge_fund(U))
+    bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+    assert np.linalg.norm(lat.get_clover(fwd) - bf) <= 1e-13 * np.linalg.norm(bf)
+    assert np.linalg.norm(lat.get_clover(inv) - bi) <= 1e-11 * np.linalg.norm(bi)
+    count = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+    for blocks in (fwd, inv):
+        hr.hr_clover_count_nonfinite(lat.g, blocks, count, hr.stream_ptr())
+        assert int(count.item()) == 0
+    inv.view(torch.float64)[5] = float("nan")
+    inv.view(torch.float64)[77] = float("inf")
+    hr.hr_clover_count_nonfinite(lat.g, inv, count, hr.stream_ptr())
+    assert int(count.item()) == 2
