@@ -205,6 +205,37 @@ int hr_dirac_apply_host(const hr_geom* g, double m0, const void* u_canon_host, c
 int hr_dirac_eo_apply_host(const hr_geom* g, int op, double m0, const void* u_canon_host,
                            const void* in_canon_host, void* out_canon_host, void* workspace, void* stream);
 
+/* ---- the sharded hop: one rank of a 4-D domain decomposition (§2.1 "inner computations
+ * ... boundary calculation ... send buffer", Fig. 4 "all four dimensions parallelized").
+ * g describes the rank's LOCAL lattice (ordinary device layout); hr_decomp says which directions are cut between ranks.
+ * Across a cut the hopping sum needs the neighbour rank's boundary spinors; they travel as FACES of spin-projected
+ * half spinors (2N complex numbers per face site instead of 4N; the backward face is already multiplied by the
+ * sender's link, so links never move):
+ *   face index 2*mu   "down": the sender's sites with x_mu = 0,        (1 - gamma_mu) psi projected; goes to the rank at -mu
+ *   face index 2*mu+1 "up"  : the sender's sites with x_mu = L_mu - 1, U_mu^dag (1 + gamma_mu) psi;   goes to the rank at +mu
+ * A face holds the sites of one parity (the hop's input parity) indexed by the other three coordinates, in 16-byte
+ * chunks [chunk][face site]; hr_halo_face_bytes(g, mu) bytes, opaque to the caller, 16-byte aligned.
+ *   hr_halo_pack : writes the 2 faces of every cut direction from the half field `in_half` of parity in_parity.
+ *                  face_out[8] (host array of device pointers, entries of uncut directions ignored) may point into the
+ *                  neighbour's receive buffer when that memory is peer-mapped (NVLink): then packing IS the transfer.
+ *   hr_hop_local : out_half (parity out_parity) = epilogue( H in_half ) on the local lattice: an interior kernel that
+ *                  leaves out the terms crossing a cut, then one boundary kernel per received face that adds them.
+ *                  face_in[2*mu] = the down face of the rank at +mu, face_in[2*mu+1] = the up face of the rank at -mu.
+ *                  epi / a / c / clover / phi_half as the epilogues of the single-GPU hop:
+ *                    HR_EPI_NONE        out = H in                      HR_EPI_AXPY        out = a phi + c H in
+ *                    HR_EPI_CLOVER_INV  out = B (H in)                  HR_EPI_CLOVER_AXPY out = B phi + c H in
+ *                  (B = the blocks of `clover`, a full-lattice block field).  With no cut direction this is the
+ *                  single-GPU hop.  The transfer between pack and hop is the caller's (NCCL send/recv, peer copies):
+ *                  Dhat = hop, exchange, hop — see paper_2411_18511_b200/halo.py for the composition. */
+typedef struct hr_decomp {
+    int split[4];   /* split[mu] != 0: direction mu is cut between ranks; 0: periodic inside the local lattice */
+} hr_decomp;
+enum { HR_EPI_NONE = 0, HR_EPI_AXPY = 1, HR_EPI_CLOVER_INV = 2, HR_EPI_CLOVER_AXPY = 3 };
+size_t hr_halo_face_bytes(const hr_geom* g, int mu);
+int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void* u, const void* in_half, void* const* face_out, void* stream);
+int hr_hop_local(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
+                 const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream);
+
 /* ---- host path with the gauge field resident on the device ----
  * The gauge field changes once per molecular-dynamics step and the operator is applied many times in between
  * (PAPER.md:53-59): upload the links once, then stream right-hand sides through.

@@ -19,6 +19,11 @@ int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int ex
 int run_clover_apply(const Geo& g, int rep, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
 int run_count_nonfinite(int prec, const void* x, size_t bytes, unsigned long long* count_dev, cudaStream_t st);
 
+// hr_halo.cu
+int run_halo_pack(const hr_geom* hg, const int* split, int par, const void* gauge, const void* in_half, void* const* face_out, cudaStream_t st);
+int run_halo_boundary(const hr_geom* hg, const int* split, const HopArgs& a, int epi, const void* const* face_in, cudaStream_t st);
+size_t halo_face_bytes(const hr_geom* hg, int mu);
+
 // hr_solver.cu
 size_t cg_workspace_bytes(const hr_geom* g);
 int run_cg(const hr_geom* g, double m0, const void* u, const void* cf, const void* ci, const void* b, void* x, void* workspace, double tol,
@@ -242,6 +247,53 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
     HR_TRY(run_hop(g, a, EPI_NONE, st));
     a.in = tmp; a.out = out; a.parity = HR_EVEN; a.phi = in; a.a = d; a.c = -1.0 / (4.0 * d);
     return run_hop(g, a, EPI_AXPY, st);
+}
+
+// ---------------------------------------------------------------- sharded hop
+size_t hr_halo_face_bytes(const hr_geom* g, int mu) {
+    if (!geom_ok(g) || mu < 0 || mu > 3) return 0;
+    return halo_face_bytes(g, mu);
+}
+
+static int check_decomp(const hr_decomp* d) {
+    if (!d) { set_error("hr_decomp is NULL"); return HR_EINVAL; }
+    return HR_OK;
+}
+
+int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void* u, const void* in_half, void* const* face_out, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
+    if (in_parity != HR_EVEN && in_parity != HR_ODD) { set_error("hr_halo_pack: in_parity %d", in_parity); return HR_EINVAL; }
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(in_half, "in_half"));
+    if (!face_out) { set_error("hr_halo_pack: face_out is NULL"); return HR_EINVAL; }
+    for (int mu = 0; mu < 4; ++mu)
+        if (d->split[mu]) { HR_TRY(check_ptr(face_out[2 * mu], "face_out (down)")); HR_TRY(check_ptr(face_out[2 * mu + 1], "face_out (up)")); }
+    return run_halo_pack(g, d->split, in_parity, u, in_half, face_out, (cudaStream_t)stream);
+}
+
+int hr_hop_local(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
+                 const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
+    if (out_parity != HR_EVEN && out_parity != HR_ODD) { set_error("hr_hop_local: out_parity %d", out_parity); return HR_EINVAL; }
+    if (epi < HR_EPI_NONE || epi > HR_EPI_CLOVER_AXPY) { set_error("hr_hop_local: unknown epilogue %d", epi); return HR_EINVAL; }
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(in_half, "in_half")); HR_TRY(check_ptr(out_half, "out_half"));
+    if (epi == HR_EPI_AXPY || epi == HR_EPI_CLOVER_AXPY) HR_TRY(check_ptr(phi_half, "phi_half"));
+    if (epi == HR_EPI_CLOVER_INV || epi == HR_EPI_CLOVER_AXPY) HR_TRY(check_ptr(clover, "clover"));
+    const size_t half = half_spinor_bytes(g);
+    if (overlap(in_half, half, out_half, half)) { set_error("hr_hop_local: out aliases in (gather operation)"); return HR_EINVAL; }
+    int mask = 0;
+    for (int mu = 0; mu < 4; ++mu)
+        if (d->split[mu]) {
+            if (!face_in) { set_error("hr_hop_local: face_in is NULL"); return HR_EINVAL; }
+            HR_TRY(check_ptr(face_in[2 * mu], "face_in (down face of the +mu neighbour)"));
+            HR_TRY(check_ptr(face_in[2 * mu + 1], "face_in (up face of the -mu neighbour)"));
+            mask |= 1 << mu;
+        }
+    HopArgs h;
+    h.gauge = u; h.in = in_half; h.out = out_half; h.phi = phi_half; h.clover = clover;
+    h.a = a; h.c = epi == HR_EPI_NONE ? 1.0 : c; h.parity = out_parity; h.both = 0; h.open_mask = mask;
+    HR_TRY(run_hop(g, h, epi, (cudaStream_t)stream));
+    if (mask) HR_TRY(run_halo_boundary(g, d->split, h, epi, face_in, (cudaStream_t)stream));
+    return HR_OK;
 }
 
 // ---------------------------------------------------------------- C1 / C2 / C3

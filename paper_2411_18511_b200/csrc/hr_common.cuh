@@ -286,11 +286,18 @@ __device__ __forceinline__ void hop_project(cplx<T>* h0, cplx<T>* h1, const cplx
         }
     }
 }
+// acc += the four spin components rebuilt from the link-multiplied half spinor (c0, c1)
+template <typename T, int N, int MU, bool FWD>
+__device__ __forceinline__ void hop_rebuild(cplx<T>* acc, const cplx<T>* c0, const cplx<T>* c1);
 template <typename T, int N, int MU, bool FWD>
 __device__ __forceinline__ void hop_apply(cplx<T>* acc, const cplx<T>* h0, const cplx<T>* h1, const Link<T, N>& u) {
     cplx<T> c0[N], c1[N];
     if (FWD) { mul_link(c0, u, h0); mul_link(c1, u, h1); }
     else     { mul_link_dag(c0, u, h0); mul_link_dag(c1, u, h1); }
+    hop_rebuild<T, N, MU, FWD>(acc, c0, c1);
+}
+template <typename T, int N, int MU, bool FWD>
+__device__ __forceinline__ void hop_rebuild(cplx<T>* acc, const cplx<T>* c0, const cplx<T>* c1) {
 #pragma unroll
     for (int c = 0; c < N; ++c) {
         acc[c] = acc[c] + c0[c];

@@ -1,0 +1,218 @@
+// hr_halo.cu — the sharded (domain-decomposed) hop: face packing and the boundary kernel.
+//
+// PAPER.md:31 §2.1: "inner computations ... boundary calculation ... a kernel that synchronizes the send buffer";
+// communications overlap the inner kernel; Fig. 4: all four dimensions parallelised.
+// Each rank holds a local lattice in the ordinary device layout.  For a direction mu that is cut between ranks, the
+// terms of the hopping sum that cross the cut are left out of the local kernel (HopArgs::open_mask) and arrive as
+// faces of spin-projected half spinors — 2N complex numbers per face site instead of 4N, and the backward face already
+// multiplied by the sender's link, so links never move:
+//   face 2mu   ("down", sites with x_mu = 0,       sent to the rank at -mu): (h0, h1) of (1 - gamma_mu) psi(y)
+//             -> the receiver's forward term at x = y - mu (its x_mu = L_mu-1):  acc += rebuild(U_mu(x) h)
+//   face 2mu+1 ("up",   sites with x_mu = L_mu-1,  sent to the rank at +mu): U_mu(y)^dag (h0, h1) of (1 + gamma_mu) psi(y)
+//             -> the receiver's backward term at x = y + mu (its x_mu = 0):      acc += rebuild(w)
+// A face holds the sites of ONE parity (the input parity of the hop), indexed by the three other coordinates:
+//   fi = lex3(other coordinates, last one fastest) / 2, chunk c of face site fi at 16-byte index c*nface + fi
+// (sender and receiver agree on fi because they share the other three coordinates).  hr_halo_pack may write a face
+// straight into the neighbour's receive buffer when that is peer-mapped (NVLink): the pointer is the caller's.
+#include "hr_hop_generic.cuh"
+
+namespace hr {
+
+struct FaceGeo {
+    int mu;          // the cut direction
+    int o[3];        // the other directions, increasing
+    int E[3];        // their extents
+    int nface;       // face sites of one parity = E0*E1*E2/2
+};
+
+static FaceGeo make_face(const hr_geom* hg, int mu) {
+    FaceGeo f;
+    f.mu = mu;
+    int k = 0;
+    for (int d = 0; d < 4; ++d)
+        if (d != mu) { f.o[k] = d; f.E[k] = hg->L[d]; ++k; }
+    f.nface = f.E[0] * f.E[1] * f.E[2] / 2;
+    return f;
+}
+
+// coordinates of face site fi of parity `par` on the plane x_mu = xmu
+__device__ __forceinline__ void face_site(const FaceGeo& f, int fi, int xmu, int par, int x[4]) {
+    const int pair = 2 * fi;
+    const int c2 = pair % f.E[2];
+    const int t = pair / f.E[2];
+    const int c1 = t % f.E[1], c0 = t / f.E[1];
+    const int r = (par + xmu + c0 + c1 + c2) & 1;      // c2 is even: the two sites of the pair are c2 and c2+1
+    x[f.mu] = xmu;
+    x[f.o[0]] = c0;
+    x[f.o[1]] = c1;
+    x[f.o[2]] = c2 + r;
+}
+
+// half spinor (2N complex) <-> face buffer chunks
+template <typename T, int N>
+__device__ __forceinline__ void face_store(void* face, int nface, int fi, const cplx<T>* h0, const cplx<T>* h1) {
+    cplx<T> v[2 * N];
+#pragma unroll
+    for (int c = 0; c < N; ++c) { v[c] = h0[c]; v[N + c] = h1[c]; }
+    SiteIO<T, 2 * N>::store(face, (size_t)fi, nface, v);
+}
+template <typename T, int N>
+__device__ __forceinline__ void face_load(const void* face, int nface, int fi, cplx<T>* h0, cplx<T>* h1) {
+    cplx<T> v[2 * N];
+    SiteIO<T, 2 * N>::template load<LD_STREAM>(v, face, (size_t)fi, nface);
+#pragma unroll
+    for (int c = 0; c < N; ++c) { h0[c] = v[c]; h1[c] = v[N + c]; }
+}
+
+template <typename T, int N, int MU, bool UP, bool ONFLY>
+__device__ __forceinline__ void pack_one(const Geo& g, const FaceGeo& f, int par, const void* gauge, const void* in_half, void* face, int fi) {
+    constexpr int NC = 4 * N;
+    int x[4];
+    face_site(f, fi, UP ? (MU == 0 ? g.L0 : MU == 1 ? g.L1 : MU == 2 ? g.L2 : 2 * g.L3h) - 1 : 0, par, x);
+    const int row = (x[0] * g.L1 + x[1]) * g.L2 + x[2], h = x[3] >> 1;
+    cplx<T> psi[NC], h0[N], h1[N];
+    SiteIO<T, NC>::template load<LD_KEEP>(psi, in_half, (size_t)row * (SiteIO<T, NC>::NCH * g.L3h) + h, g.L3h);
+    if (!UP) {
+        hop_project<T, N, MU, true>(h0, h1, psi);                  // (1 - gamma_mu) psi: the neighbour's forward term
+        face_store<T, N>(face, f.nface, fi, h0, h1);
+    } else {
+        hop_project<T, N, MU, false>(h0, h1, psi);                 // (1 + gamma_mu) psi, times this site's link^dag
+        Link<T, N> u;
+        load_link_rep<T, LD_STREAM, ONFLY>(u, gauge, g, par, MU, row, h);
+        cplx<T> c0[N], c1[N];
+        mul_link_dag(c0, u, h0);
+        mul_link_dag(c1, u, h1);
+        face_store<T, N>(face, f.nface, fi, c0, c1);
+    }
+}
+
+// one thread per face site; in_half: half field of parity `par`
+template <typename T, int N, bool ONFLY>
+__global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, FaceGeo f, int up, int par, const void* gauge, const void* in_half, void* face) {
+    const int fi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (fi >= f.nface) return;
+#define HR_PACK(MU)                                                                        \
+    if (f.mu == MU) {                                                                      \
+        if (up) pack_one<T, N, MU, true, ONFLY>(g, f, par, gauge, in_half, face, fi);      \
+        else pack_one<T, N, MU, false, ONFLY>(g, f, par, gauge, in_half, face, fi);        \
+    }
+    HR_PACK(0) HR_PACK(1) HR_PACK(2) HR_PACK(3)
+#undef HR_PACK
+}
+
+// Boundary kernel: the term of the hopping sum that crossed the cut, for the output sites on one face, combined into
+// `out` the way the local kernel's epilogue would have: out += c * t (EPI_NONE: c = 1; EPI_AXPY, EPI_CLOVER_AXPY) or
+// out += B(x) t (EPI_CLOVER_INV).  up == 1: output sites with x_mu = L_mu-1 and the face received from the rank at +mu
+// (its "down" face); up == 0: output sites with x_mu = 0 and the "up" face of the rank at -mu.  par = output parity.
+template <typename T, int N, int MU, bool UP, int EPI, bool ONFLY>
+__device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int par, const HopArgs& a, const void* face, int fi) {
+    constexpr int NC = 4 * N;
+    typedef SiteIO<T, NC> IO;
+    int x[4];
+    face_site(f, fi, UP ? (MU == 0 ? g.L0 : MU == 1 ? g.L1 : MU == 2 ? g.L2 : 2 * g.L3h) - 1 : 0, par, x);
+    const int row = (x[0] * g.L1 + x[1]) * g.L2 + x[2], h = x[3] >> 1;
+    cplx<T> t[NC], h0[N], h1[N];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) t[c] = mk<T>((T)0, (T)0);
+    face_load<T, N>(face, f.nface, fi, h0, h1);
+    if (UP) {
+        Link<T, N> u;
+        load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, par, MU, row, h);
+        hop_apply<T, N, MU, true>(t, h0, h1, u);
+    } else {
+        hop_rebuild<T, N, MU, false>(t, h0, h1);
+    }
+    const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
+    cplx<T> o[NC];
+    IO::template load<LD_KEEP>(o, a.out, first, g.L3h);
+    if (EPI == EPI_CLOVER_INV) {
+        T blk[CloverSize<N>::reals];
+        cplx<T> y[NC];
+        load_clover<T, N>(blk, a.clover, g, par, row, h);
+        clover_matvec<T, N>(y, blk, t);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) o[c] = o[c] + y[c];
+    } else {
+        const T cc = EPI == EPI_NONE ? (T)1 : (T)a.c;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) { o[c].re = fma(cc, t[c].re, o[c].re); o[c].im = fma(cc, t[c].im, o[c].im); }
+    }
+    IO::store(a.out, first, g.L3h, o);
+}
+
+template <typename T, int N, int EPI, bool ONFLY>
+__global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, int up, int par, HopArgs a, const void* face) {
+    const int fi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (fi >= f.nface) return;
+#define HR_BND(MU)                                                                         \
+    if (f.mu == MU) {                                                                      \
+        if (up) boundary_one<T, N, MU, true, EPI, ONFLY>(g, f, par, a, face, fi);          \
+        else boundary_one<T, N, MU, false, EPI, ONFLY>(g, f, par, a, face, fi);            \
+    }
+    HR_BND(0) HR_BND(1) HR_BND(2) HR_BND(3)
+#undef HR_BND
+}
+
+template <typename T, int N, bool ONFLY>
+static int pack_faces(const hr_geom* hg, const int* split, int par, const void* gauge, const void* in_half, void* const* face_out, cudaStream_t st) {
+    const Geo g = make_geo(hg);
+    for (int mu = 0; mu < 4; ++mu) {
+        if (!split[mu]) continue;
+        const FaceGeo f = make_face(hg, mu);
+        for (int up = 0; up < 2; ++up) {
+            halo_pack_kernel<T, N, ONFLY><<<(f.nface + 127) / 128, 128, 0, st>>>(g, f, up, par, gauge, in_half, face_out[2 * mu + up]);
+            count_launch();
+        }
+    }
+    return check_launch("halo_pack_kernel");
+}
+
+template <typename T, int N, bool ONFLY>
+static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, int epi, const void* const* face_in, cudaStream_t st) {
+    const Geo g = make_geo(hg);
+    for (int mu = 0; mu < 4; ++mu) {
+        if (!split[mu]) continue;
+        const FaceGeo f = make_face(hg, mu);
+        const dim3 grid((f.nface + 127) / 128);
+        for (int up = 0; up < 2; ++up) {
+            // output sites at x_mu = L-1 take the +mu neighbour's down face (index 2mu); those at x_mu = 0 its up face
+            const void* face = face_in[2 * mu + (up ? 0 : 1)];
+            switch (epi) {
+                case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
+                case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
+                case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
+                case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
+                default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
+            }
+            count_launch();
+        }
+    }
+    return check_launch("halo_boundary_kernel");
+}
+
+#define HR_DISPATCH_REP(FN, ...)                                                                      \
+    if (hg->rep == HR_REP_FUND) {                                                                     \
+        if (hg->prec == HR_PREC_F64) return FN<double, 2, false>(__VA_ARGS__);                        \
+        return FN<float, 2, false>(__VA_ARGS__);                                                      \
+    }                                                                                                 \
+    if (hg->link_storage == HR_LINKS_ONTHEFLY) {                                                      \
+        if (hg->prec == HR_PREC_F64) return FN<double, 3, true>(__VA_ARGS__);                         \
+        return FN<float, 3, true>(__VA_ARGS__);                                                       \
+    }                                                                                                 \
+    if (hg->prec == HR_PREC_F64) return FN<double, 3, false>(__VA_ARGS__);                            \
+    return FN<float, 3, false>(__VA_ARGS__);
+
+int run_halo_pack(const hr_geom* hg, const int* split, int par, const void* gauge, const void* in_half, void* const* face_out, cudaStream_t st) {
+    HR_DISPATCH_REP(pack_faces, hg, split, par, gauge, in_half, face_out, st)
+}
+
+int run_halo_boundary(const hr_geom* hg, const int* split, const HopArgs& a, int epi, const void* const* face_in, cudaStream_t st) {
+    HR_DISPATCH_REP(add_boundary, hg, split, a, epi, face_in, st)
+}
+
+size_t halo_face_bytes(const hr_geom* hg, int mu) {
+    const FaceGeo f = make_face(hg, mu);
+    return (size_t)f.nface * 2 * ncolour(hg->rep) * 2 * real_bytes(hg->prec);
+}
+
+}  // namespace hr

@@ -57,8 +57,9 @@ int kernel_plan(const hr_geom* g, int both, int* info) {
 int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
     const Geo geo = make_geo(g);
     TiledPlan pl;
-    const bool fits = g->kernel != HR_KERNEL_GENERIC && tiled_plan(g, a.both, sm_count(), pl);
-    if (g->kernel == HR_KERNEL_TILED && !fits) {
+    // (a hop with cut directions, hr_hop_local, runs on the generic kernel: the tiled march has no open-boundary form yet)
+    const bool fits = g->kernel != HR_KERNEL_GENERIC && a.open_mask == 0 && tiled_plan(g, a.both, sm_count(), pl);
+    if (g->kernel == HR_KERNEL_TILED && !fits && a.open_mask == 0) {
         set_error("HR_KERNEL_TILED: lattice %dx%dx%dx%d does not fit the tiled kernel", g->L[0], g->L[1], g->L[2], g->L[3]);
         return HR_EUNSUPPORTED;
     }

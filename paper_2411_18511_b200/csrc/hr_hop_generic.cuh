@@ -24,6 +24,9 @@ struct HopArgs {
     double a, c;
     int parity;          // output parity when both == 0
     int both;            // 1: gridDim.y == 2 and blockIdx.y is the output parity (full D in one launch)
+    int open_mask = 0;   // bit mu set: direction mu is cut between ranks (hr_hop_local): the forward term of sites with
+                         // x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out here and added from
+                         // the received faces by the boundary kernel (hr_halo.cu)
 };
 
 // PHI_POLICY: LD_STREAM when phi is read by this kernel only; LD_KEEP in the full-lattice launch (H3), where
@@ -99,21 +102,26 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
 
     const int stride = g.L3h;
     const int rowlen = IO::NCH * g.L3h;
-#define HR_HOP_DIR(MU, ROWF, HF, ROWB, HB)                                                      \
+    const int om = a.open_mask;   // terms that cross a rank boundary are the boundary kernel's (0 on one GPU)
+#define HR_HOP_DIR(MU, ROWF, HF, ROWB, HB, ATHI, ATLO)                                          \
     {                                                                                           \
         cplx<T> nb[NC];                                                                         \
         Link<T, N> u;                                                                           \
-        load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, p, MU, row, h);                                  \
-        IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWF) * rowlen + (HF), stride);        \
-        hop_term<T, N, MU, true>(acc, nb, u);                                                   \
-        load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, 1 - p, MU, ROWB, HB);                            \
-        IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWB) * rowlen + (HB), stride);        \
-        hop_term<T, N, MU, false>(acc, nb, u);                                                  \
+        if (!(((om >> MU) & 1) && (ATHI))) {                                                    \
+            load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, p, MU, row, h);                   \
+            IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWF) * rowlen + (HF), stride);    \
+            hop_term<T, N, MU, true>(acc, nb, u);                                               \
+        }                                                                                       \
+        if (!(((om >> MU) & 1) && (ATLO))) {                                                    \
+            load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, 1 - p, MU, ROWB, HB);             \
+            IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWB) * rowlen + (HB), stride);    \
+            hop_term<T, N, MU, false>(acc, nb, u);                                              \
+        }                                                                                       \
     }
-    HR_HOP_DIR(0, row_f0, h, row_b0, h)
-    HR_HOP_DIR(1, row_f1, h, row_b1, h)
-    HR_HOP_DIR(2, row_f2, h, row_b2, h)
-    HR_HOP_DIR(3, row, h_f3, row, h_b3)
+    HR_HOP_DIR(0, row_f0, h, row_b0, h, x0 == g.L0 - 1, x0 == 0)
+    HR_HOP_DIR(1, row_f1, h, row_b1, h, x1 == g.L1 - 1, x1 == 0)
+    HR_HOP_DIR(2, row_f2, h, row_b2, h, x2 == g.L2 - 1, x2 == 0)
+    HR_HOP_DIR(3, row, h_f3, row, h_b3, r == 1 && h == g.L3h - 1, r == 0 && h == 0)
 #undef HR_HOP_DIR
 
     hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row, h);

@@ -21,6 +21,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2
 EVEN, ODD, BOTH = 0, 1, 2
 EO_HOP_OE, EO_HOP_EO, EO_DHAT = 0, 1, 2
 HOST_DIRAC = 3
+EPI_NONE, EPI_AXPY, EPI_CLOVER_INV, EPI_CLOVER_AXPY = 0, 1, 2, 3
 OP_HOP, OP_DIRAC, OP_DHAT, OP_CLOVER, OP_DHAT_CLOVER, OP_REPRESENT = 0, 1, 2, 3, 4, 5
 
 # every symbol include/hr_dslash.h declares (tests/test_abi.py checks the header against this list)
@@ -30,7 +31,7 @@ SYMBOLS = [
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
     "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_gauge_upload_host",
-    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_last_error",
+    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_kernel_plan", "hr_cg_workspace_bytes", "hr_cg_solve",
     "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed", "hr_cg_solve_mixed_clover",
 ]
@@ -39,6 +40,10 @@ SYMBOLS = [
 class hr_geom(ctypes.Structure):
     _fields_ = [("L", ctypes.c_int * 4), ("rep", ctypes.c_int), ("prec", ctypes.c_int),
                 ("link_storage", ctypes.c_int), ("kernel", ctypes.c_int)]
+
+
+class hr_decomp(ctypes.Structure):
+    _fields_ = [("split", ctypes.c_int * 4)]
 
 
 class HrError(RuntimeError):
@@ -82,6 +87,9 @@ def lib():
             "hr_gauge_upload_host": (I, [G, I, V, V, V, V]),
             "hr_host_batch_workspace_bytes": (S, [G]),
             "hr_apply_host_batch": (I, [G, I, D, V, V, V, I, ctypes.POINTER(V), ctypes.POINTER(V), V, V]),
+            "hr_halo_face_bytes": (S, [G, I]),
+            "hr_halo_pack": (I, [G, ctypes.POINTER(hr_decomp), I, V, V, ctypes.POINTER(V), V]),
+            "hr_hop_local": (I, [G, ctypes.POINTER(hr_decomp), I, I, D, D, V, V, V, V, V, ctypes.POINTER(V), V]),
             "hr_last_error": (S, [ctypes.c_char_p, S]),
             "hr_launch_count": (ctypes.c_ulonglong, []),
             "hr_kernel_name": (ctypes.c_char_p, [G]),
@@ -224,6 +232,31 @@ def hr_apply_host_batch(g, op, m0, u_dev, clover_fwd, clover_inv, ins, outs, wor
     pout = (ctypes.c_void_p * n)(*[_ptr(a) for a in outs])
     _check(lib().hr_apply_host_batch(ctypes.byref(g), int(op), float(m0), _ptr(u_dev), _ptr(clover_fwd), _ptr(clover_inv), n, pin, pout,
                                      _ptr(workspace), stream))
+
+
+def decomp(split) -> hr_decomp:
+    d = hr_decomp()
+    for i in range(4):
+        d.split[i] = int(bool(split[i]))
+    return d
+
+
+def hr_halo_face_bytes(g, mu): return lib().hr_halo_face_bytes(ctypes.byref(g), int(mu))
+
+
+def _faces(faces):
+    """8 device buffers (or None) -> C array of 8 pointers"""
+    assert len(faces) == 8
+    return (ctypes.c_void_p * 8)(*[_ptr(f) for f in faces])
+
+
+def hr_halo_pack(g, d, in_parity, u, in_half, face_out, stream=0):
+    _check(lib().hr_halo_pack(ctypes.byref(g), ctypes.byref(d), int(in_parity), _ptr(u), _ptr(in_half), _faces(face_out), stream))
+
+
+def hr_hop_local(g, d, out_parity, epi, a, c, u, clover, in_half, phi_half, out_half, face_in, stream=0):
+    _check(lib().hr_hop_local(ctypes.byref(g), ctypes.byref(d), int(out_parity), int(epi), float(a), float(c), _ptr(u), _ptr(clover),
+                              _ptr(in_half), _ptr(phi_half), _ptr(out_half), _faces(face_in), stream))
 
 
 def hr_cg_workspace_bytes(g): return lib().hr_cg_workspace_bytes(ctypes.byref(g))
