@@ -409,6 +409,33 @@ def other_configs(hr, inputs, Lattice):
                                                             "gflops": round(f * sites / ms / 1e6, 1), "gbs": round(bc * sites / ms / 1e6, 1),
                                                             "kernel": hr.hr_kernel_name(g),
                                                             "note": "working set 0.1-0.2 GB: partly L2-resident, HBM fraction indicative only"}
+    # 48^4 adjoint fermions (the paper's local volume; higher representations are HiRep's purpose):
+    # HBM-sized, so the fraction of the measured copy bandwidth is meaningful here
+    import json as _json
+    peak = peaks()[0]
+    L = (48,) * 4
+    V = 48 ** 4
+    for prec, ptag in ((hr.PREC_F64, "f64"), (hr.PREC_F32, "f32")):
+        for storage, tag in ((hr.LINKS_COMPRESSED, "stored"), (hr.LINKS_ONTHEFLY, "onthefly")):
+            lat = Lattice(L, hr.REP_ADJ, prec, hr.KERNEL_AUTO, link_storage=storage)
+            g = lat.g
+            # timing only: random bytes of the right sizes (the cost is value-independent; parity is tests/test_gpu_parity.py)
+            Uf_dev = torch.randn(hr.hr_gauge_bytes(g, hr.REP_FUND) // 4, device="cuda").view(torch.uint8)
+            U_dev = lat.represent(Uf_dev) if storage == hr.LINKS_COMPRESSED else Uf_dev
+            p_dev = torch.randn(hr.hr_spinor_bytes(g, hr.BOTH) // 4, device="cuda").view(torch.uint8)
+            o_dev, tmp = lat.empty_spinor(), lat.empty_spinor(hr.ODD)
+            st0 = hr.stream_ptr()
+            for name, op, sites, fn in (
+                    ("hop", hr.OP_HOP, V // 2, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_OE, 0.0, U_dev, None, None, lat.even(p_dev), lat.odd(o_dev), None, st0)),
+                    ("dirac", hr.OP_DIRAC, V, lambda: hr.hr_dirac_apply(g, -0.3, U_dev, p_dev, o_dev, st0)),
+                    ("dhat", hr.OP_DHAT, V // 2, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.3, U_dev, None, None, lat.even(p_dev), lat.even(o_dev), tmp, st0))):
+                ms = timed(fn, 20)
+                f, bc, _ = hr.hr_dirac_flops_bytes(g, op)
+                out["adjoint_48^4_%s_%s_%s" % (name, tag, ptag)] = {"us_per_apply": round(ms * 1e3, 1), "gsites_per_s": round(sites / ms / 1e6, 3),
+                                                                    "gflops": round(f * sites / ms / 1e6, 1), "gbs": round(bc * sites / ms / 1e6, 1),
+                                                                    "frac": round(bc * sites / ms / 1e6 / peak, 4), "bytes_per_site": bc,
+                                                                    "kernel": hr.hr_kernel_name(g)}
+            del Uf_dev, U_dev, p_dev, o_dev, tmp
     return out
 
 

@@ -235,6 +235,14 @@ size_t hr_halo_face_bytes(const hr_geom* g, int mu);
 int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void* u, const void* in_half, void* const* face_out, void* stream);
 int hr_hop_local(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
                  const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream);
+/* The two halves of hr_hop_local, for overlapping the face transfer with the interior kernel ("the inner Dirac
+ * kernel ... [while] the communications take place"): enqueue hr_halo_pack and the transfer on one stream, the interior on
+ * another, make the second stream wait for the transfer, then enqueue the boundary part (paper_2411_18511_b200/halo.py:
+ * hop_all(overlap=True)).  Same arguments as hr_hop_local; the boundary part needs neither in_half nor phi_half. */
+int hr_hop_local_interior(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
+                          const void* in_half, const void* phi_half, void* out_half, void* stream);
+int hr_hop_local_boundary(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double c, const void* u, const void* clover,
+                          void* out_half, const void* const* face_in, void* stream);
 
 /* ---- host path with the gauge field resident on the device ----
  * The gauge field changes once per molecular-dynamics step and the operator is applied many times in between

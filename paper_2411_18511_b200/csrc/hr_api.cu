@@ -270,30 +270,49 @@ int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void
     return run_halo_pack(g, d->split, in_parity, u, in_half, face_out, (cudaStream_t)stream);
 }
 
-int hr_hop_local(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
-                 const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream) {
+// phases: 1 = interior kernel, 2 = boundary kernels, 3 = both
+static int hop_local_phases(int phases, const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u,
+                            const void* clover, const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream) {
     HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
     if (out_parity != HR_EVEN && out_parity != HR_ODD) { set_error("hr_hop_local: out_parity %d", out_parity); return HR_EINVAL; }
     if (epi < HR_EPI_NONE || epi > HR_EPI_CLOVER_AXPY) { set_error("hr_hop_local: unknown epilogue %d", epi); return HR_EINVAL; }
-    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(in_half, "in_half")); HR_TRY(check_ptr(out_half, "out_half"));
-    if (epi == HR_EPI_AXPY || epi == HR_EPI_CLOVER_AXPY) HR_TRY(check_ptr(phi_half, "phi_half"));
+    HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(out_half, "out_half"));
+    if (phases & 1) HR_TRY(check_ptr(in_half, "in_half"));
+    if ((phases & 1) && (epi == HR_EPI_AXPY || epi == HR_EPI_CLOVER_AXPY)) HR_TRY(check_ptr(phi_half, "phi_half"));
     if (epi == HR_EPI_CLOVER_INV || epi == HR_EPI_CLOVER_AXPY) HR_TRY(check_ptr(clover, "clover"));
     const size_t half = half_spinor_bytes(g);
-    if (overlap(in_half, half, out_half, half)) { set_error("hr_hop_local: out aliases in (gather operation)"); return HR_EINVAL; }
+    if ((phases & 1) && overlap(in_half, half, out_half, half)) { set_error("hr_hop_local: out aliases in (gather operation)"); return HR_EINVAL; }
     int mask = 0;
     for (int mu = 0; mu < 4; ++mu)
         if (d->split[mu]) {
-            if (!face_in) { set_error("hr_hop_local: face_in is NULL"); return HR_EINVAL; }
-            HR_TRY(check_ptr(face_in[2 * mu], "face_in (down face of the +mu neighbour)"));
-            HR_TRY(check_ptr(face_in[2 * mu + 1], "face_in (up face of the -mu neighbour)"));
+            if (phases & 2) {
+                if (!face_in) { set_error("hr_hop_local: face_in is NULL"); return HR_EINVAL; }
+                HR_TRY(check_ptr(face_in[2 * mu], "face_in (down face of the +mu neighbour)"));
+                HR_TRY(check_ptr(face_in[2 * mu + 1], "face_in (up face of the -mu neighbour)"));
+            }
             mask |= 1 << mu;
         }
     HopArgs h;
     h.gauge = u; h.in = in_half; h.out = out_half; h.phi = phi_half; h.clover = clover;
     h.a = a; h.c = epi == HR_EPI_NONE ? 1.0 : c; h.parity = out_parity; h.both = 0; h.open_mask = mask;
-    HR_TRY(run_hop(g, h, epi, (cudaStream_t)stream));
-    if (mask) HR_TRY(run_halo_boundary(g, d->split, h, epi, face_in, (cudaStream_t)stream));
+    if (phases & 1) HR_TRY(run_hop(g, h, epi, (cudaStream_t)stream));
+    if ((phases & 2) && mask) HR_TRY(run_halo_boundary(g, d->split, h, epi, face_in, (cudaStream_t)stream));
     return HR_OK;
+}
+
+int hr_hop_local(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
+                 const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream) {
+    return hop_local_phases(3, g, d, out_parity, epi, a, c, u, clover, in_half, phi_half, out_half, face_in, stream);
+}
+
+int hr_hop_local_interior(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u, const void* clover,
+                          const void* in_half, const void* phi_half, void* out_half, void* stream) {
+    return hop_local_phases(1, g, d, out_parity, epi, a, c, u, clover, in_half, phi_half, out_half, nullptr, stream);
+}
+
+int hr_hop_local_boundary(const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double c, const void* u, const void* clover,
+                          void* out_half, const void* const* face_in, void* stream) {
+    return hop_local_phases(2, g, d, out_parity, epi, 0.0, c, u, clover, nullptr, nullptr, out_half, face_in, stream);
 }
 
 // ---------------------------------------------------------------- C1 / C2 / C3

@@ -86,13 +86,24 @@ __device__ __forceinline__ void pack_one(const Geo& g, const FaceGeo& f, int par
     }
 }
 
-// one thread per face site; in_half: half field of parity `par`
+// one thread per face site, blockIdx.y = the face (2 per cut direction): ONE launch packs every face of the rank.
+// in_half: half field of parity `par`
+struct PackJob {
+    FaceGeo f[4];
+    void* face[8];
+    int slot[8];     // slot[j] = face index 2*mu + up of the j-th face to pack
+    int nslots;
+};
 template <typename T, int N, bool ONFLY>
-__global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, FaceGeo f, int up, int par, const void* gauge, const void* in_half, void* face) {
+__global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, PackJob job, int par, const void* gauge, const void* in_half) {
+    const int fidx = job.slot[blockIdx.y];
+    const int mu = fidx >> 1, up = fidx & 1;
+    const FaceGeo& f = job.f[mu];
     const int fi = blockIdx.x * blockDim.x + threadIdx.x;
     if (fi >= f.nface) return;
+    void* face = job.face[fidx];
 #define HR_PACK(MU)                                                                        \
-    if (f.mu == MU) {                                                                      \
+    if (mu == MU) {                                                                        \
         if (up) pack_one<T, N, MU, true, ONFLY>(g, f, par, gauge, in_half, face, fi);      \
         else pack_one<T, N, MU, false, ONFLY>(g, f, par, gauge, in_half, face, fi);        \
     }
@@ -140,10 +151,15 @@ __device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int
     IO::store(a.out, first, g.L3h, o);
 }
 
+// blockIdx.y = 0: the sites with x_mu = 0 (up face of the rank at -mu); 1: the sites with x_mu = L_mu-1 (down face of the rank
+// at +mu).  The two site sets are disjoint, so one launch serves both faces of a direction; different directions share edge and
+// corner sites and run as consecutive launches.
 template <typename T, int N, int EPI, bool ONFLY>
-__global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, int up, int par, HopArgs a, const void* face) {
+__global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, int par, HopArgs a, const void* face_lo, const void* face_hi) {
     const int fi = blockIdx.x * blockDim.x + threadIdx.x;
     if (fi >= f.nface) return;
+    const int up = blockIdx.y;
+    const void* face = up ? face_hi : face_lo;
 #define HR_BND(MU)                                                                         \
     if (f.mu == MU) {                                                                      \
         if (up) boundary_one<T, N, MU, true, EPI, ONFLY>(g, f, par, a, face, fi);          \
@@ -156,14 +172,22 @@ __global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, in
 template <typename T, int N, bool ONFLY>
 static int pack_faces(const hr_geom* hg, const int* split, int par, const void* gauge, const void* in_half, void* const* face_out, cudaStream_t st) {
     const Geo g = make_geo(hg);
+    PackJob job;
+    job.nslots = 0;
+    int maxface = 0;
     for (int mu = 0; mu < 4; ++mu) {
+        job.f[mu] = make_face(hg, mu);
+        job.face[2 * mu] = job.face[2 * mu + 1] = nullptr;
         if (!split[mu]) continue;
-        const FaceGeo f = make_face(hg, mu);
         for (int up = 0; up < 2; ++up) {
-            halo_pack_kernel<T, N, ONFLY><<<(f.nface + 127) / 128, 128, 0, st>>>(g, f, up, par, gauge, in_half, face_out[2 * mu + up]);
-            count_launch();
+            job.face[2 * mu + up] = face_out[2 * mu + up];
+            job.slot[job.nslots++] = 2 * mu + up;
         }
+        if (job.f[mu].nface > maxface) maxface = job.f[mu].nface;
     }
+    if (job.nslots == 0) return HR_OK;
+    halo_pack_kernel<T, N, ONFLY><<<dim3((maxface + 127) / 128, job.nslots), 128, 0, st>>>(g, job, par, gauge, in_half);
+    count_launch();
     return check_launch("halo_pack_kernel");
 }
 
@@ -173,19 +197,18 @@ static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, i
     for (int mu = 0; mu < 4; ++mu) {
         if (!split[mu]) continue;
         const FaceGeo f = make_face(hg, mu);
-        const dim3 grid((f.nface + 127) / 128);
-        for (int up = 0; up < 2; ++up) {
-            // output sites at x_mu = L-1 take the +mu neighbour's down face (index 2mu); those at x_mu = 0 its up face
-            const void* face = face_in[2 * mu + (up ? 0 : 1)];
-            switch (epi) {
-                case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
-                case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
-                case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
-                case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, up, a.parity, a, face); break;
-                default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
-            }
-            count_launch();
+        const dim3 grid((f.nface + 127) / 128, 2);
+        // output sites at x_mu = 0 take the -mu neighbour's up face (index 2mu+1); those at x_mu = L-1 the +mu neighbour's down face
+        const void* lo = face_in[2 * mu + 1];
+        const void* hi = face_in[2 * mu];
+        switch (epi) {
+            case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
         }
+        count_launch();
     }
     return check_launch("halo_boundary_kernel");
 }

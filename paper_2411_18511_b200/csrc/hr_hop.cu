@@ -57,9 +57,10 @@ int kernel_plan(const hr_geom* g, int both, int* info) {
 int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
     const Geo geo = make_geo(g);
     TiledPlan pl;
-    // (a hop with cut directions, hr_hop_local, runs on the generic kernel: the tiled march has no open-boundary form yet)
-    const bool fits = g->kernel != HR_KERNEL_GENERIC && a.open_mask == 0 && tiled_plan(g, a.both, sm_count(), pl);
-    if (g->kernel == HR_KERNEL_TILED && !fits && a.open_mask == 0) {
+    // a hop with cut directions (hr_hop_local): tiled open-boundary kernel for the fundamental representation, else generic
+    const bool open_ok = a.open_mask == 0 || (g->rep == HR_REP_FUND && !a.both);
+    const bool fits = g->kernel != HR_KERNEL_GENERIC && open_ok && tiled_plan(g, a.both, sm_count(), pl);
+    if (g->kernel == HR_KERNEL_TILED && !fits && open_ok) {
         set_error("HR_KERNEL_TILED: lattice %dx%dx%dx%d does not fit the tiled kernel", g->L[0], g->L[1], g->L[2], g->L[3]);
         return HR_EUNSUPPORTED;
     }
@@ -68,6 +69,10 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
         if (a.both && epi == EPI_AXPY && a.phi == a.in && dirac_plan(g, sm_count(), dp)) {   // H3: hr_dirac_tiled.cuh
             if (g->prec == HR_PREC_F64) return launch_dirac_tiled<double>(geo, a, dp, st);
             return launch_dirac_tiled<float>(geo, a, dp, st);
+        }
+        if (a.open_mask) {
+            if (g->prec == HR_PREC_F64) return launch_hop_tiled_open<double>(geo, a, epi, pl, st);
+            return launch_hop_tiled_open<float>(geo, a, epi, pl, st);
         }
         if (g->rep == HR_REP_FUND) {
             if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 2>(geo, a, epi, pl, st);

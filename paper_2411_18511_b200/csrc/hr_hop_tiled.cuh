@@ -126,7 +126,10 @@ struct TiledPlan {
 //         its own kernel, hr_dirac_tiled.cuh; this path serves the clover-improved one and the adjoint representation.)
 // L3H: compile-time L3/2 (0 = read it from the geometry): the strides between the 16-byte chunks of a site are then
 // immediates in every LDS / LDG / STG (about a quarter fewer instructions per site)
-template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H>
+// OPEN: the hop of one rank of a decomposed lattice (hr_hop_local): for the directions in HopArgs::open_mask the forward term of
+// sites with x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out (the boundary kernel of hr_halo.cu adds them
+// from the received faces); the producer still copies the wrapped-around rows, they are simply not used.
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H, bool OPEN = false>
 __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g_in, HopArgs a, TiledPlan pl) {
     Geo g = g_in;
@@ -235,6 +238,10 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
     const int rowb1_0 = ((x1 == 0 ? L1 - 1 : x1 - 1)) * g.s1 + x2;
     const int rowb2_0 = x1 * g.s1 + (x2 == 0 ? L2 - 1 : x2 - 1);
 
+    const int om = OPEN ? a.open_mask : 0;
+    const bool cut_f1 = ((om >> 1) & 1) && x1 == L1 - 1, cut_b1 = ((om >> 1) & 1) && x1 == 0;
+    const bool cut_f2 = ((om >> 2) & 1) && x2 == L2 - 1, cut_b2 = ((om >> 2) & 1) && x2 == 0;
+
     Link<T, N> uf[4], ub[4];
     {   // links of the first step
         const int row = row0 + xs * g.s0;
@@ -254,6 +261,8 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         const int r = (x0 + x1 + x2 + p) & 1;
         const int hf3 = r ? (h == L3h - 1 ? 0 : h + 1) : h;
         const int hb3 = r ? h : (h == 0 ? L3h - 1 : h - 1);
+        const bool cut_f0 = (om & 1) && x0 == L0 - 1, cut_b0 = (om & 1) && x0 == 0;
+        const bool cut_f3 = ((om >> 3) & 1) && r == 1 && h == L3h - 1, cut_b3 = ((om >> 3) & 1) && r == 0 && h == 0;
         const char* sprev = ring + (k & 3) * planeb;
         const char* scur = ring + ((k + 1) & 3) * planeb;
         const char* snext = ring + ((k + 2) & 3) * planeb;
@@ -294,35 +303,35 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         const char* const a3b = scur + off_c + hb3 * 16;
         HR_NB_NEXT(nb0, a0f);
         HR_NB_NEXT(nb1, a0b); HR_NB_NOW(nb0, a0f);
-        hop_term<T, N, 0, true>(acc, nb0, uf[0]);
+        if (!(OPEN && cut_f0)) hop_term<T, N, 0, true>(acc, nb0, uf[0]);
         load_link_rep<T, LP, ONFLY>(uf[0], a.gauge, g, p, 0, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a1f); HR_NB_NOW(nb1, a0b);
-        hop_term<T, N, 0, false>(acc, nb1, ub[0]);
+        if (!(OPEN && cut_b0)) hop_term<T, N, 0, false>(acc, nb1, ub[0]);
         load_link_rep<T, LP, ONFLY>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a1b); HR_NB_NOW(nb0, a1f);
-        hop_term<T, N, 1, true>(acc, nb0, uf[1]);
+        if (!(OPEN && cut_f1)) hop_term<T, N, 1, true>(acc, nb0, uf[1]);
         load_link_rep<T, LP, ONFLY>(uf[1], a.gauge, g, p, 1, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a2f); HR_NB_NOW(nb1, a1b);
-        hop_term<T, N, 1, false>(acc, nb1, ub[1]);
+        if (!(OPEN && cut_b1)) hop_term<T, N, 1, false>(acc, nb1, ub[1]);
         load_link_rep<T, LP, ONFLY>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a2b); HR_NB_NOW(nb0, a2f);
-        hop_term<T, N, 2, true>(acc, nb0, uf[2]);
+        if (!(OPEN && cut_f2)) hop_term<T, N, 2, true>(acc, nb0, uf[2]);
         load_link_rep<T, LP, ONFLY>(uf[2], a.gauge, g, p, 2, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a3f); HR_NB_NOW(nb1, a2b);
-        hop_term<T, N, 2, false>(acc, nb1, ub[2]);
+        if (!(OPEN && cut_b2)) hop_term<T, N, 2, false>(acc, nb1, ub[2]);
         load_link_rep<T, LP, ONFLY>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a3b); HR_NB_NOW(nb0, a3f);
-        hop_term<T, N, 3, true>(acc, nb0, uf[3]);
+        if (!(OPEN && cut_f3)) hop_term<T, N, 3, true>(acc, nb0, uf[3]);
         load_link_rep<T, LP, ONFLY>(uf[3], a.gauge, g, p, 3, rown, h);
         HR_PIN();
         HR_NB_NOW(nb1, a3b);
-        hop_term<T, N, 3, false>(acc, nb1, ub[3]);
+        if (!(OPEN && cut_b3)) hop_term<T, N, 3, false>(acc, nb1, ub[3]);
         load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
 #undef HR_NB_NEXT
 #undef HR_NB_NOW
@@ -398,9 +407,9 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) 
     return hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, num_sms, 2, 2, pl);
 }
 
-template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H, bool OPEN = false>
 inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H>;
+    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H, OPEN>;
     static std::atomic<unsigned char> configured[64];
     const int rc = opt_in_shared_memory(reinterpret_cast<const void*>(kern), configured, "hop_tiled_kernel");
     if (rc != HR_OK) return rc;
@@ -410,20 +419,20 @@ inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan&
     return check_launch("hop_tiled_kernel");
 }
 
-template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, bool OPEN = false>
 inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
     // compile-time L3/2 = 24 for the fp64 fundamental kernels (measured at 48^4: hop 219.3 -> 216.1 us; the fp32 4 x 4
     // kernel got slower with it)
     constexpr bool SPECIALISE = N == 2 && sizeof(T) == 8;
-    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0)>(g, a, pl, st);
-    return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, 0>(g, a, pl, st);
+    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0), OPEN>(g, a, pl, st);
+    return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, 0, OPEN>(g, a, pl, st);
 }
 
-template <typename T, int N, int EPI, bool SHARE, bool ONFLY>
+template <typename T, int N, int EPI, bool SHARE, bool ONFLY, bool OPEN = false>
 inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4, ONFLY>(g, a, pl, st);
-    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, SHARE, 2, 2, false>(g, a, pl, st);
-    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4, false>(g, a, pl, st);
+    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4, ONFLY, OPEN>(g, a, pl, st);
+    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, SHARE, 2, 2, false, OPEN>(g, a, pl, st);
+    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4, false, OPEN>(g, a, pl, st);
     set_error("hop_tiled_kernel: no instantiation for a %d x %d tile", pl.t1, pl.t2);
     return HR_EUNSUPPORTED;
 }
@@ -442,5 +451,10 @@ inline int launch_hop_tiled(const Geo& g, const HopArgs& a, int epi, const Tiled
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
 }
+
+// the open-boundary instantiations (fundamental representation, one parity per launch) live in their own translation unit,
+// hr_hop_open.cu, so that they compile in parallel with the rest
+template <typename T>
+int launch_hop_tiled_open(const Geo& g, const HopArgs& a, int epi, const TiledPlan& pl, cudaStream_t st);
 
 }  // namespace hr

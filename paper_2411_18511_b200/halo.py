@@ -97,6 +97,14 @@ class Shard(RankGrid):
         hr.hr_hop_local(self.lat.g, self.d, out_parity, epi, a, c, u, clover, in_half, phi, out_half, self.recv,
                         hr.stream_ptr() if stream is None else stream)
 
+    def hop_interior(self, out_parity, u, in_half, out_half, epi=hr.EPI_NONE, a=0.0, c=1.0, clover=None, phi=None, stream=None):
+        hr.hr_hop_local_interior(self.lat.g, self.d, out_parity, epi, a, c, u, clover, in_half, phi, out_half,
+                                 hr.stream_ptr() if stream is None else stream)
+
+    def hop_boundary(self, out_parity, u, out_half, epi=hr.EPI_NONE, c=1.0, clover=None, stream=None):
+        hr.hr_hop_local_boundary(self.lat.g, self.d, out_parity, epi, c, u, clover, out_half, self.recv,
+                                 hr.stream_ptr() if stream is None else stream)
+
 
 # ------------------------------------------------------------------ transport
 def exchange_in_process(shards):
@@ -134,25 +142,55 @@ def exchange_distributed(shard, dist, send=None, recv=None):
 
 
 # ------------------------------------------------------------------ operators on a set of shards in one process
-def hop_all(shards, exchange, out_parity, U, inp, out, **kw):
-    """out[c] (half field of parity out_parity) = epilogue(H inp[c]) on every shard c; U, inp, out: {coords: buffer}"""
-    for c, sh in shards.items():
-        sh.pack(1 - out_parity, U[c], inp[c])
-    exchange(shards)
-    for c, sh in shards.items():
-        kwc = {k: (v[c] if isinstance(v, dict) else v) for k, v in kw.items()}
-        sh.hop(out_parity, U[c], inp[c], out[c], **kwc)
+_comm_streams = {}
 
 
-def dhat_all(shards, exchange, m0, U, in_e, out_e, tmp_o, clover_fwd=None, clover_inv=None):
+def comm_stream(device):
+    """the side stream pack + transfer run on when they overlap the interior kernel (one per device, made on first use)"""
+    import torch
+    if device not in _comm_streams:
+        _comm_streams[device] = torch.cuda.Stream(device=device)
+    return _comm_streams[device]
+
+
+def hop_all(shards, exchange, out_parity, U, inp, out, overlap=False, **kw):
+    """out[c] (half field of parity out_parity) = epilogue(H inp[c]) on every shard c; U, inp, out: {coords: buffer}.
+    overlap=True: pack and transfer run on a side stream while the interior kernels run on the current one,
+    the boundary kernels follow once the faces have arrived."""
+    def per_shard(c):
+        return {k: (v[c] if isinstance(v, dict) else v) for k, v in kw.items()}
+    if not overlap:
+        for c, sh in shards.items():
+            sh.pack(1 - out_parity, U[c], inp[c])
+        exchange(shards)
+        for c, sh in shards.items():
+            sh.hop(out_parity, U[c], inp[c], out[c], **per_shard(c))
+        return
+    import torch
+    main = torch.cuda.current_stream()
+    side = comm_stream(next(iter(shards.values())).lat.device)
+    side.wait_stream(main)                       # the input (and the face buffers' last readers) are ready
+    with torch.cuda.stream(side):
+        for c, sh in shards.items():
+            sh.pack(1 - out_parity, U[c], inp[c])
+        exchange(shards)
+    for c, sh in shards.items():
+        sh.hop_interior(out_parity, U[c], inp[c], out[c], **per_shard(c))
+    main.wait_stream(side)
+    for c, sh in shards.items():
+        kwc = per_shard(c)
+        sh.hop_boundary(out_parity, U[c], out[c], epi=kwc.get("epi", hr.EPI_NONE), c=kwc.get("c", 1.0), clover=kwc.get("clover"))
+
+
+def dhat_all(shards, exchange, m0, U, in_e, out_e, tmp_o, clover_fwd=None, clover_inv=None, overlap=False):
     """the even-odd operator on the global lattice: hop o<-e, exchange, hop e<-o with its epilogue (E1 / E2)"""
     if clover_fwd is None:
         d = 4.0 + m0
-        hop_all(shards, exchange, hr.ODD, U, in_e, tmp_o)
-        hop_all(shards, exchange, hr.EVEN, U, tmp_o, out_e, epi=hr.EPI_AXPY, a=d, c=-1.0 / (4.0 * d), phi=in_e)
+        hop_all(shards, exchange, hr.ODD, U, in_e, tmp_o, overlap=overlap)
+        hop_all(shards, exchange, hr.EVEN, U, tmp_o, out_e, overlap=overlap, epi=hr.EPI_AXPY, a=d, c=-1.0 / (4.0 * d), phi=in_e)
     else:
-        hop_all(shards, exchange, hr.ODD, U, in_e, tmp_o, epi=hr.EPI_CLOVER_INV, clover=clover_inv)
-        hop_all(shards, exchange, hr.EVEN, U, tmp_o, out_e, epi=hr.EPI_CLOVER_AXPY, c=-0.25, clover=clover_fwd, phi=in_e)
+        hop_all(shards, exchange, hr.ODD, U, in_e, tmp_o, overlap=overlap, epi=hr.EPI_CLOVER_INV, clover=clover_inv)
+        hop_all(shards, exchange, hr.EVEN, U, tmp_o, out_e, overlap=overlap, epi=hr.EPI_CLOVER_AXPY, c=-0.25, clover=clover_fwd, phi=in_e)
 
 
 def dirac_all(shards, exchange, m0, U, psi, out):

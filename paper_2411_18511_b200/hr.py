@@ -31,7 +31,8 @@ SYMBOLS = [
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
     "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_gauge_upload_host",
-    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local", "hr_last_error",
+    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local",
+    "hr_hop_local_interior", "hr_hop_local_boundary", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_kernel_plan", "hr_cg_workspace_bytes", "hr_cg_solve",
     "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed", "hr_cg_solve_mixed_clover",
 ]
@@ -90,6 +91,8 @@ def lib():
             "hr_halo_face_bytes": (S, [G, I]),
             "hr_halo_pack": (I, [G, ctypes.POINTER(hr_decomp), I, V, V, ctypes.POINTER(V), V]),
             "hr_hop_local": (I, [G, ctypes.POINTER(hr_decomp), I, I, D, D, V, V, V, V, V, ctypes.POINTER(V), V]),
+            "hr_hop_local_interior": (I, [G, ctypes.POINTER(hr_decomp), I, I, D, D, V, V, V, V, V, V]),
+            "hr_hop_local_boundary": (I, [G, ctypes.POINTER(hr_decomp), I, I, D, V, V, V, ctypes.POINTER(V), V]),
             "hr_last_error": (S, [ctypes.c_char_p, S]),
             "hr_launch_count": (ctypes.c_ulonglong, []),
             "hr_kernel_name": (ctypes.c_char_p, [G]),
@@ -257,6 +260,16 @@ def hr_halo_pack(g, d, in_parity, u, in_half, face_out, stream=0):
 def hr_hop_local(g, d, out_parity, epi, a, c, u, clover, in_half, phi_half, out_half, face_in, stream=0):
     _check(lib().hr_hop_local(ctypes.byref(g), ctypes.byref(d), int(out_parity), int(epi), float(a), float(c), _ptr(u), _ptr(clover),
                               _ptr(in_half), _ptr(phi_half), _ptr(out_half), _faces(face_in), stream))
+
+
+def hr_hop_local_interior(g, d, out_parity, epi, a, c, u, clover, in_half, phi_half, out_half, stream=0):
+    _check(lib().hr_hop_local_interior(ctypes.byref(g), ctypes.byref(d), int(out_parity), int(epi), float(a), float(c), _ptr(u), _ptr(clover),
+                                       _ptr(in_half), _ptr(phi_half), _ptr(out_half), stream))
+
+
+def hr_hop_local_boundary(g, d, out_parity, epi, c, u, clover, out_half, face_in, stream=0):
+    _check(lib().hr_hop_local_boundary(ctypes.byref(g), ctypes.byref(d), int(out_parity), int(epi), float(c), _ptr(u), _ptr(clover),
+                                       _ptr(out_half), _faces(face_in), stream))
 
 
 def hr_cg_workspace_bytes(g): return lib().hr_cg_workspace_bytes(ctypes.byref(g))

@@ -93,12 +93,13 @@ def hr():
     return _hr
 
 
-def make_shards(hr, Lg, P, rep, prec, split=None, link_storage=None):
+def make_shards(hr, Lg, P, rep, prec, split=None, link_storage=None, kernel=None):
     from paper_2411_18511_b200 import halo
     from paper_2411_18511_b200.lattice import Lattice
     L = halo.local_extents(Lg, P)
     ls = hr.LINKS_COMPRESSED if link_storage is None else link_storage
-    return {c: halo.Shard(Lattice(L, rep, prec, hr.KERNEL_AUTO, link_storage=ls), P, c, split) for c in halo.rank_coords(P)}
+    k = hr.KERNEL_AUTO if kernel is None else kernel
+    return {c: halo.Shard(Lattice(L, rep, prec, k, link_storage=ls), P, c, split) for c in halo.rank_coords(P)}
 
 
 CASES = [((8, 4, 4, 8), (2, 1, 1, 1), None),            # one cut direction, two ranks
@@ -112,8 +113,10 @@ CASES = [((8, 4, 4, 8), (2, 1, 1, 1), None),            # one cut direction, two
 @pytest.mark.gpu
 @pytest.mark.parametrize("Lg,P,split", CASES)
 @pytest.mark.parametrize("prec", [0, 1])
-def test_sharded_fundamental_operators(hr, orc, Lg, P, split, prec):
-    """bare hops, full D, Dhat and the clover-improved Dhat on a cut lattice against the oracle on the whole lattice"""
+@pytest.mark.parametrize("kernel", ["generic", "tiled"])
+def test_sharded_fundamental_operators(hr, orc, Lg, P, split, prec, kernel):
+    """bare hops, full D, Dhat and the clover-improved Dhat on a cut lattice against the oracle on the whole lattice, with
+    both interior kernels (generic, and the x0-marching tiled kernel in its open-boundary instantiation)"""
     import torch
     from paper_2411_18511_b200 import halo
     from test_gpu_parity import dense_to_blocks
@@ -125,7 +128,9 @@ def test_sharded_fundamental_operators(hr, orc, Lg, P, split, prec):
     A = orc.clover_dense(Lg, 4.0 + m0, csw, U)
     Ainv = orc.invert(A)
     bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
-    shards = make_shards(hr, Lg, P, hr.REP_FUND, prec, split)
+    kid = hr.KERNEL_GENERIC if kernel == "generic" else hr.KERNEL_TILED
+    shards = make_shards(hr, Lg, P, hr.REP_FUND, prec, split, kernel=kid)
+    assert all(hr.hr_kernel_name(sh.lat.g) == kernel for sh in shards.values())
     Ud, pd, od, td, cf, ci = {}, {}, {}, {}, {}, {}
     for c, sh in shards.items():
         lat = sh.lat
@@ -156,9 +161,13 @@ def test_sharded_fundamental_operators(hr, orc, Lg, P, split, prec):
         od[c].zero_()
     halo.dhat_all(shards, halo.exchange_in_process, m0, Ud, {c: ev[c](pd[c]) for c in shards}, {c: ev[c](od[c]) for c in shards}, td)
     assert rel(gather(), orc.dirac_eo(Lg, 0, m0, U, psi, nthreads=NTHREADS)) <= TOL[prec]
-    halo.dhat_all(shards, halo.exchange_in_process, m0, Ud, {c: ev[c](pd[c]) for c in shards}, {c: ev[c](od[c]) for c in shards}, td,
-                  clover_fwd=cf, clover_inv=ci)
-    assert rel(gather(), orc.dirac_eo_clover(Lg, U, A, Ainv, psi, nthreads=NTHREADS)) <= TOL[prec]
+    want_e2 = orc.dirac_eo_clover(Lg, U, A, Ainv, psi, nthreads=NTHREADS)
+    for overlap in (False, True):      # True: pack + transfer on a side stream while the interior kernels run
+        for c in shards:
+            od[c].zero_()
+        halo.dhat_all(shards, halo.exchange_in_process, m0, Ud, {c: ev[c](pd[c]) for c in shards}, {c: ev[c](od[c]) for c in shards}, td,
+                      clover_fwd=cf, clover_inv=ci, overlap=overlap)
+        assert rel(gather(), want_e2) <= TOL[prec], overlap
 
 
 @pytest.mark.gpu
