@@ -47,6 +47,9 @@ def _c(a):
     return a
 
 
+REP_FUND, REP_ADJ, REP_SU3 = 0, 1, 2      # rep argument of dirac / hop / dirac_eo: link format of oracle.cpp link()
+
+
 def _vol(L):
     return int(L[0]) * int(L[1]) * int(L[2]) * int(L[3])
 

@@ -19,6 +19,7 @@
 //   spinor      [lex][spin 0..3][colour 0..N-1][re,im]
 //   fund gauge  [lex][mu][row][col][re,im]         (2x2 complex)
 //   adj gauge   [lex][mu][a][b]                    (3x3 real)
+//   rep-2 gauge [lex][mu][row][col][re,im]         (3x3 complex, e.g. SU(3) fundamental)
 //   dense site matrix (clover) [lex][8][8][re,im], row/col index = spin*2 + colour
 #include <complex>
 #include <cstring>
@@ -81,12 +82,19 @@ void gamma_matrices(cd G[4][4][4]) {
         }
 }
 
-// link U_mu(x) in the fermion representation as a complex NxN matrix
+// link U_mu(x) in the fermion representation as a complex NxN matrix.  rep 0: SU(2) fundamental (2x2 complex);
+// rep 1: SU(2) adjoint (3x3 real); rep 2: a complex 3x3 link per direction, e.g. SU(3) fundamental (PAPER.md:13, 21
+// "various gauge groups ... numbers of colors of 2 to 5") — O1-O3 are the same formulas, only
+// the colour matrix that multiplies the spinor changes.
 void link(int rep, const double* U, long x, int mu, cd M[3][3]) {
     if (rep == 0) {
         const cd* u = reinterpret_cast<const cd*>(U) + (x * 4 + mu) * 4;
         for (int r = 0; r < 2; ++r)
             for (int c = 0; c < 2; ++c) M[r][c] = u[r * 2 + c];
+    } else if (rep == 2) {
+        const cd* u = reinterpret_cast<const cd*>(U) + (x * 4 + mu) * 9;
+        for (int r = 0; r < 3; ++r)
+            for (int c = 0; c < 3; ++c) M[r][c] = u[r * 3 + c];
     } else {
         const double* u = U + (x * 4 + mu) * 9;
         for (int r = 0; r < 3; ++r)
@@ -273,7 +281,7 @@ void orc_gamma(double* G) {
     std::memcpy(G, g, sizeof(g));
 }
 
-// O1 on lex sites [begin, end): out[x] = D psi(x).  rep 0: fund (N=2), rep 1: adjoint (N=3).
+// O1 on lex sites [begin, end): out[x] = D psi(x).  rep 0: fund (N=2), rep 1: adjoint (N=3, real links), rep 2: N=3, complex links.
 // Contiguous output ranges are split over `nthreads` std::threads (SURVEY §8(d) CPU baseline).
 int orc_dirac(const int* L, int rep, double m0, const double* U, const double* psi, double* out,
               long begin, long end, int nthreads) {

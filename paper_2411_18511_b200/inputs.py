@@ -137,6 +137,31 @@ def unit_gauge(L) -> np.ndarray:
     return u
 
 
+def haar_su3(n: int, seed: int, field: int) -> np.ndarray:
+    """n Haar-random SU(3) matrices: QR of a complex Gaussian 3x3 matrix with the phases of R's diagonal moved into Q (Haar
+    on U(3)), then divided by a cube root of the determinant."""
+    out = np.empty((n, 3, 3), dtype=np.complex128)
+    for s, m in _chunks(n, 1 << 16):
+        z = normals(seed, field, 18 * s, 18 * m).reshape(m, 3, 3, 2)
+        q, r = np.linalg.qr(z[..., 0] + 1j * z[..., 1])
+        d = np.diagonal(r, axis1=-2, axis2=-1)
+        q = q * (d / np.abs(d))[:, None, :]
+        det = np.linalg.det(q)
+        out[s:s + m] = q / np.exp(1j * np.angle(det) / 3.0)[:, None, None]
+    return out
+
+
+def haar_gauge_su3(L, seed: int = 1) -> np.ndarray:
+    """SU(3) fundamental gauge field [V,4,3,3], Haar-random links (the rep-2 link format: complex 3 x 3)."""
+    V = volume(L)
+    return haar_su3(4 * V, seed, FIELD_GAUGE).reshape(V, 4, 3, 3)
+
+
+def haar_sites_su3(L, seed: int = 4) -> np.ndarray:
+    """One Haar SU(3) matrix per site [V,3,3] (a local gauge transformation g)."""
+    return haar_su3(volume(L), seed, FIELD_GAUGE_TRANSFORM)
+
+
 def haar_sites(L, seed: int = 4) -> np.ndarray:
     """One Haar SU(2) matrix per site [V,2,2] (a local gauge transformation g)."""
     return haar_su2(volume(L), seed, FIELD_GAUGE_TRANSFORM)

@@ -694,3 +694,61 @@ def test_P19_adjoint_exponential_clover(orc):
     assert 3.5 < ratio < 4.7          # quadratic in csw
     f0, i0 = orc.clover_exp_dense_adj(L, d, 0.0, R)
     assert np.abs(f0 - d * eye).max() <= 1e-14 and np.abs(i0 - eye / d).max() <= 1e-15
+
+
+# ---------------------------------------------------------------- P21: complex 3x3 links (rep 2, e.g. SU(3) fundamental)
+def test_P21_complex_3x3_links(orc):
+    """oracle rep 2 (complex 3 x 3 links, 3 complex colours): the same pins that hold
+    O1-O3 for SU(2) — P1 plane wave at U = 1, P2 gamma5-hermiticity, P3 gauge covariance under a random local SU(3)
+    transformation, P4 Schur identity, P9 hop = off-diagonal part of D, P14 an independent numpy restatement — and, as the
+    special case that ties the new link format to the pinned one, SU(2) links embedded in the upper-left 2 x 2 block of a
+    3 x 3 matrix (third colour decoupled): colours 0, 1 must reproduce the rep-0 operator, colour 2 the free one."""
+    L = (4, 4, 2, 6)
+    V = inputs.volume(L)
+    m0 = -0.2
+    d = 4.0 + m0
+    U = inputs.haar_gauge_su3(L, 1)
+    assert np.abs(U @ dagger(U) - np.eye(3)).max() < 1e-14 and np.abs(np.linalg.det(U) - 1.0).max() < 1e-13
+    psi = inputs.gaussian_spinor(L, 3, 2)
+    chi = inputs.gaussian_spinor(L, 3, 3, inputs.FIELD_SPINOR2)
+    D = lambda v, links=U: orc.dirac(L, 2, m0, links, v)
+    # P14: independent restatement (whole-lattice shifts, dense gamma matrices)
+    assert rel_l2(D(psi), wilson_dirac_numpy(L, U, psi, m0, GAM)) < 1e-14
+    # P2
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[None, :, None]
+    a, b = inner(chi, D(psi)), inner(g5 * D(g5 * chi), psi)
+    assert abs(a - b) <= 1e-14 * abs(a)
+    # P3: U^g_mu(x) = g(x) U_mu(x) g(x+mu)^dag, D[U^g](g psi) = g D[U] psi
+    g = inputs.haar_sites_su3(L, 4)
+    Ug = gauge_transform(U, g, L)
+    gpsi = np.einsum("xab,xsb->xsa", g, psi)
+    assert rel_l2(D(gpsi, Ug), np.einsum("xab,xsb->xsa", g, D(psi))) < 1e-14
+    # P9 + P4
+    par = inputs.site_parity(L)
+    even = (par == 0)[:, None, None]
+    eta = D(psi)
+    H = orc.hop(L, 2, 0, U, psi)
+    H = orc.hop(L, 2, 1, U, psi, out=H)
+    assert rel_l2(eta, d * psi - 0.5 * H) < 1e-14
+    rhs = eta * even + 0.5 / d * orc.hop(L, 2, 0, U, eta * ~even)
+    assert rel_l2(orc.dirac_eo(L, 2, m0, U, psi), rhs) < 1e-14
+    # P1: U = 1, plane wave
+    n = np.array([1, 0, 1, 2])
+    p = 2 * np.pi * n / np.array(L)
+    x = inputs.site_coords(L)
+    w = inputs.normals(5, 7, 0, 24).reshape(4, 3, 2)
+    w = w[..., 0] + 1j * w[..., 1]
+    wave = np.exp(1j * (x @ p))[:, None, None] * w[None]
+    one = np.broadcast_to(np.eye(3, dtype=np.complex128), (V, 4, 3, 3)).copy()
+    M = (m0 + np.sum(1 - np.cos(p))) * np.eye(4) + 1j * sum(np.sin(p[mu]) * GAM[mu] for mu in range(4))
+    want = np.exp(1j * (x @ p))[:, None, None] * np.einsum("st,tc->sc", M, w)[None]
+    assert rel_l2(orc.dirac(L, 2, m0, one, wave), want) < 1e-14
+    # embedded SU(2): block-diagonal links diag(U2, 1)
+    U2 = inputs.haar_gauge(L, 1)
+    emb = np.zeros((V, 4, 3, 3), dtype=np.complex128)
+    emb[..., :2, :2] = U2
+    emb[..., 2, 2] = 1.0
+    got = orc.dirac(L, 2, m0, emb, psi)
+    assert rel_l2(got[..., :2], orc.dirac(L, 0, m0, U2, np.ascontiguousarray(psi[..., :2]))) < 1e-14
+    free = orc.dirac(L, 2, m0, one, psi)
+    assert rel_l2(got[..., 2], free[..., 2]) < 1e-14
