@@ -21,6 +21,7 @@
  *         spinor        [V][4 spin][N colour][re,im]
  *         fund gauge    [V][4 mu][2 row][2 col][re,im]
  *         adj gauge     [V][4 mu][3 a][3 b]                       (real)
+ *         SU(3) gauge   [V][4 mu][3 row][3 col][re,im]            (HR_REP_SU3)
  *         clover blocks [V][2 chirality +,-][(2N)^2 reals]        one hermitian 2N x 2N block per chirality, N = 2 / 3
  *                        colours: 2N real diagonal entries, then the strictly-lower complex entries column by
  *                        column ((1,0) (2,0) .. (2N-1,0) (2,1) ..) as re,im — 16 reals (fundamental), 36 (adjoint);
@@ -41,7 +42,12 @@ extern "C" {
 
 enum { HR_OK = 0, HR_EINVAL = 1, HR_EUNSUPPORTED = 2, HR_EALIGN = 3, HR_ECUDA = 4 };
 
-enum { HR_REP_FUND = 0, HR_REP_ADJ = 1 };
+/* fermion representation / gauge group.  HR_REP_FUND and HR_REP_ADJ are the two SU(2) representations of BASELINE.json;
+ * HR_REP_SU3 is the first step towards HiRep's other gauge groups: 3 complex
+ * colours and complex 3 x 3 links stored in full (link_storage = HR_LINKS_FULL; canonical [V][4 mu][3][3][re,im]).  It is
+ * served by the generic hopping kernel: bare hops, full D, the even-odd operator without clover and the CG solvers; the
+ * clover, representation and sharded-hop calls return HR_EUNSUPPORTED for it. */
+enum { HR_REP_FUND = 0, HR_REP_ADJ = 1, HR_REP_SU3 = 2 };
 enum { HR_PREC_F64 = 0, HR_PREC_F32 = 1 };
 /* fundamental links are stored as their first row (alpha, beta): U = [[alpha, beta], [-conj(beta), conj(alpha)]]
  * is exact for SU(2).  HR_LINKS_FULL (all four entries) is declared for the byte model only and is

@@ -12,7 +12,7 @@ namespace hr {
 // hr_fields.cu
 int permute_chunks(bool pack, const Geo& g, int NI, int NCH, int SRC, const void* src, void* dst, cudaStream_t st);
 int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st);
-int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st);
+int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries = false);
 int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
@@ -70,6 +70,10 @@ static int check_ptr(const void* p, const char* name) {
     }
     return HR_OK;
 }
+static int check_no_su3(const hr_geom* g, const char* what) {
+    if (g->rep == HR_REP_SU3) { set_error("%s: not available for HR_REP_SU3 (bare hops, D, Dhat without clover and CG are)", what); return HR_EUNSUPPORTED; }
+    return HR_OK;
+}
 static int check_links(const hr_geom* g) {
     if (g->rep == HR_REP_FUND && g->link_storage != HR_LINKS_COMPRESSED) {
         set_error("HR_LINKS_FULL is a byte-model option only; kernels read HR_LINKS_COMPRESSED fundamental links");
@@ -105,11 +109,11 @@ size_t hr_spinor_bytes(const hr_geom* g, int parity) {
 }
 
 size_t hr_gauge_bytes(const hr_geom* g, int rep) {
-    if (!geom_ok(g) || (rep != HR_REP_FUND && rep != HR_REP_ADJ)) return 0;
+    if (!geom_ok(g) || (rep != HR_REP_FUND && rep != HR_REP_ADJ && rep != HR_REP_SU3)) return 0;
     const Geo geo = make_geo(g);
     const size_t links = 8 * (size_t)geo.Vh;
     if (rep == HR_REP_FUND) return links * link_chunks(g->prec) * 16;
-    return links * 9 * real_bytes(g->prec);
+    return links * (rep == HR_REP_SU3 ? 18 : 9) * real_bytes(g->prec);
 }
 
 size_t hr_clover_bytes(const hr_geom* g) {
@@ -125,9 +129,9 @@ size_t hr_canonical_spinor_bytes(const hr_geom* g) {
 }
 
 size_t hr_canonical_gauge_bytes(const hr_geom* g, int rep) {
-    if (!geom_ok(g) || (rep != HR_REP_FUND && rep != HR_REP_ADJ)) return 0;
+    if (!geom_ok(g) || (rep != HR_REP_FUND && rep != HR_REP_ADJ && rep != HR_REP_SU3)) return 0;
     const Geo geo = make_geo(g);
-    return 8 * (size_t)geo.Vh * (rep == HR_REP_FUND ? 8 : 9) * real_bytes(g->prec);
+    return 8 * (size_t)geo.Vh * (rep == HR_REP_FUND ? 8 : rep == HR_REP_SU3 ? 18 : 9) * real_bytes(g->prec);
 }
 
 size_t hr_canonical_clover_bytes(const hr_geom* g) {
@@ -156,6 +160,7 @@ int hr_pack_gauge(const hr_geom* g, int rep, const void* canon, void* dev, void*
         return permute_chunks(true, make_geo(g), 4, lch, 2 * lch, canon, dev, (cudaStream_t)stream);
     }
     if (rep == HR_REP_ADJ) return permute_adj(true, make_geo(g), g->prec, canon, dev, (cudaStream_t)stream);
+    if (rep == HR_REP_SU3) return permute_adj(true, make_geo(g), g->prec, canon, dev, (cudaStream_t)stream, true);
     set_error("unknown representation %d", rep);
     return HR_EINVAL;
 }
@@ -169,6 +174,7 @@ int hr_unpack_gauge(const hr_geom* g, int rep, const void* dev, void* canon, voi
         return rebuild_second_row(geo, g->prec, canon, (cudaStream_t)stream);
     }
     if (rep == HR_REP_ADJ) return permute_adj(false, make_geo(g), g->prec, dev, canon, (cudaStream_t)stream);
+    if (rep == HR_REP_SU3) return permute_adj(false, make_geo(g), g->prec, dev, canon, (cudaStream_t)stream, true);
     set_error("unknown representation %d", rep);
     return HR_EINVAL;
 }
@@ -185,7 +191,7 @@ int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* strea
 
 // ---------------------------------------------------------------- R1
 int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund")); HR_TRY(check_ptr(u_adj, "u_adj"));
+    HR_TRY(check_geom(g)); HR_TRY(check_no_su3(g, "hr_represent_gauge")); HR_TRY(check_ptr(u_fund, "u_fund")); HR_TRY(check_ptr(u_adj, "u_adj"));
     if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     return run_represent(make_geo(g), g->prec, u_fund, u_adj, (cudaStream_t)stream);
 }
@@ -203,7 +209,7 @@ int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, 
 }
 
 int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fwd, const void* psi, void* out, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_no_su3(g, "hr_dirac_clover_apply"));
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(psi, "psi")); HR_TRY(check_ptr(out, "out"));
     const size_t full = 2 * half_spinor_bytes(g);
     if (overlap(psi, full, out, full)) { set_error("hr_dirac_clover_apply: out aliases psi (gather operation)"); return HR_EINVAL; }
@@ -232,6 +238,7 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
     if (overlap(tmp, half, in, half) || overlap(tmp, half, out, half)) { set_error("hr_dirac_eo_apply: tmp aliases in or out"); return HR_EINVAL; }
     const bool clover = clover_fwd || clover_inv;
     if (clover) {
+        HR_TRY(check_no_su3(g, "hr_dirac_eo_apply with clover"));
         if (!clover_fwd || !clover_inv) { set_error("hr_dirac_eo_apply: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
         HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(clover_inv, "clover_inv"));
             // E2: tmp_o = A_oo^-1 H_oe in_e ;  out_e = A_ee in_e - 1/4 H_eo tmp_o
@@ -261,7 +268,7 @@ static int check_decomp(const hr_decomp* d) {
 }
 
 int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void* u, const void* in_half, void* const* face_out, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d)); HR_TRY(check_no_su3(g, "hr_halo_pack"));
     if (in_parity != HR_EVEN && in_parity != HR_ODD) { set_error("hr_halo_pack: in_parity %d", in_parity); return HR_EINVAL; }
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(in_half, "in_half"));
     if (!face_out) { set_error("hr_halo_pack: face_out is NULL"); return HR_EINVAL; }
@@ -273,7 +280,7 @@ int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void
 // phases: 1 = interior kernel, 2 = boundary kernels, 3 = both
 static int hop_local_phases(int phases, const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u,
                             const void* clover, const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d)); HR_TRY(check_no_su3(g, "hr_hop_local"));
     if (out_parity != HR_EVEN && out_parity != HR_ODD) { set_error("hr_hop_local: out_parity %d", out_parity); return HR_EINVAL; }
     if (epi < HR_EPI_NONE || epi > HR_EPI_CLOVER_AXPY) { set_error("hr_hop_local: unknown epilogue %d", epi); return HR_EINVAL; }
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(out_half, "out_half"));
@@ -317,7 +324,7 @@ int hr_hop_local_boundary(const hr_geom* g, const hr_decomp* d, int out_parity, 
 
 // ---------------------------------------------------------------- C1 / C2 / C3
 static int clover_build_any(const hr_geom* g, double m0, double csw, int expo, const void* u_fund, void* clover_fwd, void* clover_inv, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund"));
+    HR_TRY(check_geom(g)); HR_TRY(check_no_su3(g, "hr_clover_build")); HR_TRY(check_ptr(u_fund, "u_fund"));
     if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     if (!clover_fwd && !clover_inv) { set_error("hr_clover_build: nothing to build"); return HR_EINVAL; }
     if (4.0 + m0 == 0.0) { set_error("hr_clover_build: 4+m0 = 0"); return HR_EINVAL; }
@@ -338,7 +345,7 @@ int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_f
 }
 
 int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream) {
-    HR_TRY(check_geom(g));
+    HR_TRY(check_geom(g)); HR_TRY(check_no_su3(g, "hr_clover_apply"));
     if (parity < HR_EVEN || parity > HR_BOTH) { set_error("hr_clover_apply: parity %d", parity); return HR_EINVAL; }
     HR_TRY(check_ptr(blocks, "blocks")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
     return run_clover_apply(make_geo(g), g->rep, g->prec, parity, blocks, in, out, (cudaStream_t)stream);
@@ -363,6 +370,7 @@ int hr_cg_solve(const hr_geom* g, double m0, const void* u, const void* clover_f
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(b, "b")); HR_TRY(check_ptr(x, "x")); HR_TRY(check_ptr(workspace, "workspace"));
     if (!(tol > 0.0) || max_iter < 0 || check_every < 1) { set_error("hr_cg_solve: tol must be > 0, max_iter >= 0, check_every >= 1"); return HR_EINVAL; }
     if ((clover_fwd == nullptr) != (clover_inv == nullptr)) { set_error("hr_cg_solve: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
+    if (clover_fwd) HR_TRY(check_no_su3(g, "hr_cg_solve with clover"));
     const size_t half = half_spinor_bytes(g);
     if (overlap(b, half, x, half)) { set_error("hr_cg_solve: x aliases b"); return HR_EINVAL; }
     if (overlap(workspace, cg_workspace_bytes(g), x, half) || overlap(workspace, cg_workspace_bytes(g), b, half)) {
@@ -422,13 +430,14 @@ int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, doubl
     const double N = ncolour(g->rep), w = (double)real_bytes(g->prec);
     const double nr = 8.0 * N, S = nr * w;
     const double Gf = (g->link_storage != HR_LINKS_FULL ? 4.0 : 8.0) * w, Ga = 9.0 * w;
-    const double G = g->rep == HR_REP_FUND ? Gf : (g->link_storage == HR_LINKS_ONTHEFLY ? 4.0 * w : Ga);
+    const double G = g->rep == HR_REP_FUND ? Gf : g->rep == HR_REP_SU3 ? 18.0 * w : (g->link_storage == HR_LINKS_ONTHEFLY ? 4.0 * w : Ga);
     const double Bk = 2.0 * (2 * N) * (2 * N) * w;            // two hermitian 2N x 2N blocks per site
     // per direction: 4N adds to project, two colour mat-vecs, 8N adds to accumulate; x8, minus the first accumulate
     // (rebuilding R from the quaternion, ~30 flops per link, is not counted: the model counts the operator's flops)
-    const double Fhop = g->rep == HR_REP_FUND ? 8.0 * N * (16.0 * N + 7.0) : 8.0 * N * (8.0 * N + 7.0);
+    const double Fhop = g->rep != HR_REP_ADJ ? 8.0 * N * (16.0 * N + 7.0) : 8.0 * N * (8.0 * N + 7.0);   // complex links (624, SU(3): 1320) : real links (744)
     const double Fblk = 2.0 * (2.0 * (2 * N) + 8.0 * (2 * N) * (2 * N - 1));   // two hermitian 2N x 2N mat-vecs: 208 (fund), 504 (adj)
     double f = 0, bc = 0, br = 0;
+    if (g->rep == HR_REP_SU3 && (op == HR_OP_CLOVER || op == HR_OP_DHAT_CLOVER || op == HR_OP_REPRESENT)) return check_no_su3(g, "hr_dirac_flops_bytes of a clover / representation op");
     switch (op) {
         case HR_OP_HOP: f = Fhop; bc = 2 * S + 8 * G; br = 9 * S + 8 * G; break;
         case HR_OP_DIRAC: f = Fhop + 3 * nr; bc = 2 * S + 4 * G; br = 10 * S + 8 * G; break;

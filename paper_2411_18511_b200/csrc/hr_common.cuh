@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "../../include/hr_dslash.h"
 
 namespace hr {
@@ -31,7 +33,8 @@ inline bool geom_ok(const hr_geom* g) {
         if (g->L[m] < 2 || (g->L[m] & 1)) return false;
     double v = (double)g->L[0] * g->L[1] * g->L[2] * g->L[3];
     if (v > 2.0e9) return false;  // 32-bit site indices
-    if (g->rep != HR_REP_FUND && g->rep != HR_REP_ADJ) return false;
+    if (g->rep != HR_REP_FUND && g->rep != HR_REP_ADJ && g->rep != HR_REP_SU3) return false;
+    if (g->rep == HR_REP_SU3 && g->link_storage != HR_LINKS_FULL) return false;   // complex 3 x 3 links are stored in full
     if (g->prec != HR_PREC_F64 && g->prec != HR_PREC_F32) return false;
     if (g->link_storage != HR_LINKS_FULL && g->link_storage != HR_LINKS_COMPRESSED && g->link_storage != HR_LINKS_ONTHEFLY) return false;
     if (g->link_storage == HR_LINKS_ONTHEFLY && g->rep != HR_REP_ADJ) return false;
@@ -177,6 +180,8 @@ template <int NC> struct SiteIO<float, NC> {
 template <typename T, int N> struct Link;
 template <typename T> struct Link<T, 2> { cplx<T> a, b; };
 template <typename T> struct Link<T, 3> { T r[9]; };
+// complex 3 x 3 (HR_REP_SU3): row-major, m[3*row + col]
+template <typename T> struct LinkC3 { cplx<T> m[9]; };
 
 // chunk index of link (parity half `par`, direction mu, row, h): the gauge field is [par][mu][row][chunk][h]
 template <typename T, int POLICY>
@@ -215,6 +220,36 @@ __device__ __forceinline__ void load_link_rep(Link<T, 3>& u, const void* gauge, 
     u.r[0] = d + 2 * a1 * a1;          u.r[1] = 2 * (a1 * a2 + a0 * a3);  u.r[2] = 2 * (a1 * a3 - a0 * a2);
     u.r[3] = 2 * (a2 * a1 - a0 * a3);  u.r[4] = d + 2 * a2 * a2;          u.r[5] = 2 * (a2 * a3 + a0 * a1);
     u.r[6] = 2 * (a3 * a1 + a0 * a2);  u.r[7] = 2 * (a3 * a2 - a0 * a1);  u.r[8] = d + 2 * a3 * a3;
+}
+
+// complex 3 x 3 links: 9 complex planes per row, complex index (((par*4 + mu)*R + row)*9 + k)*L3h + h (128-bit loads in fp64, 64-bit in fp32)
+template <typename T, int POLICY, bool ONFLY>
+__device__ __forceinline__ void load_link_rep(LinkC3<T>& u, const void* gauge, const Geo& g, int par, int mu, int row, int h) {
+    typedef typename std::conditional<sizeof(T) == 8, double2, float2>::type pair_t;
+    const pair_t* p = reinterpret_cast<const pair_t*>(gauge) + ((size_t)(par * 4 + mu) * g.R + row) * (9 * g.L3h) + h;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const pair_t v = POLICY == LD_KEEP ? __ldg(p + (size_t)k * g.L3h) : __ldcs(p + (size_t)k * g.L3h);
+        u.m[k] = mk<T>(v.x, v.y);
+    }
+}
+template <typename T>
+__device__ __forceinline__ void mul_link(cplx<T>* chi, const LinkC3<T>& u, const cplx<T>* h) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        chi[a] = u.m[3 * a] * h[0];
+        cmad(chi[a], u.m[3 * a + 1], h[1]);
+        cmad(chi[a], u.m[3 * a + 2], h[2]);
+    }
+}
+template <typename T>
+__device__ __forceinline__ void mul_link_dag(cplx<T>* chi, const LinkC3<T>& u, const cplx<T>* h) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        chi[a] = conj(u.m[a]) * h[0];
+        cmadc(chi[a], u.m[3 + a], h[1]);
+        cmadc(chi[a], u.m[6 + a], h[2]);
+    }
 }
 
 // chi = U h  /  chi = U^dag h  on the colour index of one spin component
@@ -289,8 +324,8 @@ __device__ __forceinline__ void hop_project(cplx<T>* h0, cplx<T>* h1, const cplx
 // acc += the four spin components rebuilt from the link-multiplied half spinor (c0, c1)
 template <typename T, int N, int MU, bool FWD>
 __device__ __forceinline__ void hop_rebuild(cplx<T>* acc, const cplx<T>* c0, const cplx<T>* c1);
-template <typename T, int N, int MU, bool FWD>
-__device__ __forceinline__ void hop_apply(cplx<T>* acc, const cplx<T>* h0, const cplx<T>* h1, const Link<T, N>& u) {
+template <typename T, int N, int MU, bool FWD, typename LinkT>
+__device__ __forceinline__ void hop_apply(cplx<T>* acc, const cplx<T>* h0, const cplx<T>* h1, const LinkT& u) {
     cplx<T> c0[N], c1[N];
     if (FWD) { mul_link(c0, u, h0); mul_link(c1, u, h1); }
     else     { mul_link_dag(c0, u, h0); mul_link_dag(c1, u, h1); }
@@ -317,8 +352,8 @@ __device__ __forceinline__ void hop_rebuild(cplx<T>* acc, const cplx<T>* c0, con
         }
     }
 }
-template <typename T, int N, int MU, bool FWD>
-__device__ __forceinline__ void hop_term(cplx<T>* acc, const cplx<T>* p, const Link<T, N>& u) {
+template <typename T, int N, int MU, bool FWD, typename LinkT>
+__device__ __forceinline__ void hop_term(cplx<T>* acc, const cplx<T>* p, const LinkT& u) {
     cplx<T> h0[N], h1[N];
     hop_project<T, N, MU, FWD>(h0, h1, p);
     hop_apply<T, N, MU, FWD>(acc, h0, h1, u);

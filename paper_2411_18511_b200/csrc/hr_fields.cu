@@ -60,7 +60,8 @@ __global__ void rebuild_second_row_kernel(long long nlinks, T* canon) {
     u[6] = u[0]; u[7] = -u[1];
 }
 
-// adjoint links: canonical [lex][mu][9] reals <-> device [par][mu][row][9][h]
+// adjoint links: canonical [lex][mu][9] reals <-> device [par][mu][row][9][h]; the same permutation with T = double2 / float2
+// moves the 9 complex entries of an HR_REP_SU3 link
 template <typename T, bool PACK>
 __global__ void permute_adj_kernel(Geo g, const T* __restrict__ src, T* __restrict__ dst) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -95,10 +96,18 @@ int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st) {
     return check_launch("rebuild_second_row_kernel");
 }
 
-int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st) {
+int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries) {
     const long long total = 2LL * g.Vh * 36;
     const unsigned nb = blocks_for(total, 256);
-    if (prec == HR_PREC_F64) {
+    if (complex_entries) {
+        if (prec == HR_PREC_F64) {
+            if (pack) permute_adj_kernel<double2, true><<<nb, 256, 0, st>>>(g, (const double2*)src, (double2*)dst);
+            else permute_adj_kernel<double2, false><<<nb, 256, 0, st>>>(g, (const double2*)src, (double2*)dst);
+        } else {
+            if (pack) permute_adj_kernel<float2, true><<<nb, 256, 0, st>>>(g, (const float2*)src, (float2*)dst);
+            else permute_adj_kernel<float2, false><<<nb, 256, 0, st>>>(g, (const float2*)src, (float2*)dst);
+        }
+    } else if (prec == HR_PREC_F64) {
         if (pack) permute_adj_kernel<double, true><<<nb, 256, 0, st>>>(g, (const double*)src, (double*)dst);
         else permute_adj_kernel<double, false><<<nb, 256, 0, st>>>(g, (const double*)src, (double*)dst);
     } else {

@@ -23,6 +23,7 @@ static int sm_count() {   // of the calling thread's current device (cached per 
 }
 
 bool tiled_supported(const hr_geom* g) {
+    if (g->rep == HR_REP_SU3) return false;     // complex 3 x 3 links: generic kernel only
     TiledPlan pl;
     return tiled_plan(g, 0, 148, pl);     // (whether a tile shape fits does not depend on the SM count)
 }
@@ -59,7 +60,7 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
     TiledPlan pl;
     // a hop with cut directions (hr_hop_local): tiled open-boundary kernel for the fundamental representation, else generic
     const bool open_ok = a.open_mask == 0 || (g->rep == HR_REP_FUND && !a.both);
-    const bool fits = g->kernel != HR_KERNEL_GENERIC && open_ok && tiled_plan(g, a.both, sm_count(), pl);
+    const bool fits = g->kernel != HR_KERNEL_GENERIC && g->rep != HR_REP_SU3 && open_ok && tiled_plan(g, a.both, sm_count(), pl);
     if (g->kernel == HR_KERNEL_TILED && !fits && open_ok) {
         set_error("HR_KERNEL_TILED: lattice %dx%dx%dx%d does not fit the tiled kernel", g->L[0], g->L[1], g->L[2], g->L[3]);
         return HR_EUNSUPPORTED;
@@ -84,6 +85,10 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
         }
         if (g->prec == HR_PREC_F64) return launch_hop_tiled<double, 3>(geo, a, epi, pl, st);
         return launch_hop_tiled<float, 3>(geo, a, epi, pl, st);
+    }
+    if (g->rep == HR_REP_SU3) {
+        if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 3, false, true>(geo, a, epi, st);
+        return launch_hop_generic<float, 3, false, true>(geo, a, epi, st);
     }
     if (g->rep == HR_REP_FUND) {
         if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 2>(geo, a, epi, st);

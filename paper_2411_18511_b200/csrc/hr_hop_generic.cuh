@@ -69,8 +69,11 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
     IO::store(out_half, first, g.L3h, acc);
 }
 
-template <typename T, int N, int EPI, bool ONFLY>
+// C3: the links are complex 3 x 3 matrices stored in full (HR_REP_SU3; N = 3)
+template <typename T, int N, int EPI, bool ONFLY, bool C3 = false>
 __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
+    static_assert(!C3 || (N == 3 && !ONFLY), "complex 3 x 3 links: N = 3, stored");
+    typedef typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type link_t;
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
@@ -106,7 +109,7 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
 #define HR_HOP_DIR(MU, ROWF, HF, ROWB, HB, ATHI, ATLO)                                          \
     {                                                                                           \
         cplx<T> nb[NC];                                                                         \
-        Link<T, N> u;                                                                           \
+        link_t u;                                                                               \
         if (!(((om >> MU) & 1) && (ATHI))) {                                                    \
             load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, p, MU, row, h);                   \
             IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWF) * rowlen + (HF), stride);    \
@@ -127,14 +130,15 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row, h);
 }
 
-template <typename T, int N, bool ONFLY = false>
+template <typename T, int N, bool ONFLY = false, bool C3 = false>
 inline int launch_hop_generic(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
     dim3 block(128), grid((g.Vh + 127) / 128, a.both ? 2 : 1);
+    if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
     switch (epi) {
-        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE, ONFLY><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY, ONFLY><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE, ONFLY, C3><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY, ONFLY, C3><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY, false><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false><<<grid, block, 0, st>>>(g, a); break;
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
     count_launch();

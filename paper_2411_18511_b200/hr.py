@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libhr_dslash.so")
 
 OK, EINVAL, EUNSUPPORTED, EALIGN, ECUDA = 0, 1, 2, 3, 4
-REP_FUND, REP_ADJ = 0, 1
+REP_FUND, REP_ADJ, REP_SU3 = 0, 1, 2
 PREC_F64, PREC_F32 = 0, 1
 LINKS_FULL, LINKS_COMPRESSED, LINKS_ONTHEFLY = 0, 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED = 0, 1, 2

@@ -12,10 +12,12 @@ from . import hr
 
 class Lattice:
     def __init__(self, L, rep=hr.REP_FUND, prec=hr.PREC_F64, kernel=hr.KERNEL_AUTO, device=None,
-                 link_storage=hr.LINKS_COMPRESSED):
+                 link_storage=None):
         self.L = tuple(int(v) for v in L)
         self.V = int(np.prod(self.L))
         self.N = 2 if rep == hr.REP_FUND else 3
+        if link_storage is None:      # SU(2): first-row compressed fundamental links; SU(3): complex 3 x 3 links in full
+            link_storage = hr.LINKS_FULL if rep == hr.REP_SU3 else hr.LINKS_COMPRESSED
         self.g = hr.geom(self.L, rep, prec, link_storage, kernel)
         self.device = hr.current_device() if device is None else device     # every buffer of this object lives here
         self.real = hr.np_real(self.g)
@@ -71,6 +73,19 @@ class Lattice:
         dev = self.empty_gauge(hr.REP_ADJ)
         hr.hr_pack_gauge(self.g, hr.REP_ADJ, canon, dev, hr.stream_ptr())
         return dev
+
+    def put_gauge_su3(self, U):
+        """complex [V,4,3,3] -> device layout of HR_REP_SU3 links (stored in full)"""
+        assert U.shape == (self.V, 4, 3, 3), U.shape
+        canon = hr.upload(U.astype(self.cplx), self.device)
+        dev = self.empty_gauge(hr.REP_SU3)
+        hr.hr_pack_gauge(self.g, hr.REP_SU3, canon, dev, hr.stream_ptr())
+        return dev
+
+    def get_gauge_su3(self, dev):
+        canon = hr.device_buffer(hr.hr_canonical_gauge_bytes(self.g, hr.REP_SU3), self.device)
+        hr.hr_unpack_gauge(self.g, hr.REP_SU3, dev, canon, hr.stream_ptr())
+        return hr.download(canon, self.cplx, (self.V, 4, 3, 3))
 
     def get_gauge_adj(self, dev):
         canon = hr.device_buffer(hr.hr_canonical_gauge_bytes(self.g, hr.REP_ADJ), self.device)

@@ -188,3 +188,16 @@ def test_lattice_stages_on_its_own_device(monkeypatch):
     lat.put_gauge_adj(np.zeros((256, 4, 3, 3)))
     lat.put_clover(np.zeros((256, 2, 36)))
     assert len(seen) == 8 and all(dev == "cuda:3" for _, dev in seen), seen
+
+
+def test_su3_geometry_and_sizes(L):
+    """HR_REP_SU3: complex 3 x 3 links stored in full (18 reals per link), 3 complex colours; other link storages are rejected"""
+    g = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_FULL)
+    V = 4 * 4 * 4 * 8
+    assert hr.hr_spinor_bytes(g, hr.BOTH) == V * 24 * 8
+    assert hr.hr_gauge_bytes(g, hr.REP_SU3) == hr.hr_canonical_gauge_bytes(g, hr.REP_SU3) == 4 * V * 18 * 8
+    assert hr.hr_dirac_flops_bytes(g, hr.OP_DHAT) == (2 * 1320.0 + 72.0, 5 * 192.0 + 16 * 144.0, 19 * 192.0 + 16 * 144.0)
+    bad = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_COMPRESSED)
+    assert hr.hr_spinor_bytes(bad, hr.BOTH) == 0
+    with pytest.raises(hr.HrError):
+        hr.hr_dirac_flops_bytes(g, hr.OP_CLOVER)

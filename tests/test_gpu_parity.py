@@ -872,3 +872,37 @@ def test_clover_inverse_of_indefinite_blocks(hr, orc):
     inv.view(torch.float64)[77] = float("inf")
     hr.hr_clover_count_nonfinite(lat.g, inv, count, hr.stream_ptr())
     assert int(count.item()) == 2
+
+
+# ------------------------------------------------------------------ complex 3 x 3 links (HR_REP_SU3)
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (6, 2, 4, 12)])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_su3_small_lattices(hr, orc, L, prec):
+    """Haar SU(3) links, 3 complex colours: pack/unpack round trip, bare hops, full D, Dhat and the CG solver against the
+    oracle's rep-2 operators (pinned by P21); the clover / sharded calls refuse the representation"""
+    import torch
+    m0 = -0.2
+    U = rounded(inputs.haar_gauge_su3(L, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
+    lat = lattice(hr, L, hr.REP_SU3, prec)
+    assert hr.hr_kernel_name(lat.g) == "generic"
+    U_dev = lat.put_gauge_su3(U)
+    assert np.array_equal(lat.get_gauge_su3(U_dev), U.astype(lat.cplx))
+    want = oracle_ops(orc, L, 2, U, psi, m0)
+    got = gpu_ops(hr, lat, U_dev, psi, m0)
+    for k in want:
+        assert rel(got[k], want[k]) <= TOL[prec], k
+    f, bc, _ = hr.hr_dirac_flops_bytes(lat.g, hr.OP_HOP)
+    w = 8 if prec == 0 else 4
+    assert f == 1320.0 and bc == 2 * 24 * w + 8 * 18 * w
+    with pytest.raises(hr.HrError):
+        lat.clover_build(m0, 1.0, U_dev)
+    if prec == 0 and L == (4, 4, 4, 4):
+        b = psi.copy()
+        b[inputs.site_parity(L) == 1] = 0
+        x_orc, it_orc, _ = orc.cg_normal(L, 2, m0, U, b, tol=1e-12, max_iter=500, nthreads=NTHREADS)
+        b_dev = lat.put_spinor(b)
+        x_half, it, relres = lat.cg(m0, U_dev, lat.even(b_dev), 1e-12, 500, check_every=1)
+        full = torch.zeros_like(b_dev)
+        lat.even(full).copy_(x_half)
+        assert relres <= 1e-12 and abs(it - it_orc) <= 2 and rel(lat.get_spinor(full), x_orc) <= 1e-9
