@@ -1,7 +1,7 @@
 """In-tree nvcc build of libhr_dslash.so for sm_100a (no torch extension machinery: the library is a
 plain C-ABI shared object, include/hr_dslash.h).
 
-    python -m paper_2411_18511_b200.build [--force] [--verbose]        (env HR_NVCC_DEFS: extra -D switches)
+    python -m paper_2411_18511_b200.build [--force] [--verbose]
 """
 from __future__ import annotations
 
@@ -49,7 +49,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-    flags += os.environ.get("HR_NVCC_DEFS", "").split()   # tuning switches of csrc/hr_hop_tiled.cuh, e.g. "-DHR_T_PIN_F64=1"
 
     def compile_one(src):
         obj = os.path.join(objdir, src.replace(".cu", ".o"))

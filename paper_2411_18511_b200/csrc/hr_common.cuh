@@ -121,13 +121,10 @@ template <int POLICY> __device__ __forceinline__ float ldg_real(const float* p) 
     if (POLICY != LD_KEEP) return __ldcs(p);
     return __ldg(p);
 }
-#ifdef HR_STORE_PLAIN
-__device__ __forceinline__ void stg16_stream(double2* p, double2 v) { *p = v; }
-__device__ __forceinline__ void stg16_stream(float4* p, float4 v) { *p = v; }
-#else
+// outputs are written once and not read again by the same kernel: streaming stores (plain stores measured 2-25 % slower,
+// profiles/r01_tiled_variants.md)
 __device__ __forceinline__ void stg16_stream(double2* p, double2 v) { __stcs(p, v); }
 __device__ __forceinline__ void stg16_stream(float4* p, float4 v) { __stcs(p, v); }
-#endif
 
 __device__ __forceinline__ void chunk_to_reals(double2 v, double* e) { e[0] = v.x; e[1] = v.y; }
 __device__ __forceinline__ void chunk_to_reals(float4 v, float* e) { e[0] = v.x; e[1] = v.y; e[2] = v.z; e[3] = v.w; }

@@ -23,7 +23,7 @@ struct HopArgs {
     const void* clover;  // full-lattice block field (EPI_CLOVER_*)
     double a, c;
     int parity;          // output parity when both == 0
-    int both;            // 1: gridDim.y == 2 and blockIdx.y is the output parity (full D in one launch)
+    int both;            // 1: full-lattice launch, both output parities (in / out / phi are full fields)
     int open_mask = 0;   // bit mu set: direction mu is cut between ranks (hr_hop_local): the forward term of sites with
                          // x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out here and added from
                          // the received faces by the boundary kernel (hr_halo.cu)
@@ -70,19 +70,24 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
 }
 
 // C3: the links are complex 3 x 3 matrices stored in full (HR_REP_SU3; N = 3)
-template <typename T, int N, int EPI, bool ONFLY, bool C3 = false>
+template <typename T, int N, int EPI, bool ONFLY, bool C3 = false, bool BOTH = false>
 __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     static_assert(!C3 || (N == 3 && !ONFLY), "complex 3 x 3 links: N = 3, stored");
     typedef typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type link_t;
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
-    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    // full-lattice launch: the output parity is the fastest-varying part of blockIdx.x, so the two CTAs that use a link
+    // (forward term of parity p, backward term of parity 1-p at the neighbouring sites) run next to each other and the second
+    // use hits L2 — links and phi are then loaded at normal priority (BOTH), else streamed
+    const int bid = BOTH ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+    const int cb = bid * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
-    const int p = a.both ? (int)blockIdx.y : a.parity;
+    const int p = BOTH ? (int)(blockIdx.x & 1) : a.parity;
+    constexpr int LINKPOL = BOTH ? LD_KEEP : LD_STREAM;
     const size_t half_bytes = (size_t)g.Vh * IO::NCH * 16;
-    const char* in_half = reinterpret_cast<const char*>(a.in) + (a.both ? (size_t)(1 - p) * half_bytes : 0);
-    char* out_half = reinterpret_cast<char*>(a.out) + (a.both ? (size_t)p * half_bytes : 0);
-    const char* phi_half = a.phi ? reinterpret_cast<const char*>(a.phi) + (a.both ? (size_t)p * half_bytes : 0) : nullptr;
+    const char* in_half = reinterpret_cast<const char*>(a.in) + (BOTH ? (size_t)(1 - p) * half_bytes : 0);
+    char* out_half = reinterpret_cast<char*>(a.out) + (BOTH ? (size_t)p * half_bytes : 0);
+    const char* phi_half = a.phi ? reinterpret_cast<const char*>(a.phi) + (BOTH ? (size_t)p * half_bytes : 0) : nullptr;
 
     const int row = cb / g.L3h, h = cb - row * g.L3h;
     const int x0 = row / g.s0, rem = row - x0 * g.s0;
@@ -111,12 +116,12 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
         cplx<T> nb[NC];                                                                         \
         link_t u;                                                                               \
         if (!(((om >> MU) & 1) && (ATHI))) {                                                    \
-            load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, p, MU, row, h);                   \
+            load_link_rep<T, LINKPOL, ONFLY>(u, a.gauge, g, p, MU, row, h);                     \
             IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWF) * rowlen + (HF), stride);    \
             hop_term<T, N, MU, true>(acc, nb, u);                                               \
         }                                                                                       \
         if (!(((om >> MU) & 1) && (ATLO))) {                                                    \
-            load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, 1 - p, MU, ROWB, HB);             \
+            load_link_rep<T, LINKPOL, ONFLY>(u, a.gauge, g, 1 - p, MU, ROWB, HB);               \
             IO::template load<LD_KEEP>(nb, in_half, (size_t)(ROWB) * rowlen + (HB), stride);    \
             hop_term<T, N, MU, false>(acc, nb, u);                                              \
         }                                                                                       \
@@ -127,22 +132,28 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     HR_HOP_DIR(3, row, h_f3, row, h_b3, r == 1 && h == g.L3h - 1, r == 0 && h == 0)
 #undef HR_HOP_DIR
 
-    hop_epilogue<T, N, EPI>(acc, g, a, phi_half, out_half, p, row, h);
+    hop_epilogue<T, N, EPI, (BOTH ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row, h);
 }
 
-template <typename T, int N, bool ONFLY = false, bool C3 = false>
-inline int launch_hop_generic(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
-    dim3 block(128), grid((g.Vh + 127) / 128, a.both ? 2 : 1);
+template <typename T, int N, bool ONFLY, bool C3, bool BOTH>
+inline int launch_hop_generic_both(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
+    dim3 block(128), grid(((g.Vh + 127) / 128) * (BOTH ? 2 : 1));
     if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
     switch (epi) {
-        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE, ONFLY, C3><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY, ONFLY, C3><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY, false><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY, false, BOTH><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false, BOTH><<<grid, block, 0, st>>>(g, a); break;
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
     count_launch();
     return check_launch("hop_generic_kernel");
+}
+
+template <typename T, int N, bool ONFLY = false, bool C3 = false>
+inline int launch_hop_generic(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
+    if (a.both) return launch_hop_generic_both<T, N, ONFLY, C3, true>(g, a, epi, st);
+    return launch_hop_generic_both<T, N, ONFLY, C3, false>(g, a, epi, st);
 }
 
 }  // namespace hr
