@@ -906,3 +906,30 @@ def test_su3_small_lattices(hr, orc, L, prec):
         full = torch.zeros_like(b_dev)
         lat.even(full).copy_(x_half)
         assert relres <= 1e-12 and abs(it - it_orc) <= 2 and rel(lat.get_spinor(full), x_orc) <= 1e-9
+
+
+def test_48to4_host_batch_on_sampled_sites(hr, orc, big_inputs):
+    """the gauge-resident host path at the bench size: hr_gauge_upload_host + hr_apply_host_batch of 3 right-hand sides (full D
+    and Dhat, fp64) at 48^4, checked on sampled sites against the oracle's per-site operator"""
+    import torch
+    L, U, psi = big_inputs
+    m0 = -0.2
+    lat = lattice(hr, L, 0, 0)
+    g, st = lat.g, hr.stream_ptr()
+    Uh = torch.from_numpy(U).pin_memory()
+    u_dev = lat.empty_gauge(hr.REP_FUND)
+    ws = hr.device_buffer(max(hr.hr_host_batch_workspace_bytes(g), hr.hr_canonical_gauge_bytes(g, hr.REP_FUND)))
+    hr.hr_gauge_upload_host(g, hr.REP_FUND, Uh, u_dev, ws, st)
+    V = inputs.volume(L)
+    ins = [torch.from_numpy(psi).pin_memory(), torch.from_numpy(np.ascontiguousarray(psi[::-1])).pin_memory(), torch.from_numpy(1j * psi).pin_memory()]
+    outs = [torch.empty_like(a).pin_memory() for a in ins]
+    sites = np.unique(np.concatenate([np.array([0, 1, 47, 48, V - 1, V - 48, V // 2 + 5]), (inputs.normals(9, 9, 0, 40) * 1e9).astype(np.int64) % V]))
+    hr.hr_apply_host_batch(g, hr.HOST_DIRAC, m0, u_dev, None, None, ins, outs, ws, st)
+    for a, o in zip(ins, outs):
+        want = orc.dirac_sites(L, 0, m0, U, a.numpy(), sites)
+        assert rel(o.numpy()[sites], want) <= 1e-13
+    hr.hr_apply_host_batch(g, hr.EO_HOP_OE, m0, u_dev, None, None, ins[:2], outs[:2], ws, st)
+    odd = sites[inputs.site_parity(L)[sites] == 1]
+    for a, o in zip(ins[:2], outs[:2]):
+        assert rel(o.numpy()[odd], orc.hop_sites(L, 0, U, a.numpy(), odd)) <= 1e-13
+        assert not o.numpy()[sites[inputs.site_parity(L)[sites] == 0]].any()
