@@ -436,6 +436,25 @@ def other_configs(hr, inputs, Lattice):
                                                                     "frac": round(bc * sites / ms / 1e6 / peak, 4), "bytes_per_site": bc,
                                                                     "kernel": hr.hr_kernel_name(g)}
             del Uf_dev, U_dev, p_dev, o_dev, tmp
+    # the sharded hop on this one GPU: a 48^4 local lattice whose four directions are all cut onto the rank itself;
+    # pack + device-to-device face copies + interior kernel + boundary kernels per hop o<-e, in order and with pack / copies
+    # on a side stream (no multi-GPU hardware in this run: this measures what a cut costs a rank, not the transport)
+    from paper_2411_18511_b200 import halo
+    for prec, ptag in ((hr.PREC_F64, "f64"), (hr.PREC_F32, "f32")):
+        lat = Lattice(L, hr.REP_FUND, prec, hr.KERNEL_AUTO)
+        g = lat.g
+        U_dev = torch.randn(hr.hr_gauge_bytes(g, hr.REP_FUND) // 4, device="cuda").view(torch.uint8)
+        p_dev = torch.randn(hr.hr_spinor_bytes(g, hr.BOTH) // 4, device="cuda").view(torch.uint8)
+        o_dev = lat.empty_spinor()
+        for split in ((1, 0, 0, 0), (1, 1, 1, 1)):
+            sh = halo.Shard(lat, (1, 1, 1, 1), (0, 0, 0, 0), split)
+            shards, Ud, ind, outd = {(0, 0, 0, 0): sh}, {(0, 0, 0, 0): U_dev}, {(0, 0, 0, 0): lat.even(p_dev)}, {(0, 0, 0, 0): lat.odd(o_dev)}
+            ms_seq = timed(lambda: halo.hop_all(shards, halo.exchange_in_process, hr.ODD, Ud, ind, outd), 20)
+            ms_ovl = timed(lambda: halo.hop_all(shards, halo.exchange_in_process, hr.ODD, Ud, ind, outd, overlap=True), 20)
+            out["sharded_hop_48^4_local_%dcuts_%s" % (sum(split), ptag)] = {
+                "us_in_order": round(ms_seq * 1e3, 1), "us_overlapped": round(ms_ovl * 1e3, 1),
+                "face_bytes": hr.hr_halo_face_bytes(g, 0), "faces_per_hop": 2 * sum(split), "interior_kernel": hr.hr_kernel_name(g)}
+        del U_dev, p_dev, o_dev
     return out
 
 
