@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--L 48]
 
 One "step" = the fp64 Dslash group of BASELINE.json configs[3] over one 48^4 lattice of synthetic seeded fields (Haar
-links, Gaussian spinors), inputs resident in HBM:  H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat  (6 kernel launches).
+links, Gaussian spinors), inputs resident in HBM:  H1 hop o<-e, H1 hop e<-o, H3 full D, E1 Dhat  (5 kernel launches: Dhat is two hops).
 `value` = compulsory (algorithmic) bytes of the step (hr_dirac_flops_bytes) / step time, in GB/s — the paper's
 bandwidth metric; `dtype` = "f64".  The same four operators in fp32 and the clover / represent rows
 (configs[4]: C2, C3, E2, H3c, R1) are timed right after, K steps each, and reported under `roofline.fp32_step`,
@@ -277,7 +277,7 @@ def run_ours(args):
     hop_ms = 0.5 * (op_ms["hop_oe_f64"] + op_ms["hop_eo_f64"])
     hop_bytes = model["hop_oe_f64"]["bytes"]
     achieved = hop_bytes / hop_ms / 1e6
-    roofline = {"bound": "hbm", "kernel": "parity hop fp64 (%s): 4 of the 6 launches of the step and %d%% of its time" % (
+    roofline = {"bound": "hbm", "kernel": "parity hop fp64 (%s): 4 of the 5 launches of the step and %d%% of its time" % (
                     kname, round(100 * (op_ms["hop_oe_f64"] + op_ms["hop_eo_f64"] + op_ms["dhat_f64"]) / sum(ms64))),
                 "achieved": round(achieved, 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
                 "frac_of_datasheet_8000": round(achieved / 8000.0, 4), "bytes_per_launch": hop_bytes, "avg_launch_ms": round(hop_ms, 4),

@@ -3,7 +3,7 @@
 //
 // Same pipeline as hop_tiled_kernel (hr_hop_tiled.cuh): a producer thread moves whole x3-rows of the input field into
 // shared memory with 1-D bulk asynchronous copies that complete on mbarriers; consumer threads gather from there.
-// What differs, and why (profiles/r02_dirac_tiled.md):
+// What differs, and why (profiles/r02_kernels.md):
 //   * A consumer thread owns a spatial column (x1, x2, x3) and keeps it for the whole march, so the parity of its site
 //     alternates from plane to plane.  Its own spinors are then the x0 neighbours of its own sites: psi(x0+1) is read
 //     from shared memory once and serves three steps from registers — as the forward neighbour, as the axpy operand
@@ -25,7 +25,7 @@ namespace hr {
 // Buffers: DT_RING ring slots hold planes x0, x0+1 and two planes in flight; DT_HALO halo buffers hold the halo of the
 // centre plane and one in flight.  Deeper halo buffering (3 buffers, with a 3- or 4-slot ring) measured slower in both
 // precisions: above ~196 KiB of shared memory the L1 that the link loads go through is too small
-// (profiles/r02_dirac_tiled.md).
+// (profiles/r02_kernels.md).
 constexpr int DT_RING = 4;
 constexpr int DT_HALO = 2;
 
