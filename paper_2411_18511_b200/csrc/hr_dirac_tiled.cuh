@@ -11,9 +11,14 @@
 //     step after.  Per output site that is 7 spinor reads from shared memory instead of 9 + a global phi read.
 //   * The link U_0(x) is used by the forward term at x and by the backward term at x+0 — the same thread one step
 //     later: it stays in registers (7 link loads per site instead of 8).
-//   * Plane x0-1 is never read from shared memory, so a 4-slot ring holds planes x0, x0+1 and TWO planes in flight;
-//     the halo rows (x1 and x2 neighbours of the tile edge, centre plane only) have their own double buffer and their
-//     own mbarriers so that they do not hold the plane copies back.
+//   * The other seven links of a site do NOT travel through registers: each thread owns seven slots in shared memory that it
+//     fills with cp.async and re-requests right after use (ALINK, see cp_async16 below) — a register load requested a step
+//     ahead is in fact waited for together with every later global load of the warp (one scoreboard).
+//   * Plane x0-1 is never read from shared memory: the ring holds planes x0, x0+1 and the plane(s) in flight (3 slots with
+//     ALINK, 4 without); the halo rows (x1 and x2 neighbours of the tile edge, centre plane only) have their own buffers
+//     and their own mbarriers so that they do not hold the plane copies back, and are requested before the plane.
+//   * The eight terms run x0-1, x3+-, [halo wait] x1+-, x2+-, x0+1, and the neighbour of term t+1 is read from shared memory
+//     before term t is computed (two register images).
 //   * Every plane and halo buffer holds the even and the odd half-rows ([parity][row]); both uses of a link happen in
 //     the same CTA in the same step, so the second one hits L1/L2 and DRAM sees every link once.
 #pragma once
@@ -22,12 +27,15 @@
 
 namespace hr {
 
-// Buffers: DT_RING ring slots hold planes x0, x0+1 and two planes in flight; DT_HALO halo buffers hold the halo of the
-// centre plane and one in flight.  Deeper halo buffering (3 buffers, with a 3- or 4-slot ring) measured slower in both
-// precisions: above ~196 KiB of shared memory the L1 that the link loads go through is too small
-// (profiles/r02_kernels.md).
+// Buffers with the links in registers (ALINK = false, the form for rows too long for the link slots): DT_RING ring slots hold
+// planes x0, x0+1 and two planes in flight, DT_HALO halo buffers the halo of the centre plane and one in flight; more than
+// ~196 KiB of shared memory then starves the L1 the link loads go through (profiles/r02_kernels.md).
 constexpr int DT_RING = 4;
 constexpr int DT_HALO = 2;
+// With the links in shared-memory slots (ALINK) nothing goes through L1 and all 227 KiB can be used: 3 planes + 2 halo buffers +
+// link slots in fp64 (211 KiB at L3 = 48), 3 planes + 3 halo buffers + link slots in fp32 (223 KiB).
+__host__ __device__ constexpr int dt_ring(bool alink, size_t real_bytes) { return alink ? 3 : DT_RING; }
+__host__ __device__ constexpr int dt_nhalo(bool alink, size_t real_bytes) { return (alink && real_bytes == 4) ? 3 : DT_HALO; }
 
 // consumer threads the kernel is compiled for: one per site of a T1 x T2 tile of full x3-rows of up to 48 sites
 constexpr int dt_max_consumers(int t1, int t2) { return t1 * t2 * 48; }
@@ -38,16 +46,100 @@ struct DiracPlan {
     int nseg, seglen;  // x0 segments per tile and their length
     int nconsumer;     // consumer threads: 2 * (T1*T2*L3h rounded up to a warp)
     int rowb;          // bytes of one x3-row of one parity
+    int alink;         // links through cp.async slots in shared memory (else in registers)
     size_t smem;
 };
+
+// Links through shared memory.  A load into registers that is requested one step ahead does not get a step of lead: ptxas puts
+// every global load of the loop on ONE scoreboard, so the first use of a link at the top of a step waits for ALL outstanding link
+// loads, the ones requested a few hundred instructions earlier included, and a DRAM latency is exposed in every step (18-24 % of the
+// stall samples, profiles/r02_kernels.md).  cp.async groups complete in order and cp.async.wait_group N waits for all but the N
+// newest: each link has its own slot (32 bytes fp64, 16 bytes fp32), is re-requested into it right after its use, and is waited
+// for with N = 6 — exactly the seven-requests-ago one.  A thread reads only slots it filled itself, so no barrier is needed.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING> __device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory");
+}
+
+// (alpha, beta) of a compressed link from its slot; volatile keeps the reads behind the wait_group
+__device__ __forceinline__ void lds_link(cplx<double>* ab, uint32_t slot, int chunk_stride) {
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(ab[0].re), "=d"(ab[0].im) : "r"(slot));
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(ab[1].re), "=d"(ab[1].im) : "r"(slot + chunk_stride));
+}
+__device__ __forceinline__ void lds_link(cplx<float>* ab, uint32_t slot, int) {
+    asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ab[0].re), "=f"(ab[0].im), "=f"(ab[1].re), "=f"(ab[1].im) : "r"(slot));
+}
+
+// The producer of the full-lattice kernels (one thread): per iteration the T1 x T2 tile rows of plane j, both parity images, into
+// ring slot j % DT_RING and the halo rows of centre plane j - HLAG into halo buffer (pc-1) % DT_HALO; waits on the slot's "empty"
+// mbarrier, arms its "full" mbarrier with the byte count.  Shared by dirac_tiled_kernel and dirac_split_kernel (hr_dirac_split.cuh).
+template <int T1, int T2, int RING, int NHALO>
+__device__ __forceinline__ void dirac_producer(const char* in, size_t half_bytes, char* ring, char* halo, int rowb, uint32_t bar_full,
+                                               uint32_t bar_empty, uint32_t bar_hfull, uint32_t bar_hempty, int t1, int t2, int xs,
+                                               int nsteps, int L0, int L1, int L2) {
+    constexpr int TR = T1 * T2, HR = 2 * T2 + 2 * T1;
+    const int planeb = 2 * TR * rowb, halob = 2 * HR * rowb;
+    const int x1base = t1 * T1, x2base = t2 * T2;
+    const int x1lo = (x1base - 1 + L1) % L1, x1hi = (x1base + T1) % L1;
+    const int x2lo = (x2base - 1 + L2) % L2, x2hi = (x2base + T2) % L2;
+    // plane P can be requested once plane P - RING is dead (after step P - RING - 1), the halo of centre Pc once
+    // that of centre Pc - NHALO is (after step Pc - NHALO - 1): iteration j issues plane j and the halo of centre
+    // j - (RING - NHALO), which become free at the same time
+    constexpr int HLAG = RING - NHALO;
+    static_assert(HLAG >= 0 && HLAG <= RING - 2, "iterations up to the request of the halo of plane 1 must not wait for a consumer");
+    for (int j = 0; j < nsteps + 2 + HLAG; ++j) {
+        const int pc = j - HLAG;   // halo of a centre plane (the planes 1..nsteps are centres)
+        if (pc >= 1 && pc <= nsteps) {
+            const int hb = (pc - 1) % NHALO;
+            mbar_wait(bar_hempty + 8 * hb, (((uint32_t)(pc - 1) / NHALO) & 1) ^ 1);
+            const uint32_t full = bar_hfull + 8 * hb;
+            mbar_expect_tx(full, (uint32_t)halob);
+            const int x0h = (xs - 1 + pc + L0) % L0;
+#pragma unroll
+            for (int pp = 0; pp < 2; ++pp) {
+                const char* src = in + pp * half_bytes;
+                const uint32_t hd = smem_u32(halo + hb * halob + pp * HR * rowb);
+                bulk_g2s(hd, src + (((size_t)x0h * L1 + x1lo) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
+                bulk_g2s(hd + T2 * rowb, src + (((size_t)x0h * L1 + x1hi) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
+#pragma unroll
+                for (int aa = 0; aa < T1; ++aa) {
+                    const size_t rb = ((size_t)x0h * L1 + x1base + aa) * L2;
+                    bulk_g2s(hd + (2 * T2 + aa) * rowb, src + (rb + x2lo) * rowb, (uint32_t)rowb, full);
+                    bulk_g2s(hd + (2 * T2 + T1 + aa) * rowb, src + (rb + x2hi) * rowb, (uint32_t)rowb, full);
+                }
+            }
+        }
+        if (j < nsteps + 2) {   // plane P = j
+            const int slot = j % RING;
+            mbar_wait(bar_empty + 8 * slot, (((uint32_t)j / RING) & 1) ^ 1);
+            const uint32_t full = bar_full + 8 * slot;
+            mbar_expect_tx(full, (uint32_t)planeb);
+            const int x0p = (xs - 1 + j + L0) % L0;
+#pragma unroll
+            for (int pp = 0; pp < 2; ++pp) {
+                const uint32_t dst = smem_u32(ring + slot * planeb + pp * TR * rowb);
+#pragma unroll
+                for (int aa = 0; aa < T1; ++aa) {
+                    const size_t row = ((size_t)x0p * L1 + x1base + aa) * L2 + x2base;
+                    bulk_g2s(dst + aa * T2 * rowb, in + pp * half_bytes + row * rowb, (uint32_t)(T2 * rowb), full);
+                }
+            }
+        }
+    }
+}
 
 // grid.x = nt1 * nt2 * nseg.  Shared memory: [16 mbarriers][DT_RING planes][DT_HALO halo buffers],
 //   plane: [parity 0,1][T1*T2 rows];  halo buffer: [parity 0,1][x1-1 line: T2 rows][x1+T1 line: T2][x2-1: T1][x2+T2: T1]
 // Plane index P = x0 - xs + 1 (P = 0 is the plane below the segment, read once in the prologue), ring slot P % DT_RING;
 // the halo of centre plane P sits in halo buffer (P-1) % NHALO.
-template <typename T, int T1, int T2, int L3H>
+// ALINK: links through cp.async slots in shared memory (see above) instead of registers; the fp64 form then has a 3-slot ring.
+template <typename T, int T1, int T2, int L3H, bool ALINK>
 __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_kernel(Geo g_in, HopArgs a, DiracPlan pl) {
     constexpr int N = 2, NC = 8;
+    constexpr int RING = dt_ring(ALINK, sizeof(T)), NHALO = dt_nhalo(ALINK, sizeof(T));
     typedef SiteIO<T, NC> IO;
     constexpr int TR = T1 * T2, HR = 2 * T2 + 2 * T1;
     constexpr int LP = LD_KEEP;   // both uses of a link are in this CTA: keep the line for the second one
@@ -58,18 +150,19 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
     char* ring = smem + 128;
     const int rowb = L3H > 0 ? IO::NCH * L3H * 16 : pl.rowb;
     const int planeb = 2 * TR * rowb, halob = 2 * HR * rowb;
-    char* halo = ring + DT_RING * planeb;
-    static_assert(DT_RING >= 3 && DT_RING <= 4 && DT_HALO >= 2 && DT_HALO <= 4, "16 mbarriers: 4 + 4 + 4 + 4");
-    const uint32_t bar_full = smem_u32(bars);          // [DT_RING]
-    const uint32_t bar_empty = smem_u32(bars + 4);     // [DT_RING]
-    const uint32_t bar_hfull = smem_u32(bars + 8);     // [DT_HALO]
-    const uint32_t bar_hempty = smem_u32(bars + 12);   // [DT_HALO]
+    char* halo = ring + RING * planeb;
+    char* lbuf = halo + NHALO * halob;   // ALINK: link slots [link][chunk][consumer thread]
+    static_assert(RING >= 3 && RING <= 4 && NHALO >= 2 && NHALO <= 4, "16 mbarriers: 4 + 4 + 4 + 4");
+    const uint32_t bar_full = smem_u32(bars);          // [RING]
+    const uint32_t bar_empty = smem_u32(bars + 4);     // [RING]
+    const uint32_t bar_hfull = smem_u32(bars + 8);     // [NHALO]
+    const uint32_t bar_hempty = smem_u32(bars + 12);   // [NHALO]
 
     const int tid = threadIdx.x;
     const int ncw = pl.nconsumer >> 5;
     if (tid == 0) {
-        for (int i = 0; i < DT_RING; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, ncw); }
-        for (int i = 0; i < DT_HALO; ++i) { mbar_init(bar_hfull + 8 * i, 1); mbar_init(bar_hempty + 8 * i, ncw); }
+        for (int i = 0; i < RING; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, ncw); }
+        for (int i = 0; i < NHALO; ++i) { mbar_init(bar_hfull + 8 * i, 1); mbar_init(bar_hempty + 8 * i, ncw); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -86,53 +179,7 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
     if (tid >= pl.nconsumer) {
         // ================================================================ producer (one thread)
         if (tid != pl.nconsumer) return;
-        const int x1base = t1 * T1, x2base = t2 * T2;
-        const int x1lo = (x1base - 1 + L1) % L1, x1hi = (x1base + T1) % L1;
-        const int x2lo = (x2base - 1 + L2) % L2, x2hi = (x2base + T2) % L2;
-        // plane P can be requested once plane P - DT_RING is dead (after step P - DT_RING - 1), the halo of centre Pc once
-        // that of centre Pc - DT_HALO is (after step Pc - DT_HALO - 1): iteration j issues plane j and the halo of centre
-        // j - (DT_RING - DT_HALO), which become free at the same time
-        constexpr int HLAG = DT_RING - DT_HALO;
-        static_assert(HLAG >= 0 && HLAG <= DT_RING - 2, "iterations up to the request of the halo of plane 1 must not wait for a consumer");
-        for (int j = 0; j < nsteps + 2 + HLAG; ++j) {
-            if (j < nsteps + 2) {   // plane P = j
-                const int slot = j % DT_RING;
-                mbar_wait(bar_empty + 8 * slot, (((uint32_t)j / DT_RING) & 1) ^ 1);
-                const uint32_t full = bar_full + 8 * slot;
-                mbar_expect_tx(full, (uint32_t)planeb);
-                const int x0p = (xs - 1 + j + L0) % L0;
-#pragma unroll
-                for (int pp = 0; pp < 2; ++pp) {
-                    const uint32_t dst = smem_u32(ring + slot * planeb + pp * TR * rowb);
-#pragma unroll
-                    for (int aa = 0; aa < T1; ++aa) {
-                        const size_t row = ((size_t)x0p * L1 + x1base + aa) * L2 + x2base;
-                        bulk_g2s(dst + aa * T2 * rowb, in + pp * half_bytes + row * rowb, (uint32_t)(T2 * rowb), full);
-                    }
-                }
-            }
-            const int pc = j - HLAG;   // halo of a centre plane (the planes 1..nsteps are centres)
-            if (pc >= 1 && pc <= nsteps) {
-                const int hb = (pc - 1) % DT_HALO;
-                mbar_wait(bar_hempty + 8 * hb, (((uint32_t)(pc - 1) / DT_HALO) & 1) ^ 1);
-                const uint32_t full = bar_hfull + 8 * hb;
-                mbar_expect_tx(full, (uint32_t)halob);
-                const int x0h = (xs - 1 + pc + L0) % L0;
-#pragma unroll
-                for (int pp = 0; pp < 2; ++pp) {
-                    const char* src = in + pp * half_bytes;
-                    const uint32_t hd = smem_u32(halo + hb * halob + pp * HR * rowb);
-                    bulk_g2s(hd, src + (((size_t)x0h * L1 + x1lo) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
-                    bulk_g2s(hd + T2 * rowb, src + (((size_t)x0h * L1 + x1hi) * L2 + x2base) * rowb, (uint32_t)(T2 * rowb), full);
-#pragma unroll
-                    for (int aa = 0; aa < T1; ++aa) {
-                        const size_t rb = ((size_t)x0h * L1 + x1base + aa) * L2;
-                        bulk_g2s(hd + (2 * T2 + aa) * rowb, src + (rb + x2lo) * rowb, (uint32_t)rowb, full);
-                        bulk_g2s(hd + (2 * T2 + T1 + aa) * rowb, src + (rb + x2hi) * rowb, (uint32_t)rowb, full);
-                    }
-                }
-            }
-        }
+        dirac_producer<T1, T2, RING, NHALO>(in, half_bytes, ring, halo, rowb, bar_full, bar_empty, bar_hfull, bar_hempty, t1, t2, xs, nsteps, L0, L1, L2);
         return;
     }
 
@@ -165,9 +212,43 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
 
     // ---- prologue: psi(xs) of this column, the projected psi(xs-1), U_0(xs-1), the links of the first step
     cplx<T> psic[NC], hb0[N], hb1[N];
-    Link<T, N> uf[4], ub[4];    // ub[0] = U_0(x - 0): carried over from the previous step's uf[0]
+    Link<T, N> ul[ALINK ? 1 : 7], ub0;    // ub0 = U_0(x - 0): the U_0(x) of the previous step; ul: the seven others when they live in registers
+    // link j of this site: 0..5 = U_1(x), U_1(x-1), U_2(x), U_2(x-2), U_3(x), U_3(x-3); 6 = U_0(x)
+    constexpr int LCH = SiteIO<T, 2>::NCH;                     // 16-byte chunks of a compressed link
+    const uint32_t lslot = smem_u32(lbuf) + (uint32_t)tid * 16;
+    const int lchb = pl.nconsumer * 16;                        // one chunk of one link for all consumer threads
+    auto link_request = [&](int j, int par, int mu, int row, int hh) {
+        if constexpr (ALINK) {
+            const char* src = reinterpret_cast<const char*>(a.gauge) + (((size_t)(par * 4 + mu) * g.R + row) * (LCH * L3h) + hh) * 16;
+#pragma unroll
+            for (int c = 0; c < LCH; ++c) cp_async16(lslot + (j * LCH + c) * lchb, src + (size_t)c * cs);
+            cp_async_commit();
+        } else {
+            load_link_rep<T, LP, false>(ul[j], a.gauge, g, par, mu, row, hh);
+        }
+    };
+    auto link_get = [&](Link<T, N>& u, int j) {
+        if constexpr (ALINK) {
+            cp_async_wait<6>();      // all but the six newest requests have landed: slot j has
+            cplx<T> ab[2];
+            lds_link(ab, lslot + j * LCH * lchb, lchb);
+            u.a = ab[0];
+            u.b = ab[1];
+        } else {
+            u = ul[j];
+        }
+    };
     {
         const int p0 = (xs + x1 + x2 + q) & 1;
+        const int row = row0 + xs * g.s0;
+        link_request(0, p0, 3, row, h);
+        link_request(1, 1 - p0, 3, row, hb3);
+        link_request(2, p0, 1, row, h);
+        link_request(3, 1 - p0, 1, rowb1_0 + xs * g.s0, h);
+        link_request(4, p0, 2, row, h);
+        link_request(5, 1 - p0, 2, rowb2_0 + xs * g.s0, h);
+        link_request(6, p0, 0, row, h);
+        load_link_rep<T, LP, false>(ub0, a.gauge, g, 1 - p0, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
         mbar_wait(bar_full, 0);
         mbar_wait(bar_full + 8, 0);
         cplx<T> below[NC];
@@ -176,71 +257,64 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
         lds_site<T, NC>(psic, ring + planeb + p0 * pimg + off_c, cs);
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(bar_empty);
-        const int row = row0 + xs * g.s0;
-        load_link_rep<T, LP, false>(ub[0], a.gauge, g, 1 - p0, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
-        load_link_rep<T, LP, false>(uf[0], a.gauge, g, p0, 0, row, h);
-        load_link_rep<T, LP, false>(uf[1], a.gauge, g, p0, 1, row, h);
-        load_link_rep<T, LP, false>(ub[1], a.gauge, g, 1 - p0, 1, rowb1_0 + xs * g.s0, h);
-        load_link_rep<T, LP, false>(uf[2], a.gauge, g, p0, 2, row, h);
-        load_link_rep<T, LP, false>(ub[2], a.gauge, g, 1 - p0, 2, rowb2_0 + xs * g.s0, h);
-        load_link_rep<T, LP, false>(uf[3], a.gauge, g, p0, 3, row, h);
-        load_link_rep<T, LP, false>(ub[3], a.gauge, g, 1 - p0, 3, row, hb3);
     }
 
     for (int k = 0; k < nsteps; ++k) {
         const int x0 = xs + k;
         const int p = (x0 + x1 + x2 + q) & 1;
-        const char* scur = ring + ((k + 1) % DT_RING) * planeb + (1 - p) * pimg;     // neighbours live in the other parity's image
-        const char* snext = ring + ((k + 2) % DT_RING) * planeb + (1 - p) * pimg;
-        const int hbuf = k % DT_HALO;
+        const char* scur = ring + ((k + 1) % RING) * planeb + (1 - p) * pimg;     // neighbours live in the other parity's image
+        const char* snext = ring + ((k + 2) % RING) * planeb + (1 - p) * pimg;
+        const int hbuf = k % NHALO;
         const char* shalo = halo + hbuf * halob + (1 - p) * himg;
         // next step's plane and parity (clamped on the last step: the reload is then harmless and unused)
         const int xn = (k + 1 < nsteps) ? x0 + 1 : x0;
         const int pn = (xn + x1 + x2 + q) & 1;
         const int rown = row0 + xn * g.s0;
 
-        // Eight terms: x0-1 from registers, the x1 / x2 / x3 neighbours from the centre plane and its halo rows, last x0+1
-        // from the newest plane (doing the x3 terms before the halo wait measured slower).  Each link is re-loaded for the
-        // next step right after its use; __syncwarp() keeps ptxas from sinking those loads to the end of the step.
-        cplx<T> acc[NC], nb[NC];
+        // Eight terms: x0-1 from registers, x3+- from the centre plane, then (halo wait) x1+-, x2+- from the centre plane and its halo
+        // rows, last x0+1 from the newest plane.  Each link is re-requested for the next step right after its use.
+        cplx<T> acc[NC], nb[NC], nb2[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[c] = mk<T>((T)0, (T)0);
-        hop_apply<T, N, 0, false>(acc, hb0, hb1, ub[0]);
-        mbar_wait(bar_hfull + 8 * hbuf, ((uint32_t)k / DT_HALO) & 1);
-        lds_site<T, NC>(nb, (f1_in ? scur : shalo) + off_f1, cs);
-        hop_term<T, N, 1, true>(acc, nb, uf[1]);
-        load_link_rep<T, LP, false>(uf[1], a.gauge, g, pn, 1, rown, h);
-        __syncwarp();
-        lds_site<T, NC>(nb, (b1_in ? scur : shalo) + off_b1, cs);
-        hop_term<T, N, 1, false>(acc, nb, ub[1]);
-        load_link_rep<T, LP, false>(ub[1], a.gauge, g, 1 - pn, 1, rowb1_0 + xn * g.s0, h);
-        __syncwarp();
-        lds_site<T, NC>(nb, (f2_in ? scur : shalo) + off_f2, cs);
-        hop_term<T, N, 2, true>(acc, nb, uf[2]);
-        load_link_rep<T, LP, false>(uf[2], a.gauge, g, pn, 2, rown, h);
-        __syncwarp();
-        lds_site<T, NC>(nb, (b2_in ? scur : shalo) + off_b2, cs);
-        hop_term<T, N, 2, false>(acc, nb, ub[2]);
-        load_link_rep<T, LP, false>(ub[2], a.gauge, g, 1 - pn, 2, rowb2_0 + xn * g.s0, h);
-        __syncwarp();
+        Link<T, N> u;
+        // the neighbour of term t+1 is read from shared memory before term t is computed (two register images)
         lds_site<T, NC>(nb, scur + off_f3, cs);
-        hop_term<T, N, 3, true>(acc, nb, uf[3]);
-        load_link_rep<T, LP, false>(uf[3], a.gauge, g, pn, 3, rown, h);
-        __syncwarp();
-        lds_site<T, NC>(nb, scur + off_b3, cs);
-        hop_term<T, N, 3, false>(acc, nb, ub[3]);
-        load_link_rep<T, LP, false>(ub[3], a.gauge, g, 1 - pn, 3, rown, hb3);
-        __syncwarp();
-        // x0+1: this column's own spinor of the next plane — needed only now, so its copy had the whole step to land
-        mbar_wait(bar_full + 8 * ((k + 2) % DT_RING), ((uint32_t)(k + 2) / DT_RING) & 1);
+        hop_apply<T, N, 0, false>(acc, hb0, hb1, ub0);
+        lds_site<T, NC>(nb2, scur + off_b3, cs);
+        link_get(u, 0);
+        hop_term<T, N, 3, true>(acc, nb, u);
+        link_request(0, pn, 3, rown, h);
+        mbar_wait(bar_hfull + 8 * hbuf, ((uint32_t)k / NHALO) & 1);
+        lds_site<T, NC>(nb, (f1_in ? scur : shalo) + off_f1, cs);
+        link_get(u, 1);
+        hop_term<T, N, 3, false>(acc, nb2, u);
+        link_request(1, 1 - pn, 3, rown, hb3);
+        lds_site<T, NC>(nb2, (b1_in ? scur : shalo) + off_b1, cs);
+        link_get(u, 2);
+        hop_term<T, N, 1, true>(acc, nb, u);
+        link_request(2, pn, 1, rown, h);
+        lds_site<T, NC>(nb, (f2_in ? scur : shalo) + off_f2, cs);
+        link_get(u, 3);
+        hop_term<T, N, 1, false>(acc, nb2, u);
+        link_request(3, 1 - pn, 1, rowb1_0 + xn * g.s0, h);
+        lds_site<T, NC>(nb2, (b2_in ? scur : shalo) + off_b2, cs);
+        link_get(u, 4);
+        hop_term<T, N, 2, true>(acc, nb, u);
+        link_request(4, pn, 2, rown, h);
+        // x0+1: this column's own spinor of the next plane — its copy had two steps to land
+        mbar_wait(bar_full + 8 * ((k + 2) % RING), ((uint32_t)(k + 2) / RING) & 1);
         lds_site<T, NC>(nb, snext + off_c, cs);
-        hop_term<T, N, 0, true>(acc, nb, uf[0]);
-        ub[0] = uf[0];
-        load_link_rep<T, LP, false>(uf[0], a.gauge, g, pn, 0, rown, h);
+        link_get(u, 5);
+        hop_term<T, N, 2, false>(acc, nb2, u);
+        link_request(5, 1 - pn, 2, rowb2_0 + xn * g.s0, h);
+        link_get(u, 6);
+        hop_term<T, N, 0, true>(acc, nb, u);
+        ub0 = u;
+        link_request(6, pn, 0, rown, h);
         // the centre plane and its halo are consumed
         __syncwarp();
         if ((tid & 31) == 0) {
-            mbar_arrive(bar_empty + 8 * ((k + 1) % DT_RING));
+            mbar_arrive(bar_empty + 8 * ((k + 1) % RING));
             mbar_arrive(bar_hempty + 8 * hbuf);
         }
         // out = (4+m0) psi(x) - 1/2 H psi(x)
@@ -254,10 +328,11 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
 #pragma unroll
         for (int c = 0; c < NC; ++c) psic[c] = nb[c];
     }
+    if constexpr (ALINK) cp_async_wait<0>();   // the unused requests of the last step must not outlive the CTA
 }
 
 // ------------------------------------------------------------------ host side
-inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, DiracPlan& pl) {
+inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, DiracPlan& pl, bool alink = true) {
     const Geo g = make_geo(hg);
     const int L1 = hg->L[1], L2 = hg->L[2], L0 = hg->L[0];
     if (L1 % t1 || L2 % t2) return false;
@@ -268,8 +343,11 @@ inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, Dir
     pl.nconsumer = 2 * ((sites + 31) & ~31);
     if (pl.nconsumer > dt_max_consumers(t1, t2)) return false;
     pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
-    pl.smem = 128 + (size_t)pl.rowb * 2 * (DT_RING * t1 * t2 + DT_HALO * (2 * t1 + 2 * t2));
-    if (pl.smem > TILED_SMEM_LIMIT) return false;
+    pl.alink = alink ? 1 : 0;
+    const int ring = dt_ring(alink, real_bytes(hg->prec)), nhalo = dt_nhalo(alink, real_bytes(hg->prec));
+    pl.smem = 128 + (size_t)pl.rowb * 2 * (ring * t1 * t2 + nhalo * (2 * t1 + 2 * t2)) +
+              (alink ? (size_t)7 * link_chunks(hg->prec) * 16 * pl.nconsumer : 0);
+    if (pl.smem > TILED_SMEM_LIMIT) return alink ? dirac_plan_shape(hg, num_sms, t1, t2, pl, false) : false;
     pl.nt1 = L1 / t1;
     pl.nt2 = L2 / t2;
     pl.nseg = tiled_segments(L0, (long)pl.nt1 * pl.nt2, num_sms > 0 ? num_sms : 148);
@@ -278,15 +356,15 @@ inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, Dir
 }
 
 // fundamental representation only: 2 x 2 rows in fp64, 2 x 4 in fp32 (rows half as long)
-inline bool dirac_plan(const hr_geom* hg, int num_sms, DiracPlan& pl) {
+inline bool dirac_plan(const hr_geom* hg, int num_sms, DiracPlan& pl, bool alink = true) {
     if (hg->rep != HR_REP_FUND) return false;
-    if (hg->prec == HR_PREC_F32 && dirac_plan_shape(hg, num_sms, 2, 4, pl)) return true;
-    return dirac_plan_shape(hg, num_sms, 2, 2, pl);
+    if (hg->prec == HR_PREC_F32 && dirac_plan_shape(hg, num_sms, 2, 4, pl, alink)) return true;
+    return dirac_plan_shape(hg, num_sms, 2, 2, pl, alink);
 }
 
-template <typename T, int T1, int T2, int L3H>
+template <typename T, int T1, int T2, int L3H, bool ALINK>
 inline int launch_dirac_tiled_l3h(const Geo& g, const HopArgs& a, const DiracPlan& pl, cudaStream_t st) {
-    auto kern = dirac_tiled_kernel<T, T1, T2, L3H>;
+    auto kern = dirac_tiled_kernel<T, T1, T2, L3H, ALINK>;
     static std::atomic<unsigned char> configured[64];
     const int rc = opt_in_shared_memory(reinterpret_cast<const void*>(kern), configured, "dirac_tiled_kernel");
     if (rc != HR_OK) return rc;
@@ -295,16 +373,20 @@ inline int launch_dirac_tiled_l3h(const Geo& g, const HopArgs& a, const DiracPla
     return check_launch("dirac_tiled_kernel");
 }
 
-template <typename T>
-inline int launch_dirac_tiled(const Geo& g, const HopArgs& a, const DiracPlan& pl, cudaStream_t st) {
+template <typename T, bool ALINK>
+inline int launch_dirac_tiled_a(const Geo& g, const HopArgs& a, const DiracPlan& pl, cudaStream_t st) {
     if constexpr (sizeof(T) == 4) {
         if (pl.t1 == 2 && pl.t2 == 4) {
-            if (g.L3h == 24) return launch_dirac_tiled_l3h<T, 2, 4, 24>(g, a, pl, st);
-            return launch_dirac_tiled_l3h<T, 2, 4, 0>(g, a, pl, st);
+            if (g.L3h == 24) return launch_dirac_tiled_l3h<T, 2, 4, 24, ALINK>(g, a, pl, st);
+            return launch_dirac_tiled_l3h<T, 2, 4, 0, ALINK>(g, a, pl, st);
         }
     }
-    if (g.L3h == 24) return launch_dirac_tiled_l3h<T, 2, 2, 24>(g, a, pl, st);
-    return launch_dirac_tiled_l3h<T, 2, 2, 0>(g, a, pl, st);
+    if (g.L3h == 24) return launch_dirac_tiled_l3h<T, 2, 2, 24, ALINK>(g, a, pl, st);
+    return launch_dirac_tiled_l3h<T, 2, 2, 0, ALINK>(g, a, pl, st);
+}
+template <typename T>
+inline int launch_dirac_tiled(const Geo& g, const HopArgs& a, const DiracPlan& pl, cudaStream_t st) {
+    return pl.alink ? launch_dirac_tiled_a<T, true>(g, a, pl, st) : launch_dirac_tiled_a<T, false>(g, a, pl, st);
 }
 
 }  // namespace hr

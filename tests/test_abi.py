@@ -208,9 +208,9 @@ def test_kernel_plan_of_the_bench_lattice(L):
     g64 = hr.geom((48,) * 4, hr.REP_FUND, hr.PREC_F64)
     g32 = hr.geom((48,) * 4, hr.REP_FUND, hr.PREC_F32)
     assert hr.hr_kernel_plan(g64, hr.OP_HOP) == {"kernel": 1, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 224, "smem": 172160, "grid": 288}
-    assert hr.hr_kernel_plan(g64, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 2, "nseg": 1, "seglen": 48, "threads": 224, "smem": 196736, "grid": 576}
+    assert hr.hr_kernel_plan(g64, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 2, "nseg": 1, "seglen": 48, "threads": 224, "smem": 215168, "grid": 576}
     assert hr.hr_kernel_plan(g32, hr.OP_HOP)["grid"] == 144 and hr.hr_kernel_plan(g32, hr.OP_HOP)["t1"] == 4
-    assert hr.hr_kernel_plan(g32, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 416, "smem": 172160, "grid": 288}
+    assert hr.hr_kernel_plan(g32, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 416, "smem": 227456, "grid": 288}
     # below 32^4 and for adjoint / SU(3) fermions AUTO keeps the generic kernel
     assert hr.hr_kernel_plan(hr.geom((16,) * 4), hr.OP_HOP)["kernel"] == 0
     assert hr.hr_kernel_plan(hr.geom((48,) * 4, hr.REP_ADJ), hr.OP_HOP)["kernel"] == 0
