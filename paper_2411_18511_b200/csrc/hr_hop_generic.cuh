@@ -24,6 +24,7 @@ struct HopArgs {
     double a, c;
     int parity;          // output parity when both == 0
     int both;            // 1: full-lattice launch, both output parities (in / out / phi are full fields)
+    int slab_w1 = 0;     // > 0: the generic kernel walks the lattice in x1-slabs of this width (launch_hop_generic sets it)
     int open_mask = 0;   // bit mu set: direction mu is cut between ranks (hr_hop_local): the forward term of sites with
                          // x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out here and added from
                          // the received faces by the boundary kernel (hr_halo.cu)
@@ -89,7 +90,21 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     char* out_half = reinterpret_cast<char*>(a.out) + (BOTH ? (size_t)p * half_bytes : 0);
     const char* phi_half = a.phi ? reinterpret_cast<const char*>(a.phi) + (BOTH ? (size_t)p * half_bytes : 0) : nullptr;
 
-    const int row = cb / g.L3h, h = cb - row * g.L3h;
+    // Site order.  Default: checkerboard index = (row, h) with row = (x0 L1 + x1) L2 + x2.  With slabs (full-lattice launches on
+    // lattices whose x0-plane does not stay in L2 between its uses as x0-1, x0 and x0+1 neighbour): slab of x1 first, then x0, then
+    // the rows of the slab — the reuse distance along x0 shrinks from a plane to a slab of it.
+    int row, h;
+    if (a.slab_w1 > 0) {
+        const int slab_rows = a.slab_w1 * g.s1, slab_plane = slab_rows * g.L3h, per_slab = g.L0 * slab_plane;
+        const int sl = cb / per_slab, r0 = cb - sl * per_slab;
+        const int xx0 = r0 / slab_plane, r1 = r0 - xx0 * slab_plane;
+        const int lrow = r1 / g.L3h;
+        h = r1 - lrow * g.L3h;
+        row = xx0 * g.s0 + sl * slab_rows + lrow;
+    } else {
+        row = cb / g.L3h;
+        h = cb - row * g.L3h;
+    }
     const int x0 = row / g.s0, rem = row - x0 * g.s0;
     const int x1 = rem / g.s1, x2 = rem - x1 * g.s1;
     const int r = (x0 + x1 + x2 + p) & 1;  // x3 = 2h + r
@@ -135,8 +150,23 @@ __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
     hop_epilogue<T, N, EPI, (BOTH ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row, h);
 }
 
+// x1-slab width for the generic kernel's site order (0 = plain order): full-lattice launches whose two live x0-planes (both
+// parities, spinors + links + output) exceed what L2 keeps; the widest divisor of L1 whose slab fits (profiles/r02_adjoint.md)
+inline int generic_slab_w1(const Geo& g, bool both, size_t site_bytes) {
+    if (!both) return 0;
+    const int L1 = g.s0 / g.s1;
+    const double plane = 2.0 * 2.0 * (double)g.s0 * g.L3h * site_bytes;      // two planes, two parities
+    if (plane <= 64e6) return 0;          // half of L2: the plain order already gets the x0 neighbours from L2
+    int best = 1;                          // 48^4 adjoint fp64: widths 8-12 are best (915 -> 815 us), 16+ lose again
+    for (int w = 1; w < L1; ++w)
+        if (L1 % w == 0 && plane * w / L1 <= 40e6) best = w;
+    return best;
+}
+
 template <typename T, int N, bool ONFLY, bool C3, bool BOTH>
-inline int launch_hop_generic_both(const Geo& g, const HopArgs& a, int epi, cudaStream_t st) {
+inline int launch_hop_generic_both(const Geo& g, const HopArgs& a_in, int epi, cudaStream_t st) {
+    HopArgs a = a_in;
+    a.slab_w1 = generic_slab_w1(g, BOTH, (size_t)(16 * N + 4 * (C3 ? 18 : ONFLY ? 4 : N == 2 ? 4 : 9)) * sizeof(T));
     dim3 block(128), grid(((g.Vh + 127) / 128) * (BOTH ? 2 : 1));
     if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
     switch (epi) {

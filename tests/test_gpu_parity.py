@@ -277,6 +277,29 @@ def test_config2_24to4_adjoint(hr, orc):
             assert rel(got[k], want[k]) <= 1e-13, (k, kernel, "on the fly")
 
 
+def test_48to4_adjoint_full_lattice_slab_order(hr, orc):
+    """adjoint fermions at 48^4 (the paper's local volume): the full-lattice launch of the generic kernel walks the
+    lattice in x1-slabs there (hr_hop_generic.cuh: generic_slab_w1).  Full D with stored and with on-the-fly links against the
+    oracle's per-site operator on sampled sites that include both sides of every slab boundary and the lattice corners."""
+    L, m0 = (48, 48, 48, 48), -0.3
+    Uf = inputs.haar_gauge(L, 1)
+    psi = inputs.gaussian_spinor(L, 3, 2)
+    R, _ = orc.represent(Uf)
+    V = inputs.volume(L)
+    lex = lambda x0, x1, x2, x3: ((x0 * 48 + x1) * 48 + x2) * 48 + x3
+    fixed = [lex(x0, x1, x2, x3) for x0 in (0, 17, 47) for x1 in (0, 5, 7, 8, 11, 12, 15, 16, 23, 24, 35, 36, 47) for (x2, x3) in ((0, 0), (47, 47), (20, 31))]
+    sites = np.unique(np.concatenate([np.array(fixed), (inputs.normals(11, 9, 0, 60) * 1e9).astype(np.int64) % V]))
+    want = orc.dirac_sites(L, 1, m0, R, psi, sites)
+    from paper_2411_18511_b200.lattice import Lattice
+    lat = Lattice(L, hr.REP_ADJ, hr.PREC_F64, hr.KERNEL_AUTO)
+    assert hr.hr_kernel_plan(lat.g, hr.OP_DIRAC)["kernel"] == 0          # the generic kernel
+    got = lat.get_spinor(lat.dirac(m0, lat.represent(lat.put_gauge_fund(Uf)), lat.put_spinor(psi)))
+    assert rel(got[sites], want) <= 1e-13 and site_err(got[sites], want) <= SITE_TOL[0]
+    fly = Lattice(L, hr.REP_ADJ, hr.PREC_F64, hr.KERNEL_AUTO, link_storage=hr.LINKS_ONTHEFLY)
+    got = fly.get_spinor(fly.dirac(m0, fly.put_gauge_fund(Uf), fly.put_spinor(psi)))
+    assert rel(got[sites], want) <= 1e-13 and site_err(got[sites], want) <= SITE_TOL[0]
+
+
 # ------------------------------------------------------------------ config 3
 @pytest.fixture(scope="module")
 def big_inputs():
