@@ -268,7 +268,7 @@ static int check_decomp(const hr_decomp* d) {
 }
 
 int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void* u, const void* in_half, void* const* face_out, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d)); HR_TRY(check_no_su3(g, "hr_halo_pack"));
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
     if (in_parity != HR_EVEN && in_parity != HR_ODD) { set_error("hr_halo_pack: in_parity %d", in_parity); return HR_EINVAL; }
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(in_half, "in_half"));
     if (!face_out) { set_error("hr_halo_pack: face_out is NULL"); return HR_EINVAL; }
@@ -280,13 +280,13 @@ int hr_halo_pack(const hr_geom* g, const hr_decomp* d, int in_parity, const void
 // phases: 1 = interior kernel, 2 = boundary kernels, 3 = both
 static int hop_local_phases(int phases, const hr_geom* g, const hr_decomp* d, int out_parity, int epi, double a, double c, const void* u,
                             const void* clover, const void* in_half, const void* phi_half, void* out_half, const void* const* face_in, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d)); HR_TRY(check_no_su3(g, "hr_hop_local"));
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_decomp(d));
     if (out_parity != HR_EVEN && out_parity != HR_ODD) { set_error("hr_hop_local: out_parity %d", out_parity); return HR_EINVAL; }
     if (epi < HR_EPI_NONE || epi > HR_EPI_CLOVER_AXPY) { set_error("hr_hop_local: unknown epilogue %d", epi); return HR_EINVAL; }
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(out_half, "out_half"));
     if (phases & 1) HR_TRY(check_ptr(in_half, "in_half"));
     if ((phases & 1) && (epi == HR_EPI_AXPY || epi == HR_EPI_CLOVER_AXPY)) HR_TRY(check_ptr(phi_half, "phi_half"));
-    if (epi == HR_EPI_CLOVER_INV || epi == HR_EPI_CLOVER_AXPY) HR_TRY(check_ptr(clover, "clover"));
+    if (epi == HR_EPI_CLOVER_INV || epi == HR_EPI_CLOVER_AXPY) { HR_TRY(check_no_su3(g, "hr_hop_local with a clover epilogue")); HR_TRY(check_ptr(clover, "clover")); }
     const size_t half = half_spinor_bytes(g);
     if ((phases & 1) && overlap(in_half, half, out_half, half)) { set_error("hr_hop_local: out aliases in (gather operation)"); return HR_EINVAL; }
     int mask = 0;

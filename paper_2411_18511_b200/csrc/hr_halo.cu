@@ -64,7 +64,7 @@ __device__ __forceinline__ void face_load(const void* face, int nface, int fi, c
     for (int c = 0; c < N; ++c) { h0[c] = v[c]; h1[c] = v[N + c]; }
 }
 
-template <typename T, int N, int MU, bool UP, bool ONFLY>
+template <typename T, int N, int MU, bool UP, bool ONFLY, bool C3>
 __device__ __forceinline__ void pack_one(const Geo& g, const FaceGeo& f, int par, const void* gauge, const void* in_half, void* face, int fi) {
     constexpr int NC = 4 * N;
     int x[4];
@@ -77,7 +77,7 @@ __device__ __forceinline__ void pack_one(const Geo& g, const FaceGeo& f, int par
         face_store<T, N>(face, f.nface, fi, h0, h1);
     } else {
         hop_project<T, N, MU, false>(h0, h1, psi);                 // (1 + gamma_mu) psi, times this site's link^dag
-        Link<T, N> u;
+        typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type u;    // C3: complex 3 x 3 links (HR_REP_SU3)
         load_link_rep<T, LD_STREAM, ONFLY>(u, gauge, g, par, MU, row, h);
         cplx<T> c0[N], c1[N];
         mul_link_dag(c0, u, h0);
@@ -94,7 +94,7 @@ struct PackJob {
     int slot[8];     // slot[j] = face index 2*mu + up of the j-th face to pack
     int nslots;
 };
-template <typename T, int N, bool ONFLY>
+template <typename T, int N, bool ONFLY, bool C3>
 __global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, PackJob job, int par, const void* gauge, const void* in_half) {
     const int fidx = job.slot[blockIdx.y];
     const int mu = fidx >> 1, up = fidx & 1;
@@ -104,8 +104,8 @@ __global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, PackJob job, int 
     void* face = job.face[fidx];
 #define HR_PACK(MU)                                                                        \
     if (mu == MU) {                                                                        \
-        if (up) pack_one<T, N, MU, true, ONFLY>(g, f, par, gauge, in_half, face, fi);      \
-        else pack_one<T, N, MU, false, ONFLY>(g, f, par, gauge, in_half, face, fi);        \
+        if (up) pack_one<T, N, MU, true, ONFLY, C3>(g, f, par, gauge, in_half, face, fi);      \
+        else pack_one<T, N, MU, false, ONFLY, C3>(g, f, par, gauge, in_half, face, fi);      \
     }
     HR_PACK(0) HR_PACK(1) HR_PACK(2) HR_PACK(3)
 #undef HR_PACK
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, PackJob job, int 
 // `out` the way the local kernel's epilogue would have: out += c * t (EPI_NONE: c = 1; EPI_AXPY, EPI_CLOVER_AXPY) or
 // out += B(x) t (EPI_CLOVER_INV).  up == 1: output sites with x_mu = L_mu-1 and the face received from the rank at +mu
 // (its "down" face); up == 0: output sites with x_mu = 0 and the "up" face of the rank at -mu.  par = output parity.
-template <typename T, int N, int MU, bool UP, int EPI, bool ONFLY>
+template <typename T, int N, int MU, bool UP, int EPI, bool ONFLY, bool C3>
 __device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int par, const HopArgs& a, const void* face, int fi) {
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
@@ -127,7 +127,7 @@ __device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int
     for (int c = 0; c < NC; ++c) t[c] = mk<T>((T)0, (T)0);
     face_load<T, N>(face, f.nface, fi, h0, h1);
     if (UP) {
-        Link<T, N> u;
+        typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type u;
         load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, par, MU, row, h);
         hop_apply<T, N, MU, true>(t, h0, h1, u);
     } else {
@@ -136,7 +136,7 @@ __device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int
     const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
     cplx<T> o[NC];
     IO::template load<LD_KEEP>(o, a.out, first, g.L3h);
-    if (EPI == EPI_CLOVER_INV) {
+    if (EPI == EPI_CLOVER_INV && !C3) {
         T blk[CloverSize<N>::reals];
         cplx<T> y[NC];
         load_clover<T, N>(blk, a.clover, g, par, row, h);
@@ -154,7 +154,7 @@ __device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int
 // blockIdx.y = 0: the sites with x_mu = 0 (up face of the rank at -mu); 1: the sites with x_mu = L_mu-1 (down face of the rank
 // at +mu).  The two site sets are disjoint, so one launch serves both faces of a direction; different directions share edge and
 // corner sites and run as consecutive launches.
-template <typename T, int N, int EPI, bool ONFLY>
+template <typename T, int N, int EPI, bool ONFLY, bool C3>
 __global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, int par, HopArgs a, const void* face_lo, const void* face_hi) {
     const int fi = blockIdx.x * blockDim.x + threadIdx.x;
     if (fi >= f.nface) return;
@@ -162,14 +162,14 @@ __global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, in
     const void* face = up ? face_hi : face_lo;
 #define HR_BND(MU)                                                                         \
     if (f.mu == MU) {                                                                      \
-        if (up) boundary_one<T, N, MU, true, EPI, ONFLY>(g, f, par, a, face, fi);          \
-        else boundary_one<T, N, MU, false, EPI, ONFLY>(g, f, par, a, face, fi);            \
+        if (up) boundary_one<T, N, MU, true, EPI, ONFLY, C3>(g, f, par, a, face, fi);          \
+        else boundary_one<T, N, MU, false, EPI, ONFLY, C3>(g, f, par, a, face, fi);           \
     }
     HR_BND(0) HR_BND(1) HR_BND(2) HR_BND(3)
 #undef HR_BND
 }
 
-template <typename T, int N, bool ONFLY>
+template <typename T, int N, bool ONFLY, bool C3 = false>
 static int pack_faces(const hr_geom* hg, const int* split, int par, const void* gauge, const void* in_half, void* const* face_out, cudaStream_t st) {
     const Geo g = make_geo(hg);
     PackJob job;
@@ -186,12 +186,12 @@ static int pack_faces(const hr_geom* hg, const int* split, int par, const void* 
         if (job.f[mu].nface > maxface) maxface = job.f[mu].nface;
     }
     if (job.nslots == 0) return HR_OK;
-    halo_pack_kernel<T, N, ONFLY><<<dim3((maxface + 127) / 128, job.nslots), 128, 0, st>>>(g, job, par, gauge, in_half);
+    halo_pack_kernel<T, N, ONFLY, C3><<<dim3((maxface + 127) / 128, job.nslots), 128, 0, st>>>(g, job, par, gauge, in_half);
     count_launch();
     return check_launch("halo_pack_kernel");
 }
 
-template <typename T, int N, bool ONFLY>
+template <typename T, int N, bool ONFLY, bool C3 = false>
 static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, int epi, const void* const* face_in, cudaStream_t st) {
     const Geo g = make_geo(hg);
     for (int mu = 0; mu < 4; ++mu) {
@@ -201,11 +201,12 @@ static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, i
         // output sites at x_mu = 0 take the -mu neighbour's up face (index 2mu+1); those at x_mu = L-1 the +mu neighbour's down face
         const void* lo = face_in[2 * mu + 1];
         const void* hi = face_in[2 * mu];
+        if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
         switch (epi) {
-            case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY, C3><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY, C3><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY, false><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
+            case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
             default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
         }
         count_launch();
@@ -214,6 +215,10 @@ static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, i
 }
 
 #define HR_DISPATCH_REP(FN, ...)                                                                      \
+    if (hg->rep == HR_REP_SU3) {                                                                      \
+        if (hg->prec == HR_PREC_F64) return FN<double, 3, false, true>(__VA_ARGS__);                  \
+        return FN<float, 3, false, true>(__VA_ARGS__);                                                \
+    }                                                                                                 \
     if (hg->rep == HR_REP_FUND) {                                                                     \
         if (hg->prec == HR_PREC_F64) return FN<double, 2, false>(__VA_ARGS__);                        \
         return FN<float, 2, false>(__VA_ARGS__);                                                      \

@@ -205,6 +205,45 @@ def test_sharded_adjoint_operators(hr, orc, Lg, P, split, onfly):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("Lg,P,split", [CASES[1], CASES[3], CASES[4]])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_sharded_su3_operators(hr, orc, Lg, P, split, prec):
+    """complex 3 x 3 links (HR_REP_SU3) on a cut lattice: the up faces are multiplied by the sender's U^dag, the receiver applies its own
+    U to the down faces; full D and Dhat stitched from the shards against the oracle's global operator (rep 2)"""
+    import torch
+    from paper_2411_18511_b200 import halo
+    m0 = -0.3
+    U = inputs.haar_gauge_su3(Lg, 1)
+    psi = inputs.gaussian_spinor(Lg, 3, 2)
+    if prec:
+        U, psi = U.astype(np.complex64).astype(np.complex128), psi.astype(np.complex64).astype(np.complex128)
+    shards = make_shards(hr, Lg, P, hr.REP_SU3, prec, split, hr.LINKS_FULL)
+    Ud, pd, od, td = {}, {}, {}, {}
+    for c, sh in shards.items():
+        lat = sh.lat
+        Ud[c] = lat.put_gauge_su3(halo.local_block(U, Lg, P, c))
+        pd[c] = lat.put_spinor(halo.local_block(psi, Lg, P, c))
+        od[c] = torch.zeros_like(pd[c])
+        td[c] = lat.empty_spinor(hr.ODD)
+
+    def gather():
+        torch.cuda.synchronize()
+        return halo.assemble({c: sh.lat.get_spinor(od[c]) for c, sh in shards.items()}, Lg, P)
+
+    halo.dirac_all(shards, halo.exchange_in_process, m0, Ud, pd, od)
+    assert rel(gather(), orc.dirac(Lg, 2, m0, U, psi, nthreads=NTHREADS)) <= TOL[prec]
+    for c in shards:
+        od[c].zero_()
+    halo.dhat_all(shards, halo.exchange_in_process, m0, Ud, {c: sh.lat.even(pd[c]) for c, sh in shards.items()},
+                  {c: sh.lat.even(od[c]) for c, sh in shards.items()}, td)
+    assert rel(gather(), orc.dirac_eo(Lg, 2, m0, U, psi, nthreads=NTHREADS)) <= TOL[prec]
+    # the clover epilogues are not there for this representation: refused, not silently wrong
+    sh = next(iter(shards.values()))
+    with pytest.raises(hr.HrError):
+        sh.hop(hr.ODD, Ud[sh.coords], sh.lat.even(pd[sh.coords]), sh.lat.odd(od[sh.coords]), epi=hr.EPI_CLOVER_INV, clover=pd[sh.coords])
+
+
+@pytest.mark.gpu
 def test_uncut_hop_local_is_the_single_gpu_hop(hr):
     """with no cut direction hr_hop_local is hr_dirac_eo_apply bit for bit (same kernel, no boundary pass)"""
     import torch
