@@ -111,62 +111,90 @@ __global__ void __launch_bounds__(128) halo_pack_kernel(Geo g, PackJob job, int 
 #undef HR_PACK
 }
 
-// Boundary kernel: the term of the hopping sum that crossed the cut, for the output sites on one face, combined into
-// `out` the way the local kernel's epilogue would have: out += c * t (EPI_NONE: c = 1; EPI_AXPY, EPI_CLOVER_AXPY) or
-// out += B(x) t (EPI_CLOVER_INV).  up == 1: output sites with x_mu = L_mu-1 and the face received from the rank at +mu
-// (its "down" face); up == 0: output sites with x_mu = 0 and the "up" face of the rank at -mu.  par = output parity.
-template <typename T, int N, int MU, bool UP, int EPI, bool ONFLY, bool C3>
-__device__ __forceinline__ void boundary_one(const Geo& g, const FaceGeo& f, int par, const HopArgs& a, const void* face, int fi) {
-    constexpr int NC = 4 * N;
-    typedef SiteIO<T, NC> IO;
-    int x[4];
-    face_site(f, fi, UP ? (MU == 0 ? g.L0 : MU == 1 ? g.L1 : MU == 2 ? g.L2 : 2 * g.L3h) - 1 : 0, par, x);
-    const int row = (x[0] * g.L1 + x[1]) * g.L2 + x[2], h = x[3] >> 1;
-    cplx<T> t[NC], h0[N], h1[N];
-#pragma unroll
-    for (int c = 0; c < NC; ++c) t[c] = mk<T>((T)0, (T)0);
-    face_load<T, N>(face, f.nface, fi, h0, h1);
-    if (UP) {
-        typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type u;
+// Boundary kernel: the terms of the hopping sum that crossed a cut, for the output sites on the faces, combined into `out` the way
+// the local kernel's epilogue would have: out += c * t (EPI_NONE: c = 1; EPI_AXPY, EPI_CLOVER_AXPY) or out += B(x) t (EPI_CLOVER_INV).
+// Output sites with x_mu = L_mu-1 take the face received from the rank at +mu (its "down" face, multiplied here by the local link),
+// output sites with x_mu = 0 the "up" face of the rank at -mu.  par = output parity.
+//
+// ONE launch serves every cut direction: blockIdx.y runs over the (direction, side) faces, one thread per face site.  Edge and corner
+// sites lie on the faces of several directions; a site is OWNED by its lowest cut direction — the thread that meets it on a face of a
+// higher direction leaves — and the owner adds the terms of all directions the site is on a face of, in increasing direction, with one
+// read-modify-write of the output spinor (no two threads touch the same site: deterministic, no atomics).
+struct BoundaryJob {
+    FaceGeo f[4];
+    const void* lo[4];   // face for the sites with x_mu = 0      (the -mu neighbour's up face)
+    const void* hi[4];   // face for the sites with x_mu = L_mu-1 (the +mu neighbour's down face)
+    int cut[4];
+    int slot[8];         // slot[j] = 2*mu + side of the j-th face
+    int nslots;
+};
+
+// index of site x in the face of direction f.mu (inverse of face_site)
+__device__ __forceinline__ int face_index(const FaceGeo& f, const int x[4]) {
+    return ((x[f.o[0]] * f.E[1] + x[f.o[1]]) * f.E[2] + x[f.o[2]]) >> 1;
+}
+
+// t += the term of direction MU that crossed the cut, for output site (row, h) = x on side `up` of that direction
+template <typename T, int N, int MU, bool ONFLY, bool C3>
+__device__ __forceinline__ void boundary_term(cplx<T>* t, const Geo& g, const BoundaryJob& job, int par, const HopArgs& a, int up, const int x[4],
+                                              int row, int h) {
+    const FaceGeo& f = job.f[MU];
+    const int fi = face_index(f, x);
+    cplx<T> h0[N], h1[N];
+    face_load<T, N>(up ? job.hi[MU] : job.lo[MU], f.nface, fi, h0, h1);
+    if (up) {
+        typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type u;    // C3: complex 3 x 3 links (HR_REP_SU3)
         load_link_rep<T, LD_STREAM, ONFLY>(u, a.gauge, g, par, MU, row, h);
         hop_apply<T, N, MU, true>(t, h0, h1, u);
     } else {
         hop_rebuild<T, N, MU, false>(t, h0, h1);
     }
+}
+
+template <typename T, int N, int EPI, bool ONFLY, bool C3>
+__global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, BoundaryJob job, int par, HopArgs a) {
+    constexpr int NC = 4 * N;
+    typedef SiteIO<T, NC> IO;
+    const int fidx = job.slot[blockIdx.y];
+    const int mu = fidx >> 1, side = fidx & 1;
+    const int fi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (fi >= job.f[mu].nface) return;
+    const int L[4] = {g.L0, g.L1, g.L2, 2 * g.L3h};
+    int x[4];
+    face_site(job.f[mu], fi, side ? L[mu] - 1 : 0, par, x);
+    for (int nu = 0; nu < mu; ++nu)
+        if (job.cut[nu] && (x[nu] == 0 || x[nu] == L[nu] - 1)) return;      // owned by a lower direction
+    const int row = (x[0] * g.L1 + x[1]) * g.L2 + x[2], h = x[3] >> 1;
     const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
-    cplx<T> o[NC];
+    cplx<T> o[NC], t[NC];
     IO::template load<LD_KEEP>(o, a.out, first, g.L3h);
-    if (EPI == EPI_CLOVER_INV && !C3) {
+    const T cc = EPI == EPI_NONE ? (T)1 : (T)a.c;
+    bool any = false;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) t[c] = mk<T>((T)0, (T)0);
+#define HR_BND(MU)                                                                                         \
+    if (MU >= mu && job.cut[MU] && (x[MU] == 0 || x[MU] == L[MU] - 1)) {                                   \
+        boundary_term<T, N, MU, ONFLY, C3>(t, g, job, par, a, x[MU] == 0 ? 0 : 1, x, row, h);              \
+        any = true;                                                                                        \
+        if (EPI != EPI_CLOVER_INV) {   /* one direction at a time, like consecutive passes would */         \
+            _Pragma("unroll") for (int c = 0; c < NC; ++c) {                                               \
+                o[c].re = fma(cc, t[c].re, o[c].re); o[c].im = fma(cc, t[c].im, o[c].im);                  \
+                t[c] = mk<T>((T)0, (T)0);                                                                  \
+            }                                                                                              \
+        }                                                                                                  \
+    }
+    HR_BND(0) HR_BND(1) HR_BND(2) HR_BND(3)
+#undef HR_BND
+    if (!any) return;
+    if (EPI == EPI_CLOVER_INV && !C3) {      // B(x) is linear: one block product for the sum of the crossing terms
         T blk[CloverSize<N>::reals];
         cplx<T> y[NC];
         load_clover<T, N>(blk, a.clover, g, par, row, h);
         clover_matvec<T, N>(y, blk, t);
 #pragma unroll
         for (int c = 0; c < NC; ++c) o[c] = o[c] + y[c];
-    } else {
-        const T cc = EPI == EPI_NONE ? (T)1 : (T)a.c;
-#pragma unroll
-        for (int c = 0; c < NC; ++c) { o[c].re = fma(cc, t[c].re, o[c].re); o[c].im = fma(cc, t[c].im, o[c].im); }
     }
     IO::store(a.out, first, g.L3h, o);
-}
-
-// blockIdx.y = 0: the sites with x_mu = 0 (up face of the rank at -mu); 1: the sites with x_mu = L_mu-1 (down face of the rank
-// at +mu).  The two site sets are disjoint, so one launch serves both faces of a direction; different directions share edge and
-// corner sites and run as consecutive launches.
-template <typename T, int N, int EPI, bool ONFLY, bool C3>
-__global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, FaceGeo f, int par, HopArgs a, const void* face_lo, const void* face_hi) {
-    const int fi = blockIdx.x * blockDim.x + threadIdx.x;
-    if (fi >= f.nface) return;
-    const int up = blockIdx.y;
-    const void* face = up ? face_hi : face_lo;
-#define HR_BND(MU)                                                                         \
-    if (f.mu == MU) {                                                                      \
-        if (up) boundary_one<T, N, MU, true, EPI, ONFLY, C3>(g, f, par, a, face, fi);          \
-        else boundary_one<T, N, MU, false, EPI, ONFLY, C3>(g, f, par, a, face, fi);           \
-    }
-    HR_BND(0) HR_BND(1) HR_BND(2) HR_BND(3)
-#undef HR_BND
 }
 
 template <typename T, int N, bool ONFLY, bool C3 = false>
@@ -194,23 +222,32 @@ static int pack_faces(const hr_geom* hg, const int* split, int par, const void* 
 template <typename T, int N, bool ONFLY, bool C3 = false>
 static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, int epi, const void* const* face_in, cudaStream_t st) {
     const Geo g = make_geo(hg);
+    BoundaryJob job;
+    job.nslots = 0;
+    int maxface = 0;
     for (int mu = 0; mu < 4; ++mu) {
+        job.f[mu] = make_face(hg, mu);
+        job.cut[mu] = split[mu] ? 1 : 0;
+        job.lo[mu] = job.hi[mu] = nullptr;
         if (!split[mu]) continue;
-        const FaceGeo f = make_face(hg, mu);
-        const dim3 grid((f.nface + 127) / 128, 2);
         // output sites at x_mu = 0 take the -mu neighbour's up face (index 2mu+1); those at x_mu = L-1 the +mu neighbour's down face
-        const void* lo = face_in[2 * mu + 1];
-        const void* hi = face_in[2 * mu];
-        if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
-        switch (epi) {
-            case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY, C3><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY, C3><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY, false><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false><<<grid, 128, 0, st>>>(g, f, a.parity, a, lo, hi); break;
-            default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
-        }
-        count_launch();
+        job.lo[mu] = face_in[2 * mu + 1];
+        job.hi[mu] = face_in[2 * mu];
+        job.slot[job.nslots++] = 2 * mu;
+        job.slot[job.nslots++] = 2 * mu + 1;
+        if (job.f[mu].nface > maxface) maxface = job.f[mu].nface;
     }
+    if (job.nslots == 0) return HR_OK;
+    if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
+    const dim3 grid((maxface + 127) / 128, job.nslots);
+    switch (epi) {
+        case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY, C3><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
+        case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY, C3><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
+        case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY, false><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
+        case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
+        default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
+    }
+    count_launch();
     return check_launch("halo_boundary_kernel");
 }
 

@@ -104,6 +104,27 @@ __device__ __forceinline__ void lds_site<float, 12>(cplx<float>* s, const char* 
     }
 }
 
+// OPEN kernels: a term that crosses a cut is left out by multiplying its link by zero — branch-free, so that the instruction
+// schedule stays that of the periodic kernel (skipping the term with a branch cost 14 % of the interior kernel: 247 against 216 us)
+template <bool OPEN, typename T>
+__device__ __forceinline__ Link<T, 2> open_link(const Link<T, 2>& u, bool cut) {
+    if (!OPEN) return u;
+    const T m = cut ? (T)0 : (T)1;
+    Link<T, 2> v;
+    v.a = mk<T>(u.a.re * m, u.a.im * m);
+    v.b = mk<T>(u.b.re * m, u.b.im * m);
+    return v;
+}
+template <bool OPEN, typename T>
+__device__ __forceinline__ Link<T, 3> open_link(const Link<T, 3>& u, bool cut) {
+    if (!OPEN) return u;
+    const T m = cut ? (T)0 : (T)1;
+    Link<T, 3> v;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) v.r[k] = u.r[k] * m;
+    return v;
+}
+
 // launch geometry chosen on the host (hr_hop.cu)
 struct TiledPlan {
     int t1, t2;        // tile shape in rows (x1, x2): selects the kernel instantiation
@@ -303,35 +324,35 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         const char* const a3b = scur + off_c + hb3 * 16;
         HR_NB_NEXT(nb0, a0f);
         HR_NB_NEXT(nb1, a0b); HR_NB_NOW(nb0, a0f);
-        if (!(OPEN && cut_f0)) hop_term<T, N, 0, true>(acc, nb0, uf[0]);
+        hop_term<T, N, 0, true>(acc, nb0, open_link<OPEN>(uf[0], cut_f0));
         load_link_rep<T, LP, ONFLY>(uf[0], a.gauge, g, p, 0, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a1f); HR_NB_NOW(nb1, a0b);
-        if (!(OPEN && cut_b0)) hop_term<T, N, 0, false>(acc, nb1, ub[0]);
+        hop_term<T, N, 0, false>(acc, nb1, open_link<OPEN>(ub[0], cut_b0));
         load_link_rep<T, LP, ONFLY>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a1b); HR_NB_NOW(nb0, a1f);
-        if (!(OPEN && cut_f1)) hop_term<T, N, 1, true>(acc, nb0, uf[1]);
+        hop_term<T, N, 1, true>(acc, nb0, open_link<OPEN>(uf[1], cut_f1));
         load_link_rep<T, LP, ONFLY>(uf[1], a.gauge, g, p, 1, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a2f); HR_NB_NOW(nb1, a1b);
-        if (!(OPEN && cut_b1)) hop_term<T, N, 1, false>(acc, nb1, ub[1]);
+        hop_term<T, N, 1, false>(acc, nb1, open_link<OPEN>(ub[1], cut_b1));
         load_link_rep<T, LP, ONFLY>(ub[1], a.gauge, g, 1 - p, 1, rowb1_0 + xn * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a2b); HR_NB_NOW(nb0, a2f);
-        if (!(OPEN && cut_f2)) hop_term<T, N, 2, true>(acc, nb0, uf[2]);
+        hop_term<T, N, 2, true>(acc, nb0, open_link<OPEN>(uf[2], cut_f2));
         load_link_rep<T, LP, ONFLY>(uf[2], a.gauge, g, p, 2, rown, h);
         HR_PIN();
         HR_NB_NEXT(nb0, a3f); HR_NB_NOW(nb1, a2b);
-        if (!(OPEN && cut_b2)) hop_term<T, N, 2, false>(acc, nb1, ub[2]);
+        hop_term<T, N, 2, false>(acc, nb1, open_link<OPEN>(ub[2], cut_b2));
         load_link_rep<T, LP, ONFLY>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xn * g.s0, h);
         HR_PIN();
         HR_NB_NEXT(nb1, a3b); HR_NB_NOW(nb0, a3f);
-        if (!(OPEN && cut_f3)) hop_term<T, N, 3, true>(acc, nb0, uf[3]);
+        hop_term<T, N, 3, true>(acc, nb0, open_link<OPEN>(uf[3], cut_f3));
         load_link_rep<T, LP, ONFLY>(uf[3], a.gauge, g, p, 3, rown, h);
         HR_PIN();
         HR_NB_NOW(nb1, a3b);
-        if (!(OPEN && cut_b3)) hop_term<T, N, 3, false>(acc, nb1, ub[3]);
+        hop_term<T, N, 3, false>(acc, nb1, open_link<OPEN>(ub[3], cut_b3));
         load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
 #undef HR_NB_NEXT
 #undef HR_NB_NOW
