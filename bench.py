@@ -385,6 +385,8 @@ def other_configs(hr, inputs, Lattice):
 
     def timed(fn, n):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        time.sleep(0.25)          # every side row starts below the power cap (burst regime, as the back-to-back table)
         for _ in range(3):
             fn()
         torch.cuda.synchronize()
@@ -474,6 +476,25 @@ def other_configs(hr, inputs, Lattice):
                                                                     "frac": round(bc * sites / ms / 1e6 / peak, 4), "bytes_per_site": bc,
                                                                     "kernel": hr.hr_kernel_name(g)}
             del Uf_dev, U_dev, p_dev, o_dev, tmp
+    # complex 3 x 3 links (HR_REP_SU3, DESIGN.md §1 row f4b) at the same volume: generic kernel, links stored in full or as two rows
+    for prec, storage, ptag in ((hr.PREC_F64, hr.LINKS_FULL, "f64"), (hr.PREC_F32, hr.LINKS_FULL, "f32"),
+                                (hr.PREC_F64, hr.LINKS_COMPRESSED, "tworows_f64"), (hr.PREC_F32, hr.LINKS_COMPRESSED, "tworows_f32")):
+        lat = Lattice(L, hr.REP_SU3, prec, hr.KERNEL_AUTO, link_storage=storage)
+        g = lat.g
+        U_dev = torch.randn(hr.hr_gauge_bytes(g, hr.REP_SU3) // 4, device="cuda").view(torch.uint8)
+        p_dev = torch.randn(hr.hr_spinor_bytes(g, hr.BOTH) // 4, device="cuda").view(torch.uint8)
+        o_dev, tmp = lat.empty_spinor(), lat.empty_spinor(hr.ODD)
+        st0 = hr.stream_ptr()
+        for name, op, sites, fn in (
+                ("hop", hr.OP_HOP, V // 2, lambda: hr.hr_dirac_eo_apply(g, hr.EO_HOP_OE, 0.0, U_dev, None, None, lat.even(p_dev), lat.odd(o_dev), None, st0)),
+                ("dirac", hr.OP_DIRAC, V, lambda: hr.hr_dirac_apply(g, -0.3, U_dev, p_dev, o_dev, st0)),
+                ("dhat", hr.OP_DHAT, V // 2, lambda: hr.hr_dirac_eo_apply(g, hr.EO_DHAT, -0.3, U_dev, None, None, lat.even(p_dev), lat.even(o_dev), tmp, st0))):
+            ms = timed(fn, 20)
+            f, bc, _ = hr.hr_dirac_flops_bytes(g, op)
+            out["su3_48^4_%s_%s" % (name, ptag)] = {"us_per_apply": round(ms * 1e3, 1), "gsites_per_s": round(sites / ms / 1e6, 3),
+                                                   "gflops": round(f * sites / ms / 1e6, 1), "gbs": round(bc * sites / ms / 1e6, 1),
+                                                   "frac": round(bc * sites / ms / 1e6 / peak, 4), "bytes_per_site": bc, "kernel": hr.hr_kernel_name(g)}
+        del U_dev, p_dev, o_dev, tmp
     # the sharded hop on this one GPU: a 48^4 local lattice whose four directions are all cut onto the rank itself;
     # pack + device-to-device face copies + interior kernel + boundary kernels per hop o<-e, in order and with pack / copies
     # on a side stream (no multi-GPU hardware in this run: this measures what a cut costs a rank, not the transport)
@@ -484,7 +505,7 @@ def other_configs(hr, inputs, Lattice):
         U_dev = torch.randn(hr.hr_gauge_bytes(g, hr.REP_FUND) // 4, device="cuda").view(torch.uint8)
         p_dev = torch.randn(hr.hr_spinor_bytes(g, hr.BOTH) // 4, device="cuda").view(torch.uint8)
         o_dev = lat.empty_spinor()
-        for split in ((1, 0, 0, 0), (1, 1, 1, 1)):
+        for split in ((1, 0, 0, 0), (1, 1, 1, 0), (1, 1, 1, 1)):
             sh = halo.Shard(lat, (1, 1, 1, 1), (0, 0, 0, 0), split)
             shards, Ud, ind, outd = {(0, 0, 0, 0): sh}, {(0, 0, 0, 0): U_dev}, {(0, 0, 0, 0): lat.even(p_dev)}, {(0, 0, 0, 0): lat.odd(o_dev)}
             ms_seq = timed(lambda: halo.hop_all(shards, halo.exchange_in_process, hr.ODD, Ud, ind, outd), 20)

@@ -44,7 +44,9 @@ enum { HR_OK = 0, HR_EINVAL = 1, HR_EUNSUPPORTED = 2, HR_EALIGN = 3, HR_ECUDA = 
 
 /* fermion representation / gauge group.  HR_REP_FUND and HR_REP_ADJ are the two SU(2) representations of BASELINE.json;
  * HR_REP_SU3 is the first step towards HiRep's other gauge groups: 3 complex
- * colours and complex 3 x 3 links stored in full (link_storage = HR_LINKS_FULL; canonical [V][4 mu][3][3][re,im]).  It is
+ * colours and complex 3 x 3 links (canonical [V][4 mu][3][3][re,im]) kept on the device in full (link_storage = HR_LINKS_FULL, 18 reals)
+ * or as their first two rows (HR_LINKS_COMPRESSED, 12 reals: the kernels and hr_unpack_gauge rebuild row 2 = conj(row 0 x row 1),
+ * exact for unitary links of determinant 1).  It is
  * served by the generic hopping kernel: bare hops, full D, the even-odd operator without clover, the CG solvers and the sharded hop
  * (hr_halo_pack / hr_hop_local with the epilogues HR_EPI_NONE and HR_EPI_AXPY); the clover and representation calls and the clover
  * epilogues return HR_EUNSUPPORTED for it. */

@@ -12,7 +12,7 @@ namespace hr {
 // hr_fields.cu
 int permute_chunks(bool pack, const Geo& g, int NI, int NCH, int SRC, const void* src, void* dst, cudaStream_t st);
 int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st);
-int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries = false);
+int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries = false, bool two_rows = false);
 int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
@@ -113,7 +113,7 @@ size_t hr_gauge_bytes(const hr_geom* g, int rep) {
     const Geo geo = make_geo(g);
     const size_t links = 8 * (size_t)geo.Vh;
     if (rep == HR_REP_FUND) return links * link_chunks(g->prec) * 16;
-    return links * (rep == HR_REP_SU3 ? 18 : 9) * real_bytes(g->prec);
+    return links * (rep == HR_REP_SU3 ? (g->link_storage == HR_LINKS_COMPRESSED ? 12 : 18) : 9) * real_bytes(g->prec);
 }
 
 size_t hr_clover_bytes(const hr_geom* g) {
@@ -160,7 +160,7 @@ int hr_pack_gauge(const hr_geom* g, int rep, const void* canon, void* dev, void*
         return permute_chunks(true, make_geo(g), 4, lch, 2 * lch, canon, dev, (cudaStream_t)stream);
     }
     if (rep == HR_REP_ADJ) return permute_adj(true, make_geo(g), g->prec, canon, dev, (cudaStream_t)stream);
-    if (rep == HR_REP_SU3) return permute_adj(true, make_geo(g), g->prec, canon, dev, (cudaStream_t)stream, true);
+    if (rep == HR_REP_SU3) return permute_adj(true, make_geo(g), g->prec, canon, dev, (cudaStream_t)stream, true, g->link_storage == HR_LINKS_COMPRESSED);
     set_error("unknown representation %d", rep);
     return HR_EINVAL;
 }
@@ -174,7 +174,7 @@ int hr_unpack_gauge(const hr_geom* g, int rep, const void* dev, void* canon, voi
         return rebuild_second_row(geo, g->prec, canon, (cudaStream_t)stream);
     }
     if (rep == HR_REP_ADJ) return permute_adj(false, make_geo(g), g->prec, dev, canon, (cudaStream_t)stream);
-    if (rep == HR_REP_SU3) return permute_adj(false, make_geo(g), g->prec, dev, canon, (cudaStream_t)stream, true);
+    if (rep == HR_REP_SU3) return permute_adj(false, make_geo(g), g->prec, dev, canon, (cudaStream_t)stream, true, g->link_storage == HR_LINKS_COMPRESSED);
     set_error("unknown representation %d", rep);
     return HR_EINVAL;
 }
@@ -430,7 +430,7 @@ int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, doubl
     const double N = ncolour(g->rep), w = (double)real_bytes(g->prec);
     const double nr = 8.0 * N, S = nr * w;
     const double Gf = (g->link_storage != HR_LINKS_FULL ? 4.0 : 8.0) * w, Ga = 9.0 * w;
-    const double G = g->rep == HR_REP_FUND ? Gf : g->rep == HR_REP_SU3 ? 18.0 * w : (g->link_storage == HR_LINKS_ONTHEFLY ? 4.0 * w : Ga);
+    const double G = g->rep == HR_REP_FUND ? Gf : g->rep == HR_REP_SU3 ? (g->link_storage == HR_LINKS_COMPRESSED ? 12.0 : 18.0) * w : (g->link_storage == HR_LINKS_ONTHEFLY ? 4.0 * w : Ga);
     const double Bk = 2.0 * (2 * N) * (2 * N) * w;            // two hermitian 2N x 2N blocks per site
     // per direction: 4N adds to project, two colour mat-vecs, 8N adds to accumulate; x8, minus the first accumulate
     // (rebuilding R from the quaternion, ~30 flops per link, is not counted: the model counts the operator's flops)

@@ -34,7 +34,7 @@ inline bool geom_ok(const hr_geom* g) {
     double v = (double)g->L[0] * g->L[1] * g->L[2] * g->L[3];
     if (v > 2.0e9) return false;  // 32-bit site indices
     if (g->rep != HR_REP_FUND && g->rep != HR_REP_ADJ && g->rep != HR_REP_SU3) return false;
-    if (g->rep == HR_REP_SU3 && g->link_storage != HR_LINKS_FULL) return false;   // complex 3 x 3 links are stored in full
+    if (g->rep == HR_REP_SU3 && g->link_storage == HR_LINKS_ONTHEFLY) return false;   // complex 3 x 3 links: all three rows, or the first two
     if (g->prec != HR_PREC_F64 && g->prec != HR_PREC_F32) return false;
     if (g->link_storage != HR_LINKS_FULL && g->link_storage != HR_LINKS_COMPRESSED && g->link_storage != HR_LINKS_ONTHEFLY) return false;
     if (g->link_storage == HR_LINKS_ONTHEFLY && g->rep != HR_REP_ADJ) return false;
@@ -219,15 +219,24 @@ __device__ __forceinline__ void load_link_rep(Link<T, 3>& u, const void* gauge, 
     u.r[6] = 2 * (a3 * a1 + a0 * a2);  u.r[7] = 2 * (a3 * a2 - a0 * a1);  u.r[8] = d + 2 * a3 * a3;
 }
 
-// complex 3 x 3 links: 9 complex planes per row, complex index (((par*4 + mu)*R + row)*9 + k)*L3h + h (128-bit loads in fp64, 64-bit in fp32)
-template <typename T, int POLICY, bool ONFLY>
+// complex 3 x 3 links: NK complex planes per row, complex index (((par*4 + mu)*R + row)*NK + k)*L3h + h (128-bit loads in fp64,
+// 64-bit in fp32).  TWOROWS = false: all nine entries stored (NK = 9).  TWOROWS = true (HR_LINKS_COMPRESSED): the first two rows are
+// stored (NK = 6, 96 instead of 144 bytes in fp64) and the third is rebuilt in registers, row2 = conj(row0 x row1) — exact for
+// det U = 1, U unitary, the usual two-row storage of SU(3) links.
+template <typename T, int POLICY, bool TWOROWS>
 __device__ __forceinline__ void load_link_rep(LinkC3<T>& u, const void* gauge, const Geo& g, int par, int mu, int row, int h) {
     typedef typename std::conditional<sizeof(T) == 8, double2, float2>::type pair_t;
-    const pair_t* p = reinterpret_cast<const pair_t*>(gauge) + ((size_t)(par * 4 + mu) * g.R + row) * (9 * g.L3h) + h;
+    constexpr int NK = TWOROWS ? 6 : 9;
+    const pair_t* p = reinterpret_cast<const pair_t*>(gauge) + ((size_t)(par * 4 + mu) * g.R + row) * (NK * g.L3h) + h;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) {
+    for (int k = 0; k < NK; ++k) {
         const pair_t v = POLICY == LD_KEEP ? __ldg(p + (size_t)k * g.L3h) : __ldcs(p + (size_t)k * g.L3h);
         u.m[k] = mk<T>(v.x, v.y);
+    }
+    if (TWOROWS) {
+        u.m[6] = conj(u.m[1] * u.m[5] - u.m[2] * u.m[4]);
+        u.m[7] = conj(u.m[2] * u.m[3] - u.m[0] * u.m[5]);
+        u.m[8] = conj(u.m[0] * u.m[4] - u.m[1] * u.m[3]);
     }
 }
 template <typename T>

@@ -62,18 +62,32 @@ __global__ void rebuild_second_row_kernel(long long nlinks, T* canon) {
 
 // adjoint links: canonical [lex][mu][9] reals <-> device [par][mu][row][9][h]; the same permutation with T = double2 / float2
 // moves the 9 complex entries of an HR_REP_SU3 link
-template <typename T, bool PACK>
+// NK: entries of a link kept on the device (9, or 6 = the first two rows of an HR_REP_SU3 link with HR_LINKS_COMPRESSED); the
+// canonical array always has 9 per link
+template <typename T, bool PACK, int NK>
 __global__ void permute_adj_kernel(Geo g, const T* __restrict__ src, T* __restrict__ dst) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long total = 2LL * g.Vh * 36;
+    const long long total = 2LL * g.Vh * 4 * NK;
     if (t >= total) return;
-    const int k = (int)(t % 9);
-    const int mu = (int)((t / 9) % 4);
-    const int lex = (int)(t / 36);
+    const int k = (int)(t % NK);
+    const int mu = (int)((t / NK) % 4);
+    const int lex = (int)(t / (4 * NK));
     const SiteRef s = site_of_lex(g, lex);
-    const size_t id = (((size_t)(s.par * 4 + mu) * g.R + s.row) * 9 + k) * g.L3h + s.h;
-    if (PACK) dst[id] = src[t];
-    else dst[t] = src[id];
+    const size_t id = (((size_t)(s.par * 4 + mu) * g.R + s.row) * NK + k) * g.L3h + s.h;
+    const size_t ic = ((size_t)lex * 4 + mu) * 9 + k;
+    if (PACK) dst[id] = src[ic];
+    else dst[ic] = src[id];
+}
+
+// third row of every canonical complex 3 x 3 link from the first two: row2 = conj(row0 x row1) (unpack of two-row storage)
+template <typename T>
+__global__ void rebuild_third_row_kernel(long long nlinks, T* __restrict__ canon) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nlinks) return;
+    cplx<T>* m = reinterpret_cast<cplx<T>*>(canon) + t * 9;
+    m[6] = conj(m[1] * m[5] - m[2] * m[4]);
+    m[7] = conj(m[2] * m[3] - m[0] * m[5]);
+    m[8] = conj(m[0] * m[4] - m[1] * m[3]);
 }
 
 static inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
@@ -96,23 +110,34 @@ int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st) {
     return check_launch("rebuild_second_row_kernel");
 }
 
-int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries) {
-    const long long total = 2LL * g.Vh * 36;
-    const unsigned nb = blocks_for(total, 256);
-    if (complex_entries) {
-        if (prec == HR_PREC_F64) {
-            if (pack) permute_adj_kernel<double2, true><<<nb, 256, 0, st>>>(g, (const double2*)src, (double2*)dst);
-            else permute_adj_kernel<double2, false><<<nb, 256, 0, st>>>(g, (const double2*)src, (double2*)dst);
-        } else {
-            if (pack) permute_adj_kernel<float2, true><<<nb, 256, 0, st>>>(g, (const float2*)src, (float2*)dst);
-            else permute_adj_kernel<float2, false><<<nb, 256, 0, st>>>(g, (const float2*)src, (float2*)dst);
+template <typename T, int NK>
+static void permute_adj_launch(bool pack, const Geo& g, const void* src, void* dst, cudaStream_t st) {
+    const unsigned nb = blocks_for(2LL * g.Vh * 4 * NK, 256);
+    if (pack) permute_adj_kernel<T, true, NK><<<nb, 256, 0, st>>>(g, (const T*)src, (T*)dst);
+    else permute_adj_kernel<T, false, NK><<<nb, 256, 0, st>>>(g, (const T*)src, (T*)dst);
+}
+
+// complex_entries: HR_REP_SU3 links; two_rows: only their first two rows live on the device (unpack rebuilds the third)
+int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries, bool two_rows) {
+    if (complex_entries && two_rows) {
+        if (prec == HR_PREC_F64) permute_adj_launch<double2, 6>(pack, g, src, dst, st);
+        else permute_adj_launch<float2, 6>(pack, g, src, dst, st);
+        count_launch();
+        if (!pack) {
+            const long long nl = 8LL * g.Vh;
+            if (prec == HR_PREC_F64) rebuild_third_row_kernel<double><<<blocks_for(nl, 256), 256, 0, st>>>(nl, (double*)dst);
+            else rebuild_third_row_kernel<float><<<blocks_for(nl, 256), 256, 0, st>>>(nl, (float*)dst);
+            count_launch();
         }
+        return check_launch("permute_adj_kernel");
+    }
+    if (complex_entries) {
+        if (prec == HR_PREC_F64) permute_adj_launch<double2, 9>(pack, g, src, dst, st);
+        else permute_adj_launch<float2, 9>(pack, g, src, dst, st);
     } else if (prec == HR_PREC_F64) {
-        if (pack) permute_adj_kernel<double, true><<<nb, 256, 0, st>>>(g, (const double*)src, (double*)dst);
-        else permute_adj_kernel<double, false><<<nb, 256, 0, st>>>(g, (const double*)src, (double*)dst);
+        permute_adj_launch<double, 9>(pack, g, src, dst, st);
     } else {
-        if (pack) permute_adj_kernel<float, true><<<nb, 256, 0, st>>>(g, (const float*)src, (float*)dst);
-        else permute_adj_kernel<float, false><<<nb, 256, 0, st>>>(g, (const float*)src, (float*)dst);
+        permute_adj_launch<float, 9>(pack, g, src, dst, st);
     }
     count_launch();
     return check_launch("permute_adj_kernel");

@@ -253,6 +253,10 @@ static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, i
 
 #define HR_DISPATCH_REP(FN, ...)                                                                      \
     if (hg->rep == HR_REP_SU3) {                                                                      \
+        if (hg->link_storage == HR_LINKS_COMPRESSED) {                                                \
+            if (hg->prec == HR_PREC_F64) return FN<double, 3, true, true>(__VA_ARGS__);               \
+            return FN<float, 3, true, true>(__VA_ARGS__);                                             \
+        }                                                                                             \
         if (hg->prec == HR_PREC_F64) return FN<double, 3, false, true>(__VA_ARGS__);                  \
         return FN<float, 3, false, true>(__VA_ARGS__);                                                \
     }                                                                                                 \

@@ -87,6 +87,10 @@ int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st) {
         return launch_hop_tiled<float, 3>(geo, a, epi, pl, st);
     }
     if (g->rep == HR_REP_SU3) {
+        if (g->link_storage == HR_LINKS_COMPRESSED) {     // two rows stored
+            if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 3, true, true>(geo, a, epi, st);
+            return launch_hop_generic<float, 3, true, true>(geo, a, epi, st);
+        }
         if (g->prec == HR_PREC_F64) return launch_hop_generic<double, 3, false, true>(geo, a, epi, st);
         return launch_hop_generic<float, 3, false, true>(geo, a, epi, st);
     }

@@ -73,7 +73,7 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
 // C3: the links are complex 3 x 3 matrices stored in full (HR_REP_SU3; N = 3)
 template <typename T, int N, int EPI, bool ONFLY, bool C3 = false, bool BOTH = false>
 __global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
-    static_assert(!C3 || (N == 3 && !ONFLY), "complex 3 x 3 links: N = 3, stored");
+    static_assert(!C3 || N == 3, "complex 3 x 3 links: N = 3 (ONFLY then means: two rows stored, third rebuilt)");
     typedef typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type link_t;
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
@@ -166,7 +166,7 @@ inline int generic_slab_w1(const Geo& g, bool both, size_t site_bytes) {
 template <typename T, int N, bool ONFLY, bool C3, bool BOTH>
 inline int launch_hop_generic_both(const Geo& g, const HopArgs& a_in, int epi, cudaStream_t st) {
     HopArgs a = a_in;
-    a.slab_w1 = generic_slab_w1(g, BOTH, (size_t)(16 * N + 4 * (C3 ? 18 : ONFLY ? 4 : N == 2 ? 4 : 9)) * sizeof(T));
+    a.slab_w1 = generic_slab_w1(g, BOTH, (size_t)(16 * N + 4 * (C3 ? (ONFLY ? 12 : 18) : ONFLY ? 4 : N == 2 ? 4 : 9)) * sizeof(T));
     dim3 block(128), grid(((g.Vh + 127) / 128) * (BOTH ? 2 : 1));
     if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
     switch (epi) {

@@ -75,7 +75,7 @@ class Lattice:
         return dev
 
     def put_gauge_su3(self, U):
-        """complex [V,4,3,3] -> device layout of HR_REP_SU3 links (stored in full)"""
+        """complex [V,4,3,3] -> device layout of HR_REP_SU3 links (all three rows, or the first two with LINKS_COMPRESSED)"""
         assert U.shape == (self.V, 4, 3, 3), U.shape
         canon = hr.upload(U.astype(self.cplx), self.device)
         dev = self.empty_gauge(hr.REP_SU3)

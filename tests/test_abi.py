@@ -191,13 +191,17 @@ def test_lattice_stages_on_its_own_device(monkeypatch):
 
 
 def test_su3_geometry_and_sizes(L):
-    """HR_REP_SU3: complex 3 x 3 links stored in full (18 reals per link), 3 complex colours; other link storages are rejected"""
+    """HR_REP_SU3: complex 3 x 3 links stored in full (18 reals per link) or as their first two rows (12 reals, HR_LINKS_COMPRESSED),
+    3 complex colours; HR_LINKS_ONTHEFLY is rejected"""
     g = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_FULL)
     V = 4 * 4 * 4 * 8
     assert hr.hr_spinor_bytes(g, hr.BOTH) == V * 24 * 8
     assert hr.hr_gauge_bytes(g, hr.REP_SU3) == hr.hr_canonical_gauge_bytes(g, hr.REP_SU3) == 4 * V * 18 * 8
     assert hr.hr_dirac_flops_bytes(g, hr.OP_DHAT) == (2 * 1320.0 + 72.0, 5 * 192.0 + 16 * 144.0, 19 * 192.0 + 16 * 144.0)
-    bad = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_COMPRESSED)
+    g2 = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_COMPRESSED)
+    assert hr.hr_gauge_bytes(g2, hr.REP_SU3) == 4 * V * 12 * 8 and hr.hr_canonical_gauge_bytes(g2, hr.REP_SU3) == 4 * V * 18 * 8
+    assert hr.hr_dirac_flops_bytes(g2, hr.OP_HOP)[1] == 2 * 192.0 + 8 * 96.0
+    bad = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_ONTHEFLY)
     assert hr.hr_spinor_bytes(bad, hr.BOTH) == 0
     with pytest.raises(hr.HrError):
         hr.hr_dirac_flops_bytes(g, hr.OP_CLOVER)

@@ -900,24 +900,33 @@ def test_clover_inverse_of_indefinite_blocks(hr, orc):
 # ------------------------------------------------------------------ complex 3 x 3 links (HR_REP_SU3)
 @pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 2, 2, 2), (2, 4, 6, 8), (6, 2, 4, 12)])
 @pytest.mark.parametrize("prec", [0, 1])
-def test_su3_small_lattices(hr, orc, L, prec):
+@pytest.mark.parametrize("two_rows", [False, True])
+def test_su3_small_lattices(hr, orc, L, prec, two_rows):
     """Haar SU(3) links, 3 complex colours: pack/unpack round trip, bare hops, full D, Dhat and the CG solver against the
-    oracle's rep-2 operators (pinned by P21); the clover / sharded calls refuse the representation"""
+    oracle's rep-2 operators (pinned by P21); the clover calls refuse the representation.  two_rows: HR_LINKS_COMPRESSED — the
+    device keeps the first two rows of a link and the kernels (and unpack) rebuild the third, row2 = conj(row0 x row1)."""
     import torch
+    from paper_2411_18511_b200.lattice import Lattice
     m0 = -0.2
     U = rounded(inputs.haar_gauge_su3(L, 1), prec)
     psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
-    lat = lattice(hr, L, hr.REP_SU3, prec)
+    lat = Lattice(L, hr.REP_SU3, prec, 0, link_storage=hr.LINKS_COMPRESSED if two_rows else hr.LINKS_FULL)
     assert hr.hr_kernel_name(lat.g) == "generic"
     U_dev = lat.put_gauge_su3(U)
-    assert np.array_equal(lat.get_gauge_su3(U_dev), U.astype(lat.cplx))
+    assert hr.hr_gauge_bytes(lat.g, hr.REP_SU3) == inputs.volume(L) * 4 * (12 if two_rows else 18) * (8 if prec == 0 else 4)
+    back = lat.get_gauge_su3(U_dev)
+    if two_rows:      # rows 0 and 1 are a permutation, row 2 is recomputed from them
+        assert np.array_equal(back[:, :, :2], U.astype(lat.cplx)[:, :, :2])
+        assert np.abs(back[:, :, 2] - U[:, :, 2]).max() <= (1e-15 if prec == 0 else 5e-7)
+    else:
+        assert np.array_equal(back, U.astype(lat.cplx))
     want = oracle_ops(orc, L, 2, U, psi, m0)
     got = gpu_ops(hr, lat, U_dev, psi, m0)
     for k in want:
         assert rel(got[k], want[k]) <= TOL[prec], k
     f, bc, _ = hr.hr_dirac_flops_bytes(lat.g, hr.OP_HOP)
     w = 8 if prec == 0 else 4
-    assert f == 1320.0 and bc == 2 * 24 * w + 8 * 18 * w
+    assert f == 1320.0 and bc == 2 * 24 * w + 8 * (12 if two_rows else 18) * w
     with pytest.raises(hr.HrError):
         lat.clover_build(m0, 1.0, U_dev)
     if prec == 0 and L == (4, 4, 4, 4):

@@ -207,7 +207,8 @@ def test_sharded_adjoint_operators(hr, orc, Lg, P, split, onfly):
 @pytest.mark.gpu
 @pytest.mark.parametrize("Lg,P,split", [CASES[1], CASES[3], CASES[4]])
 @pytest.mark.parametrize("prec", [0, 1])
-def test_sharded_su3_operators(hr, orc, Lg, P, split, prec):
+@pytest.mark.parametrize("two_rows", [False, True])
+def test_sharded_su3_operators(hr, orc, Lg, P, split, prec, two_rows):
     """complex 3 x 3 links (HR_REP_SU3) on a cut lattice: the up faces are multiplied by the sender's U^dag, the receiver applies its own
     U to the down faces; full D and Dhat stitched from the shards against the oracle's global operator (rep 2)"""
     import torch
@@ -217,7 +218,7 @@ def test_sharded_su3_operators(hr, orc, Lg, P, split, prec):
     psi = inputs.gaussian_spinor(Lg, 3, 2)
     if prec:
         U, psi = U.astype(np.complex64).astype(np.complex128), psi.astype(np.complex64).astype(np.complex128)
-    shards = make_shards(hr, Lg, P, hr.REP_SU3, prec, split, hr.LINKS_FULL)
+    shards = make_shards(hr, Lg, P, hr.REP_SU3, prec, split, hr.LINKS_COMPRESSED if two_rows else hr.LINKS_FULL)
     Ud, pd, od, td = {}, {}, {}, {}
     for c, sh in shards.items():
         lat = sh.lat
