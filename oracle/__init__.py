@@ -312,3 +312,60 @@ def dirac_eo_clover_adj(L, R, A, Ainv, psi, nthreads=1):
     t = site_matvec_n(Ainv, t, odd)
     h = hop(L, 1, 0, R, t, nthreads=nthreads)               # H_eo (...) on even sites
     return site_matvec_n(A, pe, even) - 0.25 * h
+
+
+# ------------------------------------------------------------------ O12: clover term for complex 3 x 3 links (HR_REP_SU3)
+def clover_dense_su3(L, diag, csw, U):
+    """O12 (SURVEY.md §8(f) item 4 "other groups"): the clover term of O5 for complex 3 x 3 links U
+    (dagger = conjugate transpose), acting on 4 spin x 3 colour:
+        A(x) = diag + C(x),  C = csw (i/2) sum_{mu<nu} sigma_mu,nu (x) F^_mu,nu,  sigma_mu,nu = (i/2)[gamma_mu, gamma_nu],
+        F^_mu,nu = (Q - Q^dag)/8,  Q = P1 + P2 + P3 + P4 the four leaves of O5 that start and end at x (mu -> nu sense).
+    U: complex [V,4,3,3].  Returns dense [V,12,12] complex (row/col = spin*3 + colour).  Whole-lattice numpy shifts; the
+    same construction as O10 with the real adjoint links replaced by complex ones.  Pinned by P22."""
+    U = np.ascontiguousarray(U, dtype=np.complex128)
+    Lt = tuple(int(v) for v in L)
+    V = _vol(L)
+    Ug = U.reshape(Lt + (4, 3, 3))
+    gam = gamma()
+
+    def at(mu, shift):      # U_mu(x + shift), shift a dict {axis: displacement}
+        a = Ug[..., mu, :, :]
+        for ax, d in shift.items():
+            a = np.roll(a, -d, axis=ax)
+        return a
+
+    def H(m):
+        return np.conj(np.swapaxes(m, -1, -2))
+
+    A = np.zeros((V, 12, 12), dtype=np.complex128)
+    A += diag * np.eye(12)[None]
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            P1 = at(mu, {}) @ at(nu, {mu: 1}) @ H(at(mu, {nu: 1})) @ H(at(nu, {}))
+            P2 = at(nu, {}) @ H(at(mu, {mu: -1, nu: 1})) @ H(at(nu, {mu: -1})) @ at(mu, {mu: -1})
+            P3 = H(at(mu, {mu: -1})) @ H(at(nu, {mu: -1, nu: -1})) @ at(mu, {mu: -1, nu: -1}) @ at(nu, {nu: -1})
+            P4 = H(at(nu, {nu: -1})) @ at(mu, {nu: -1}) @ at(nu, {mu: 1, nu: -1}) @ H(at(mu, {}))
+            Q = P1 + P2 + P3 + P4
+            F = ((Q - H(Q)) / 8.0).reshape(V, 3, 3)
+            sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
+            A += csw * 0.5j * np.einsum("st,xab->xsatb", sig, F).reshape(V, 12, 12)
+    return A
+
+
+def clover_exp_dense_su3(L, diag, csw, U):
+    """the exponential site-diagonal term (O9 / O11, reading B4) for complex 3 x 3 links: (diag exp(C/diag), exp(-C/diag)/diag) with
+    C = clover_dense_su3(L, 0, csw, U); dense [V,12,12]."""
+    return _exp_hermitian_pair(clover_dense_su3(L, 0.0, csw, U), diag)
+
+
+def dirac_eo_clover_n(L, rep, U, A, Ainv, psi, nthreads=1):
+    """O7 for any representation of link() with dense site matrices: Dhat psi_e = A_ee psi_e - 1/4 H_eo A_oo^-1 H_oe psi_e (odd
+    output = 0); A, Ainv dense [V,4N,4N].  The construction of dirac_eo_clover_adj (pinned by P18) with the hop's representation
+    as an argument; rep = 2 (complex 3 x 3 links) is pinned by P22."""
+    par = (np.indices(tuple(int(v) for v in L)).sum(axis=0) % 2).reshape(-1)
+    even, odd = par == 0, par == 1
+    pe = np.where(even[:, None, None], psi, 0.0)
+    t = hop(L, rep, 1, U, pe, nthreads=nthreads)
+    t = site_matvec_n(Ainv, t, odd)
+    h = hop(L, rep, 0, U, t, nthreads=nthreads)
+    return site_matvec_n(A, pe, even) - 0.25 * h

@@ -752,3 +752,122 @@ def test_P21_complex_3x3_links(orc):
     assert rel_l2(got[..., :2], orc.dirac(L, 0, m0, U2, np.ascontiguousarray(psi[..., :2]))) < 1e-14
     free = orc.dirac(L, 2, m0, one, psi)
     assert rel_l2(got[..., 2], free[..., 2]) < 1e-14
+
+
+def test_P22_su3_clover(orc):
+    """O12 (clover term for complex 3 x 3 links) and dirac_eo_clover_n(rep = 2).  (a) SU(2) links embedded in the upper-left 2 x 2
+    block of a 3 x 3 unit matrix: the colour-(0,1) sub-block of O12 must be the FUNDAMENTAL SU(2) clover term of the C++ oracle
+    (O5/O6, explicit site loops — an independent implementation) and colour 2 must see the bare diagonal; (b) every site of a
+    Haar SU(3) field against leaves multiplied out here with explicit (x +- mu) mod L site arithmetic; (c) C hermitian,
+    traceless, commuting with gamma5; (d) gauge covariance under SU(3); (e) abelian links diag(e^{i a}, e^{i b}, e^{-i(a+b)}):
+    F^_mu,nu = (i/4) diag(sum over the four leaves of sin(plaquette angle)) per colour; (f) the Schur identity P4 for
+    dirac_eo_clover_n with D_sw = D[U] + C applied site by site here."""
+    L = (2, 2, 2, 4)
+    V = inputs.volume(L)
+    gam = orc.gamma()
+    d, csw = 3.7, 1.3
+    # (a)
+    U2 = inputs.haar_gauge(L, 1)
+    U3 = np.zeros((V, 4, 3, 3), dtype=complex)
+    U3[:, :, :2, :2] = U2
+    U3[:, :, 2, 2] = 1.0
+    A3 = orc.clover_dense_su3(L, d, csw, U3).reshape(V, 4, 3, 4, 3)
+    A2 = orc.clover_dense(L, d, csw, U2).reshape(V, 4, 2, 4, 2)
+    assert np.abs(A3[:, :, :2, :, :2] - A2).max() <= 1e-13
+    assert np.abs(A3[:, :, 2, :, 2] - d * np.eye(4)[None]).max() <= 1e-14
+    assert np.abs(A3[:, :, :2, :, 2]).max() == 0 and np.abs(A3[:, :, 2, :, :2]).max() == 0
+    # (b)
+    U = inputs.haar_gauge_su3(L, 1)
+    x_of = inputs.site_coords(L)
+
+    def lex(x):
+        return ((x[0] % L[0] * L[1] + x[1] % L[1]) * L[2] + x[2] % L[2]) * L[3] + x[3] % L[3]
+
+    def u(x, mu, dag=False):
+        m = U[lex(x), mu]
+        return m.conj().T if dag else m
+
+    def e(mu):
+        v = np.zeros(4, dtype=int)
+        v[mu] = 1
+        return v
+
+    A = orc.clover_dense_su3(L, d, csw, U)
+    for s_ in range(0, V, 3):
+        x = x_of[s_]
+        C = np.zeros((12, 12), dtype=complex)
+        for mu in range(4):
+            for nu in range(mu + 1, 4):
+                m, n = e(mu), e(nu)
+                Q = (u(x, mu) @ u(x + m, nu) @ u(x + n, mu, True) @ u(x, nu, True)
+                     + u(x, nu) @ u(x - m + n, mu, True) @ u(x - m, nu, True) @ u(x - m, mu)
+                     + u(x - m, mu, True) @ u(x - m - n, nu, True) @ u(x - m - n, mu) @ u(x - n, nu)
+                     + u(x - n, nu, True) @ u(x - n, mu) @ u(x + m - n, nu) @ u(x, mu, True))
+                F = (Q - Q.conj().T) / 8.0
+                sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
+                C += csw * 0.5j * np.kron(sig, F)
+        assert np.abs(A[s_] - d * np.eye(12) - C).max() <= 1e-13
+    # (c)
+    Cf = A - d * np.eye(12)[None]
+    assert np.abs(Cf - np.conj(np.swapaxes(Cf, -1, -2))).max() <= 1e-15
+    assert np.abs(np.trace(Cf, axis1=1, axis2=2)).max() <= 1e-14
+    g5 = np.kron(np.diag([1, 1, -1, -1]), np.eye(3)).astype(complex)
+    assert np.abs(g5 @ Cf - Cf @ g5).max() <= 1e-15
+    # (d) U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag  ->  C'(x) = g(x) C(x) g(x)^dag on colour
+    g = inputs.haar_sites_su3(L, 4)
+    Ug = np.empty_like(U)
+    gl = g.reshape(L + (3, 3))
+    for mu in range(4):
+        gs = np.roll(gl, -1, axis=mu).reshape(V, 3, 3)
+        Ug[:, mu] = g @ U[:, mu] @ np.conj(np.swapaxes(gs, -1, -2))
+    big = np.einsum("st,xab->xsatb", np.eye(4), g).reshape(V, 12, 12)
+    Cg = orc.clover_dense_su3(L, 0.0, csw, Ug)
+    assert np.abs(Cg - big @ Cf @ np.conj(np.swapaxes(big, -1, -2))).max() <= 1e-13
+    # (e)
+    ph = 0.4 * inputs.normals(11, 9, 0, V * 8).reshape(L + (4, 2))
+    ang = np.concatenate([ph, -ph.sum(axis=-1, keepdims=True)], axis=-1)          # three colour phases per link, sum 0
+    Uab = np.zeros((V, 4, 3, 3), dtype=complex)
+    for c in range(3):
+        Uab[:, :, c, c] = np.exp(1j * ang[..., c].reshape(V, 4))
+    Aab = orc.clover_dense_su3(L, 0.0, 1.0, Uab)
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            sig = 0.5j * (gam[mu] @ gam[nu] - gam[nu] @ gam[mu])
+            Fo = np.einsum("ts,xsatb->xab", sig, Aab.reshape(V, 4, 3, 4, 3)) / 4.0 / 0.5j
+            for c in range(3):
+                a = ang[..., c]
+                P = a[..., mu] + np.roll(a[..., nu], -1, mu) - np.roll(a[..., mu], -1, nu) - a[..., nu]
+                S = np.sin(P) + np.sin(np.roll(P, 1, mu)) + np.sin(np.roll(np.roll(P, 1, mu), 1, nu)) + np.sin(np.roll(P, 1, nu))
+                assert np.abs(Fo[:, c, c] - 0.25j * S.reshape(V)).max() <= 1e-13, (mu, nu, c)
+            off = Fo.copy()
+            off[:, range(3), range(3)] = 0
+            assert np.abs(off).max() <= 1e-15
+    # (f)
+    L4 = (2, 4, 2, 4)
+    m0 = -0.25
+    dd = 4.0 + m0
+    Uw = inputs.haar_gauge_su3(L4, 1)
+    par = inputs.site_parity(L4)
+    even, odd = par == 0, par == 1
+    Aw = orc.clover_dense_su3(L4, dd, 1.2, Uw)
+    Cw = Aw - dd * np.eye(12)[None]
+    Awinv = np.linalg.inv(Aw)
+    x = inputs.gaussian_spinor(L4, 3, seed=2)
+    eta = orc.dirac(L4, 2, m0, Uw, x) + _site_loop_matvec(Cw, x)
+    t = np.where(odd[:, None, None], _site_loop_matvec(Awinv, eta), 0.0)
+    rhs = np.where(even[:, None, None], eta, 0.0) + 0.5 * orc.hop(L4, 2, 0, Uw, t)
+    lhs = orc.dirac_eo_clover_n(L4, 2, Uw, Aw, Awinv, x)
+    assert rel_l2(lhs, rhs) < 1e-14 and not lhs[odd].any()
+    # the exponential pair: scipy's Pade expm on three sites, det = d^12
+    import scipy.linalg
+    Ae, Aei = orc.clover_exp_dense_su3(L4, dd, 1.2, Uw)
+    for s_ in (0, 17, inputs.volume(L4) - 1):
+        assert np.abs(Ae[s_] - dd * scipy.linalg.expm(Cw[s_] / dd)).max() <= 1e-12
+        assert np.abs(Ae[s_] @ Aei[s_] - np.eye(12)).max() <= 1e-13
+    assert np.abs(np.linalg.det(Ae) / dd ** 12 - 1).max() <= 1e-11
+    # and the adjoint wrapper is this function
+    Uf = inputs.weak_gauge(L4, 0.3, seed=1)
+    R, _ = orc.represent(Uf)
+    Ar = orc.clover_dense_adj(L4, dd, 1.2, R)
+    xa = inputs.gaussian_spinor(L4, 3, seed=2)
+    assert np.array_equal(orc.dirac_eo_clover_n(L4, 1, R, Ar, np.linalg.inv(Ar), xa), orc.dirac_eo_clover_adj(L4, R, Ar, np.linalg.inv(Ar), xa))
