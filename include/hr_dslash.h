@@ -47,9 +47,10 @@ enum { HR_OK = 0, HR_EINVAL = 1, HR_EUNSUPPORTED = 2, HR_EALIGN = 3, HR_ECUDA = 
  * colours and complex 3 x 3 links (canonical [V][4 mu][3][3][re,im]) kept on the device in full (link_storage = HR_LINKS_FULL, 18 reals)
  * or as their first two rows (HR_LINKS_COMPRESSED, 12 reals: the kernels and hr_unpack_gauge rebuild row 2 = conj(row 0 x row 1),
  * exact for unitary links of determinant 1).  It is
- * served by the generic hopping kernel: bare hops, full D, the even-odd operator without clover, the CG solvers and the sharded hop
- * (hr_halo_pack / hr_hop_local with the epilogues HR_EPI_NONE and HR_EPI_AXPY); the clover and representation calls and the clover
- * epilogues return HR_EUNSUPPORTED for it. */
+ * served by the generic hopping kernel: bare hops, full D, the even-odd operator with and without clover, the clover-improved full
+ * operator, the clover block builders (regular and exponential; hr_clover_build takes the SU(3) gauge field itself as u_fund;
+ * blocks are 6 x 6 like the adjoint ones), hr_clover_apply, the CG solvers and the sharded hop with every epilogue; only
+ * hr_represent_gauge returns HR_EUNSUPPORTED for it. */
 enum { HR_REP_FUND = 0, HR_REP_ADJ = 1, HR_REP_SU3 = 2 };
 enum { HR_PREC_F64 = 0, HR_PREC_F32 = 1 };
 /* fundamental links are stored as their first row (alpha, beta): U = [[alpha, beta], [-conj(beta), conj(alpha)]]

@@ -16,6 +16,7 @@ int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, c
 int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
+int run_clover_build_c3(const Geo& g, int prec, bool two_rows, double diag, double csw, int expo, const void* gauge, void* fwd, void* inv, cudaStream_t st);
 int run_clover_apply(const Geo& g, int rep, int prec, int parity, const void* blocks, const void* in, void* out, cudaStream_t st);
 int run_count_nonfinite(int prec, const void* x, size_t bytes, unsigned long long* count_dev, cudaStream_t st);
 
@@ -71,7 +72,7 @@ static int check_ptr(const void* p, const char* name) {
     return HR_OK;
 }
 static int check_no_su3(const hr_geom* g, const char* what) {
-    if (g->rep == HR_REP_SU3) { set_error("%s: not available for HR_REP_SU3 (bare hops, D, Dhat without clover and CG are)", what); return HR_EUNSUPPORTED; }
+    if (g->rep == HR_REP_SU3) { set_error("%s: not available for HR_REP_SU3", what); return HR_EUNSUPPORTED; }
     return HR_OK;
 }
 static int check_links(const hr_geom* g) {
@@ -209,7 +210,7 @@ int hr_dirac_apply(const hr_geom* g, double m0, const void* u, const void* psi, 
 }
 
 int hr_dirac_clover_apply(const hr_geom* g, const void* u, const void* clover_fwd, const void* psi, void* out, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_links(g)); HR_TRY(check_no_su3(g, "hr_dirac_clover_apply"));
+    HR_TRY(check_geom(g)); HR_TRY(check_links(g));
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(psi, "psi")); HR_TRY(check_ptr(out, "out"));
     const size_t full = 2 * half_spinor_bytes(g);
     if (overlap(psi, full, out, full)) { set_error("hr_dirac_clover_apply: out aliases psi (gather operation)"); return HR_EINVAL; }
@@ -238,7 +239,6 @@ int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const 
     if (overlap(tmp, half, in, half) || overlap(tmp, half, out, half)) { set_error("hr_dirac_eo_apply: tmp aliases in or out"); return HR_EINVAL; }
     const bool clover = clover_fwd || clover_inv;
     if (clover) {
-        HR_TRY(check_no_su3(g, "hr_dirac_eo_apply with clover"));
         if (!clover_fwd || !clover_inv) { set_error("hr_dirac_eo_apply: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
         HR_TRY(check_ptr(clover_fwd, "clover_fwd")); HR_TRY(check_ptr(clover_inv, "clover_inv"));
             // E2: tmp_o = A_oo^-1 H_oe in_e ;  out_e = A_ee in_e - 1/4 H_eo tmp_o
@@ -286,7 +286,7 @@ static int hop_local_phases(int phases, const hr_geom* g, const hr_decomp* d, in
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(out_half, "out_half"));
     if (phases & 1) HR_TRY(check_ptr(in_half, "in_half"));
     if ((phases & 1) && (epi == HR_EPI_AXPY || epi == HR_EPI_CLOVER_AXPY)) HR_TRY(check_ptr(phi_half, "phi_half"));
-    if (epi == HR_EPI_CLOVER_INV || epi == HR_EPI_CLOVER_AXPY) { HR_TRY(check_no_su3(g, "hr_hop_local with a clover epilogue")); HR_TRY(check_ptr(clover, "clover")); }
+    if (epi == HR_EPI_CLOVER_INV || epi == HR_EPI_CLOVER_AXPY) HR_TRY(check_ptr(clover, "clover"));
     const size_t half = half_spinor_bytes(g);
     if ((phases & 1) && overlap(in_half, half, out_half, half)) { set_error("hr_hop_local: out aliases in (gather operation)"); return HR_EINVAL; }
     int mask = 0;
@@ -324,12 +324,14 @@ int hr_hop_local_boundary(const hr_geom* g, const hr_decomp* d, int out_parity, 
 
 // ---------------------------------------------------------------- C1 / C2 / C3
 static int clover_build_any(const hr_geom* g, double m0, double csw, int expo, const void* u_fund, void* clover_fwd, void* clover_inv, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_no_su3(g, "hr_clover_build")); HR_TRY(check_ptr(u_fund, "u_fund"));
-    if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund"));
+    if (g->rep != HR_REP_SU3 && g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     if (!clover_fwd && !clover_inv) { set_error("hr_clover_build: nothing to build"); return HR_EINVAL; }
     if (4.0 + m0 == 0.0) { set_error("hr_clover_build: 4+m0 = 0"); return HR_EINVAL; }
     if (clover_fwd) HR_TRY(check_ptr(clover_fwd, "clover_fwd"));
     if (clover_inv) HR_TRY(check_ptr(clover_inv, "clover_inv"));
+    if (g->rep == HR_REP_SU3)     // u_fund is then the SU(3) gauge field itself (all three rows, or two with HR_LINKS_COMPRESSED)
+        return run_clover_build_c3(make_geo(g), g->prec, g->link_storage == HR_LINKS_COMPRESSED, 4.0 + m0, csw, expo, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
     if (g->rep == HR_REP_ADJ) return run_clover_build_adj(make_geo(g), g->prec, 4.0 + m0, csw, expo, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
     return run_clover_build(make_geo(g), g->prec, 4.0 + m0, csw, expo, u_fund, clover_fwd, clover_inv, (cudaStream_t)stream);
 }
@@ -345,7 +347,7 @@ int hr_clover_build_exp(const hr_geom* g, double m0, double csw, const void* u_f
 }
 
 int hr_clover_apply(const hr_geom* g, int parity, const void* blocks, const void* in, void* out, void* stream) {
-    HR_TRY(check_geom(g)); HR_TRY(check_no_su3(g, "hr_clover_apply"));
+    HR_TRY(check_geom(g));
     if (parity < HR_EVEN || parity > HR_BOTH) { set_error("hr_clover_apply: parity %d", parity); return HR_EINVAL; }
     HR_TRY(check_ptr(blocks, "blocks")); HR_TRY(check_ptr(in, "in")); HR_TRY(check_ptr(out, "out"));
     return run_clover_apply(make_geo(g), g->rep, g->prec, parity, blocks, in, out, (cudaStream_t)stream);
@@ -370,7 +372,6 @@ int hr_cg_solve(const hr_geom* g, double m0, const void* u, const void* clover_f
     HR_TRY(check_ptr(u, "u")); HR_TRY(check_ptr(b, "b")); HR_TRY(check_ptr(x, "x")); HR_TRY(check_ptr(workspace, "workspace"));
     if (!(tol > 0.0) || max_iter < 0 || check_every < 1) { set_error("hr_cg_solve: tol must be > 0, max_iter >= 0, check_every >= 1"); return HR_EINVAL; }
     if ((clover_fwd == nullptr) != (clover_inv == nullptr)) { set_error("hr_cg_solve: clover_fwd and clover_inv must both be given"); return HR_EINVAL; }
-    if (clover_fwd) HR_TRY(check_no_su3(g, "hr_cg_solve with clover"));
     const size_t half = half_spinor_bytes(g);
     if (overlap(b, half, x, half)) { set_error("hr_cg_solve: x aliases b"); return HR_EINVAL; }
     if (overlap(workspace, cg_workspace_bytes(g), x, half) || overlap(workspace, cg_workspace_bytes(g), b, half)) {
@@ -437,7 +438,7 @@ int hr_dirac_flops_bytes(const hr_geom* g, int op, double* flops_per_site, doubl
     const double Fhop = g->rep != HR_REP_ADJ ? 8.0 * N * (16.0 * N + 7.0) : 8.0 * N * (8.0 * N + 7.0);   // complex links (624, SU(3): 1320) : real links (744)
     const double Fblk = 2.0 * (2.0 * (2 * N) + 8.0 * (2 * N) * (2 * N - 1));   // two hermitian 2N x 2N mat-vecs: 208 (fund), 504 (adj)
     double f = 0, bc = 0, br = 0;
-    if (g->rep == HR_REP_SU3 && (op == HR_OP_CLOVER || op == HR_OP_DHAT_CLOVER || op == HR_OP_REPRESENT)) return check_no_su3(g, "hr_dirac_flops_bytes of a clover / representation op");
+    if (g->rep == HR_REP_SU3 && op == HR_OP_REPRESENT) return check_no_su3(g, "hr_dirac_flops_bytes of the representation op");
     switch (op) {
         case HR_OP_HOP: f = Fhop; bc = 2 * S + 8 * G; br = 9 * S + 8 * G; break;
         case HR_OP_DIRAC: f = Fhop + 3 * nr; bc = 2 * S + 4 * G; br = 10 * S + 8 * G; break;

@@ -509,6 +509,152 @@ __global__ void clover_build_adj_kernel(Geo g, double diag, double csw, int expo
     }
 }
 
+// C1 for complex 3 x 3 links (HR_REP_SU3; oracle O12): the same 6 x 6 chirality blocks on (2 spin x 3 colour),
+//   A+- = (4+m0) + (csw/2) [ tau1 (x) i(+-F01 - F23) + tau2 (x) i(+-F02 + F13) + tau3 (x) i(+-F03 - F12) ],
+// with F^_mu,nu = (Q - Q^dag)/8 the anti-hermitian part of the four leaves, multiplied out as complex 3 x 3 matrices.
+template <typename T, bool TWOROWS>
+__device__ __forceinline__ void link_c3(dcplx (*m)[3], const void* gauge, const Geo& g, int x0, int x1, int x2, int x3, int mu, bool dag) {
+    const SiteRef s = site_of_coords(g, x0, x1, x2, x3);
+    LinkC3<T> u;
+    load_link_rep<T, LD_KEEP, TWOROWS>(u, gauge, g, s.par, mu, s.row, s.h);
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            const cplx<T> z = dag ? u.m[3 * b + a] : u.m[3 * a + b];
+            m[a][b].re = (double)z.re;
+            m[a][b].im = dag ? -(double)z.im : (double)z.im;
+        }
+}
+
+// F[a][b] = ((Q - Q^dag)/8)[a][b] of the mu-nu plane at x
+template <typename T, bool TWOROWS>
+__device__ void clover_leaves_c3(dcplx (*F)[3], const void* gauge, const Geo& g, const int* x, int mu, int nu) {
+    int e[4] = {0, 0, 0, 0}, f[4] = {0, 0, 0, 0};
+    e[mu] = 1;
+    f[nu] = 1;
+    dcplx Q[3][3], A[3][3], B[3][3], C[3][3];
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) Q[a][b].re = Q[a][b].im = 0.0;
+    // the four links of a leaf as (displacement in mu, displacement in nu, direction, dagger), in path order
+    const int path[4][4][4] = {
+        {{0, 0, 0, 0}, {1, 0, 1, 0}, {0, 1, 0, 1}, {0, 0, 1, 1}},
+        {{0, 0, 1, 0}, {-1, 1, 0, 1}, {-1, 0, 1, 1}, {-1, 0, 0, 0}},
+        {{-1, 0, 0, 1}, {-1, -1, 1, 1}, {-1, -1, 0, 0}, {0, -1, 1, 0}},
+        {{0, -1, 1, 1}, {0, -1, 0, 0}, {1, -1, 1, 0}, {0, 0, 0, 1}}};
+    for (int leaf = 0; leaf < 4; ++leaf) {
+        for (int k = 0; k < 4; ++k) {
+            const int dm = path[leaf][k][0], dn = path[leaf][k][1], dir = path[leaf][k][2] ? nu : mu;
+            link_c3<T, TWOROWS>(B, gauge, g, x[0] + dm * e[0] + dn * f[0], x[1] + dm * e[1] + dn * f[1], x[2] + dm * e[2] + dn * f[2],
+                                x[3] + dm * e[3] + dn * f[3], dir, path[leaf][k][3] != 0);
+            if (k == 0) {
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) A[a][b] = B[a][b];
+            } else {
+                matmul_d<3>(C, A, B);
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) A[a][b] = C[a][b];
+            }
+        }
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) Q[a][b] = dadd(Q[a][b], A[a][b]);
+    }
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+            F[a][b].re = (Q[a][b].re - Q[b][a].re) / 8.0;
+            F[a][b].im = (Q[a][b].im + Q[b][a].im) / 8.0;
+        }
+}
+
+// the two 6 x 6 blocks and their inverses (or the exponential pair) from the six F matrices (planes 01 02 03 12 13 23)
+__device__ __noinline__ void clover_c3_blocks(double diag, double csw, int expo, const dcplx (*F)[3][3], double* reals_f, double* reals_i) {
+    const dcplx Z = {0.0, 0.0}, P1 = {1.0, 0.0}, M1 = {-1.0, 0.0}, PI = {0.0, 1.0}, MI = {0.0, -1.0};
+    const dcplx pauli[3][2][2] = {{{Z, P1}, {P1, Z}}, {{Z, MI}, {PI, Z}}, {{P1, Z}, {Z, M1}}};
+    for (int chi = 0; chi < 2; ++chi) {
+        const double s = chi == 0 ? 1.0 : -1.0;
+        dcplx A[6][6];
+        for (int sp = 0; sp < 2; ++sp)
+            for (int c = 0; c < 3; ++c)
+                for (int tp = 0; tp < 2; ++tp)
+                    for (int d = 0; d < 3; ++d) {
+                        dcplx acc = {(sp == tp && c == d) ? diag : 0.0, 0.0};
+                        for (int k = 0; k < 3; ++k) {
+                            // G_k = +-F0k -+ ... : (s F01 - F23), (s F02 + F13), (s F03 - F12)
+                            const dcplx a0 = F[k][c][d], a1 = F[k == 0 ? 5 : k == 1 ? 4 : 3][c][d];
+                            const double sg = k == 1 ? 1.0 : -1.0;
+                            const dcplx G = {s * a0.re + sg * a1.re, s * a0.im + sg * a1.im};
+                            const dcplx iG = {-G.im, G.re};
+                            const dcplx tx = dmul(pauli[k][sp][tp], iG);
+                            acc.re += 0.5 * csw * tx.re;
+                            acc.im += 0.5 * csw * tx.im;
+                        }
+                        A[sp * 3 + c][tp * 3 + d] = acc;
+                    }
+        if (expo) {
+            dcplx X[6][6], E[6][6];
+            for (int i = 0; i < 6; ++i)
+                for (int j = 0; j < 6; ++j) { X[i][j].re = (A[i][j].re - (i == j ? diag : 0.0)) / diag; X[i][j].im = A[i][j].im / diag; }
+            expm_d<6>(E, X);
+            for (int i = 0; i < 6; ++i)
+                for (int j = 0; j < 6; ++j) { A[i][j].re = diag * E[i][j].re; A[i][j].im = diag * E[i][j].im; X[i][j].re = -X[i][j].re; X[i][j].im = -X[i][j].im; }
+            herm_to_reals_d<double, 6>(reals_f + 36 * chi, A);
+            expm_d<6>(E, X);
+            for (int i = 0; i < 6; ++i)
+                for (int j = 0; j < 6; ++j) { A[i][j].re = E[i][j].re / diag; A[i][j].im = E[i][j].im / diag; }
+            herm_to_reals_d<double, 6>(reals_i + 36 * chi, A);
+        } else {
+            herm_to_reals_d<double, 6>(reals_f + 36 * chi, A);
+            invert_d<6>(A);
+            herm_to_reals_d<double, 6>(reals_i + 36 * chi, A);
+        }
+    }
+}
+
+template <typename T, bool TWOROWS>
+__global__ void clover_build_c3_kernel(Geo g, double diag, double csw, int expo, const void* __restrict__ gauge, void* fwd, void* inv) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 2 * g.Vh) return;
+    const int par = t / g.Vh, cb = t - par * g.Vh;
+    const int row = cb / g.L3h, h = cb - row * g.L3h;
+    int x[4];
+    x[0] = row / g.s0;
+    const int rem = row - x[0] * g.s0;
+    x[1] = rem / g.s1;
+    x[2] = rem - x[1] * g.s1;
+    x[3] = 2 * h + ((x[0] + x[1] + x[2] + par) & 1);
+    dcplx F[6][3][3];
+    clover_leaves_c3<T, TWOROWS>(F[0], gauge, g, x, 0, 1);
+    clover_leaves_c3<T, TWOROWS>(F[1], gauge, g, x, 0, 2);
+    clover_leaves_c3<T, TWOROWS>(F[2], gauge, g, x, 0, 3);
+    clover_leaves_c3<T, TWOROWS>(F[3], gauge, g, x, 1, 2);
+    clover_leaves_c3<T, TWOROWS>(F[4], gauge, g, x, 1, 3);
+    clover_leaves_c3<T, TWOROWS>(F[5], gauge, g, x, 2, 3);
+    constexpr int NR = 72;
+    double rf[NR], ri[NR];
+    clover_c3_blocks(diag, csw, expo, F, rf, ri);
+    constexpr int CCH = NR * sizeof(T) / 16;
+    constexpr int PER = 16 / sizeof(T);
+    typedef typename Chunk<T>::type chunk_t;
+    const size_t first = ((size_t)par * g.R + row) * (CCH * g.L3h) + h;
+    for (int c = 0; c < CCH; ++c) {
+        T ef[PER], ei[PER];
+        for (int k = 0; k < PER; ++k) { ef[k] = (T)rf[c * PER + k]; ei[k] = (T)ri[c * PER + k]; }
+        if (fwd) reinterpret_cast<chunk_t*>(fwd)[first + (size_t)c * g.L3h] = reals_to_chunk(ef);
+        if (inv) reinterpret_cast<chunk_t*>(inv)[first + (size_t)c * g.L3h] = reals_to_chunk(ei);
+    }
+}
+
+int run_clover_build_c3(const Geo& g, int prec, bool two_rows, double diag, double csw, int expo, const void* gauge, void* fwd, void* inv, cudaStream_t st) {
+    const unsigned nb = blocks_for(2LL * g.Vh, 64);
+    if (prec == HR_PREC_F64) {
+        if (two_rows) clover_build_c3_kernel<double, true><<<nb, 64, 0, st>>>(g, diag, csw, expo, gauge, fwd, inv);
+        else clover_build_c3_kernel<double, false><<<nb, 64, 0, st>>>(g, diag, csw, expo, gauge, fwd, inv);
+    } else {
+        if (two_rows) clover_build_c3_kernel<float, true><<<nb, 64, 0, st>>>(g, diag, csw, expo, gauge, fwd, inv);
+        else clover_build_c3_kernel<float, false><<<nb, 64, 0, st>>>(g, diag, csw, expo, gauge, fwd, inv);
+    }
+    count_launch();
+    return check_launch("clover_build_c3_kernel");
+}
+
 int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st) {
     const unsigned nb = blocks_for(2LL * g.Vh, 64);
     if (prec == HR_PREC_F64) clover_build_adj_kernel<double><<<nb, 64, 0, st>>>(g, diag, csw, expo, ufund, fwd, inv);

@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(128) halo_boundary_kernel(Geo g, BoundaryJob j
     HR_BND(0) HR_BND(1) HR_BND(2) HR_BND(3)
 #undef HR_BND
     if (!any) return;
-    if (EPI == EPI_CLOVER_INV && !C3) {      // B(x) is linear: one block product for the sum of the crossing terms
+    if (EPI == EPI_CLOVER_INV) {      // B(x) is linear: one block product for the sum of the crossing terms
         T blk[CloverSize<N>::reals];
         cplx<T> y[NC];
         load_clover<T, N>(blk, a.clover, g, par, row, h);
@@ -238,13 +238,12 @@ static int add_boundary(const hr_geom* hg, const int* split, const HopArgs& a, i
         if (job.f[mu].nface > maxface) maxface = job.f[mu].nface;
     }
     if (job.nslots == 0) return HR_OK;
-    if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
     const dim3 grid((maxface + 127) / 128, job.nslots);
     switch (epi) {
         case EPI_NONE: halo_boundary_kernel<T, N, EPI_NONE, ONFLY, C3><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
         case EPI_AXPY: halo_boundary_kernel<T, N, EPI_AXPY, ONFLY, C3><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
-        case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY, false><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
-        case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
+        case EPI_CLOVER_INV: halo_boundary_kernel<T, N, EPI_CLOVER_INV, ONFLY, C3><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
+        case EPI_CLOVER_AXPY: halo_boundary_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, C3><<<grid, 128, 0, st>>>(g, job, a.parity, a); break;
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
     count_launch();

@@ -168,12 +168,11 @@ inline int launch_hop_generic_both(const Geo& g, const HopArgs& a_in, int epi, c
     HopArgs a = a_in;
     a.slab_w1 = generic_slab_w1(g, BOTH, (size_t)(16 * N + 4 * (C3 ? (ONFLY ? 12 : 18) : ONFLY ? 4 : N == 2 ? 4 : 9)) * sizeof(T));
     dim3 block(128), grid(((g.Vh + 127) / 128) * (BOTH ? 2 : 1));
-    if (C3 && (epi == EPI_CLOVER_INV || epi == EPI_CLOVER_AXPY)) { set_error("HR_REP_SU3 has no clover term yet"); return HR_EUNSUPPORTED; }
     switch (epi) {
         case EPI_NONE: hop_generic_kernel<T, N, EPI_NONE, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
         case EPI_AXPY: hop_generic_kernel<T, N, EPI_AXPY, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY, false, BOTH><<<grid, block, 0, st>>>(g, a); break;
-        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, false, BOTH><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_INV: hop_generic_kernel<T, N, EPI_CLOVER_INV, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
+        case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
     count_launch();

@@ -203,8 +203,9 @@ def test_su3_geometry_and_sizes(L):
     assert hr.hr_dirac_flops_bytes(g2, hr.OP_HOP)[1] == 2 * 192.0 + 8 * 96.0
     bad = hr.geom((4, 4, 4, 8), hr.REP_SU3, hr.PREC_F64, hr.LINKS_ONTHEFLY)
     assert hr.hr_spinor_bytes(bad, hr.BOTH) == 0
+    assert hr.hr_dirac_flops_bytes(g, hr.OP_CLOVER)[1] == 2 * 192.0 + 2 * 36 * 8.0        # two hermitian 6 x 6 blocks per site
     with pytest.raises(hr.HrError):
-        hr.hr_dirac_flops_bytes(g, hr.OP_CLOVER)
+        hr.hr_dirac_flops_bytes(g, hr.OP_REPRESENT)
 
 
 def test_kernel_plan_of_the_bench_lattice(L):

@@ -800,6 +800,57 @@ def test_adjoint_clover(hr, orc, L, prec, exponential):
             assert rel(lat.get_spinor(lat.dirac_clover(U_dev, fwd, psi_dev)), want_dsw) <= TOL[prec], (storage, kernel)
 
 
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 4, 6, 8)])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("exponential", [False, True])
+@pytest.mark.parametrize("two_rows", [False, True])
+def test_su3_clover(hr, orc, L, prec, exponential, two_rows):
+    """complex 3 x 3 links (HR_REP_SU3): 6 x 6 blocks and inverses (regular and exponential) against the oracle's O12 (pinned by
+    P22), C2/C3 on them, the even-odd operator with clover (E2), the full clover-improved operator and the CG solver on the
+    clover-improved system; links stored in full and as two rows"""
+    import torch
+    from paper_2411_18511_b200.lattice import Lattice
+    m0, csw = -0.25, 1.2
+    d = 4.0 + m0
+    U = rounded(inputs.haar_gauge_su3(L, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
+    if exponential:
+        A, Ainv = orc.clover_exp_dense_su3(L, d, csw, U)
+    else:
+        A = orc.clover_dense_su3(L, d, csw, U)
+        Ainv = np.linalg.inv(A)
+    bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+    tol_blk = 1e-13 if prec == 0 else 2e-6
+    want_dhat = orc.dirac_eo_clover_n(L, 2, U, A, Ainv, psi, nthreads=NTHREADS)
+    H = orc.hop(L, 2, 0, U, psi, nthreads=NTHREADS)
+    H = orc.hop(L, 2, 1, U, psi, nthreads=NTHREADS, out=H)
+    want_dsw = orc.site_matvec_n(A, psi) - 0.5 * H
+    lat = Lattice(L, hr.REP_SU3, prec, 0, link_storage=hr.LINKS_COMPRESSED if two_rows else hr.LINKS_FULL)
+    U_dev, psi_dev = lat.put_gauge_su3(U), lat.put_spinor(psi)
+    fwd, inv = lat.clover_build(m0, csw, U_dev, exponential=exponential)
+    assert np.linalg.norm(lat.get_clover(fwd) - bf) <= tol_blk * np.linalg.norm(bf)
+    assert np.linalg.norm(lat.get_clover(inv) - bi) <= tol_blk * np.linalg.norm(bi)
+    got = lat.get_spinor(lat.clover_apply(hr.BOTH, fwd, psi_dev))
+    assert rel(got, orc.site_matvec_n(A, psi)) <= TOL[prec]
+    half = torch.zeros_like(psi_dev)
+    lat.clover_apply(hr.ODD, inv, lat.odd(psi_dev), lat.odd(half))
+    assert rel(lat.get_spinor(half), orc.site_matvec_n(Ainv, psi, inputs.site_parity(L) == 1)) <= TOL[prec]
+    out = torch.zeros_like(psi_dev)
+    lat.dhat(m0, U_dev, lat.even(psi_dev), lat.even(out), clover_fwd=fwd, clover_inv=inv)
+    assert rel(lat.get_spinor(out), want_dhat) <= TOL[prec]
+    assert rel(lat.get_spinor(lat.dirac_clover(U_dev, fwd, psi_dev)), want_dsw) <= TOL[prec]
+    if prec == 0 and L == (4, 4, 4, 4) and not exponential:
+        b = psi.copy()
+        b[inputs.site_parity(L) == 1] = 0
+        dh = lambda v: orc.dirac_eo_clover_n(L, 2, U, A, Ainv, v, nthreads=NTHREADS)
+        x_orc, it_orc, _ = orc.cg_normal(L, 2, m0, U, b, tol=1e-12, max_iter=500, dhat=dh)
+        b_dev = lat.put_spinor(b)
+        x_half, it, relres = lat.cg(m0, U_dev, lat.even(b_dev), 1e-12, 500, clover_fwd=fwd, clover_inv=inv, check_every=1)
+        full = torch.zeros_like(b_dev)
+        lat.even(full).copy_(x_half)
+        assert relres <= 1e-12 and abs(it - it_orc) <= 2 and rel(lat.get_spinor(full), x_orc) <= 1e-9
+
+
 @pytest.mark.parametrize("rep", [0, 1])
 def test_cg_with_clover_all_variants(hr, orc, rep):
     """hr_cg_solve and hr_cg_solve_mixed_clover on the clover-improved even-odd system, fundamental and adjoint,
@@ -927,8 +978,6 @@ def test_su3_small_lattices(hr, orc, L, prec, two_rows):
     f, bc, _ = hr.hr_dirac_flops_bytes(lat.g, hr.OP_HOP)
     w = 8 if prec == 0 else 4
     assert f == 1320.0 and bc == 2 * 24 * w + 8 * (12 if two_rows else 18) * w
-    with pytest.raises(hr.HrError):
-        lat.clover_build(m0, 1.0, U_dev)
     if prec == 0 and L == (4, 4, 4, 4):
         b = psi.copy()
         b[inputs.site_parity(L) == 1] = 0

@@ -238,10 +238,20 @@ def test_sharded_su3_operators(hr, orc, Lg, P, split, prec, two_rows):
     halo.dhat_all(shards, halo.exchange_in_process, m0, Ud, {c: sh.lat.even(pd[c]) for c, sh in shards.items()},
                   {c: sh.lat.even(od[c]) for c, sh in shards.items()}, td)
     assert rel(gather(), orc.dirac_eo(Lg, 2, m0, U, psi, nthreads=NTHREADS)) <= TOL[prec]
-    # the clover epilogues are not there for this representation: refused, not silently wrong
-    sh = next(iter(shards.values()))
-    with pytest.raises(hr.HrError):
-        sh.hop(hr.ODD, Ud[sh.coords], sh.lat.even(pd[sh.coords]), sh.lat.odd(od[sh.coords]), epi=hr.EPI_CLOVER_INV, clover=pd[sh.coords])
+    # Dhat with clover (E2) through the clover epilogues of the interior and boundary kernels
+    m0c, csw = -0.25, 1.2
+    A = orc.clover_dense_su3(Lg, 4.0 + m0c, csw, U)
+    Ainv = np.linalg.inv(A)
+    from test_gpu_parity import dense_to_blocks
+    bf, bi = dense_to_blocks(A), dense_to_blocks(Ainv)
+    fw, iv = {}, {}
+    for c, sh in shards.items():
+        fw[c] = sh.lat.put_clover(halo.local_block(bf, Lg, P, c))
+        iv[c] = sh.lat.put_clover(halo.local_block(bi, Lg, P, c))
+        od[c].zero_()
+    halo.dhat_all(shards, halo.exchange_in_process, m0c, Ud, {c: sh.lat.even(pd[c]) for c, sh in shards.items()},
+                  {c: sh.lat.even(od[c]) for c, sh in shards.items()}, td, clover_fwd=fw, clover_inv=iv)
+    assert rel(gather(), orc.dirac_eo_clover_n(Lg, 2, U, A, Ainv, psi, nthreads=NTHREADS)) <= TOL[prec]
 
 
 @pytest.mark.gpu
