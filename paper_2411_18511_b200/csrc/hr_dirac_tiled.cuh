@@ -37,8 +37,9 @@ constexpr int DT_HALO = 2;
 __host__ __device__ constexpr int dt_ring(bool alink, size_t real_bytes) { return alink ? 3 : DT_RING; }
 __host__ __device__ constexpr int dt_nhalo(bool alink, size_t real_bytes) { return (alink && real_bytes == 4) ? 3 : DT_HALO; }
 
-// consumer threads the kernel is compiled for: one per site of a T1 x T2 tile of full x3-rows of up to 48 sites
-constexpr int dt_max_consumers(int t1, int t2) { return t1 * t2 * 48; }
+// consumer threads the kernel is compiled for: one per site of a T1 x T2 tile of full x3-rows of up to 48 sites (2 x 2, 2 x 4 tiles) or
+// up to 96 sites (the 1 x 2 tile of long rows, L3 = 50 .. 96)
+constexpr int dt_max_consumers(int t1, int t2) { return t1 * t2 * (t1 * t2 <= 2 ? 96 : 48); }
 
 struct DiracPlan {
     int t1, t2;        // tile shape in rows (x1, x2)
@@ -355,11 +356,12 @@ inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, Dir
     return true;
 }
 
-// fundamental representation only: 2 x 2 rows in fp64, 2 x 4 in fp32 (rows half as long)
+// fundamental representation only: 2 x 2 rows in fp64, 2 x 4 in fp32 (rows half as long), 1 x 2 for rows too long for those
 inline bool dirac_plan(const hr_geom* hg, int num_sms, DiracPlan& pl, bool alink = true) {
     if (hg->rep != HR_REP_FUND) return false;
     if (hg->prec == HR_PREC_F32 && dirac_plan_shape(hg, num_sms, 2, 4, pl, alink)) return true;
-    return dirac_plan_shape(hg, num_sms, 2, 2, pl, alink);
+    if (dirac_plan_shape(hg, num_sms, 2, 2, pl, alink)) return true;
+    return dirac_plan_shape(hg, num_sms, 1, 2, pl, alink);      // long rows (L3 = 50 .. 96)
 }
 
 template <typename T, int T1, int T2, int L3H, bool ALINK>
@@ -381,6 +383,7 @@ inline int launch_dirac_tiled_a(const Geo& g, const HopArgs& a, const DiracPlan&
             return launch_dirac_tiled_l3h<T, 2, 4, 0, ALINK>(g, a, pl, st);
         }
     }
+    if (pl.t1 == 1 && pl.t2 == 2) return launch_dirac_tiled_l3h<T, 1, 2, 0, ALINK>(g, a, pl, st);
     if (g.L3h == 24) return launch_dirac_tiled_l3h<T, 2, 2, 24, ALINK>(g, a, pl, st);
     return launch_dirac_tiled_l3h<T, 2, 2, 0, ALINK>(g, a, pl, st);
 }
