@@ -70,9 +70,13 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
     IO::store(out_half, first, g.L3h, acc);
 }
 
+// resident CTAs per SM the kernel is compiled for: the fp64 kernels with three colours need 130-138 registers left alone (3 CTAs of
+// 4 warps per SM: 18 % of the warp slots, DRAM 58-68 % busy); held to 128 registers (4 CTAs, a few bytes of spills) the SU(3) hop at
+// 48^4 goes from 729 to 634 us.  5 CTAs (102 registers) spill heavily and lose 25 %; the other instantiations gain nothing.
+template <typename T, int N> constexpr int generic_min_ctas() { return (N == 3 && sizeof(T) == 8) ? 4 : 1; }
 // C3: the links are complex 3 x 3 matrices stored in full (HR_REP_SU3; N = 3)
 template <typename T, int N, int EPI, bool ONFLY, bool C3 = false, bool BOTH = false>
-__global__ void __launch_bounds__(128) hop_generic_kernel(Geo g, HopArgs a) {
+__global__ void __launch_bounds__(128, generic_min_ctas<T, N>()) hop_generic_kernel(Geo g, HopArgs a) {
     static_assert(!C3 || N == 3, "complex 3 x 3 links: N = 3 (ONFLY then means: two rows stored, third rebuilt)");
     typedef typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type link_t;
     constexpr int NC = 4 * N;
