@@ -431,6 +431,11 @@ struct HopArgs;
 int run_hop(const hr_geom* g, const HopArgs& a, int epi, cudaStream_t st);
 bool tiled_supported(const hr_geom* g);
 bool tiled_chosen(const hr_geom* g);
-int kernel_plan(const hr_geom* g, int both, int* info);   // both: 0 parity hop, 1 paired-parity launch, 2 full D with phi == in
+int kernel_plan(const hr_geom* g, int both, int* info);
+int sm_count();
+// hr_hop_cg.cu: a parity hop with an axpy-type epilogue followed by a POST_* stage of the CG solver (hr_hop_generic.cuh);
+// hop_post_blocks = the number of partial sums such a launch writes to HopArgs::partial
+int run_hop_post(const hr_geom* g, const HopArgs& a, int epi, int post, cudaStream_t st);
+int hop_post_blocks(const hr_geom* g);   // both: 0 parity hop, 1 paired-parity launch, 2 full D with phi == in
 
 }  // namespace hr

@@ -7,7 +7,7 @@ namespace hr {
 // many small CTAs spread better there than one marching CTA per tile
 static const double TILED_AUTO_MIN_SITES = 32.0 * 32.0 * 32.0 * 32.0;
 
-static int sm_count() {   // of the calling thread's current device (cached per device)
+int sm_count() {   // of the calling thread's current device (cached per device)
     static std::atomic<int> cache[64];
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return 148; }

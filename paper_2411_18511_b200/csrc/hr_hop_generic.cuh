@@ -15,6 +15,12 @@ enum {
     EPI_CLOVER_AXPY = 3  // out = B(x) phi(x) + c*h      (B = A_ee)
 };
 
+// what happens to the epilogue's result w(x) (SURVEY.md §8(f) item 2 "fused dot products and axpys in the hop epilogue"):
+//   POST_STORE     : out = w
+//   POST_G5_NORM   : out = gamma5 w,  partial += |w|^2                                        (s = gamma5 Dhat p and <p, Dhat^dag Dhat p>)
+//   POST_CG_UPDATE : r -= alpha gamma5 w,  partial += |r|^2,  x += alpha p   (w is not stored)   (the CG update after the second Dhat)
+enum { POST_STORE = 0, POST_G5_NORM = 1, POST_CG_UPDATE = 2 };
+
 struct HopArgs {
     const void* gauge;   // gauge field in the fermion representation, device layout
     const void* in;      // both == 0: half field of parity 1-parity; both == 1: full field
@@ -24,6 +30,12 @@ struct HopArgs {
     double a, c;
     int parity;          // output parity when both == 0
     int both;            // 1: full-lattice launch, both output parities (in / out / phi are full fields)
+    // POST_* stages of the CG solver (hr_solver.cu), applied to the value the epilogue would have stored:
+    double* partial = nullptr;        // one partial sum per CTA (fixed order inside the CTA)
+    const double* cg_alpha = nullptr; // device scalar alpha (POST_CG_UPDATE)
+    void* cg_r = nullptr;             // half fields of the output parity (POST_CG_UPDATE): r -= alpha gamma5 w,
+    void* cg_x = nullptr;             //   x += alpha p
+    const void* cg_p = nullptr;
     int slab_w1 = 0;     // > 0: the generic kernel walks the lattice in x1-slabs of this width (launch_hop_generic sets it)
     int open_mask = 0;   // bit mu set: direction mu is cut between ranks (hr_hop_local): the forward term of sites with
                          // x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out here and added from
@@ -32,9 +44,9 @@ struct HopArgs {
 
 // PHI_POLICY: LD_STREAM when phi is read by this kernel only; LD_KEEP in the full-lattice launch (H3), where
 // phi is the other parity pass's gather input
-template <typename T, int N, int EPI, int PHI_POLICY = LD_STREAM>
+template <typename T, int N, int EPI, int PHI_POLICY = LD_STREAM, int POST = POST_STORE>
 __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const HopArgs& a, const void* phi_half,
-                                             void* out_half, int p, int row, int h) {
+                                             void* out_half, int p, int row, int h, double* part = nullptr, T alpha = (T)0) {
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
     const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
@@ -67,7 +79,51 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
             acc[k].im = fma(cc, acc[k].im, y[k].im);
         }
     }
-    IO::store(out_half, first, g.L3h, acc);
+    if (POST == POST_STORE) {
+        IO::store(out_half, first, g.L3h, acc);
+    } else if (POST == POST_G5_NORM) {
+        double n2 = 0.0;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            n2 += (double)acc[k].re * (double)acc[k].re + (double)acc[k].im * (double)acc[k].im;
+            if (k >= 2 * N) acc[k] = -acc[k];              // gamma5 = diag(1, 1, -1, -1) on the spin index
+        }
+        *part += n2;
+        IO::store(out_half, first, g.L3h, acc);
+    } else {
+        cplx<T> v[NC];
+        IO::template load<LD_STREAM>(v, a.cg_r, first, g.L3h);
+        double n2 = 0.0;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            const T sa = k >= 2 * N ? alpha : -alpha;      // r -= alpha gamma5 w
+            v[k].re = fma(sa, acc[k].re, v[k].re);
+            v[k].im = fma(sa, acc[k].im, v[k].im);
+            n2 += (double)v[k].re * (double)v[k].re + (double)v[k].im * (double)v[k].im;
+        }
+        *part += n2;
+        IO::store(a.cg_r, first, g.L3h, v);
+        cplx<T> pv[NC];
+        IO::template load<LD_KEEP>(pv, a.cg_p, first, g.L3h);
+        IO::template load<LD_STREAM>(v, a.cg_x, first, g.L3h);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) { v[k].re = fma(alpha, pv[k].re, v[k].re); v[k].im = fma(alpha, pv[k].im, v[k].im); }
+        IO::store(a.cg_x, first, g.L3h, v);
+    }
+}
+
+// sum of `v` over the first `nthreads` threads of the CTA in a fixed order (warp tree, then warp sums in index order); valid in
+// thread 0.  `red`: at least nthreads / 32 doubles of shared memory; `barrier_id`: a named barrier all nthreads threads reach.
+__device__ __forceinline__ double cta_sum_fixed(double v, double* red, int nthreads, int barrier_id) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    asm volatile("bar.sync %0, %1;" ::"r"(barrier_id), "r"(nthreads) : "memory");     // everybody is done with the memory `red` aliases
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    asm volatile("bar.sync %0, %1;" ::"r"(barrier_id), "r"(nthreads) : "memory");
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < nthreads / 32; ++i) t += red[i];
+    return t;
 }
 
 // resident CTAs per SM the kernel is compiled for: the fp64 kernels with three colours need 130-138 registers left alone (3 CTAs of
@@ -75,7 +131,7 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
 // 48^4 goes from 729 to 634 us.  5 CTAs (102 registers) spill heavily and lose 25 %; the other instantiations gain nothing.
 template <typename T, int N> constexpr int generic_min_ctas() { return (N == 3 && sizeof(T) == 8) ? 4 : 1; }
 // C3: the links are complex 3 x 3 matrices stored in full (HR_REP_SU3; N = 3)
-template <typename T, int N, int EPI, bool ONFLY, bool C3 = false, bool BOTH = false>
+template <typename T, int N, int EPI, bool ONFLY, bool C3 = false, bool BOTH = false, int POST = POST_STORE>
 __global__ void __launch_bounds__(128, generic_min_ctas<T, N>()) hop_generic_kernel(Geo g, HopArgs a) {
     static_assert(!C3 || N == 3, "complex 3 x 3 links: N = 3 (ONFLY then means: two rows stored, third rebuilt)");
     typedef typename std::conditional<C3, LinkC3<T>, Link<T, N>>::type link_t;
@@ -85,8 +141,12 @@ __global__ void __launch_bounds__(128, generic_min_ctas<T, N>()) hop_generic_ker
     // (forward term of parity p, backward term of parity 1-p at the neighbouring sites) run next to each other and the second
     // use hits L2 — links and phi are then loaded at normal priority (BOTH), else streamed
     const int bid = BOTH ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
-    const int cb = bid * blockDim.x + threadIdx.x;
-    if (cb >= g.Vh) return;
+    int cb = bid * blockDim.x + threadIdx.x;
+    const bool valid = cb < g.Vh;
+    if (!valid) {
+        if (POST == POST_STORE) return;
+        cb = g.Vh - 1;        // a reduction follows: stay, shadow the last site, store and add nothing
+    }
     const int p = BOTH ? (int)(blockIdx.x & 1) : a.parity;
     constexpr int LINKPOL = BOTH ? LD_KEEP : LD_STREAM;
     const size_t half_bytes = (size_t)g.Vh * IO::NCH * 16;
@@ -151,7 +211,15 @@ __global__ void __launch_bounds__(128, generic_min_ctas<T, N>()) hop_generic_ker
     HR_HOP_DIR(3, row, h_f3, row, h_b3, r == 1 && h == g.L3h - 1, r == 0 && h == 0)
 #undef HR_HOP_DIR
 
-    hop_epilogue<T, N, EPI, (BOTH ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row, h);
+    if (POST == POST_STORE) {
+        hop_epilogue<T, N, EPI, (BOTH ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row, h);
+    } else {
+        __shared__ double red[4];
+        double part = 0.0;
+        if (valid) hop_epilogue<T, N, EPI, LD_STREAM, POST>(acc, g, a, phi_half, out_half, p, row, h, &part, POST == POST_CG_UPDATE ? (T)*a.cg_alpha : (T)0);
+        const double tot = cta_sum_fixed(part, red, 128, 1);
+        if (threadIdx.x == 0) a.partial[blockIdx.x] = tot;
+    }
 }
 
 // x1-slab width for the generic kernel's site order (0 = plain order): full-lattice launches whose two live x0-planes (both
@@ -179,6 +247,19 @@ inline int launch_hop_generic_both(const Geo& g, const HopArgs& a_in, int epi, c
         case EPI_CLOVER_AXPY: hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, C3, BOTH><<<grid, block, 0, st>>>(g, a); break;
         default: set_error("unknown epilogue %d", epi); return HR_EINVAL;
     }
+    count_launch();
+    return check_launch("hop_generic_kernel");
+}
+
+// the CG stages: parity hop with an axpy-type epilogue and a POST stage; blocks = the number of partial sums written
+template <typename T, int N, bool ONFLY, bool C3>
+inline int launch_hop_generic_post(const Geo& g, const HopArgs& a, int epi, int post, cudaStream_t st) {
+    dim3 block(128), grid((g.Vh + 127) / 128);
+    if (epi == EPI_AXPY && post == POST_G5_NORM) hop_generic_kernel<T, N, EPI_AXPY, ONFLY, C3, false, POST_G5_NORM><<<grid, block, 0, st>>>(g, a);
+    else if (epi == EPI_AXPY && post == POST_CG_UPDATE) hop_generic_kernel<T, N, EPI_AXPY, ONFLY, C3, false, POST_CG_UPDATE><<<grid, block, 0, st>>>(g, a);
+    else if (epi == EPI_CLOVER_AXPY && post == POST_G5_NORM) hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, C3, false, POST_G5_NORM><<<grid, block, 0, st>>>(g, a);
+    else if (epi == EPI_CLOVER_AXPY && post == POST_CG_UPDATE) hop_generic_kernel<T, N, EPI_CLOVER_AXPY, ONFLY, C3, false, POST_CG_UPDATE><<<grid, block, 0, st>>>(g, a);
+    else { set_error("hop with a CG stage: epilogue %d / stage %d", epi, post); return HR_EINVAL; }
     count_launch();
     return check_launch("hop_generic_kernel");
 }

@@ -150,7 +150,8 @@ struct TiledPlan {
 // OPEN: the hop of one rank of a decomposed lattice (hr_hop_local): for the directions in HopArgs::open_mask the forward term of
 // sites with x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out (the boundary kernel of hr_halo.cu adds them
 // from the received faces); the producer still copies the wrapped-around rows, they are simply not used.
-template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H, bool OPEN = false>
+// POST: a stage of the CG solver applied to the epilogue's result (hr_hop_generic.cuh: POST_*); the CTA then writes one partial sum
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H, bool OPEN = false, int POST = POST_STORE>
 __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g_in, HopArgs a, TiledPlan pl) {
     Geo g = g_in;
@@ -277,6 +278,8 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, row, r ? h : (h == 0 ? L3h - 1 : h - 1));
     }
 
+    double cg_part = 0.0;                                                           // POST stages: this thread's share of the CTA's partial sum
+    const T cg_alpha = POST == POST_CG_UPDATE ? (T)*a.cg_alpha : (T)0;
     for (int k = 0; k < nsteps; ++k) {
         const int x0 = xs + k;
         const int r = (x0 + x1 + x2 + p) & 1;
@@ -365,7 +368,15 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
             mbar_arrive(bar_hempty + 8 * hb);
         }
         // (requesting phi before the eight terms was measured slower at 48^4)
-        if (active) hop_epilogue<T, N, EPI, (SHARE ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
+        if (POST == POST_STORE) {
+            if (active) hop_epilogue<T, N, EPI, (SHARE ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
+        } else {
+            if (active) hop_epilogue<T, N, EPI, LD_STREAM, POST>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h, &cg_part, cg_alpha);
+        }
+    }
+    if (POST != POST_STORE) {   // every plane and halo copy has been waited for and read: the ring is free to hold the warp sums
+        const double tot = cta_sum_fixed(cg_part, reinterpret_cast<double*>(ring), pl.nconsumer, 1);
+        if (tid == 0) a.partial[blockIdx.x] = tot;
     }
 }
 
@@ -428,9 +439,9 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) 
     return hg->rep == HR_REP_FUND && tiled_plan_shape(hg, both, num_sms, 2, 2, pl);
 }
 
-template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H, bool OPEN = false>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H, bool OPEN = false, int POST = POST_STORE>
 inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H, OPEN>;
+    auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H, OPEN, POST>;
     static std::atomic<unsigned char> configured[64];
     const int rc = opt_in_shared_memory(reinterpret_cast<const void*>(kern), configured, "hop_tiled_kernel");
     if (rc != HR_OK) return rc;
@@ -440,20 +451,20 @@ inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan&
     return check_launch("hop_tiled_kernel");
 }
 
-template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, bool OPEN = false>
+template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, bool OPEN = false, int POST = POST_STORE>
 inline int launch_hop_tiled_shape(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
     // compile-time L3/2 = 24 for the fp64 fundamental kernels (measured at 48^4: hop 219.3 -> 216.1 us; the fp32 4 x 4
     // kernel got slower with it)
     constexpr bool SPECIALISE = N == 2 && sizeof(T) == 8;
-    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0), OPEN>(g, a, pl, st);
-    return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, 0, OPEN>(g, a, pl, st);
+    if (SPECIALISE && g.L3h == 24) return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, (SPECIALISE ? 24 : 0), OPEN, POST>(g, a, pl, st);
+    return launch_hop_tiled_l3h<T, N, EPI, SHARE, T1, T2, ONFLY, 0, OPEN, POST>(g, a, pl, st);
 }
 
-template <typename T, int N, int EPI, bool SHARE, bool ONFLY, bool OPEN = false>
+template <typename T, int N, int EPI, bool SHARE, bool ONFLY, bool OPEN = false, int POST = POST_STORE>
 inline int launch_hop_tiled_epi(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
-    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4, ONFLY, OPEN>(g, a, pl, st);
-    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, SHARE, 2, 2, false, OPEN>(g, a, pl, st);
-    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4, false, OPEN>(g, a, pl, st);
+    if (pl.t1 == 2 && pl.t2 == 4) return launch_hop_tiled_shape<T, N, EPI, SHARE, 2, 4, ONFLY, OPEN, POST>(g, a, pl, st);
+    if (N == 2 && pl.t1 == 2 && pl.t2 == 2) return launch_hop_tiled_shape<T, 2, EPI, SHARE, 2, 2, false, OPEN, POST>(g, a, pl, st);
+    if (sizeof(T) == 4 && N == 2 && pl.t1 == 4 && pl.t2 == 4) return launch_hop_tiled_shape<float, 2, EPI, SHARE, 4, 4, false, OPEN, POST>(g, a, pl, st);
     set_error("hop_tiled_kernel: no instantiation for a %d x %d tile", pl.t1, pl.t2);
     return HR_EUNSUPPORTED;
 }

@@ -1,11 +1,12 @@
 // hr_solver.cu — conjugate gradient on the normal equations of the even-odd operator (
 // PAPER.md:13 "range of inverters", PAPER.md:39 the even-odd operator "used mainly in the HMC"):
 //     Dhat^dag Dhat x = b   on the even sites,   Dhat^dag = gamma5 Dhat gamma5.
-// The operator applications are hr_dirac_eo_apply (the hopping kernels); this file adds the linear algebra
-// between them as three fused streaming kernels and keeps every scalar on the device, so an iteration is
-// enqueued without a host round trip.  Reductions are two-stage with a fixed order (per-block partial sums in
-// double, then one block sums them): results are bitwise reproducible from run to run.
-#include "hr_common.cuh"
+// The operator applications are the hopping kernels; the linear algebra between them rides in the epilogue of the second hop
+// of each Dhat (POST_G5_NORM, POST_CG_UPDATE of hr_hop_generic.cuh: s = gamma5 Dhat p with |Dhat p|^2, and r -= alpha gamma5 Dhat s
+// with |r|^2 and x += alpha p), so Dhat p and Dhat s never reach memory; p = r + beta p is the one vector kernel left.  Every scalar
+// stays on the device, so an iteration is enqueued without a host round trip.  Reductions are two-stage with a fixed order (one
+// partial sum per CTA in double, then one block sums them): results are bitwise reproducible from run to run.
+#include "hr_hop_generic.cuh"
 
 namespace hr {
 
@@ -91,39 +92,6 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_finalize_kernel(int what, int npa
     }
 }
 
-// x += alpha p;  r -= alpha gamma5 w;  partial = sum |r|^2          (w = Dhat gamma5 Dhat p, so gamma5 w = Dhat^dag Dhat p)
-template <typename T>
-__global__ void __launch_bounds__(CG_BLOCK) cg_update_kernel(size_t nchunks, int L3h, int NCH, const CgScalars* __restrict__ sc, const void* __restrict__ p_,
-                                                             const void* __restrict__ w_, void* __restrict__ x_, void* __restrict__ r_,
-                                                             double* __restrict__ partial) {
-    typedef typename Chunk<T>::type chunk_t;
-    constexpr int R = RealsPerChunk<T>::value;
-    const chunk_t* p = reinterpret_cast<const chunk_t*>(p_);
-    const chunk_t* w = reinterpret_cast<const chunk_t*>(w_);
-    chunk_t* x = reinterpret_cast<chunk_t*>(x_);
-    chunk_t* r = reinterpret_cast<chunk_t*>(r_);
-    const T alpha = (T)sc->alpha;
-    double acc = 0.0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
-        T ep[R], ew[R], ex[R], er[R];
-        chunk_to_reals(ldg16<LD_KEEP>(p + i), ep);
-        chunk_to_reals(ldg16<LD_STREAM>(w + i), ew);
-        chunk_to_reals(x[i], ex);
-        chunk_to_reals(r[i], er);
-        const T sg = (T)g5_sign(i, L3h, NCH);
-#pragma unroll
-        for (int k = 0; k < R; ++k) {
-            ex[k] = fma(alpha, ep[k], ex[k]);
-            er[k] = fma(-alpha * sg, ew[k], er[k]);
-            acc += (double)er[k] * (double)er[k];
-        }
-        x[i] = reals_to_chunk(ex);
-        r[i] = reals_to_chunk(er);
-    }
-    const double tot = block_sum(acc);
-    if (threadIdx.x == 0) partial[blockIdx.x] = tot;
-}
-
 // p = r + beta p
 template <typename T>
 __global__ void __launch_bounds__(CG_BLOCK) cg_direction_kernel(size_t nchunks, const CgScalars* __restrict__ sc, const void* __restrict__ r_, void* __restrict__ p_) {
@@ -170,9 +138,15 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_init_kernel(size_t nchunks, const
 // ------------------------------------------------------------------ host driver
 static size_t up256s(size_t n) { return (n + 255) & ~(size_t)255; }
 
+// partial sums: one per block of the vector kernels (<= CG_MAX_PARTIALS) or per CTA of a hop that carries a CG stage
+static size_t cg_partials(const hr_geom* g) {
+    const size_t nb = (size_t)hop_post_blocks(g);
+    return nb > (size_t)CG_MAX_PARTIALS ? nb : (size_t)CG_MAX_PARTIALS;
+}
+
 size_t cg_workspace_bytes(const hr_geom* g) {
     const size_t half = hr_spinor_bytes(g, HR_EVEN);
-    return 256 + up256s(CG_MAX_PARTIALS * sizeof(double)) + 5 * up256s(half);
+    return 256 + up256s(cg_partials(g) * sizeof(double)) + 5 * up256s(half);
 }
 
 template <typename T>
@@ -184,15 +158,18 @@ static int cg_run(const hr_geom* g, double m0, const void* u, const void* cf, co
     const size_t nchunks = half / 16;
     char* w8 = (char*)workspace;
     CgScalars* sc = (CgScalars*)w8; w8 += 256;
-    double* partial = (double*)w8; w8 += up256s(CG_MAX_PARTIALS * sizeof(double));
+    double* partial = (double*)w8; w8 += up256s(cg_partials(g) * sizeof(double));
     void* r = w8; w8 += up256s(half);
     void* p = w8; w8 += up256s(half);
-    void* t = w8; w8 += up256s(half);
+    w8 += up256s(half);      // (a third vector of the unfused iteration: kept in the layout, unused)
     void* w = w8; w8 += up256s(half);
     void* tmp = w8;
     int nblk = (int)((nchunks + CG_BLOCK - 1) / CG_BLOCK);
     if (nblk > CG_MAX_PARTIALS) nblk = CG_MAX_PARTIALS;
-    void* strm = (void*)st;
+    const bool clover = cf && ci;
+    const double d = 4.0 + m0;
+    if (!clover && d == 0.0) { set_error("hr_cg_solve: 4+m0 = 0, D_oo is singular"); return HR_EINVAL; }
+    const int nhop = hop_post_blocks(g);
 
     cg_init_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, b, x, r, p, partial);
     cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_INIT, nblk, partial, sc);
@@ -214,17 +191,30 @@ static int cg_run(const hr_geom* g, double m0, const void* u, const void* cf, co
             relres = h.bb > 0.0 ? sqrt(h.rr / h.bb) : 0.0;
             if (h.bb == 0.0 || h.rr <= tol * tol * h.bb || it >= max_iter) { done = true; break; }
         }
-        // t = Dhat p ; s = gamma5 t (into w), |t|^2 ; t = Dhat s ; x += alpha p, r -= alpha gamma5 t ; p = r + beta p
-        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u, cf, ci, p, t, tmp, strm);
+        // One iteration = four hops and one vector kernel.  The linear algebra between the operator applications rides in the
+        // epilogues of the second hop of each Dhat (hr_hop_generic.cuh: POST_*), so Dhat p and Dhat s are never written out:
+        //   tmp = [A_oo^-1] H_oe p ;  s = gamma5 (Dhat p) with <p, Dhat^dag Dhat p> = |Dhat p|^2 as per-CTA partial sums      (POST_G5_NORM)
+        //   tmp = [A_oo^-1] H_oe s ;  r -= alpha gamma5 (Dhat s), |r|^2, x += alpha p                                       (POST_CG_UPDATE)
+        //   p = r + beta p
+        HopArgs a;
+        a.gauge = u; a.both = 0; a.partial = partial;
+        a.in = p; a.out = tmp; a.parity = HR_ODD; a.phi = nullptr; a.clover = clover ? ci : nullptr; a.a = 0.0; a.c = 1.0;
+        rc = run_hop(g, a, clover ? EPI_CLOVER_INV : EPI_NONE, st);
         if (rc != HR_OK) return rc;
-        cg_g5_norm_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, t, w, partial);
-        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_PAP, nblk, partial, sc);
-        rc = hr_dirac_eo_apply(g, HR_EO_DHAT, m0, u, cf, ci, w, t, tmp, strm);
+        a.in = tmp; a.out = w; a.parity = HR_EVEN; a.phi = p; a.clover = clover ? cf : nullptr; a.a = clover ? 0.0 : d; a.c = clover ? -0.25 : -1.0 / (4.0 * d);
+        rc = run_hop_post(g, a, clover ? EPI_CLOVER_AXPY : EPI_AXPY, POST_G5_NORM, st);
         if (rc != HR_OK) return rc;
-        cg_update_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, geo.L3h, NCH, sc, p, t, x, r, partial);
-        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_RR, nblk, partial, sc);
+        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_PAP, nhop, partial, sc);
+        a.in = w; a.out = tmp; a.parity = HR_ODD; a.phi = nullptr; a.clover = clover ? ci : nullptr; a.a = 0.0; a.c = 1.0;
+        rc = run_hop(g, a, clover ? EPI_CLOVER_INV : EPI_NONE, st);
+        if (rc != HR_OK) return rc;
+        a.in = tmp; a.out = nullptr; a.parity = HR_EVEN; a.phi = w; a.clover = clover ? cf : nullptr; a.a = clover ? 0.0 : d; a.c = clover ? -0.25 : -1.0 / (4.0 * d);
+        a.cg_alpha = &sc->alpha; a.cg_r = r; a.cg_x = x; a.cg_p = p;
+        rc = run_hop_post(g, a, clover ? EPI_CLOVER_AXPY : EPI_AXPY, POST_CG_UPDATE, st);
+        if (rc != HR_OK) return rc;
+        cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_RR, nhop, partial, sc);
         cg_direction_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, sc, r, p);
-        count_launch(5);
+        count_launch(3);
         rc = check_launch("cg iteration");
         if (rc != HR_OK) return rc;
         ++it;
