@@ -51,29 +51,6 @@ struct DiracPlan {
     size_t smem;
 };
 
-// Links through shared memory.  A load into registers that is requested one step ahead does not get a step of lead: ptxas puts
-// every global load of the loop on ONE scoreboard, so the first use of a link at the top of a step waits for ALL outstanding link
-// loads, the ones requested a few hundred instructions earlier included, and a DRAM latency is exposed in every step (18-24 % of the
-// stall samples, profiles/r02_kernels.md).  cp.async groups complete in order and cp.async.wait_group N waits for all but the N
-// newest: each link has its own slot (32 bytes fp64, 16 bytes fp32), is re-requested into it right after its use, and is waited
-// for with N = 6 — exactly the seven-requests-ago one.  A thread reads only slots it filled itself, so no barrier is needed.
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int NPENDING> __device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory");
-}
-
-// (alpha, beta) of a compressed link from its slot; volatile keeps the reads behind the wait_group
-__device__ __forceinline__ void lds_link(cplx<double>* ab, uint32_t slot, int chunk_stride) {
-    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(ab[0].re), "=d"(ab[0].im) : "r"(slot));
-    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(ab[1].re), "=d"(ab[1].im) : "r"(slot + chunk_stride));
-}
-__device__ __forceinline__ void lds_link(cplx<float>* ab, uint32_t slot, int) {
-    asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ab[0].re), "=f"(ab[0].im), "=f"(ab[1].re), "=f"(ab[1].im) : "r"(slot));
-}
-
 // The producer of the full-lattice kernels (one thread): per iteration the T1 x T2 tile rows of plane j, both parity images, into
 // ring slot j % DT_RING and the halo rows of centre plane j - HLAG into halo buffer (pc-1) % DT_HALO; waits on the slot's "empty"
 // mbarrier, arms its "full" mbarrier with the byte count.  Shared by dirac_tiled_kernel and dirac_split_kernel (hr_dirac_split.cuh).

@@ -18,6 +18,9 @@
 
 namespace hr {
 
+#ifndef HR_HOP_ALINK
+#define HR_HOP_ALINK 1
+#endif
 constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live + one being filled
 constexpr int TILED_HALO = 2;         // halo buffers: one in use, one being filled (a third one costs the L1 the link loads need)
 
@@ -125,6 +128,29 @@ __device__ __forceinline__ Link<T, 3> open_link(const Link<T, 3>& u, bool cut) {
     return v;
 }
 
+// Links through shared memory.  A load into registers that is requested one step ahead does not get a step of lead: ptxas puts
+// every global load of the loop on ONE scoreboard, so the first use of a link at the top of a step waits for ALL outstanding link
+// loads, the ones requested a few hundred instructions earlier included, and a DRAM latency is exposed in every step (18-24 % of the
+// stall samples, profiles/r02_kernels.md).  cp.async groups complete in order and cp.async.wait_group N waits for all but the N
+// newest: each link has its own slot (32 bytes fp64, 16 bytes fp32), is re-requested into it right after its use, and is waited
+// for with N = 6 — exactly the seven-requests-ago one.  A thread reads only slots it filled itself, so no barrier is needed.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING> __device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory");
+}
+
+// (alpha, beta) of a compressed link from its slot; volatile keeps the reads behind the wait_group
+__device__ __forceinline__ void lds_link(cplx<double>* ab, uint32_t slot, int chunk_stride) {
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(ab[0].re), "=d"(ab[0].im) : "r"(slot));
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(ab[1].re), "=d"(ab[1].im) : "r"(slot + chunk_stride));
+}
+__device__ __forceinline__ void lds_link(cplx<float>* ab, uint32_t slot, int) {
+    asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ab[0].re), "=f"(ab[0].im), "=f"(ab[1].re), "=f"(ab[1].im) : "r"(slot));
+}
+
 // launch geometry chosen on the host (hr_hop.cu)
 struct TiledPlan {
     int t1, t2;        // tile shape in rows (x1, x2): selects the kernel instantiation
@@ -151,7 +177,9 @@ struct TiledPlan {
 // sites with x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out (the boundary kernel of hr_halo.cu adds them
 // from the received faces); the producer still copies the wrapped-around rows, they are simply not used.
 // POST: a stage of the CG solver applied to the epilogue's result (hr_hop_generic.cuh: POST_*); the CTA then writes one partial sum
-template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H, bool OPEN = false, int POST = POST_STORE>
+// ALINK: the eight links of a site travel through cp.async slots in shared memory instead of registers (see cp_async16 above;
+// fundamental representation, one output parity)
+template <typename T, int N, int EPI, int T1, int T2, bool SHARE, bool ONFLY, int L3H, bool OPEN = false, int POST = POST_STORE, bool ALINK = false>
 __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && sizeof(T) == 4 && N == 2 && T1 * T2 <= 8) ? 2 : 1)
     hop_tiled_kernel(Geo g_in, HopArgs a, TiledPlan pl) {
     Geo g = g_in;
@@ -169,6 +197,8 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
     const int planeb = TR * rowb;
     const int halob = HR * rowb;
     char* halo = ring + TILED_RING * planeb;
+    char* lbuf = halo + TILED_HALO * halob;          // ALINK: link slots [link][chunk][consumer thread]
+    static_assert(!ALINK || (N == 2 && !ONFLY && !SHARE), "link slots: compressed fundamental links, one output parity");
     const uint32_t bar_full = smem_u32(bars);            // [TILED_RING]
     const uint32_t bar_empty = smem_u32(bars + 4);       // [TILED_RING]
     const uint32_t bar_hempty = smem_u32(bars + 8);      // [TILED_HALO]
@@ -264,10 +294,38 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
     const bool cut_f1 = ((om >> 1) & 1) && x1 == L1 - 1, cut_b1 = ((om >> 1) & 1) && x1 == 0;
     const bool cut_f2 = ((om >> 2) & 1) && x2 == L2 - 1, cut_b2 = ((om >> 2) & 1) && x2 == 0;
 
-    Link<T, N> uf[4], ub[4];
+    Link<T, N> uf[ALINK ? 1 : 4], ub[ALINK ? 1 : 4];
+    // ALINK: slot j of this thread holds link j of the CURRENT step, j = 0..7 in the order of use (U_0(x), U_0(x-0), U_1(x), ...);
+    // it is re-requested for the next step right after its use and waited for with cp.async.wait_group 7
+    constexpr int LCH = SiteIO<T, 2>::NCH;
+    const uint32_t lslot = smem_u32(lbuf) + (uint32_t)tid * 16;
+    const int lchb = pl.nconsumer * 16;
+    auto link_request = [&](int j, int par, int mu, int row, int hh) {
+        const char* src = reinterpret_cast<const char*>(a.gauge) + (((size_t)(par * 4 + mu) * g.R + row) * (LCH * L3h) + hh) * 16;
+#pragma unroll
+        for (int c = 0; c < LCH; ++c) cp_async16(lslot + (j * LCH + c) * lchb, src + (size_t)c * cs);
+        cp_async_commit();
+    };
+    auto link_get = [&](Link<T, 2>& u, int j) {
+        cp_async_wait<7>();
+        cplx<T> ab[2];
+        lds_link(ab, lslot + j * LCH * lchb, lchb);
+        u.a = ab[0];
+        u.b = ab[1];
+    };
     {   // links of the first step
         const int row = row0 + xs * g.s0;
         const int r = (xs + x1 + x2 + p) & 1;
+        if constexpr (ALINK) {
+            link_request(0, p, 0, row, h);
+            link_request(1, 1 - p, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
+            link_request(2, p, 1, row, h);
+            link_request(3, 1 - p, 1, rowb1_0 + xs * g.s0, h);
+            link_request(4, p, 2, row, h);
+            link_request(5, 1 - p, 2, rowb2_0 + xs * g.s0, h);
+            link_request(6, p, 3, row, h);
+            link_request(7, 1 - p, 3, row, r ? h : (h == 0 ? L3h - 1 : h - 1));
+        } else {
         load_link_rep<T, LP, ONFLY>(uf[0], a.gauge, g, p, 0, row, h);
         load_link_rep<T, LP, ONFLY>(ub[0], a.gauge, g, 1 - p, 0, row0 + (xs == 0 ? L0 - 1 : xs - 1) * g.s0, h);
         load_link_rep<T, LP, ONFLY>(uf[1], a.gauge, g, p, 1, row, h);
@@ -276,6 +334,7 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         load_link_rep<T, LP, ONFLY>(ub[2], a.gauge, g, 1 - p, 2, rowb2_0 + xs * g.s0, h);
         load_link_rep<T, LP, ONFLY>(uf[3], a.gauge, g, p, 3, row, h);
         load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, row, r ? h : (h == 0 ? L3h - 1 : h - 1));
+        }
     }
 
     double cg_part = 0.0;                                                           // POST stages: this thread's share of the CTA's partial sum
@@ -325,6 +384,41 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         const char* const a2b = (b2_in ? scur : shalo) + off_b2 + h * 16;
         const char* const a3f = scur + off_c + hf3 * 16;
         const char* const a3b = scur + off_c + hb3 * 16;
+        if constexpr (ALINK) {
+            Link<T, 2> u;
+            lds_site<T, NC>(nbA, a0f, cs);
+            lds_site<T, NC>(nbB, a0b, cs);
+            link_get(u, 0);
+            hop_term<T, N, 0, true>(acc, nbA, open_link<OPEN>(u, cut_f0));
+            link_request(0, p, 0, rown, h);
+            lds_site<T, NC>(nbA, a1f, cs);
+            link_get(u, 1);
+            hop_term<T, N, 0, false>(acc, nbB, open_link<OPEN>(u, cut_b0));
+            link_request(1, 1 - p, 0, row0 + (xn == 0 ? L0 - 1 : xn - 1) * g.s0, h);
+            lds_site<T, NC>(nbB, a1b, cs);
+            link_get(u, 2);
+            hop_term<T, N, 1, true>(acc, nbA, open_link<OPEN>(u, cut_f1));
+            link_request(2, p, 1, rown, h);
+            lds_site<T, NC>(nbA, a2f, cs);
+            link_get(u, 3);
+            hop_term<T, N, 1, false>(acc, nbB, open_link<OPEN>(u, cut_b1));
+            link_request(3, 1 - p, 1, rowb1_0 + xn * g.s0, h);
+            lds_site<T, NC>(nbB, a2b, cs);
+            link_get(u, 4);
+            hop_term<T, N, 2, true>(acc, nbA, open_link<OPEN>(u, cut_f2));
+            link_request(4, p, 2, rown, h);
+            lds_site<T, NC>(nbA, a3f, cs);
+            link_get(u, 5);
+            hop_term<T, N, 2, false>(acc, nbB, open_link<OPEN>(u, cut_b2));
+            link_request(5, 1 - p, 2, rowb2_0 + xn * g.s0, h);
+            lds_site<T, NC>(nbB, a3b, cs);
+            link_get(u, 6);
+            hop_term<T, N, 3, true>(acc, nbA, open_link<OPEN>(u, cut_f3));
+            link_request(6, p, 3, rown, h);
+            link_get(u, 7);
+            hop_term<T, N, 3, false>(acc, nbB, open_link<OPEN>(u, cut_b3));
+            link_request(7, 1 - p, 3, rown, hb3n);
+        } else {
         HR_NB_NEXT(nb0, a0f);
         HR_NB_NEXT(nb1, a0b); HR_NB_NOW(nb0, a0f);
         hop_term<T, N, 0, true>(acc, nb0, open_link<OPEN>(uf[0], cut_f0));
@@ -357,6 +451,7 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         HR_NB_NOW(nb1, a3b);
         hop_term<T, N, 3, false>(acc, nb1, open_link<OPEN>(ub[3], cut_b3));
         load_link_rep<T, LP, ONFLY>(ub[3], a.gauge, g, 1 - p, 3, rown, hb3n);
+        }
 #undef HR_NB_NEXT
 #undef HR_NB_NOW
 #undef HR_PIN
@@ -374,6 +469,7 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
             if (active) hop_epilogue<T, N, EPI, LD_STREAM, POST>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h, &cg_part, cg_alpha);
         }
     }
+    if (ALINK) cp_async_wait<0>();   // the unused requests of the last step must not outlive the CTA
     if (POST != POST_STORE) {   // every plane and halo copy has been waited for and read: the ring is free to hold the warp sums
         const double tot = cta_sum_fixed(cg_part, reinterpret_cast<double*>(ring), pl.nconsumer, 1);
         if (tid == 0) a.partial[blockIdx.x] = tot;
@@ -441,6 +537,22 @@ inline bool tiled_plan(const hr_geom* hg, int both, int num_sms, TiledPlan& pl) 
 
 template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, int L3H, bool OPEN = false, int POST = POST_STORE>
 inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
+    // Link slots (ALINK) where the instantiation has them and 8 links x 16 / 32 bytes per consumer thread still fit.  Measured at 48^4
+    // (profiles/r02_hop_alink.md): the bare and axpy hops gain (fp64 215.8 -> 206 us; 64^4 817 -> 694 us), the clover epilogues lose
+    // (their 256-byte block loads need the L1 that the slots take: E2 724 -> 768 us) and so do the fp64 CG stages; fp32 CG stages gain.
+    constexpr bool CAN_ALINK = HR_HOP_ALINK && N == 2 && !SHARE && !ONFLY && (EPI == EPI_NONE || EPI == EPI_AXPY) && (POST == POST_STORE || sizeof(T) == 4);
+    if constexpr (CAN_ALINK) {
+        const size_t smem = pl.smem + (size_t)8 * SiteIO<T, 2>::NCH * 16 * pl.nconsumer;
+        if (smem <= TILED_SMEM_LIMIT) {
+            auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H, OPEN, POST, true>;
+            static std::atomic<unsigned char> configured[64];
+            const int rc = opt_in_shared_memory(reinterpret_cast<const void*>(kern), configured, "hop_tiled_kernel");
+            if (rc != HR_OK) return rc;
+            kern<<<(unsigned)(pl.nt1 * pl.nt2 * pl.nseg), pl.nconsumer + 32, smem, st>>>(g, a, pl);
+            count_launch();
+            return check_launch("hop_tiled_kernel");
+        }
+    }
     auto kern = hop_tiled_kernel<T, N, EPI, T1, T2, SHARE, ONFLY, L3H, OPEN, POST>;
     static std::atomic<unsigned char> configured[64];
     const int rc = opt_in_shared_memory(reinterpret_cast<const void*>(kern), configured, "hop_tiled_kernel");

@@ -212,7 +212,7 @@ def test_kernel_plan_of_the_bench_lattice(L):
     """hr_kernel_plan is host-only: the 48^4 launch plans DESIGN.md §5 describes (148 SMs assumed without a device)"""
     g64 = hr.geom((48,) * 4, hr.REP_FUND, hr.PREC_F64)
     g32 = hr.geom((48,) * 4, hr.REP_FUND, hr.PREC_F32)
-    assert hr.hr_kernel_plan(g64, hr.OP_HOP) == {"kernel": 1, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 224, "smem": 172160, "grid": 288}
+    assert hr.hr_kernel_plan(g64, hr.OP_HOP) == {"kernel": 1, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 224, "smem": 221312, "grid": 288}
     assert hr.hr_kernel_plan(g64, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 2, "nseg": 1, "seglen": 48, "threads": 224, "smem": 215168, "grid": 576}
     assert hr.hr_kernel_plan(g32, hr.OP_HOP)["grid"] == 144 and hr.hr_kernel_plan(g32, hr.OP_HOP)["t1"] == 4
     assert hr.hr_kernel_plan(g32, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 416, "smem": 227456, "grid": 288}
