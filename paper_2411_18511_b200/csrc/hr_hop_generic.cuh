@@ -18,7 +18,8 @@ enum {
 // what happens to the epilogue's result w(x) (SURVEY.md §8(f) item 2 "fused dot products and axpys in the hop epilogue"):
 //   POST_STORE     : out = w
 //   POST_G5_NORM   : out = gamma5 w,  partial += |w|^2                                        (s = gamma5 Dhat p and <p, Dhat^dag Dhat p>)
-//   POST_CG_UPDATE : r -= alpha gamma5 w,  partial += |r|^2,  x += alpha p   (w is not stored)   (the CG update after the second Dhat)
+//   POST_CG_UPDATE : r -= alpha gamma5 w,  partial += |r|^2   (w is not stored)                 (the CG update after the second Dhat;
+//                    x += alpha p rides with p = r + beta p in cg_direction_kernel, which reads p anyway)
 enum { POST_STORE = 0, POST_G5_NORM = 1, POST_CG_UPDATE = 2 };
 
 struct HopArgs {
@@ -33,9 +34,7 @@ struct HopArgs {
     // POST_* stages of the CG solver (hr_solver.cu), applied to the value the epilogue would have stored:
     double* partial = nullptr;        // one partial sum per CTA (fixed order inside the CTA)
     const double* cg_alpha = nullptr; // device scalar alpha (POST_CG_UPDATE)
-    void* cg_r = nullptr;             // half fields of the output parity (POST_CG_UPDATE): r -= alpha gamma5 w,
-    void* cg_x = nullptr;             //   x += alpha p
-    const void* cg_p = nullptr;
+    void* cg_r = nullptr;             // half field of the output parity (POST_CG_UPDATE): r -= alpha gamma5 w
     int slab_w1 = 0;     // > 0: the generic kernel walks the lattice in x1-slabs of this width (launch_hop_generic sets it)
     int open_mask = 0;   // bit mu set: direction mu is cut between ranks (hr_hop_local): the forward term of sites with
                          // x_mu = L_mu-1 and the backward term of sites with x_mu = 0 are left out here and added from
@@ -103,12 +102,6 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
         }
         *part += n2;
         IO::store(a.cg_r, first, g.L3h, v);
-        cplx<T> pv[NC];
-        IO::template load<LD_KEEP>(pv, a.cg_p, first, g.L3h);
-        IO::template load<LD_STREAM>(v, a.cg_x, first, g.L3h);
-#pragma unroll
-        for (int k = 0; k < NC; ++k) { v[k].re = fma(alpha, pv[k].re, v[k].re); v[k].im = fma(alpha, pv[k].im, v[k].im); }
-        IO::store(a.cg_x, first, g.L3h, v);
     }
 }
 

@@ -539,8 +539,8 @@ template <typename T, int N, int EPI, bool SHARE, int T1, int T2, bool ONFLY, in
 inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan& pl, cudaStream_t st) {
     // Link slots (ALINK) where the instantiation has them and 8 links x 16 / 32 bytes per consumer thread still fit.  Measured at 48^4
     // (profiles/r02_hop_alink.md): the bare and axpy hops gain (fp64 215.8 -> 206 us; 64^4 817 -> 694 us), the clover epilogues lose
-    // (their 256-byte block loads need the L1 that the slots take: E2 724 -> 768 us) and so does the fp64 CG update stage (three more
-    // spinors per site); the norm stage and the fp32 CG stages gain.
+    // (their 256-byte block loads need the L1 that the slots take: E2 724 -> 768 us) and so does the fp64 CG update stage (1320 -> 1328 us per
+    // iteration); the norm stage and the fp32 CG stages gain.
     constexpr bool CAN_ALINK = HR_HOP_ALINK && N == 2 && !SHARE && !ONFLY && (EPI == EPI_NONE || EPI == EPI_AXPY) && (POST != POST_CG_UPDATE || sizeof(T) == 4);
     if constexpr (CAN_ALINK) {
         const size_t smem = pl.smem + (size_t)8 * SiteIO<T, 2>::NCH * 16 * pl.nconsumer;

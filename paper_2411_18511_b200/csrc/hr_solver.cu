@@ -3,7 +3,7 @@
 //     Dhat^dag Dhat x = b   on the even sites,   Dhat^dag = gamma5 Dhat gamma5.
 // The operator applications are the hopping kernels; the linear algebra between them rides in the epilogue of the second hop
 // of each Dhat (POST_G5_NORM, POST_CG_UPDATE of hr_hop_generic.cuh: s = gamma5 Dhat p with |Dhat p|^2, and r -= alpha gamma5 Dhat s
-// with |r|^2 and x += alpha p), so Dhat p and Dhat s never reach memory; p = r + beta p is the one vector kernel left.  Every scalar
+// with |r|^2), so Dhat p and Dhat s never reach memory; x += alpha p and p = r + beta p share the one vector kernel left.  Every scalar
 // stays on the device, so an iteration is enqueued without a host round trip.  Reductions are two-stage with a fixed order (one
 // partial sum per CTA in double, then one block sums them): results are bitwise reproducible from run to run.
 #include "hr_hop_generic.cuh"
@@ -92,20 +92,27 @@ __global__ void __launch_bounds__(CG_BLOCK) cg_finalize_kernel(int what, int npa
     }
 }
 
-// p = r + beta p
+// x += alpha p;  p = r + beta p        (alpha, beta of this iteration; r already updated by the POST_CG_UPDATE hop)
 template <typename T>
-__global__ void __launch_bounds__(CG_BLOCK) cg_direction_kernel(size_t nchunks, const CgScalars* __restrict__ sc, const void* __restrict__ r_, void* __restrict__ p_) {
+__global__ void __launch_bounds__(CG_BLOCK) cg_direction_kernel(size_t nchunks, const CgScalars* __restrict__ sc, const void* __restrict__ r_, void* __restrict__ p_,
+                                                                void* __restrict__ x_) {
     typedef typename Chunk<T>::type chunk_t;
     constexpr int R = RealsPerChunk<T>::value;
     const chunk_t* r = reinterpret_cast<const chunk_t*>(r_);
     chunk_t* p = reinterpret_cast<chunk_t*>(p_);
-    const T beta = (T)sc->beta;
+    chunk_t* x = reinterpret_cast<chunk_t*>(x_);
+    const T alpha = (T)sc->alpha, beta = (T)sc->beta;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nchunks; i += (size_t)gridDim.x * blockDim.x) {
-        T er[R], ep[R];
-        chunk_to_reals(r[i], er);
+        T er[R], ep[R], ex[R];
+        chunk_to_reals(ldg16<LD_STREAM>(r + i), er);
         chunk_to_reals(p[i], ep);
+        chunk_to_reals(x[i], ex);
 #pragma unroll
-        for (int k = 0; k < R; ++k) ep[k] = fma(beta, ep[k], er[k]);
+        for (int k = 0; k < R; ++k) {
+            ex[k] = fma(alpha, ep[k], ex[k]);
+            ep[k] = fma(beta, ep[k], er[k]);
+        }
+        x[i] = reals_to_chunk(ex);
         p[i] = reals_to_chunk(ep);
     }
 }
@@ -194,8 +201,8 @@ static int cg_run(const hr_geom* g, double m0, const void* u, const void* cf, co
         // One iteration = four hops and one vector kernel.  The linear algebra between the operator applications rides in the
         // epilogues of the second hop of each Dhat (hr_hop_generic.cuh: POST_*), so Dhat p and Dhat s are never written out:
         //   tmp = [A_oo^-1] H_oe p ;  s = gamma5 (Dhat p) with <p, Dhat^dag Dhat p> = |Dhat p|^2 as per-CTA partial sums      (POST_G5_NORM)
-        //   tmp = [A_oo^-1] H_oe s ;  r -= alpha gamma5 (Dhat s), |r|^2, x += alpha p                                       (POST_CG_UPDATE)
-        //   p = r + beta p
+        //   tmp = [A_oo^-1] H_oe s ;  r -= alpha gamma5 (Dhat s), |r|^2                                                     (POST_CG_UPDATE)
+        //   x += alpha p ;  p = r + beta p
         HopArgs a;
         a.gauge = u; a.both = 0; a.partial = partial;
         a.in = p; a.out = tmp; a.parity = HR_ODD; a.phi = nullptr; a.clover = clover ? ci : nullptr; a.a = 0.0; a.c = 1.0;
@@ -209,11 +216,11 @@ static int cg_run(const hr_geom* g, double m0, const void* u, const void* cf, co
         rc = run_hop(g, a, clover ? EPI_CLOVER_INV : EPI_NONE, st);
         if (rc != HR_OK) return rc;
         a.in = tmp; a.out = nullptr; a.parity = HR_EVEN; a.phi = w; a.clover = clover ? cf : nullptr; a.a = clover ? 0.0 : d; a.c = clover ? -0.25 : -1.0 / (4.0 * d);
-        a.cg_alpha = &sc->alpha; a.cg_r = r; a.cg_x = x; a.cg_p = p;
+        a.cg_alpha = &sc->alpha; a.cg_r = r;
         rc = run_hop_post(g, a, clover ? EPI_CLOVER_AXPY : EPI_AXPY, POST_CG_UPDATE, st);
         if (rc != HR_OK) return rc;
         cg_finalize_kernel<<<1, CG_BLOCK, 0, st>>>(CG_FIN_RR, nhop, partial, sc);
-        cg_direction_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, sc, r, p);
+        cg_direction_kernel<T><<<nblk, CG_BLOCK, 0, st>>>(nchunks, sc, r, p, x);
         count_launch(3);
         rc = check_launch("cg iteration");
         if (rc != HR_OK) return rc;
