@@ -269,10 +269,16 @@ int hr_hop_local_boundary(const hr_geom* g, const hr_decomp* d, int out_parity, 
  *                          and kept for the life of the process — the one place this library allocates anything) and
  *                          the caller's stream: upload of spinor i+1, pack + operator + unpack of spinor i and download
  *                          of result i-1 overlap, so both PCIe directions are busy.  workspace =
- *                          hr_host_batch_workspace_bytes(g) device bytes.  Returns after the last result has arrived. */
+ *                          hr_host_batch_workspace_bytes(g) device bytes.  Returns after the last result has arrived.
+ *   hr_apply_host_ops    : the same pipeline with one operator PER ITEM (ops[i], same codes): out_i = Op_i in_i.  A sequence of
+ *                          different operators then pays the pipeline's fill and drain (one upload and one download that overlap
+ *                          nothing) once, not once per operator.  With clover blocks the HR_EO_DHAT items use clover_fwd and
+ *                          clover_inv, the HR_HOST_DIRAC items clover_fwd. */
 enum { HR_HOST_DIRAC = 3 };
 int hr_gauge_upload_host(const hr_geom* g, int rep, const void* u_canon_host, void* u_dev, void* workspace, void* stream);
 size_t hr_host_batch_workspace_bytes(const hr_geom* g);
+int hr_apply_host_ops(const hr_geom* g, const int* ops, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
+                      int nitems, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream);
 int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
                         int nrhs, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream);
 

@@ -78,16 +78,20 @@ size_t hr_host_batch_workspace_bytes(const hr_geom* g) {
     return 2 * (2 * up256h(cs) + 2 * up256h(ds)) + up256h(ds / 2);
 }
 
-int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
-                        int nrhs, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream) {
+// ops == nullptr: every item applies `op`; else item i applies ops[i] (hr_apply_host_ops: one pipeline across operators)
+static int host_pipeline(const hr_geom* g, int op, const int* ops, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
+                         int nrhs, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream) {
     const size_t cs = hr_canonical_spinor_bytes(g), ds = hr_spinor_bytes(g, HR_BOTH), half = ds / 2;
     if (cs == 0) { set_error("hr_apply_host_batch: invalid geometry"); return HR_EINVAL; }
-    if (op < HR_EO_HOP_OE || op > HR_HOST_DIRAC) { set_error("hr_apply_host_batch: unknown op %d", op); return HR_EINVAL; }
+    for (int i = 0; i < (ops ? nrhs : 1); ++i) {
+        const int o = ops ? ops[i] : op;
+        if (o < HR_EO_HOP_OE || o > HR_HOST_DIRAC) { set_error("hr_apply_host_batch: unknown op %d", o); return HR_EINVAL; }
+        if (o == HR_HOST_DIRAC && clover_inv && !ops) { set_error("hr_apply_host_batch: the full operator takes clover_fwd only"); return HR_EINVAL; }
+    }
     if (nrhs < 0 || (nrhs > 0 && (!in_canon_host || !out_canon_host))) { set_error("hr_apply_host_batch: nrhs < 0 or NULL pointer arrays"); return HR_EINVAL; }
     if (!u_dev || !workspace || ((uintptr_t)workspace & 15)) { set_error("hr_apply_host_batch: u_dev / workspace NULL or misaligned"); return HR_EINVAL; }
     for (int i = 0; i < nrhs; ++i)
         if (!in_canon_host[i] || !out_canon_host[i]) { set_error("hr_apply_host_batch: host pointer %d is NULL", i); return HR_EINVAL; }
-    if (op == HR_HOST_DIRAC && clover_inv) { set_error("hr_apply_host_batch: the full operator takes clover_fwd only"); return HR_EINVAL; }
     HostPipe* q = nullptr;
     HR_TRY(pipe_for_current_device(&q));
     cudaStream_t st = (cudaStream_t)stream;
@@ -106,6 +110,7 @@ int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, 
     HR_CUDA(cudaStreamWaitEvent(q->s_out, q->start, 0));
     for (int i = 0; i < nrhs; ++i) {
         const int b = i & 1;
+        if (ops) op = ops[i];
         // stage 1 (copy-in stream): host -> canonical staging buffer
         if (i >= 2) HR_CUDA(cudaStreamWaitEvent(q->s_in, q->packed[b], 0));      // the pack of spinor i-2 has consumed it
         HR_CUDA(cudaMemcpyAsync(c_in[b], in_canon_host[i], cs, cudaMemcpyHostToDevice, q->s_in));
@@ -115,7 +120,7 @@ int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, 
         HR_TRY(hr_pack_spinor(g, c_in[b], d_in[b], stream));
         HR_CUDA(cudaEventRecord(q->packed[b], st));
         if (op == HR_HOST_DIRAC) {
-            if (clover_fwd) HR_TRY(hr_dirac_clover_apply(g, u_dev, clover_fwd, d_in[b], d_out[b], stream));
+            if (clover_fwd) HR_TRY(hr_dirac_clover_apply(g, u_dev, clover_fwd, d_in[b], d_out[b], stream));   // (clover_inv, if any, belongs to the Dhat items)
             else HR_TRY(hr_dirac_apply(g, m0, u_dev, d_in[b], d_out[b], stream));
         } else {
             HR_CUDA(cudaMemsetAsync(d_out[b], 0, ds, st));                        // the untouched parity comes back as zeros
@@ -135,6 +140,17 @@ int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, 
     HR_CUDA(cudaStreamSynchronize(st));
     HR_CUDA(cudaStreamSynchronize(q->s_out));
     return HR_OK;
+}
+
+int hr_apply_host_batch(const hr_geom* g, int op, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
+                        int nrhs, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream) {
+    return host_pipeline(g, op, nullptr, m0, u_dev, clover_fwd, clover_inv, nrhs, in_canon_host, out_canon_host, workspace, stream);
+}
+
+int hr_apply_host_ops(const hr_geom* g, const int* ops, double m0, const void* u_dev, const void* clover_fwd, const void* clover_inv,
+                      int nitems, const void* const* in_canon_host, void* const* out_canon_host, void* workspace, void* stream) {
+    if (nitems > 0 && !ops) { set_error("hr_apply_host_ops: ops is NULL"); return HR_EINVAL; }
+    return host_pipeline(g, HR_HOST_DIRAC, ops, m0, u_dev, clover_fwd, clover_inv, nitems, in_canon_host, out_canon_host, workspace, stream);
 }
 
 }  // extern "C"

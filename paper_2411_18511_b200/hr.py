@@ -31,7 +31,7 @@ SYMBOLS = [
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
     "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_gauge_upload_host",
-    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local",
+    "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_apply_host_ops", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local",
     "hr_hop_local_interior", "hr_hop_local_boundary", "hr_last_error",
     "hr_launch_count", "hr_kernel_name", "hr_kernel_plan", "hr_cg_workspace_bytes", "hr_cg_solve",
     "hr_cg_mixed_workspace_bytes", "hr_cg_solve_mixed", "hr_cg_solve_mixed_clover",
@@ -88,6 +88,7 @@ def lib():
             "hr_gauge_upload_host": (I, [G, I, V, V, V, V]),
             "hr_host_batch_workspace_bytes": (S, [G]),
             "hr_apply_host_batch": (I, [G, I, D, V, V, V, I, ctypes.POINTER(V), ctypes.POINTER(V), V, V]),
+            "hr_apply_host_ops": (I, [G, ctypes.POINTER(ctypes.c_int), D, V, V, V, I, ctypes.POINTER(V), ctypes.POINTER(V), V, V]),
             "hr_halo_face_bytes": (S, [G, I]),
             "hr_halo_pack": (I, [G, ctypes.POINTER(hr_decomp), I, V, V, ctypes.POINTER(V), V]),
             "hr_hop_local": (I, [G, ctypes.POINTER(hr_decomp), I, I, D, D, V, V, V, V, V, ctypes.POINTER(V), V]),
@@ -235,6 +236,17 @@ def hr_apply_host_batch(g, op, m0, u_dev, clover_fwd, clover_inv, ins, outs, wor
     pout = (ctypes.c_void_p * n)(*[_ptr(a) for a in outs])
     _check(lib().hr_apply_host_batch(ctypes.byref(g), int(op), float(m0), _ptr(u_dev), _ptr(clover_fwd), _ptr(clover_inv), n, pin, pout,
                                      _ptr(workspace), stream))
+
+
+def hr_apply_host_ops(g, ops, m0, u_dev, clover_fwd, clover_inv, ins, outs, workspace, stream=0):
+    """one operator per item (ops[i]): the pipeline of hr_apply_host_batch across a sequence of different operators"""
+    n = len(ins)
+    assert len(outs) == n and len(ops) == n
+    pin = (ctypes.c_void_p * n)(*[_ptr(a) for a in ins])
+    pout = (ctypes.c_void_p * n)(*[_ptr(a) for a in outs])
+    pops = (ctypes.c_int * n)(*[int(o) for o in ops])
+    _check(lib().hr_apply_host_ops(ctypes.byref(g), pops, float(m0), _ptr(u_dev), _ptr(clover_fwd), _ptr(clover_inv), n, pin, pout,
+                                   _ptr(workspace), stream))
 
 
 def decomp(split) -> hr_decomp:

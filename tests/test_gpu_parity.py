@@ -530,6 +530,23 @@ def test_host_batch_with_resident_gauge(hr, orc, prec):
     hr.hr_apply_host_batch(g, hr.HOST_DIRAC, m0, u_dev, None, None, [], [], ws, st)      # empty batch: nothing to do
     with pytest.raises(hr.HrError):
         hr.hr_apply_host_batch(g, hr.HOST_DIRAC, m0, u_dev, fwd, inv, ins[:1], outs[:1], ws, st)
+    # one pipeline across different operators (hr_apply_host_ops): item i applies ops[i]
+    ops = [hr.EO_HOP_OE, hr.EO_HOP_EO, hr.HOST_DIRAC, hr.EO_DHAT, hr.HOST_DIRAC]
+    wants = [lambda p: orc.hop(L, 0, 1, U, p), lambda p: orc.hop(L, 0, 0, U, p), lambda p: orc.dirac(L, 0, m0, U, p),
+             lambda p: orc.dirac_eo(L, 0, m0, U, p), lambda p: orc.dirac(L, 0, m0, U, p)]
+    for o in outs:
+        o.fill_(7.0)
+    hr.hr_apply_host_ops(g, ops, m0, u_dev, None, None, ins, outs, ws, st)
+    for p_, o, w in zip(psis, outs, wants):
+        assert rel(o.numpy(), w(p_)) <= TOL[prec]
+    # with clover blocks: Dhat items use both block fields, full-D items the forward one
+    for o in outs:
+        o.fill_(7.0)
+    hr.hr_apply_host_ops(g, [hr.EO_DHAT, hr.HOST_DIRAC], m0, u_dev, fwd, inv, ins[:2], outs[:2], ws, st)
+    assert rel(outs[0].numpy(), orc.dirac_eo_clover(L, U, A, Ainv, psis[0])) <= TOL[prec]
+    assert rel(outs[1].numpy(), orc.dirac_clover(L, m0, U, C, psis[1])) <= TOL[prec]
+    with pytest.raises(hr.HrError):
+        hr.hr_apply_host_ops(g, [9], m0, u_dev, None, None, ins[:1], outs[:1], ws, st)
 
 
 def test_native_library_is_the_one_loaded(hr):
