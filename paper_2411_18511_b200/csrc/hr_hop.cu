@@ -52,7 +52,7 @@ int kernel_plan(const hr_geom* g, int both, int* info) {
     if (!tiled_plan(g, both ? 1 : 0, sm_count(), pl)) return HR_OK;
     size_t smem = pl.smem;      // + the link slots where launch_hop_tiled_l3h uses them (fundamental representation, bare / axpy parity hop)
     const size_t with_links = pl.smem + (size_t)8 * link_chunks(g->prec) * 16 * pl.nconsumer;
-    if (HR_HOP_ALINK && !both && g->rep == HR_REP_FUND && with_links <= TILED_SMEM_LIMIT) smem = with_links;
+    if (HOP_ALINK && !both && g->rep == HR_REP_FUND && with_links <= TILED_SMEM_LIMIT) smem = with_links;
     const int v[8] = {1, pl.t1, pl.t2, pl.nseg, pl.seglen, pl.nconsumer + 32, (int)smem, (both ? 2 : 1) * pl.nt1 * pl.nt2 * pl.nseg};
     for (int i = 0; i < 8; ++i) info[i] = v[i];
     return HR_OK;

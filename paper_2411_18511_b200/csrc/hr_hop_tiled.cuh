@@ -18,9 +18,7 @@
 
 namespace hr {
 
-#ifndef HR_HOP_ALINK
-#define HR_HOP_ALINK 1
-#endif
+constexpr bool HOP_ALINK = true;      // link slots in shared memory where an instantiation has them (launch_hop_tiled_l3h)
 constexpr int TILED_RING = 4;         // ring slots: planes x0-1, x0, x0+1 live + one being filled
 constexpr int TILED_HALO = 2;         // halo buffers: one in use, one being filled (a third one costs the L1 the link loads need)
 
@@ -541,7 +539,7 @@ inline int launch_hop_tiled_l3h(const Geo& g, const HopArgs& a, const TiledPlan&
     // (profiles/r02_hop_alink.md): the bare and axpy hops gain (fp64 215.8 -> 206 us; 64^4 817 -> 694 us), the clover epilogues lose
     // (their 256-byte block loads need the L1 that the slots take: E2 724 -> 768 us) and so does the fp64 CG update stage (1320 -> 1328 us per
     // iteration); the norm stage and the fp32 CG stages gain.
-    constexpr bool CAN_ALINK = HR_HOP_ALINK && N == 2 && !SHARE && !ONFLY && (EPI == EPI_NONE || EPI == EPI_AXPY) && (POST != POST_CG_UPDATE || sizeof(T) == 4);
+    constexpr bool CAN_ALINK = HOP_ALINK && N == 2 && !SHARE && !ONFLY && (EPI == EPI_NONE || EPI == EPI_AXPY) && (POST != POST_CG_UPDATE || sizeof(T) == 4);
     if constexpr (CAN_ALINK) {
         const size_t smem = pl.smem + (size_t)8 * SiteIO<T, 2>::NCH * 16 * pl.nconsumer;
         if (smem <= TILED_SMEM_LIMIT) {
