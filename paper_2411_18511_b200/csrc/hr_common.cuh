@@ -397,15 +397,17 @@ __device__ __forceinline__ void herm_matvec(cplx<T>* y, const T* blk, const cplx
 // reals of the two blocks of one site: 2 (2N)^2
 template <int N> struct CloverSize { static constexpr int reals = 2 * (2 * N) * (2 * N); };
 
-// the block reals of one site from the clover field [par][row][chunk][h]
-template <typename T, int N = 2>
+// the block reals of one site from the clover field [par][row][chunk][h].  POLICY: streaming in the site-diagonal kernels; in the hop
+// epilogues the blocks bypass L1 allocation (LD_NOALLOC), which the link and phi loads need more (E2 724 -> 717 us, H3c 620 -> 607 us
+// at 48^4, while the plain clover apply loses 2.5 % with it)
+template <typename T, int N = 2, int POLICY = LD_STREAM>
 __device__ __forceinline__ void load_clover(T* blk, const void* field, const Geo& g, int par, int row, int h) {
     constexpr int CCH = CloverSize<N>::reals * sizeof(T) / 16;
     typedef typename Chunk<T>::type chunk_t;
     const chunk_t* p = reinterpret_cast<const chunk_t*>(field) + ((size_t)par * g.R + row) * (CCH * g.L3h) + h;
 #pragma unroll
     for (int c = 0; c < CCH; ++c) {
-        chunk_to_reals(ldg16<LD_STREAM>(p + (size_t)c * g.L3h), blk + c * (16 / sizeof(T)));
+        chunk_to_reals(ldg16<POLICY>(p + (size_t)c * g.L3h), blk + c * (16 / sizeof(T)));
     }
 }
 

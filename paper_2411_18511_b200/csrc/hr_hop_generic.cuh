@@ -61,14 +61,14 @@ __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const H
     } else if (EPI == EPI_CLOVER_INV) {
         T blk[CloverSize<N>::reals];
         cplx<T> y[NC];
-        load_clover<T, N>(blk, a.clover, g, p, row, h);
+        load_clover<T, N, LD_NOALLOC>(blk, a.clover, g, p, row, h);
         clover_matvec<T, N>(y, blk, acc);
 #pragma unroll
         for (int k = 0; k < NC; ++k) acc[k] = y[k];
     } else if (EPI == EPI_CLOVER_AXPY) {
         T blk[CloverSize<N>::reals];
         cplx<T> phi[NC], y[NC];
-        load_clover<T, N>(blk, a.clover, g, p, row, h);
+        load_clover<T, N, LD_NOALLOC>(blk, a.clover, g, p, row, h);
         IO::template load<PHI_POLICY>(phi, phi_half, first, g.L3h);
         clover_matvec<T, N>(y, blk, phi);
         const T cc = (T)a.c;
