@@ -45,13 +45,15 @@ struct HopArgs {
 // phi is the other parity pass's gather input
 template <typename T, int N, int EPI, int PHI_POLICY = LD_STREAM, int POST = POST_STORE>
 __device__ __forceinline__ void hop_epilogue(cplx<T>* acc, const Geo& g, const HopArgs& a, const void* phi_half,
-                                             void* out_half, int p, int row, int h, double* part = nullptr, T alpha = (T)0) {
+                                             void* out_half, int p, int row, int h, double* part = nullptr, T alpha = (T)0,
+                                             const cplx<T>* phi_pre = nullptr) {   // phi_pre: phi(x) already in registers (EPI_AXPY)
     constexpr int NC = 4 * N;
     typedef SiteIO<T, NC> IO;
     const size_t first = (size_t)row * (IO::NCH * g.L3h) + h;
     if (EPI == EPI_AXPY) {
-        cplx<T> phi[NC];
-        IO::template load<PHI_POLICY>(phi, phi_half, first, g.L3h);
+        cplx<T> phi_ld[NC];
+        if (!phi_pre) IO::template load<PHI_POLICY>(phi_ld, phi_half, first, g.L3h);
+        const cplx<T>* phi = phi_pre ? phi_pre : phi_ld;
         const T ca = (T)a.a, cc = (T)a.c;
 #pragma unroll
         for (int k = 0; k < NC; ++k) {

@@ -382,6 +382,12 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
         const char* const a2b = (b2_in ? scur : shalo) + off_b2 + h * 16;
         const char* const a3f = scur + off_c + hf3 * 16;
         const char* const a3b = scur + off_c + hb3 * 16;
+        // ALINK + axpy epilogue: phi(x) is requested here, a step's worth of arithmetic before its use — with the links in their slots it is
+        // the only global load of the loop, so its scoreboard waits for nothing else
+        cplx<T> phi_pre[(ALINK && EPI == EPI_AXPY) ? NC : 1];
+        if constexpr (ALINK && EPI == EPI_AXPY) {
+            if (active) IO::template load<LD_STREAM>(phi_pre, phi_half, (size_t)(row0 + x0 * g.s0) * (IO::NCH * L3h) + h, L3h);
+        }
         if constexpr (ALINK) {
             Link<T, 2> u;
             lds_site<T, NC>(nbA, a0f, cs);
@@ -461,10 +467,11 @@ __global__ void __launch_bounds__(tiled_max_consumers(T1, T2) + 32, (!SHARE && s
             mbar_arrive(bar_hempty + 8 * hb);
         }
         // (requesting phi before the eight terms was measured slower at 48^4)
+        constexpr bool PHI_PRE = ALINK && EPI == EPI_AXPY;
         if (POST == POST_STORE) {
-            if (active) hop_epilogue<T, N, EPI, (SHARE ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h);
+            if (active) hop_epilogue<T, N, EPI, (SHARE ? LD_KEEP : LD_STREAM)>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h, nullptr, (T)0, PHI_PRE ? phi_pre : nullptr);
         } else {
-            if (active) hop_epilogue<T, N, EPI, LD_STREAM, POST>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h, &cg_part, cg_alpha);
+            if (active) hop_epilogue<T, N, EPI, LD_STREAM, POST>(acc, g, a, phi_half, out_half, p, row0 + x0 * g.s0, h, &cg_part, cg_alpha, PHI_PRE ? phi_pre : nullptr);
         }
     }
     if (ALINK) cp_async_wait<0>();   // the unused requests of the last step must not outlive the CTA
