@@ -125,6 +125,23 @@ enum { HR_EO_HOP_OE = 0, HR_EO_HOP_EO = 1, HR_EO_DHAT = 2 };
 int hr_dirac_eo_apply(const hr_geom* g, int op, double m0, const void* u, const void* clover_fwd,
                       const void* clover_inv, const void* in, void* out, void* tmp, void* stream);
 
+/* E1/E2 without any device allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it):   out_e = Dhat in_e   exactly as hr_dirac_eo_apply(op = HR_EO_DHAT) computes
+ * it (same kernels, same bits), with the odd half field between the two hops kept in a file-scope device array of the
+ * library instead of a caller-owned `tmp`.  u, clover_fwd, clover_inv (both NULL or both given), in, out: device,
+ * caller-owned, as for hr_dirac_eo_apply.
+ *   - Limit: hr_spinor_bytes(g, HR_ODD) <= HR_STATIC_SCRATCH_BYTES (8 MiB: 16^3 x 32 SU(2)-fundamental sites in fp64,
+ *     twice that in fp32); a larger lattice returns HR_EINVAL with the two sizes in hr_last_error() and launches nothing.
+ *   - The call makes no cudaMalloc / cudaFree and calls no allocating library routine.  Every GPU that loads the library
+ *     holds the 8 MiB until the process exits.  The first call on a device looks the array's device address up
+ *     (cudaGetSymbolAddress, once per device, the device of `stream` current): make that call outside stream capture.
+ *   - All calls on one device share the array, which keeps the last call's contents.  Nothing in it has to start at
+ *     zero (the first hop writes every entry the second one reads), but two calls that overlap on the GPU — different
+ *     streams, or graphs replayed concurrently — race on it: serialise them (one stream, or an event between them). */
+#define HR_STATIC_SCRATCH_BYTES (8u << 20)
+int hr_dhat_apply_static(const hr_geom* g, double m0, const void* u, const void* clover_fwd, const void* clover_inv,
+                         const void* in, void* out, void* stream);
+
 /* C1 ("precomputing certain fields ... recomputed whenever the gauge field is updated"):
  * from the FUNDAMENTAL gauge field build, for every site, the two hermitian chirality blocks (4x4 for fundamental
  * fermions, 6x6 for adjoint ones: g->rep, the leaves mapped to the adjoint representation) of

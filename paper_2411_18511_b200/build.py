@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhr_dslash.so")
-SOURCES = ["hr_api.cu", "hr_fields.cu", "hr_hop.cu", "hr_solver.cu", "hr_host.cu", "hr_halo.cu", "hr_hop_open.cu", "hr_hop_cg.cu"]
+SOURCES = ["hr_api.cu", "hr_fields.cu", "hr_hop.cu", "hr_solver.cu", "hr_host.cu", "hr_halo.cu", "hr_hop_open.cu", "hr_hop_cg.cu", "hr_static.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "--use_fast_math=false", "-Xptxas", "-v"]
 

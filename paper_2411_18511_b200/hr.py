@@ -23,13 +23,14 @@ EO_HOP_OE, EO_HOP_EO, EO_DHAT = 0, 1, 2
 HOST_DIRAC = 3
 EPI_NONE, EPI_AXPY, EPI_CLOVER_INV, EPI_CLOVER_AXPY = 0, 1, 2, 3
 OP_HOP, OP_DIRAC, OP_DHAT, OP_CLOVER, OP_DHAT_CLOVER, OP_REPRESENT = 0, 1, 2, 3, 4, 5
+STATIC_SCRATCH_BYTES = 8 << 20   # HR_STATIC_SCRATCH_BYTES of include/hr_dslash.h
 
 # every symbol include/hr_dslash.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = [
     "hr_spinor_bytes", "hr_gauge_bytes", "hr_clover_bytes", "hr_canonical_spinor_bytes",
     "hr_canonical_gauge_bytes", "hr_canonical_clover_bytes", "hr_pack_spinor", "hr_unpack_spinor",
     "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
-    "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
+    "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_dhat_apply_static", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_gauge_upload_host",
     "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_apply_host_ops", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local",
     "hr_hop_local_interior", "hr_hop_local_boundary", "hr_last_error",
@@ -77,6 +78,7 @@ def lib():
             "hr_dirac_apply": (I, [G, D, V, V, V, V]),
             "hr_dirac_clover_apply": (I, [G, V, V, V, V, V]),
             "hr_dirac_eo_apply": (I, [G, I, D, V, V, V, V, V, V, V]),
+            "hr_dhat_apply_static": (I, [G, D, V, V, V, V, V, V]),
             "hr_clover_build": (I, [G, D, D, V, V, V, V]),
             "hr_clover_build_exp": (I, [G, D, D, V, V, V, V]),
             "hr_clover_apply": (I, [G, I, V, V, V, V]),
@@ -186,6 +188,13 @@ def hr_dirac_clover_apply(g, u, clover_fwd, psi, out, stream=0):
 def hr_dirac_eo_apply(g, op, m0, u, clover_fwd, clover_inv, inp, out, tmp, stream=0):
     _check(lib().hr_dirac_eo_apply(ctypes.byref(g), int(op), float(m0), _ptr(u), _ptr(clover_fwd), _ptr(clover_inv),
                                    _ptr(inp), _ptr(out), _ptr(tmp), stream))
+
+
+def hr_dhat_apply_static(g, m0, u, clover_fwd, clover_inv, inp, out, stream=0):
+    """Dhat with the odd half field between the two hops in the library's static device array (no allocation;
+    lattices up to STATIC_SCRATCH_BYTES per odd half field)."""
+    _check(lib().hr_dhat_apply_static(ctypes.byref(g), float(m0), _ptr(u), _ptr(clover_fwd), _ptr(clover_inv),
+                                      _ptr(inp), _ptr(out), stream))
 
 
 def hr_clover_build(g, m0, csw, u_fund, clover_fwd, clover_inv, stream=0):

@@ -133,6 +133,12 @@ class Lattice:
         hr.hr_dirac_eo_apply(self.g, hr.EO_DHAT, m0, u, clover_fwd, clover_inv, inp, out, tmp, hr.stream_ptr())
         return out
 
+    def dhat_static(self, m0, u, inp, out, clover_fwd=None, clover_inv=None):
+        """dhat() with the intermediate odd half field in the library's static scratch array: allocates nothing
+        (out is the caller's), lattices up to hr.STATIC_SCRATCH_BYTES per odd half field"""
+        hr.hr_dhat_apply_static(self.g, m0, u, clover_fwd, clover_inv, inp, out, hr.stream_ptr())
+        return out
+
     def clover_build(self, m0, csw, u_fund, exponential=False):
         fwd, inv = self.empty_clover(), self.empty_clover()
         build = hr.hr_clover_build_exp if exponential else hr.hr_clover_build
