@@ -195,12 +195,41 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
     constexpr int LCH = SiteIO<T, 2>::NCH;                     // 16-byte chunks of a compressed link
     const uint32_t lslot = smem_u32(lbuf) + (uint32_t)tid * 16;
     const int lchb = pl.nconsumer * 16;                        // one chunk of one link for all consumer threads
-    auto link_request = [&](int j, int par, int mu, int row, int hh) {
-        if constexpr (ALINK) {
-            const char* src = reinterpret_cast<const char*>(a.gauge) + (((size_t)(par * 4 + mu) * g.R + row) * (LCH * L3h) + hh) * 16;
+    // ALINK: the address of link j is carried from step to step — one x0-plane further and into the other parity half, since the
+    // parity of the column's site alternates: + s0 rows +- the parity stride, the sign swapping every step and opposite for the
+    // forward links (parity of the site) and the backward ones (other parity) — instead of the full index arithmetic
+    // ((par*4 + mu)*R + row)*W + h per link and step.  fp64: seven 64-bit pointers.  fp32 (13 warps: 128 registers at most): seven
+    // 32-bit offsets in 16-byte units from the start of the gauge field (the plan refuses fields of 2^32 chunks or more).
+    constexpr bool RUN64 = ALINK && sizeof(T) == 8, RUN32 = ALINK && sizeof(T) == 4;
+    const char* lptr[RUN64 ? 7 : 1];
+    uint32_t loff[RUN32 ? 7 : 1];
+    const long long lrow = (long long)(LCH * L3h);                                   // 16-byte chunks of one row of links of one parity and direction
+    const long long dplus = ((long long)g.s0 + 4 * (long long)g.R) * lrow, dminus = ((long long)g.s0 - 4 * (long long)g.R) * lrow;
+    long long dstep_f = 0, dstep_b = 0;                                              // this step's advance of the forward / backward links (bytes)
+    uint32_t ostep_f = 0, ostep_b = 0;                                               // the same in chunks, modulo 2^32
+    bool more = true;                                                                // a next step exists (its links are requested)
+    auto link_issue = [&](int j) {
+        const char* src = RUN64 ? lptr[RUN64 ? j : 0] : reinterpret_cast<const char*>(a.gauge) + (size_t)loff[RUN32 ? j : 0] * 16;
 #pragma unroll
-            for (int c = 0; c < LCH; ++c) cp_async16(lslot + (j * LCH + c) * lchb, src + (size_t)c * cs);
+        for (int c = 0; c < LCH; ++c) cp_async16(lslot + (j * LCH + c) * lchb, src + (size_t)c * cs);
+    };
+    auto link_request = [&](int j, int par, int mu, int row, int hh) {      // prologue (and every step with the links in registers)
+        if constexpr (ALINK) {
+            const size_t chunk = ((size_t)(par * 4 + mu) * g.R + row) * (LCH * L3h) + hh;
+            if constexpr (RUN64) lptr[j] = reinterpret_cast<const char*>(a.gauge) + chunk * 16;
+            else loff[j] = (uint32_t)chunk;
+            link_issue(j);
             cp_async_commit();
+        } else {
+            load_link_rep<T, LP, false>(ul[j], a.gauge, g, par, mu, row, hh);
+        }
+    };
+    auto link_next = [&](int j, bool fwd, int par, int mu, int row, int hh) {
+        if constexpr (ALINK) {
+            if constexpr (RUN64) lptr[j] += fwd ? dstep_f : dstep_b;
+            else loff[j] += fwd ? ostep_f : ostep_b;
+            if (more) link_issue(j);     // no request past the last plane of the segment (the address may lie outside the field)
+            cp_async_commit();           // the (possibly empty) group keeps the wait_group count
         } else {
             load_link_rep<T, LP, false>(ul[j], a.gauge, g, par, mu, row, hh);
         }
@@ -248,6 +277,16 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
         const int xn = (k + 1 < nsteps) ? x0 + 1 : x0;
         const int pn = (xn + x1 + x2 + q) & 1;
         const int rown = row0 + xn * g.s0;
+        if constexpr (ALINK) {
+            more = k + 1 < nsteps;
+            if constexpr (RUN64) {
+                dstep_f = 16 * (p ? dminus : dplus);
+                dstep_b = 16 * (p ? dplus : dminus);
+            } else {
+                ostep_f = (uint32_t)(p ? dminus : dplus);
+                ostep_b = (uint32_t)(p ? dplus : dminus);
+            }
+        }
 
         // Eight terms: x0-1 from registers, x3+- from the centre plane, then (halo wait) x1+-, x2+- from the centre plane and its halo
         // rows, last x0+1 from the newest plane.  Each link is re-requested for the next step right after its use.
@@ -261,34 +300,34 @@ __global__ void __launch_bounds__(dt_max_consumers(T1, T2) + 32, 1) dirac_tiled_
         lds_site<T, NC>(nb2, scur + off_b3, cs);
         link_get(u, 0);
         hop_term<T, N, 3, true>(acc, nb, u);
-        link_request(0, pn, 3, rown, h);
+        link_next(0, true, pn, 3, rown, h);
         mbar_wait(bar_hfull + 8 * hbuf, ((uint32_t)k / NHALO) & 1);
         lds_site<T, NC>(nb, (f1_in ? scur : shalo) + off_f1, cs);
         link_get(u, 1);
         hop_term<T, N, 3, false>(acc, nb2, u);
-        link_request(1, 1 - pn, 3, rown, hb3);
+        link_next(1, false, 1 - pn, 3, rown, hb3);
         lds_site<T, NC>(nb2, (b1_in ? scur : shalo) + off_b1, cs);
         link_get(u, 2);
         hop_term<T, N, 1, true>(acc, nb, u);
-        link_request(2, pn, 1, rown, h);
+        link_next(2, true, pn, 1, rown, h);
         lds_site<T, NC>(nb, (f2_in ? scur : shalo) + off_f2, cs);
         link_get(u, 3);
         hop_term<T, N, 1, false>(acc, nb2, u);
-        link_request(3, 1 - pn, 1, rowb1_0 + xn * g.s0, h);
+        link_next(3, false, 1 - pn, 1, rowb1_0 + xn * g.s0, h);
         lds_site<T, NC>(nb2, (b2_in ? scur : shalo) + off_b2, cs);
         link_get(u, 4);
         hop_term<T, N, 2, true>(acc, nb, u);
-        link_request(4, pn, 2, rown, h);
+        link_next(4, true, pn, 2, rown, h);
         // x0+1: this column's own spinor of the next plane — its copy had two steps to land
         mbar_wait(bar_full + 8 * ((k + 2) % RING), ((uint32_t)(k + 2) / RING) & 1);
         lds_site<T, NC>(nb, snext + off_c, cs);
         link_get(u, 5);
         hop_term<T, N, 2, false>(acc, nb2, u);
-        link_request(5, 1 - pn, 2, rowb2_0 + xn * g.s0, h);
+        link_next(5, false, 1 - pn, 2, rowb2_0 + xn * g.s0, h);
         link_get(u, 6);
         hop_term<T, N, 0, true>(acc, nb, u);
         ub0 = u;
-        link_request(6, pn, 0, rown, h);
+        link_next(6, true, pn, 0, rown, h);
         // the centre plane and its halo are consumed
         __syncwarp();
         if ((tid & 31) == 0) {
@@ -321,6 +360,7 @@ inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, Dir
     pl.nconsumer = 2 * ((sites + 31) & ~31);
     if (pl.nconsumer > dt_max_consumers(t1, t2)) return false;
     pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
+    if (alink && (unsigned long long)8 * g.R * link_chunks(hg->prec) * g.L3h >= (1ull << 32)) alink = false;   // 32-bit chunk offsets of the fp32 link slots
     pl.alink = alink ? 1 : 0;
     const int ring = dt_ring(alink, real_bytes(hg->prec)), nhalo = dt_nhalo(alink, real_bytes(hg->prec));
     pl.smem = 128 + (size_t)pl.rowb * 2 * (ring * t1 * t2 + nhalo * (2 * t1 + 2 * t2)) +
