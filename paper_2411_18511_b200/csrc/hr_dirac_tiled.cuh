@@ -360,7 +360,8 @@ inline bool dirac_plan_shape(const hr_geom* hg, int num_sms, int t1, int t2, Dir
     pl.nconsumer = 2 * ((sites + 31) & ~31);
     if (pl.nconsumer > dt_max_consumers(t1, t2)) return false;
     pl.rowb = spinor_chunks(hg->rep, hg->prec) * g.L3h * 16;
-    if (alink && (unsigned long long)8 * g.R * link_chunks(hg->prec) * g.L3h >= (1ull << 32)) alink = false;   // 32-bit chunk offsets of the fp32 link slots
+    // the fp32 kernel addresses its link slots' sources by 32-bit chunk offsets
+    if (alink && hg->prec == HR_PREC_F32 && (unsigned long long)8 * g.R * link_chunks(hg->prec) * g.L3h >= (1ull << 32)) alink = false;
     pl.alink = alink ? 1 : 0;
     const int ring = dt_ring(alink, real_bytes(hg->prec)), nhalo = dt_nhalo(alink, real_bytes(hg->prec));
     pl.smem = 128 + (size_t)pl.rowb * 2 * (ring * t1 * t2 + nhalo * (2 * t1 + 2 * t2)) +
