@@ -14,8 +14,8 @@
 //   * The other seven links of a site do NOT travel through registers: each thread owns seven slots in shared memory that it
 //     fills with cp.async and re-requests right after use (ALINK, see cp_async16 below) — a register load requested a step
 //     ahead is in fact waited for together with every later global load of the warp (one scoreboard).
-//   * Plane x0-1 is never read from shared memory: the ring holds planes x0, x0+1 and the plane(s) in flight (3 slots with
-//     ALINK, 4 without); the halo rows (x1 and x2 neighbours of the tile edge, centre plane only) have their own buffers
+//   * Plane x0-1 is never read from shared memory: the ring holds planes x0, x0+1 and the plane(s) in flight (3 slots in fp64 with
+//     ALINK, else 4); the halo rows (x1 and x2 neighbours of the tile edge, centre plane only) have their own buffers
 //     and their own mbarriers so that they do not hold the plane copies back, and are requested before the plane.
 //   * The eight terms run x0-1, x3+-, [halo wait] x1+-, x2+-, x0+1, and the neighbour of term t+1 is read from shared memory
 //     before term t is computed (two register images).
@@ -32,10 +32,12 @@ namespace hr {
 // ~196 KiB of shared memory then starves the L1 the link loads go through (profiles/r02_kernels.md).
 constexpr int DT_RING = 4;
 constexpr int DT_HALO = 2;
-// With the links in shared-memory slots (ALINK) nothing goes through L1 and all 227 KiB can be used: 3 planes + 2 halo buffers +
-// link slots in fp64 (211 KiB at L3 = 48), 3 planes + 3 halo buffers + link slots in fp32 (223 KiB).
-__host__ __device__ constexpr int dt_ring(bool alink, size_t real_bytes) { return alink ? 3 : DT_RING; }
-__host__ __device__ constexpr int dt_nhalo(bool alink, size_t real_bytes) { return (alink && real_bytes == 4) ? 3 : DT_HALO; }
+// With the links in shared-memory slots (ALINK) nothing goes through L1 and all 227 KiB can be used.  fp64 (2 x 2 tile): 3 planes + 2 halo
+// buffers + link slots = 211 KiB at L3 = 48 — no room for more.  fp32 (2 x 4 tile): 4 planes + 2 halo buffers + link slots = 210 KiB: the
+// plane in flight then has almost three steps to land instead of almost two; with 3 planes + 3 halo buffers (223 KiB) the wait for the
+// x0+1 plane was the top stall of the fp32 kernel (11.5 % of the samples, profiles/r02_dirac_alink.md section 8): 179.2 -> 175.1 us.
+__host__ __device__ constexpr int dt_ring(bool alink, size_t real_bytes) { return (alink && real_bytes == 8) ? 3 : DT_RING; }
+__host__ __device__ constexpr int dt_nhalo(bool alink, size_t real_bytes) { return DT_HALO; }
 
 // consumer threads the kernel is compiled for: one per site of a T1 x T2 tile of full x3-rows of up to 48 sites (2 x 2, 2 x 4 tiles) or
 // up to 96 sites (the 1 x 2 tile of long rows, L3 = 50 .. 96)

@@ -215,10 +215,10 @@ def test_kernel_plan_of_the_bench_lattice(L):
     assert hr.hr_kernel_plan(g64, hr.OP_HOP) == {"kernel": 1, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 224, "smem": 221312, "grid": 288}
     assert hr.hr_kernel_plan(g64, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 2, "nseg": 1, "seglen": 48, "threads": 224, "smem": 215168, "grid": 576}
     assert hr.hr_kernel_plan(g32, hr.OP_HOP)["grid"] == 144 and hr.hr_kernel_plan(g32, hr.OP_HOP)["t1"] == 4
-    assert hr.hr_kernel_plan(g32, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 416, "smem": 227456, "grid": 288}
+    assert hr.hr_kernel_plan(g32, hr.OP_DIRAC) == {"kernel": 2, "t1": 2, "t2": 4, "nseg": 1, "seglen": 48, "threads": 416, "smem": 215168, "grid": 288}
     # the fp32 full-lattice kernel addresses its links by 32-bit offsets in 16-byte chunks: a gauge field of 2^32 chunks or more
     # (8 * L0*L1*L2 * L3/2 >= 2^32) falls back to the register-link form (no link slots: less shared memory); fp64 carries pointers
-    assert hr.hr_kernel_plan(hr.geom((256, 256, 256, 48), hr.REP_FUND, hr.PREC_F32), hr.OP_DIRAC)["smem"] == 227456
+    assert hr.hr_kernel_plan(hr.geom((256, 256, 256, 48), hr.REP_FUND, hr.PREC_F32), hr.OP_DIRAC)["smem"] == 215168
     assert hr.hr_kernel_plan(hr.geom((512, 256, 256, 48), hr.REP_FUND, hr.PREC_F32), hr.OP_DIRAC)["smem"] == 172160
     assert hr.hr_kernel_plan(hr.geom((512, 256, 256, 48), hr.REP_FUND, hr.PREC_F64), hr.OP_DIRAC)["smem"] == 215168
     # below 32^4 and for adjoint / SU(3) fermions AUTO keeps the generic kernel
