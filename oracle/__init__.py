@@ -369,3 +369,22 @@ def dirac_eo_clover_n(L, rep, U, A, Ainv, psi, nthreads=1):
     t = site_matvec_n(Ainv, t, odd)
     h = hop(L, rep, 0, U, t, nthreads=nthreads)
     return site_matvec_n(A, pe, even) - 0.25 * h
+
+
+# ------------------------------------------------------------------ O13: two-index antisymmetric representation of SU(3)
+def represent_antisym_su3(U):
+    """O13 (SURVEY.md §8(f) item 4 "symmetric/antisymmetric reps", "higher representations"; DESIGN.md §3 reading B9):
+    the two-index antisymmetric representation of complex 3 x 3 links by its definition as the action U e U^T on antisymmetric
+    matrices,
+        R_ab(U) = tr( (e^a)^dag  U  e^b  U^T ),     e^a = (E_ij - E_ji) / sqrt(2)  for the pairs a = (i<j) = (0,1), (0,2), (1,2),
+    written out with explicit basis matrices and one einsum (no minors, no cofactors).  U: complex [..., 3, 3]; returns complex
+    [..., 3, 3].  For N = 3 the representation has dimension N(N-1)/2 = 3 and the result is again a special unitary 3 x 3 matrix, so
+    the operators of link() rep 2 act on it unchanged.  Pinned by P23."""
+    U = np.ascontiguousarray(U, dtype=np.complex128)
+    pairs = [(0, 1), (0, 2), (1, 2)]
+    e = np.zeros((3, 3, 3), dtype=np.complex128)
+    for a, (i, j) in enumerate(pairs):
+        e[a, i, j] = 1.0 / np.sqrt(2.0)
+        e[a, j, i] = -1.0 / np.sqrt(2.0)
+    # tr(e^a^dag U e^b U^T) = sum_{ijkl} conj(e^a_ij) U_ik e^b_kl U_jl
+    return np.einsum("aij,...ik,bkl,...jl->...ab", np.conj(e), U, e, U)

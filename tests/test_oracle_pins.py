@@ -871,3 +871,41 @@ def test_P22_su3_clover(orc):
     Ar = orc.clover_dense_adj(L4, dd, 1.2, R)
     xa = inputs.gaussian_spinor(L4, 3, seed=2)
     assert np.array_equal(orc.dirac_eo_clover_n(L4, 1, R, Ar, np.linalg.inv(Ar), xa), orc.dirac_eo_clover_adj(L4, R, Ar, np.linalg.inv(Ar), xa))
+
+
+# ---------------------------------------------------------------- P23: two-index antisymmetric representation of SU(3) (O13)
+def test_P23_antisymmetric_representation_su3(orc):
+    """O13 against what the mathematics fixes, none of it through the oracle's own formula:
+    (i) R(U) is unitary with det 1 and R(1) = 1; (ii) homomorphism R(UV) = R(U) R(V); (iii) character
+    tr R(U) = ((tr U)^2 - tr U^2) / 2; (iv) for SU(3) the antisymmetric pair (i,j) is dual to the third index k (epsilon_ijk), so
+    R(U) = P conj(U) P^T with the signed permutation P: (0,1) -> +2, (0,2) -> -1, (1,2) -> +0 — an exact closed form;
+    (v) a diagonal U = diag(z0, z1, z2) gives diag(z0 z1, z0 z2, z1 z2); (vi) an SU(2) matrix V embedded in the upper-left block acts
+    as 1 on the pair (0,1) and as V on the pairs ((0,2), (1,2)); (vii) a non-unitary matrix: the entries are the 2 x 2 minors
+    (brute force), which catches a transposed operand that unitarity would hide."""
+    rng = np.random.default_rng(23)
+    U = inputs.haar_su3(64, 5, 0)
+    Vm = inputs.haar_su3(64, 6, 0)
+    R = orc.represent_antisym_su3(U)
+    I3 = np.eye(3)
+    assert np.abs(R @ np.conj(np.swapaxes(R, -1, -2)) - I3).max() < 1e-14
+    assert np.abs(np.linalg.det(R) - 1.0).max() < 1e-13
+    assert np.abs(orc.represent_antisym_su3(I3) - I3).max() < 1e-15
+    assert np.abs(orc.represent_antisym_su3(U @ Vm) - R @ orc.represent_antisym_su3(Vm)).max() < 1e-14
+    tr = np.trace(U, axis1=-2, axis2=-1)
+    tr2 = np.trace(U @ U, axis1=-2, axis2=-1)
+    assert np.abs(np.trace(R, axis1=-2, axis2=-1) - 0.5 * (tr * tr - tr2)).max() < 1e-14
+    P = np.array([[0, 0, 1], [0, -1, 0], [1, 0, 0]], dtype=float)
+    assert np.abs(R - P @ np.conj(U) @ P.T).max() < 1e-14
+    ph = rng.uniform(0, 2 * np.pi, 2)
+    z = np.exp(1j * np.array([ph[0], ph[1], -ph[0] - ph[1]]))
+    assert np.abs(orc.represent_antisym_su3(np.diag(z)) - np.diag([z[0] * z[1], z[0] * z[2], z[1] * z[2]])).max() < 1e-15
+    V2 = inputs.haar_su2(1, 7, 0)[0]
+    E = np.eye(3, dtype=complex)
+    E[:2, :2] = V2
+    want = np.eye(3, dtype=complex)
+    want[1:, 1:] = V2
+    assert np.abs(orc.represent_antisym_su3(E) - want).max() < 1e-15
+    M = rng.normal(size=(3, 3)) + 1j * rng.normal(size=(3, 3))      # not unitary: R_ab = minor(rows pair a, columns pair b)
+    pairs = [(0, 1), (0, 2), (1, 2)]
+    minors = np.array([[M[i, k] * M[j, l] - M[i, l] * M[j, k] for (k, l) in pairs] for (i, j) in pairs])
+    assert np.abs(orc.represent_antisym_su3(M) - minors).max() < 1e-14
