@@ -49,8 +49,9 @@ enum { HR_OK = 0, HR_EINVAL = 1, HR_EUNSUPPORTED = 2, HR_EALIGN = 3, HR_ECUDA = 
  * exact for unitary links of determinant 1).  It is
  * served by the generic hopping kernel: bare hops, full D, the even-odd operator with and without clover, the clover-improved full
  * operator, the clover block builders (regular and exponential; hr_clover_build takes the SU(3) gauge field itself as u_fund;
- * blocks are 6 x 6 like the adjoint ones), hr_clover_apply, the CG solvers and the sharded hop with every epilogue; only
- * hr_represent_gauge returns HR_EUNSUPPORTED for it. */
+ * blocks are 6 x 6 like the adjoint ones), hr_clover_apply, the CG solvers and the sharded hop with every epilogue;
+ * hr_represent_gauge (the SU(2) adjoint) returns HR_EUNSUPPORTED for it, hr_represent_gauge_antisym builds its two-index
+ * antisymmetric representation. */
 enum { HR_REP_FUND = 0, HR_REP_ADJ = 1, HR_REP_SU3 = 2 };
 enum { HR_PREC_F64 = 0, HR_PREC_F32 = 1 };
 /* fundamental links are stored as their first row (alpha, beta): U = [[alpha, beta], [-conj(beta), conj(alpha)]]
@@ -98,6 +99,16 @@ int hr_unpack_clover(const hr_geom* g, const void* dev, void* canon, void* strea
  * u_fund: fundamental gauge field, u_adj: adjoint gauge field, both device layout, sized by
  * hr_gauge_bytes(g, HR_REP_FUND / HR_REP_ADJ).  g->rep is ignored. */
 int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* stream);
+
+/* R1 for complex 3 x 3 links: the two-index antisymmetric representation (SURVEY.md §8(f) item 4 "symmetric/antisymmetric reps";
+ * PAPER.md:21 "higher representations"; DESIGN.md §3 reading B9):
+ *   R_ab(x,mu) = tr( e^a^dag U_mu(x) e^b U_mu(x)^T ),  e^a = (E_ij - E_ji)/sqrt(2) for the pairs a = (i<j) = (0,1), (0,2), (1,2),
+ * i.e. the 2 x 2 minors of U (rows = pair a, columns = pair b), for all 4V links.  For three colours the representation is
+ * three-dimensional and R is again special unitary, so u_rep has the layout and size of u_fund (hr_gauge_bytes(g, HR_REP_SU3),
+ * all three rows with HR_LINKS_FULL, the first two with HR_LINKS_COMPRESSED) and every HR_REP_SU3 operator takes it as its gauge
+ * field.  g->rep must be HR_REP_SU3 (else HR_EUNSUPPORTED); both pointers on the device, 16-byte aligned, not overlapping
+ * (HR_EINVAL); the caller owns both; asynchronous on `stream`. */
+int hr_represent_gauge_antisym(const hr_geom* g, const void* u_fund, void* u_rep, void* stream);
 
 /* H3 (north_star "full form"): out = D psi on all V sites, one launch.
  * u: gauge field in representation g->rep (the fundamental field if g->link_storage == HR_LINKS_ONTHEFLY);

@@ -14,6 +14,7 @@ int permute_chunks(bool pack, const Geo& g, int NI, int NCH, int SRC, const void
 int rebuild_second_row(const Geo& g, int prec, void* canon, cudaStream_t st);
 int permute_adj(bool pack, const Geo& g, int prec, const void* src, void* dst, cudaStream_t st, bool complex_entries = false, bool two_rows = false);
 int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStream_t st);
+int run_represent_antisym_su3(const Geo& g, int prec, bool tworows, const void* ufund, void* urep, cudaStream_t st);
 int run_clover_build(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_build_adj(const Geo& g, int prec, double diag, double csw, int expo, const void* ufund, void* fwd, void* inv, cudaStream_t st);
 int run_clover_build_c3(const Geo& g, int prec, bool two_rows, double diag, double csw, int expo, const void* gauge, void* fwd, void* inv, cudaStream_t st);
@@ -195,6 +196,13 @@ int hr_represent_gauge(const hr_geom* g, const void* u_fund, void* u_adj, void* 
     HR_TRY(check_geom(g)); HR_TRY(check_no_su3(g, "hr_represent_gauge")); HR_TRY(check_ptr(u_fund, "u_fund")); HR_TRY(check_ptr(u_adj, "u_adj"));
     if (g->link_storage == HR_LINKS_FULL) { set_error("only HR_LINKS_COMPRESSED fundamental links are stored"); return HR_EUNSUPPORTED; }
     return run_represent(make_geo(g), g->prec, u_fund, u_adj, (cudaStream_t)stream);
+}
+
+int hr_represent_gauge_antisym(const hr_geom* g, const void* u_fund, void* u_rep, void* stream) {
+    HR_TRY(check_geom(g)); HR_TRY(check_ptr(u_fund, "u_fund")); HR_TRY(check_ptr(u_rep, "u_rep"));
+    if (g->rep != HR_REP_SU3) { set_error("hr_represent_gauge_antisym: complex 3 x 3 links only (g->rep must be HR_REP_SU3)"); return HR_EUNSUPPORTED; }
+    if (overlap(u_fund, hr_gauge_bytes(g, HR_REP_SU3), u_rep, hr_gauge_bytes(g, HR_REP_SU3))) { set_error("hr_represent_gauge_antisym: u_rep aliases u_fund"); return HR_EINVAL; }
+    return run_represent_antisym_su3(make_geo(g), g->prec, g->link_storage == HR_LINKS_COMPRESSED, u_fund, u_rep, (cudaStream_t)stream);
 }
 
 // ---------------------------------------------------------------- H3

@@ -177,6 +177,53 @@ int run_represent(const Geo& g, int prec, const void* ufund, void* uadj, cudaStr
     return check_launch("represent_kernel");
 }
 
+// R1 for complex 3 x 3 links: the two-index antisymmetric representation.  U acts on
+// antisymmetric matrices as e -> U e U^T; in the basis e^a = (E_ij - E_ji)/sqrt(2), a = (i<j) = (0,1), (0,2), (1,2), the matrix of
+// that action is the second compound of U — its 2 x 2 minors:
+//     R_ab = U_ik U_jl - U_il U_jk     with (i,j) the pair a (rows) and (k,l) the pair b (columns).
+// For N = 3 it is again special unitary, so it is stored like the fundamental field (all three rows, or the first two) and every
+// HR_REP_SU3 operator runs on it unchanged.  One thread per link.
+template <typename T, bool TWOROWS>
+__global__ void represent_antisym_su3_kernel(Geo g, const void* __restrict__ ufund, void* __restrict__ urep) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = 8LL * g.Vh;  // 2 parities x 4 mu x Vh
+    if (t >= total) return;
+    const int h = (int)(t % g.L3h);
+    const long long pr = t / g.L3h;      // (par*4+mu)*R + row
+    const int pm = (int)(pr / g.R), row = (int)(pr - (long long)pm * g.R);
+    LinkC3<T> u;
+    load_link_rep<T, LD_STREAM, TWOROWS>(u, ufund, g, pm >> 2, pm & 3, row, h);
+    constexpr int NK = TWOROWS ? 6 : 9;
+    typedef typename std::conditional<sizeof(T) == 8, double2, float2>::type pair_t;
+    pair_t* o = reinterpret_cast<pair_t*>(urep) + (size_t)pr * (NK * g.L3h) + h;
+    const int pi[3] = {0, 0, 1}, pj[3] = {1, 2, 2};
+#pragma unroll
+    for (int a = 0; a < (TWOROWS ? 2 : 3); ++a) {
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const cplx<T> m = u.m[3 * pi[a] + pi[b]] * u.m[3 * pj[a] + pj[b]] - u.m[3 * pi[a] + pj[b]] * u.m[3 * pj[a] + pi[b]];
+            pair_t v;
+            v.x = m.re;
+            v.y = m.im;
+            __stcs(o + (size_t)(3 * a + b) * g.L3h, v);
+        }
+    }
+}
+
+int run_represent_antisym_su3(const Geo& g, int prec, bool tworows, const void* ufund, void* urep, cudaStream_t st) {
+    const long long total = 8LL * g.Vh;
+    const unsigned nb = blocks_for(total, 256);
+    if (prec == HR_PREC_F64) {
+        if (tworows) represent_antisym_su3_kernel<double, true><<<nb, 256, 0, st>>>(g, ufund, urep);
+        else represent_antisym_su3_kernel<double, false><<<nb, 256, 0, st>>>(g, ufund, urep);
+    } else {
+        if (tworows) represent_antisym_su3_kernel<float, true><<<nb, 256, 0, st>>>(g, ufund, urep);
+        else represent_antisym_su3_kernel<float, false><<<nb, 256, 0, st>>>(g, ufund, urep);
+    }
+    count_launch();
+    return check_launch("represent_antisym_su3_kernel");
+}
+
 // ------------------------------------------------------------------ C1: clover blocks and their inverses
 // SU(2) matrices as quaternions q = (q0, q1, q2, q3) <-> q0 + i (q1 s1 + q2 s2 + q3 s3):
 //   product (a0,a)(b0,b) = (a0 b0 - a.b, a0 b + b0 a - a x b),  dagger = (a0, -a).

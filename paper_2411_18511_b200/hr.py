@@ -29,7 +29,7 @@ STATIC_SCRATCH_BYTES = 8 << 20   # HR_STATIC_SCRATCH_BYTES of include/hr_dslash.
 SYMBOLS = [
     "hr_spinor_bytes", "hr_gauge_bytes", "hr_clover_bytes", "hr_canonical_spinor_bytes",
     "hr_canonical_gauge_bytes", "hr_canonical_clover_bytes", "hr_pack_spinor", "hr_unpack_spinor",
-    "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge",
+    "hr_pack_gauge", "hr_unpack_gauge", "hr_pack_clover", "hr_unpack_clover", "hr_represent_gauge", "hr_represent_gauge_antisym",
     "hr_dirac_apply", "hr_dirac_clover_apply", "hr_dirac_eo_apply", "hr_dhat_apply_static", "hr_clover_build", "hr_clover_build_exp", "hr_clover_apply", "hr_clover_count_nonfinite", "hr_dirac_flops_bytes",
     "hr_host_workspace_bytes", "hr_dirac_apply_host", "hr_dirac_eo_apply_host", "hr_gauge_upload_host",
     "hr_host_batch_workspace_bytes", "hr_apply_host_batch", "hr_apply_host_ops", "hr_halo_face_bytes", "hr_halo_pack", "hr_hop_local",
@@ -75,6 +75,7 @@ def lib():
             "hr_pack_gauge": (I, [G, I, V, V, V]), "hr_unpack_gauge": (I, [G, I, V, V, V]),
             "hr_pack_clover": (I, [G, V, V, V]), "hr_unpack_clover": (I, [G, V, V, V]),
             "hr_represent_gauge": (I, [G, V, V, V]),
+            "hr_represent_gauge_antisym": (I, [G, V, V, V]),
             "hr_dirac_apply": (I, [G, D, V, V, V, V]),
             "hr_dirac_clover_apply": (I, [G, V, V, V, V, V]),
             "hr_dirac_eo_apply": (I, [G, I, D, V, V, V, V, V, V, V]),
@@ -175,6 +176,10 @@ def hr_unpack_clover(g, dev, canon, stream=0): _check(lib().hr_unpack_clover(cty
 # ------------------------------------------------------------------ operators
 def hr_represent_gauge(g, u_fund, u_adj, stream=0):
     _check(lib().hr_represent_gauge(ctypes.byref(g), _ptr(u_fund), _ptr(u_adj), stream))
+
+
+def hr_represent_gauge_antisym(g, u_fund, u_rep, stream=0):
+    _check(lib().hr_represent_gauge_antisym(ctypes.byref(g), _ptr(u_fund), _ptr(u_rep), stream))
 
 
 def hr_dirac_apply(g, m0, u, psi, out, stream=0):

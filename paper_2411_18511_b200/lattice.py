@@ -111,6 +111,12 @@ class Lattice:
         hr.hr_represent_gauge(self.g, u_fund, u_adj, hr.stream_ptr())
         return u_adj
 
+    def represent_antisym(self, u_fund):
+        """two-index antisymmetric representation of HR_REP_SU3 links (same layout and size as the input field)"""
+        u_rep = self.empty_gauge(hr.REP_SU3)
+        hr.hr_represent_gauge_antisym(self.g, u_fund, u_rep, hr.stream_ptr())
+        return u_rep
+
     def dirac(self, m0, u, psi, out=None):
         out = self.empty_spinor() if out is None else out
         hr.hr_dirac_apply(self.g, m0, u, psi, out, hr.stream_ptr())

@@ -1006,6 +1006,41 @@ def test_su3_small_lattices(hr, orc, L, prec, two_rows):
         assert relres <= 1e-12 and abs(it - it_orc) <= 2 and rel(lat.get_spinor(full), x_orc) <= 1e-9
 
 
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (2, 4, 6, 8), (6, 2, 4, 12)])
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("two_rows", [False, True])
+def test_su3_antisymmetric_representation(hr, orc, L, prec, two_rows):
+    """hr_represent_gauge_antisym (the 2 x 2 minors of a link) against the oracle's O13 (trace definition, pinned by P23), link by
+    link; the result is special unitary; and the operators of HR_REP_SU3 on the represented field against the oracle's rep-2
+    operators on the oracle's represented field.  Wrong representation / aliased buffers are refused."""
+    from paper_2411_18511_b200.lattice import Lattice
+    m0 = -0.2
+    U = rounded(inputs.haar_gauge_su3(L, 1), prec)
+    psi = rounded(inputs.gaussian_spinor(L, 3, 2), prec)
+    lat = Lattice(L, hr.REP_SU3, prec, 0, link_storage=hr.LINKS_COMPRESSED if two_rows else hr.LINKS_FULL)
+    U_dev = lat.put_gauge_su3(U)
+    R_dev = lat.represent_antisym(U_dev)
+    R_want = orc.represent_antisym_su3(U)
+    R_got = lat.get_gauge_su3(R_dev).astype(np.complex128)
+    # entries are sums of two products of numbers of modulus <= 1; with two rows stored the third row of U (and of R) is rebuilt
+    tol = (1e-15 if prec == 0 else 5e-7) * (4 if two_rows else 1)
+    assert np.abs(R_got - R_want).max() <= tol
+    eye = np.eye(3)
+    assert np.abs(R_got @ np.conj(np.swapaxes(R_got, -1, -2)) - eye).max() <= 10 * tol
+    assert np.abs(np.linalg.det(R_got) - 1).max() <= 10 * tol
+    assert np.array_equal(lat.get_gauge_su3(U_dev)[:, :, :2], U.astype(lat.cplx)[:, :, :2])      # the input field is untouched
+    want = oracle_ops(orc, L, 2, R_want, psi, m0)
+    got = gpu_ops(hr, lat, R_dev, psi, m0)
+    for k in want:
+        assert rel(got[k], want[k]) <= TOL[prec], k
+    with pytest.raises(hr.HrError) as e:
+        hr.hr_represent_gauge_antisym(lat.g, U_dev, U_dev, hr.stream_ptr())
+    assert e.value.status == hr.EINVAL
+    with pytest.raises(hr.HrError) as e:
+        hr.hr_represent_gauge_antisym(hr.geom(L, hr.REP_FUND, prec), U_dev, R_dev, hr.stream_ptr())
+    assert e.value.status == hr.EUNSUPPORTED
+
+
 def test_48to4_host_batch_on_sampled_sites(hr, orc, big_inputs):
     """the gauge-resident host path at the bench size: hr_gauge_upload_host + hr_apply_host_batch of 3 right-hand sides (full D
     and Dhat, fp64) at 48^4, checked on sampled sites against the oracle's per-site operator"""
