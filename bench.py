@@ -494,7 +494,14 @@ def other_configs(hr, inputs, Lattice):
             out["su3_48^4_%s_%s" % (name, ptag)] = {"us_per_apply": round(ms * 1e3, 1), "gsites_per_s": round(sites / ms / 1e6, 3),
                                                    "gflops": round(f * sites / ms / 1e6, 1), "gbs": round(bc * sites / ms / 1e6, 1),
                                                    "frac": round(bc * sites / ms / 1e6 / peak, 4), "bytes_per_site": bc, "kernel": hr.hr_kernel_name(g)}
-        del U_dev, p_dev, o_dev, tmp
+        # the two-index antisymmetric representation of the links (hr_represent_gauge_antisym): a streaming kernel that reads and
+        # writes one gauge field — bytes per link = 2 x the stored link
+        R_dev = lat.empty_gauge(hr.REP_SU3)
+        ms = timed(lambda: hr.hr_represent_gauge_antisym(g, U_dev, R_dev, st0), 20)
+        rbytes = 2.0 * hr.hr_gauge_bytes(g, hr.REP_SU3)
+        out["su3_48^4_represent_antisym_%s" % ptag] = {"us_per_apply": round(ms * 1e3, 1), "gbs": round(rbytes / ms / 1e6, 1),
+                                                       "frac": round(rbytes / ms / 1e6 / peak, 4), "bytes_per_link": rbytes / (4 * V)}
+        del U_dev, p_dev, o_dev, tmp, R_dev
     # the sharded hop on this one GPU: a 48^4 local lattice whose four directions are all cut onto the rank itself;
     # pack + device-to-device face copies + interior kernel + boundary kernels per hop o<-e, in order and with pack / copies
     # on a side stream (no multi-GPU hardware in this run: this measures what a cut costs a rank, not the transport)
